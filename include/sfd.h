@@ -1,0 +1,126 @@
+/* sfd.h — C ABI of libsfd: Shifted-Fresnel diffraction on one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (arxiv/paper_1001_4309, §2.1, Eq.(1)-(5), L50-71; step list
+ * (i)-(xi), L85-95): from one N x N in-line hologram u0 sampled at pitch p1, for each of n_views
+ * views with its own depth z, reconstruction pitch p2 and off-axis shift (Ox, Oy), the complex
+ * field
+ *
+ *     u1[n1][m1] = c0 * sum_{n0,m0} u0[n0][m0] * exp(i pi [(x1-x0)^2 + (y1-y0)^2] / (lambda z)),
+ *     x0 = (m0 - N/2) p1,  y0 = (n0 - N/2) p1,  x1 = (m1 - N/2) p2 + Ox,  y1 = (n1 - N/2) p2 + Oy,
+ *     c0 = p1^2 exp(i 2 pi z / lambda) / (i lambda z),
+ *
+ * and its intensity I = |u1|^2 (Eq. 5).  This is Eq.(1) with all of C1 (Eq. 2) kept and the area
+ * element p1^2 included (readings 1, 2, 9, 10).  It is evaluated as the paper evaluates
+ * it — pre-chirp (Eq. 3), zero-padded 2N-point FFT, multiply by the spectrum of the chirp kernel h
+ * (Eq. 4), inverse FFT, crop, post-chirp (Eq. 2) — but, h being separable, as two fused passes of
+ * 1-D length-2N transforms (first along y, then along x); see DESIGN.md §5.
+ *
+ * Conventions
+ *   - Arrays are row-major [n][m]: n <-> y <-> row, m <-> x <-> fastest index.
+ *   - All lengths are SI metres.  All per-view parameter arrays are HOST arrays of n_views doubles
+ *     and are copied at plan creation (the caller may free them afterwards).
+ *   - Pointers named *_dev are DEVICE pointers on the plan's device (the device current when the
+ *     plan was created); *_pinned are page-locked HOST pointers.  The caller owns them.
+ *   - The plan owns its device tables, the cached chirp-kernel spectra and its workspace.
+ *   - Every call returns an int: 0 = SFD_OK, negative = error.  No exception crosses the ABI.
+ *   - One sfd_execute* may be in flight per plan (shared workspace); distinct plans are
+ *     independent.  Calls on one plan must be issued from one host thread at a time.
+ */
+#ifndef SFD_H
+#define SFD_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sfd_plan sfd_plan; /* opaque */
+
+/* error codes */
+#define SFD_OK 0
+#define SFD_EINVAL (-1)       /* bad argument (NULL, size, non-finite parameter, z == 0, ...) */
+#define SFD_ENOMEM (-2)       /* host or device allocation failed */
+#define SFD_ECUDA (-3)        /* a CUDA runtime call failed; see sfd_last_cuda_error() */
+#define SFD_EUNSUPPORTED (-4) /* valid request that this build does not implement */
+
+/* hologram sample types (argument in_dtype) */
+#define SFD_U8 0  /* unsigned 8-bit CCD samples; the method sees value/255 (reading 12) */
+#define SFD_F32 1 /* float32 samples used as they are */
+
+/* Create a plan for one hologram size and a fixed set of views (S = p1 p2/(lambda z);
+ * Eq.(2)-(4)).  Builds, in float64 on the host, the 1-D chirp tables of Eq.(2)-(3) and the spectrum
+ * of the 1-D chirp kernel of Eq.(4) for every view (steps (v)-(vi) L89-90, done once here instead
+ * of every frame), uploads them as complex64 and allocates the workspace
+ * (n_views * N * N complex64 + n_views * N * N float32).
+ *   out      receives the plan; *out = NULL on failure.
+ *   N        hologram / output side; a power of two, 64 <= N <= 2048.
+ *   n_views  >= 1.
+ *   lambda   wavelength > 0.
+ *   p1,p2,z,Ox,Oy  host arrays [n_views]: hologram pitch (> 0), reconstruction pitch (> 0), depth
+ *            (finite, != 0; negative = conjugate reconstruction), shifts of the output window.
+ *   in_dtype SFD_U8 or SFD_F32.
+ * Errors: SFD_EINVAL, SFD_ENOMEM, SFD_ECUDA. */
+int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const double *p1,
+                    const double *p2, const double *z, const double *Ox, const double *Oy,
+                    int in_dtype);
+
+/* Reconstruct all views of one hologram (steps (ii)-(x), L86-94).  Asynchronous on `stream`
+ * (a cudaStream_t passed as void*; NULL = the legacy default stream); no host synchronisation.
+ *   hologram_dev   [N][N] samples of the plan's in_dtype.
+ *   field_dev      [n_views][N][N] complex64 (re, im interleaved), or NULL to skip the field.
+ *   intensity_dev  [n_views][N][N] float32, or NULL to skip the intensity.
+ * At least one output must be non-NULL.  Errors: SFD_EINVAL, SFD_ECUDA. */
+int sfd_execute(sfd_plan *plan, const void *hologram_dev, void *field_dev, float *intensity_dev,
+                void *stream);
+
+/* Real-time variant (step (xi) L95, reading 15): intensity returned as 8-bit images, per view
+ * I8 = round_half_even(255 * I / max(I)) (an all-zero view gives zeros).
+ *   intensity_u8_dev  [n_views][N][N] unsigned char.  Asynchronous on `stream`. */
+int sfd_execute_u8(sfd_plan *plan, const void *hologram_dev, unsigned char *intensity_u8_dev,
+                   void *stream);
+
+/* Real-time stream (steps (i)-(xi) repeated, L83-97): reconstruct n_frames holograms that sit in
+ * page-locked host memory, double-buffering the H2D copies against compute and the D2H copies of
+ * the 8-bit results, on three internal streams.  Blocking: returns when out_pinned is complete.
+ *   holograms_pinned  [n_frames][N][N] samples of the plan's in_dtype (pinned host memory).
+ *   out_pinned        [n_frames][n_views][N][N] unsigned char (pinned host memory).
+ *   seconds           if non-NULL, receives the device-measured time (CUDA events) from the start
+ *                     of the first H2D copy to the end of the last D2H copy. */
+int sfd_stream_run(sfd_plan *plan, const void *holograms_pinned, int n_frames,
+                   unsigned char *out_pinned, double *seconds);
+
+/* Replace the parameters of one view (0 <= view < n_views) and rebuild its tables and cached
+ * spectrum (the paper's user steers z, p2, Ox, Oy live: L33, L73, L123).  Synchronises with the
+ * device (cudaMemcpy) before returning; do not call while an execute on this plan is in flight. */
+int sfd_plan_update_view(sfd_plan *plan, int view, double p1, double p2, double z, double Ox,
+                         double Oy);
+
+/* Destroy a plan and free everything it owns.  NULL is accepted. */
+int sfd_plan_destroy(sfd_plan *plan);
+
+/* Plan queries (host): N, n_views, padded FFT length M = 2N, bytes of device memory owned. */
+int sfd_plan_get_n(const sfd_plan *plan);
+int sfd_plan_get_views(const sfd_plan *plan);
+int sfd_plan_get_m(const sfd_plan *plan);
+long long sfd_plan_device_bytes(const sfd_plan *plan);
+
+/* Timing aid for benchmarks: CUDA-event time, in milliseconds, of each of the two hot kernels
+ * (pass y, pass x) of the most recent execute call on this plan, recorded on the stream they
+ * were launched on.  Synchronises on those events.  ms[0] = pass y, ms[1] = pass x,
+ * ms[2] = quantise (0 when not run).  Requires sfd_plan_set_timing(plan, 1) beforehand. */
+int sfd_plan_set_timing(sfd_plan *plan, int enable);
+int sfd_plan_last_kernel_ms(sfd_plan *plan, float ms[3]);
+
+/* Number of kernel launches issued by all sfd_execute* / sfd_stream_run calls of this process. */
+long long sfd_launch_count(void);
+
+/* Static description of an error code / of the last CUDA error seen by this thread. */
+const char *sfd_error_string(int code);
+const char *sfd_last_cuda_error(void);
+
+/* Library version, e.g. "sfd 0.1 sm_100a". */
+const char *sfd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SFD_H */
