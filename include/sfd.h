@@ -35,6 +35,12 @@ extern "C" {
 
 typedef struct sfd_plan sfd_plan; /* opaque */
 
+#if defined(__GNUC__)
+#define SFD_API __attribute__((visibility("default")))
+#else
+#define SFD_API
+#endif
+
 /* error codes */
 #define SFD_OK 0
 #define SFD_EINVAL (-1)       /* bad argument (NULL, size, non-finite parameter, z == 0, ...) */
@@ -59,7 +65,7 @@ typedef struct sfd_plan sfd_plan; /* opaque */
  *            (finite, != 0; negative = conjugate reconstruction), shifts of the output window.
  *   in_dtype SFD_U8 or SFD_F32.
  * Errors: SFD_EINVAL, SFD_ENOMEM, SFD_ECUDA. */
-int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const double *p1,
+SFD_API int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const double *p1,
                     const double *p2, const double *z, const double *Ox, const double *Oy,
                     int in_dtype);
 
@@ -69,13 +75,13 @@ int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const dou
  *   field_dev      [n_views][N][N] complex64 (re, im interleaved), or NULL to skip the field.
  *   intensity_dev  [n_views][N][N] float32, or NULL to skip the intensity.
  * At least one output must be non-NULL.  Errors: SFD_EINVAL, SFD_ECUDA. */
-int sfd_execute(sfd_plan *plan, const void *hologram_dev, void *field_dev, float *intensity_dev,
+SFD_API int sfd_execute(sfd_plan *plan, const void *hologram_dev, void *field_dev, float *intensity_dev,
                 void *stream);
 
 /* Real-time variant (step (xi) L95, reading 15): intensity returned as 8-bit images, per view
  * I8 = round_half_even(255 * I / max(I)) (an all-zero view gives zeros).
  *   intensity_u8_dev  [n_views][N][N] unsigned char.  Asynchronous on `stream`. */
-int sfd_execute_u8(sfd_plan *plan, const void *hologram_dev, unsigned char *intensity_u8_dev,
+SFD_API int sfd_execute_u8(sfd_plan *plan, const void *hologram_dev, unsigned char *intensity_u8_dev,
                    void *stream);
 
 /* Real-time stream (steps (i)-(xi) repeated, L83-97): reconstruct n_frames holograms that sit in
@@ -85,40 +91,47 @@ int sfd_execute_u8(sfd_plan *plan, const void *hologram_dev, unsigned char *inte
  *   out_pinned        [n_frames][n_views][N][N] unsigned char (pinned host memory).
  *   seconds           if non-NULL, receives the device-measured time (CUDA events) from the start
  *                     of the first H2D copy to the end of the last D2H copy. */
-int sfd_stream_run(sfd_plan *plan, const void *holograms_pinned, int n_frames,
+SFD_API int sfd_stream_run(sfd_plan *plan, const void *holograms_pinned, int n_frames,
                    unsigned char *out_pinned, double *seconds);
 
 /* Replace the parameters of one view (0 <= view < n_views) and rebuild its tables and cached
  * spectrum (the paper's user steers z, p2, Ox, Oy live: L33, L73, L123).  Synchronises with the
  * device (cudaMemcpy) before returning; do not call while an execute on this plan is in flight. */
-int sfd_plan_update_view(sfd_plan *plan, int view, double p1, double p2, double z, double Ox,
+SFD_API int sfd_plan_update_view(sfd_plan *plan, int view, double p1, double p2, double z, double Ox,
                          double Oy);
 
 /* Destroy a plan and free everything it owns.  NULL is accepted. */
-int sfd_plan_destroy(sfd_plan *plan);
+SFD_API int sfd_plan_destroy(sfd_plan *plan);
 
 /* Plan queries (host): N, n_views, padded FFT length M = 2N, bytes of device memory owned. */
-int sfd_plan_get_n(const sfd_plan *plan);
-int sfd_plan_get_views(const sfd_plan *plan);
-int sfd_plan_get_m(const sfd_plan *plan);
-long long sfd_plan_device_bytes(const sfd_plan *plan);
+SFD_API int sfd_plan_get_n(const sfd_plan *plan);
+SFD_API int sfd_plan_get_views(const sfd_plan *plan);
+SFD_API int sfd_plan_get_m(const sfd_plan *plan);
+SFD_API long long sfd_plan_device_bytes(const sfd_plan *plan);
 
 /* Timing aid for benchmarks: CUDA-event time, in milliseconds, of each of the two hot kernels
  * (pass y, pass x) of the most recent execute call on this plan, recorded on the stream they
  * were launched on.  Synchronises on those events.  ms[0] = pass y, ms[1] = pass x,
  * ms[2] = quantise (0 when not run).  Requires sfd_plan_set_timing(plan, 1) beforehand. */
-int sfd_plan_set_timing(sfd_plan *plan, int enable);
-int sfd_plan_last_kernel_ms(sfd_plan *plan, float ms[3]);
+SFD_API int sfd_plan_set_timing(sfd_plan *plan, int enable);
+SFD_API int sfd_plan_last_kernel_ms(sfd_plan *plan, float ms[3]);
 
 /* Number of kernel launches issued by all sfd_execute* / sfd_stream_run calls of this process. */
-long long sfd_launch_count(void);
+SFD_API long long sfd_launch_count(void);
+
+/* Host-only diagnostic (no GPU needed): the float64 tables the plan builds for ONE axis of one view,
+ * before rounding to complex64: pre[N] (Eq. 3), post[N] (Eq. 2 without c0) and the cached kernel
+ * spectrum H[2N] = FFT_2N(h)/(2N) (Eq. 4), each as interleaved (re, im) doubles in caller-owned host
+ * arrays of 2N, 2N and 4N doubles.  `off` is the window shift along that axis.  N: power of two. */
+SFD_API int sfd_host_tables(int N, double lambda, double p1, double p2, double z, double off, double *pre,
+                    double *post, double *H);
 
 /* Static description of an error code / of the last CUDA error seen by this thread. */
-const char *sfd_error_string(int code);
-const char *sfd_last_cuda_error(void);
+SFD_API const char *sfd_error_string(int code);
+SFD_API const char *sfd_last_cuda_error(void);
 
 /* Library version, e.g. "sfd 0.1 sm_100a". */
-const char *sfd_version(void);
+SFD_API const char *sfd_version(void);
 
 #ifdef __cplusplus
 }

@@ -1,0 +1,277 @@
+"""ctypes binding of ``libsfd.so`` — argument marshalling only; every step of the hot path runs in
+the library's CUDA kernels.  Names mirror ``include/sfd.h``.
+
+PyTorch appears here only as the owner of device memory and streams: tensors are passed down as
+``data_ptr()`` and the stream as ``torch.cuda.current_stream().cuda_stream``.
+
+There is no CPU fallback: importing this module raises if ``libsfd.so`` is missing, and every call
+raises ``SfdError`` on a non-zero return code."""
+from __future__ import annotations
+
+import ctypes as C
+import pathlib
+import re
+
+import numpy as np
+
+_PKG = pathlib.Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libsfd.so"
+HEADER_PATH = _PKG.parent / "include" / "sfd.h"
+
+SFD_OK, SFD_EINVAL, SFD_ENOMEM, SFD_ECUDA, SFD_EUNSUPPORTED = 0, -1, -2, -3, -4
+SFD_U8, SFD_F32 = 0, 1
+
+if not LIB_PATH.exists():
+    raise ImportError(
+        f"{LIB_PATH} is not built — run `python -m paper_1001_4309_b200.build` (needs nvcc). "
+        "There is no CPU fallback for the Shifted-Fresnel hot path.")
+
+_lib = C.CDLL(str(LIB_PATH))
+
+_dp = C.POINTER(C.c_double)
+_vp = C.c_void_p
+_sig = {
+    "sfd_plan_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_double, _dp, _dp, _dp, _dp,
+                                  _dp, C.c_int]),
+    "sfd_execute": (C.c_int, [_vp, _vp, _vp, _vp, _vp]),
+    "sfd_execute_u8": (C.c_int, [_vp, _vp, _vp, _vp]),
+    "sfd_stream_run": (C.c_int, [_vp, _vp, C.c_int, _vp, _dp]),
+    "sfd_plan_update_view": (C.c_int, [_vp, C.c_int] + [C.c_double] * 5),
+    "sfd_plan_destroy": (C.c_int, [_vp]),
+    "sfd_plan_get_n": (C.c_int, [_vp]),
+    "sfd_plan_get_views": (C.c_int, [_vp]),
+    "sfd_plan_get_m": (C.c_int, [_vp]),
+    "sfd_plan_device_bytes": (C.c_longlong, [_vp]),
+    "sfd_plan_set_timing": (C.c_int, [_vp, C.c_int]),
+    "sfd_plan_last_kernel_ms": (C.c_int, [_vp, C.POINTER(C.c_float)]),
+    "sfd_launch_count": (C.c_longlong, []),
+    "sfd_host_tables": (C.c_int, [C.c_int] + [C.c_double] * 5 + [_dp, _dp, _dp]),
+    "sfd_error_string": (C.c_char_p, [C.c_int]),
+    "sfd_last_cuda_error": (C.c_char_p, []),
+    "sfd_version": (C.c_char_p, []),
+}
+for _name, (_res, _args) in _sig.items():
+    _f = getattr(_lib, _name)          # AttributeError here = the library lacks a declared symbol
+    _f.restype, _f.argtypes = _res, _args
+
+
+def declared_symbols():
+    """Names of all functions ``include/sfd.h`` declares (parsed from the header)."""
+    text = HEADER_PATH.read_text()
+    return sorted(set(re.findall(r"SFD_API[^;(]*?\b(sfd_\w+)\s*\(", text)))
+
+
+class SfdError(RuntimeError):
+    def __init__(self, code, where):
+        msg = _lib.sfd_error_string(code).decode()
+        if code == SFD_ECUDA:
+            msg += ": " + _lib.sfd_last_cuda_error().decode()
+        super().__init__(f"{where} failed with {code} ({msg})")
+        self.code = code
+
+
+def _chk(code, where):
+    if code != SFD_OK:
+        raise SfdError(code, where)
+
+
+def _darr(v, n=None):
+    a = np.ascontiguousarray(np.atleast_1d(np.asarray(v, dtype=np.float64)))
+    if n is not None and n >= 1 and a.shape != (n,):      # the C side reads n values
+        raise ValueError(f"expected {n} per-view values, got shape {a.shape}")
+    return a
+
+
+def _ptr(t):
+    """Device/host address of a torch tensor, a numpy array, an int, or None."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if isinstance(t, np.ndarray):
+        return t.ctypes.data
+    return t.data_ptr()
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+# ---- functions with the names of the C ABI -------------------------------------------------------
+def sfd_version():
+    return _lib.sfd_version().decode()
+
+
+def sfd_error_string(code):
+    return _lib.sfd_error_string(int(code)).decode()
+
+
+def sfd_last_cuda_error():
+    return _lib.sfd_last_cuda_error().decode()
+
+
+def sfd_launch_count():
+    return int(_lib.sfd_launch_count())
+
+
+def sfd_plan_create(N, n_views, lam, p1, p2, z, Ox, Oy, in_dtype=SFD_U8):
+    """Returns the opaque plan handle (an int).  Per-view arrays are host sequences of floats."""
+    arrs = [_darr(a, n_views) for a in (p1, p2, z, Ox, Oy)]
+    h = _vp()
+    _chk(_lib.sfd_plan_create(C.byref(h), int(N), int(n_views), float(lam),
+                              *[a.ctypes.data_as(_dp) for a in arrs], int(in_dtype)),
+         "sfd_plan_create")
+    return h.value
+
+
+def sfd_execute(plan, hologram_dev, field_dev, intensity_dev, stream=None):
+    _chk(_lib.sfd_execute(plan, _ptr(hologram_dev), _ptr(field_dev), _ptr(intensity_dev),
+                          _stream(stream)), "sfd_execute")
+
+
+def sfd_execute_u8(plan, hologram_dev, intensity_u8_dev, stream=None):
+    _chk(_lib.sfd_execute_u8(plan, _ptr(hologram_dev), _ptr(intensity_u8_dev), _stream(stream)),
+         "sfd_execute_u8")
+
+
+def sfd_stream_run(plan, holograms_pinned, n_frames, out_pinned):
+    """Returns the device-measured seconds from first H2D to last D2H."""
+    sec = C.c_double(0.0)
+    _chk(_lib.sfd_stream_run(plan, _ptr(holograms_pinned), int(n_frames), _ptr(out_pinned),
+                             C.byref(sec)), "sfd_stream_run")
+    return sec.value
+
+
+def sfd_plan_update_view(plan, view, p1, p2, z, Ox, Oy):
+    _chk(_lib.sfd_plan_update_view(plan, int(view), float(p1), float(p2), float(z), float(Ox),
+                                   float(Oy)), "sfd_plan_update_view")
+
+
+def sfd_plan_destroy(plan):
+    _chk(_lib.sfd_plan_destroy(plan), "sfd_plan_destroy")
+
+
+def sfd_plan_get_n(plan):
+    return int(_lib.sfd_plan_get_n(plan))
+
+
+def sfd_plan_get_views(plan):
+    return int(_lib.sfd_plan_get_views(plan))
+
+
+def sfd_plan_get_m(plan):
+    return int(_lib.sfd_plan_get_m(plan))
+
+
+def sfd_plan_device_bytes(plan):
+    return int(_lib.sfd_plan_device_bytes(plan))
+
+
+def sfd_plan_set_timing(plan, enable):
+    _chk(_lib.sfd_plan_set_timing(plan, int(bool(enable))), "sfd_plan_set_timing")
+
+
+def sfd_plan_last_kernel_ms(plan):
+    ms = (C.c_float * 3)()
+    _chk(_lib.sfd_plan_last_kernel_ms(plan, ms), "sfd_plan_last_kernel_ms")
+    return [float(x) for x in ms]
+
+
+def sfd_host_tables(N, lam, p1, p2, z, off):
+    """Host-only: (pre[N], post[N], H[2N]) complex128, one axis of one view (see sfd.h)."""
+    pre = np.empty(N, np.complex128)
+    post = np.empty(N, np.complex128)
+    H = np.empty(2 * N, np.complex128)
+    _chk(_lib.sfd_host_tables(int(N), float(lam), float(p1), float(p2), float(z), float(off),
+                              pre.ctypes.data_as(_dp), post.ctypes.data_as(_dp),
+                              H.ctypes.data_as(_dp)), "sfd_host_tables")
+    return pre, post, H
+
+
+# ---- convenience wrapper: owns the handle, allocates outputs with torch --------------------------
+class Plan:
+    """``Plan(workload)`` or ``Plan(N=..., lam=..., p1=..., p2=..., z=..., Ox=..., Oy=...,
+    in_dtype=...)``; a context manager.  Allocation of outputs is the only thing it adds."""
+
+    def __init__(self, workload=None, **kw):
+        if workload is not None:
+            kw = dict(N=workload.N, lam=workload.lam, p1=workload.p1, p2=workload.p2,
+                      z=workload.z, Ox=workload.Ox, Oy=workload.Oy, in_dtype=workload.in_dtype)
+        self.N = int(kw["N"])
+        self.V = len(np.atleast_1d(kw["z"]))
+        self.in_dtype = int(kw.get("in_dtype", SFD_U8))
+        self.handle = sfd_plan_create(self.N, self.V, kw["lam"], kw["p1"], kw["p2"], kw["z"],
+                                      kw["Ox"], kw["Oy"], self.in_dtype)
+
+    def close(self):
+        if self.handle:
+            sfd_plan_destroy(self.handle)
+            self.handle = None
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def _check_holo(self, hologram):
+        import torch
+        want = torch.uint8 if self.in_dtype == SFD_U8 else torch.float32
+        if (hologram.dtype != want or tuple(hologram.shape) != (self.N, self.N)
+                or not hologram.is_cuda or not hologram.is_contiguous()):
+            raise ValueError(f"hologram must be a contiguous CUDA tensor [{self.N},{self.N}] {want}")
+
+    def execute(self, hologram, field=True, intensity=True, stream=None):
+        """Returns ``(field complex64 [V,N,N] | None, intensity float32 [V,N,N] | None)``.
+        ``field`` / ``intensity`` may be ``True`` (allocate), ``False`` (skip) or a tensor."""
+        import torch
+        self._check_holo(hologram)
+        shape = (self.V, self.N, self.N)
+        if field is True:
+            field = torch.empty(shape, dtype=torch.complex64, device=hologram.device)
+        elif field is False:
+            field = None
+        if intensity is True:
+            intensity = torch.empty(shape, dtype=torch.float32, device=hologram.device)
+        elif intensity is False:
+            intensity = None
+        sfd_execute(self.handle, hologram, field, intensity, stream)
+        return field, intensity
+
+    def execute_u8(self, hologram, out=None, stream=None):
+        import torch
+        self._check_holo(hologram)
+        if out is None:
+            out = torch.empty((self.V, self.N, self.N), dtype=torch.uint8, device=hologram.device)
+        sfd_execute_u8(self.handle, hologram, out, stream)
+        return out
+
+    def stream_run(self, holograms_pinned, out_pinned=None):
+        """``holograms_pinned``: pinned CPU tensor [F,N,N]; returns ``(out [F,V,N,N] uint8 pinned,
+        seconds)``."""
+        import torch
+        F = int(holograms_pinned.shape[0])
+        if not holograms_pinned.is_pinned() or not holograms_pinned.is_contiguous():
+            raise ValueError("holograms must be a contiguous pinned CPU tensor")
+        if out_pinned is None:
+            out_pinned = torch.empty((F, self.V, self.N, self.N), dtype=torch.uint8).pin_memory()
+        sec = sfd_stream_run(self.handle, holograms_pinned, F, out_pinned)
+        return out_pinned, sec
+
+    def update_view(self, view, p1, p2, z, Ox, Oy):
+        sfd_plan_update_view(self.handle, view, p1, p2, z, Ox, Oy)
+
+    def set_timing(self, enable=True):
+        sfd_plan_set_timing(self.handle, enable)
+
+    def last_kernel_ms(self):
+        return sfd_plan_last_kernel_ms(self.handle)
+
+    @property
+    def device_bytes(self):
+        return sfd_plan_device_bytes(self.handle)

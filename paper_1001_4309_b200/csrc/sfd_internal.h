@@ -1,0 +1,44 @@
+// sfd_internal.h — what sfd_plan.cpp (host logic) and sfd_kernels.cu (device code) share.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <vector>
+
+struct sfd_stream_state;  // pinned double-buffer pipeline (sfd_plan.cpp)
+
+// Device-side description of a plan, passed by value to the launcher.
+struct sfd_dev {
+    int N = 0, M = 0, log2M = 0, V = 0, in_dtype = 0;
+    // complex64 tables, one device allocation; per view contiguous
+    float2 *pre_y = nullptr;   // [V][N]  Eq.(3) y-part (x 1/255 for uint8 input)
+    float2 *post_y = nullptr;  // [V][N]  Eq.(2) y-part x c0
+    float2 *pre_x = nullptr;   // [V][N]  Eq.(3) x-part
+    float2 *post_x = nullptr;  // [V][N]  Eq.(2) x-part
+    float2 *H = nullptr;       // [V][M]  FFT_M(h)/M, h of Eq.(4) wrapped (S_x = S_y: one per view)
+    float2 *tw = nullptr;      // [M]     exp(-2 pi i x / M)
+    // workspace
+    float2 *B = nullptr;           // [V][N][N] intermediate between pass y and pass x
+    float *inten_ws = nullptr;     // [V][N][N] intensity scratch of the 8-bit mode
+    unsigned int *vmax = nullptr;  // [V] per-view max intensity (float bits)
+};
+
+struct sfd_plan {
+    sfd_dev d;
+    int device = 0;
+    double lambda = 0;
+    std::vector<double> p1, p2, z, Ox, Oy;
+    void *table_alloc = nullptr;
+    long long device_bytes = 0;
+    bool timing = false;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool ev_valid = false, ev_quant = false;
+    sfd_stream_state *ss = nullptr;
+};
+
+// Enqueue the kernels of one reconstruction on `st` (sfd_kernels.cu).  `u8` non-NULL selects the
+// 8-bit mode (intensity into the plan's scratch, per-view max, quantise).  Returns a cudaError_t.
+cudaError_t sfd_launch(sfd_plan *p, const void *holo, float2 *field, float *inten,
+                       unsigned char *u8, cudaStream_t st);
+// One-time per-process kernel attribute set-up (dynamic shared memory opt-in).
+cudaError_t sfd_kernels_init();
+void sfd_count_launch(int n);

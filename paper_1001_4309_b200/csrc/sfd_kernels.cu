@@ -1,0 +1,154 @@
+// sfd_kernels.cu — the sm_100a kernels of libsfd and their launcher.
+//
+// A reconstruction (PAPER.md steps (ii)-(x), L86-94) is two kernels for all views at once:
+//   k_pass_y : grid (N/C, V); per CTA C hologram columns: u8/f32 -> float, x pre_y (Eq. 3), zero-pad,
+//              2N-point FFT, x H, inverse FFT, crop, x c0 post_y (Eq. 2) -> B[V][N][N]
+//   k_pass_x : grid (N/RPC, V); per CTA RPC rows of B: x pre_x, FFT, x H, inverse FFT, crop, x post_x
+//              -> field, |.|^2 -> intensity (Eq. 5), optional per-view max
+// plus, in the 8-bit mode (step (xi), reading 15), k_quantise.
+// The per-thread arithmetic lives in sfd_fft_core.cuh.
+#include <atomic>
+
+#include "sfd_fft_core.cuh"
+#include "sfd_internal.h"
+
+namespace {
+
+using namespace sfd;
+
+// columns per CTA in pass y / rows per CTA in pass x, by padded length
+template <int LOG2M> struct Tile {
+    static constexpr int T = Sched<LOG2M>::T;
+    static constexpr int C = LOG2M <= 7 ? 16 : LOG2M <= 9 ? 8 : LOG2M <= 11 ? 4 : 2;
+    static constexpr int RPC = T >= 128 ? 1 : 128 / T;
+    static constexpr int THREADS_Y = C * T;
+    static constexpr int THREADS_X = RPC * T;
+    static constexpr size_t SMEM_Y = sizeof(float2) * Sched<LOG2M>::PADDED * C;
+    static constexpr size_t SMEM_X = sizeof(float2) * Sched<LOG2M>::PADDED * RPC;
+};
+
+template <int LOG2M, typename TIn>
+__global__ void __launch_bounds__(Tile<LOG2M>::THREADS_Y)
+k_pass_y(const TIn *__restrict__ holo, const float2 *__restrict__ pre_y,
+         const float2 *__restrict__ H, const float2 *__restrict__ post_y,
+         const float2 *__restrict__ tw, float2 *__restrict__ B, unsigned int *vmax) {
+    extern __shared__ float2 smem[];
+    if (vmax != nullptr && blockIdx.x == 0 && threadIdx.x == 0) vmax[blockIdx.y] = 0u;
+    pass_y_body<LOG2M, Tile<LOG2M>::C, TIn>(threadIdx.x, blockIdx.x, blockIdx.y, smem, holo, pre_y,
+                                            H, post_y, tw, B, [] { __syncthreads(); });
+}
+
+template <int LOG2M>
+__global__ void __launch_bounds__(Tile<LOG2M>::THREADS_X)
+k_pass_x(const float2 *__restrict__ B, const float2 *__restrict__ pre_x,
+         const float2 *__restrict__ H, const float2 *__restrict__ post_x,
+         const float2 *__restrict__ tw, float2 *__restrict__ field, float *__restrict__ inten,
+         unsigned int *vmax) {
+    extern __shared__ float2 smem[];
+    float mx = pass_x_body<LOG2M, Tile<LOG2M>::RPC>(threadIdx.x, blockIdx.x, blockIdx.y, smem, B,
+                                                    pre_x, H, post_x, tw, field, inten,
+                                                    [] { __syncthreads(); });
+    if (vmax != nullptr) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        // intensities are >= 0, so their float bit patterns order like unsigned integers
+        if ((threadIdx.x & 31) == 0) atomicMax(vmax + blockIdx.y, __float_as_uint(mx));
+    }
+}
+
+// I8 = round_half_even(255 I / max I) per view (reading 15); 4 pixels per thread.
+__global__ void __launch_bounds__(256)
+k_quantise(const float4 *__restrict__ inten, const unsigned int *__restrict__ vmax,
+           uchar4 *__restrict__ out, int quads_per_view) {
+    const int v = blockIdx.y;
+    const float mx = __uint_as_float(vmax[v]);
+    const float sc = mx > 0.f ? 255.f / mx : 0.f;
+    const size_t base = (size_t)v * quads_per_view;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < quads_per_view;
+         i += gridDim.x * blockDim.x) {
+        const float4 I = __ldg(inten + base + i);
+        uchar4 o;
+        o.x = (unsigned char)min(__float2int_rn(I.x * sc), 255);
+        o.y = (unsigned char)min(__float2int_rn(I.y * sc), 255);
+        o.z = (unsigned char)min(__float2int_rn(I.z * sc), 255);
+        o.w = (unsigned char)min(__float2int_rn(I.w * sc), 255);
+        out[base + i] = o;
+    }
+}
+
+std::atomic<long long> g_launches{0};
+
+template <int LOG2M, typename TIn> cudaError_t set_attr() {
+    cudaError_t e = cudaFuncSetAttribute(k_pass_y<LOG2M, TIn>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)Tile<LOG2M>::SMEM_Y);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_pass_x<LOG2M>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)Tile<LOG2M>::SMEM_X);
+}
+
+template <int LOG2M>
+cudaError_t launch_t(sfd_plan *p, const void *holo, float2 *field, float *inten,
+                     unsigned char *u8, cudaStream_t st) {
+    using TL = Tile<LOG2M>;
+    const sfd_dev &d = p->d;
+    const int N = d.N, V = d.V;
+    unsigned int *vmax = u8 ? d.vmax : nullptr;
+    if (u8) {
+        field = nullptr;
+        inten = d.inten_ws;
+    }
+    const bool timing = p->timing;
+    if (timing) cudaEventRecord(p->ev[0], st);
+    dim3 gy(N / TL::C, V), gx(N / TL::RPC, V);
+    if (d.in_dtype == 0)
+        k_pass_y<LOG2M, unsigned char><<<gy, TL::THREADS_Y, TL::SMEM_Y, st>>>(
+            (const unsigned char *)holo, d.pre_y, d.H, d.post_y, d.tw, d.B, vmax);
+    else
+        k_pass_y<LOG2M, float><<<gy, TL::THREADS_Y, TL::SMEM_Y, st>>>(
+            (const float *)holo, d.pre_y, d.H, d.post_y, d.tw, d.B, vmax);
+    if (timing) cudaEventRecord(p->ev[1], st);
+    k_pass_x<LOG2M><<<gx, TL::THREADS_X, TL::SMEM_X, st>>>(d.B, d.pre_x, d.H, d.post_x, d.tw, field,
+                                                           inten, vmax);
+    if (timing) cudaEventRecord(p->ev[2], st);
+    int n = 2;
+    if (u8) {
+        const int quads = N * N / 4;
+        dim3 gq((quads + 256 * 4 - 1) / (256 * 4), V);
+        k_quantise<<<gq, 256, 0, st>>>((const float4 *)d.inten_ws, d.vmax, (uchar4 *)u8, quads);
+        if (timing) cudaEventRecord(p->ev[3], st);
+        ++n;
+    }
+    p->ev_valid = timing;
+    p->ev_quant = timing && u8 != nullptr;
+    g_launches.fetch_add(n, std::memory_order_relaxed);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+void sfd_count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+long long sfd_launch_count_impl() { return g_launches.load(std::memory_order_relaxed); }
+
+cudaError_t sfd_kernels_init() {
+    cudaError_t e;
+#define SFD_ATTR(L)                                                   \
+    if ((e = set_attr<L, unsigned char>()) != cudaSuccess) return e;  \
+    if ((e = set_attr<L, float>()) != cudaSuccess) return e;
+    SFD_ATTR(7) SFD_ATTR(8) SFD_ATTR(9) SFD_ATTR(10) SFD_ATTR(11) SFD_ATTR(12)
+#undef SFD_ATTR
+    return cudaSuccess;
+}
+
+cudaError_t sfd_launch(sfd_plan *p, const void *holo, float2 *field, float *inten,
+                       unsigned char *u8, cudaStream_t st) {
+    switch (p->d.log2M) {
+        case 7: return launch_t<7>(p, holo, field, inten, u8, st);
+        case 8: return launch_t<8>(p, holo, field, inten, u8, st);
+        case 9: return launch_t<9>(p, holo, field, inten, u8, st);
+        case 10: return launch_t<10>(p, holo, field, inten, u8, st);
+        case 11: return launch_t<11>(p, holo, field, inten, u8, st);
+        case 12: return launch_t<12>(p, holo, field, inten, u8, st);
+    }
+    return cudaErrorInvalidValue;
+}

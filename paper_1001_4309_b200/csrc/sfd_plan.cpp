@@ -1,0 +1,432 @@
+// sfd_plan.cpp — host side of libsfd: argument checking, the float64 table builder, plan life
+// cycle, execute entry points and the pinned double-buffered real-time stream.
+//
+// Tables (Eq.(2)-(4), L58-65, with the readings of DESIGN.md §3): every phase is formed in
+// cycles in extended precision, reduced modulo 1, summed and only then turned into a complex
+// number, so the float32 values that reach the GPU carry one rounding each.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cmath>
+#include <complex>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "sfd.h"
+#include "sfd_internal.h"
+
+long long sfd_launch_count_impl();
+
+namespace {
+
+typedef long double ld;
+typedef std::complex<double> cd;
+
+thread_local char g_cuda_err[256] = "no CUDA error";
+
+int cuda_fail(cudaError_t e, const char *where) {
+    std::snprintf(g_cuda_err, sizeof g_cuda_err, "%s: %s (%s)", where, cudaGetErrorName(e),
+                  cudaGetErrorString(e));
+    cudaGetLastError();  // clear the sticky-less error state
+    return SFD_ECUDA;
+}
+#define SFD_CUDA(call)                                          \
+    do {                                                        \
+        cudaError_t e_ = (call);                                \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);     \
+    } while (0)
+
+const ld TWO_PI = 6.283185307179586476925286766559005768L;
+
+inline ld frac1(ld c) { return c - rintl(c); }  // cycles -> (-1/2, 1/2]
+inline cd cis_cycles(ld c) {
+    c = frac1(c);
+    return cd((double)cosl(TWO_PI * c), (double)sinl(TWO_PI * c));
+}
+
+// In-place radix-2 FFT, double, forward sign; twiddles evaluated directly (no recurrence).
+void fft_host(std::vector<cd> &a) {
+    const size_t n = a.size();
+    for (size_t i = 1, j = 0; i < n; ++i) {
+        size_t bit = n >> 1;
+        for (; j & bit; bit >>= 1) j ^= bit;
+        j ^= bit;
+        if (i < j) std::swap(a[i], a[j]);
+    }
+    std::vector<cd> w(n / 2);
+    for (size_t k = 0; k < n / 2; ++k) w[k] = cis_cycles(-(ld)k / (ld)n);
+    for (size_t len = 2; len <= n; len <<= 1) {
+        const size_t step = n / len;
+        for (size_t i = 0; i < n; i += len)
+            for (size_t k = 0; k < len / 2; ++k) {
+                cd u = a[i + k], t = a[i + k + len / 2] * w[k * step];
+                a[i + k] = u + t;
+                a[i + k + len / 2] = u - t;
+            }
+    }
+}
+
+// One axis of one view.  `off` is the shift of the reconstruction window along this axis.
+//   pre[m]  = exp(i pi x0^2/(lambda z)) exp(-i 2 pi m p1 a1/(lambda z)) exp(-i pi S m^2)   Eq.(3)
+//   post[m] = exp(i pi x1^2/(lambda z)) exp(-i 2 pi a0 x1/(lambda z)) exp(-i pi S m^2)     Eq.(2)
+// with x0 = a0 + m p1, a0 = -N/2 p1, x1 = a1 + m p2, a1 = -N/2 p2 + off, S = p1 p2/(lambda z).
+void axis_tables(int N, double lambda, double p1, double p2, double z, double off, cd *pre,
+                 cd *post) {
+    const ld lz = (ld)lambda * (ld)z;
+    const ld S = (ld)p1 * (ld)p2 / lz;
+    const ld a0 = -(ld)N / 2 * (ld)p1;
+    const ld a1 = -(ld)N / 2 * (ld)p2 + (ld)off;
+    for (int m = 0; m < N; ++m) {
+        const ld x0 = a0 + (ld)m * p1, x1 = a1 + (ld)m * p2;
+        const ld chirp = frac1(-S * (ld)m * (ld)m / 2);
+        pre[m] = cis_cycles(frac1(x0 * x0 / (2 * lz)) + frac1(-(ld)m * p1 * a1 / lz) + chirp);
+        post[m] = cis_cycles(frac1(x1 * x1 / (2 * lz)) + frac1(-a0 * x1 / lz) + chirp);
+    }
+}
+
+// Spectrum of the wrapped 1-D chirp kernel of Eq.(4): h[j] = exp(i pi S d^2), d = j (j <= N),
+// d = j - M (j > N), M = 2N; returns FFT_M(h)/M (the 1/M of the inverse FFT folded in, reading 8).
+void kernel_spectrum(int N, double lambda, double p1, double p2, double z, cd *H) {
+    const int M = 2 * N;
+    const ld S = (ld)p1 * (ld)p2 / ((ld)lambda * (ld)z);
+    std::vector<cd> h(M);
+    for (int j = 0; j < M; ++j) {
+        const ld d = j <= N ? (ld)j : (ld)(j - M);
+        h[j] = cis_cycles(S * d * d / 2);
+    }
+    fft_host(h);
+    for (int k = 0; k < M; ++k) H[k] = h[k] / (double)M;
+}
+
+// c0 = p1^2 exp(i 2 pi z/lambda) / (i lambda z)   (constant of Eq.(2) times the area element)
+cd c0_factor(double lambda, double p1, double z) {
+    const cd e = cis_cycles((ld)z / (ld)lambda);
+    return (p1 * p1) * e / (cd(0, 1) * (lambda * z));
+}
+
+bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
+
+int check_view(double lambda, double p1, double p2, double z, double Ox, double Oy) {
+    if (!finite_pos(lambda) || !finite_pos(p1) || !finite_pos(p2)) return SFD_EINVAL;
+    if (!std::isfinite(z) || z == 0.0) return SFD_EINVAL;
+    if (!std::isfinite(Ox) || !std::isfinite(Oy)) return SFD_EINVAL;
+    return SFD_OK;
+}
+
+int log2_exact(int n) {
+    int l = 0;
+    while ((1 << l) < n) ++l;
+    return (1 << l) == n ? l : -1;
+}
+
+void to_f32(const cd *src, float2 *dst, size_t n, cd scale = cd(1, 0)) {
+    for (size_t i = 0; i < n; ++i) {
+        const cd v = src[i] * scale;
+        dst[i] = make_float2((float)v.real(), (float)v.imag());
+    }
+}
+
+// float32 tables of one view, host staging layout: pre_y[N] post_y[N] pre_x[N] post_x[N] H[M]
+void build_view_f32(const sfd_plan *p, int v, float2 *pre_y, float2 *post_y, float2 *pre_x,
+                    float2 *post_x, float2 *H) {
+    const int N = p->d.N, M = p->d.M;
+    std::vector<cd> a(N), b(N), h(M);
+    const double in_scale = p->d.in_dtype == SFD_U8 ? 1.0 / 255.0 : 1.0;
+    axis_tables(N, p->lambda, p->p1[v], p->p2[v], p->z[v], p->Oy[v], a.data(), b.data());
+    to_f32(a.data(), pre_y, N, cd(in_scale, 0));
+    to_f32(b.data(), post_y, N, c0_factor(p->lambda, p->p1[v], p->z[v]));
+    axis_tables(N, p->lambda, p->p1[v], p->p2[v], p->z[v], p->Ox[v], a.data(), b.data());
+    to_f32(a.data(), pre_x, N);
+    to_f32(b.data(), post_x, N);
+    kernel_spectrum(N, p->lambda, p->p1[v], p->p2[v], p->z[v], h.data());
+    to_f32(h.data(), H, M);
+}
+
+std::atomic<bool> g_init{false};
+
+}  // namespace
+
+// ---- real-time stream state --------------------------------------------------------------------
+struct sfd_stream_state {
+    cudaStream_t s_in = nullptr, s_comp = nullptr, s_out = nullptr;
+    void *d_holo[2] = {nullptr, nullptr};
+    unsigned char *d_out[2] = {nullptr, nullptr};
+    cudaEvent_t e_in[2] = {nullptr, nullptr}, e_comp[2] = {nullptr, nullptr},
+                e_out[2] = {nullptr, nullptr}, e_t0 = nullptr, e_t1 = nullptr;
+};
+
+namespace {
+
+void stream_state_free(sfd_stream_state *s) {
+    if (!s) return;
+    for (int b = 0; b < 2; ++b) {
+        if (s->d_holo[b]) cudaFree(s->d_holo[b]);
+        if (s->d_out[b]) cudaFree(s->d_out[b]);
+        if (s->e_in[b]) cudaEventDestroy(s->e_in[b]);
+        if (s->e_comp[b]) cudaEventDestroy(s->e_comp[b]);
+        if (s->e_out[b]) cudaEventDestroy(s->e_out[b]);
+    }
+    if (s->e_t0) cudaEventDestroy(s->e_t0);
+    if (s->e_t1) cudaEventDestroy(s->e_t1);
+    if (s->s_in) cudaStreamDestroy(s->s_in);
+    if (s->s_comp) cudaStreamDestroy(s->s_comp);
+    if (s->s_out) cudaStreamDestroy(s->s_out);
+    delete s;
+}
+
+int stream_state_make(sfd_plan *p) {
+    if (p->ss) return SFD_OK;
+    sfd_stream_state *s = new (std::nothrow) sfd_stream_state;
+    if (!s) return SFD_ENOMEM;
+    p->ss = s;  // freed by sfd_plan_destroy even when half built
+    const size_t nn = (size_t)p->d.N * p->d.N;
+    const size_t in_bytes = nn * (p->d.in_dtype == SFD_U8 ? 1 : 4);
+    SFD_CUDA(cudaStreamCreateWithFlags(&s->s_in, cudaStreamNonBlocking));
+    SFD_CUDA(cudaStreamCreateWithFlags(&s->s_comp, cudaStreamNonBlocking));
+    SFD_CUDA(cudaStreamCreateWithFlags(&s->s_out, cudaStreamNonBlocking));
+    for (int b = 0; b < 2; ++b) {
+        SFD_CUDA(cudaMalloc(&s->d_holo[b], in_bytes));
+        SFD_CUDA(cudaMalloc((void **)&s->d_out[b], nn * p->d.V));
+        SFD_CUDA(cudaEventCreateWithFlags(&s->e_in[b], cudaEventDisableTiming));
+        SFD_CUDA(cudaEventCreateWithFlags(&s->e_comp[b], cudaEventDisableTiming));
+        SFD_CUDA(cudaEventCreateWithFlags(&s->e_out[b], cudaEventDisableTiming));
+        p->device_bytes += (long long)(in_bytes + nn * p->d.V);
+    }
+    SFD_CUDA(cudaEventCreate(&s->e_t0));
+    SFD_CUDA(cudaEventCreate(&s->e_t1));
+    return SFD_OK;
+}
+
+int upload_view(sfd_plan *p, int v) {
+    const int N = p->d.N, M = p->d.M;
+    std::vector<float2> st((size_t)4 * N + M);
+    build_view_f32(p, v, st.data(), st.data() + N, st.data() + 2 * N, st.data() + 3 * N,
+                   st.data() + 4 * N);
+    const size_t nb = sizeof(float2) * N;
+    SFD_CUDA(cudaMemcpy(p->d.pre_y + (size_t)v * N, st.data(), nb, cudaMemcpyHostToDevice));
+    SFD_CUDA(cudaMemcpy(p->d.post_y + (size_t)v * N, st.data() + N, nb, cudaMemcpyHostToDevice));
+    SFD_CUDA(cudaMemcpy(p->d.pre_x + (size_t)v * N, st.data() + 2 * N, nb, cudaMemcpyHostToDevice));
+    SFD_CUDA(cudaMemcpy(p->d.post_x + (size_t)v * N, st.data() + 3 * N, nb, cudaMemcpyHostToDevice));
+    SFD_CUDA(cudaMemcpy(p->d.H + (size_t)v * M, st.data() + 4 * N, sizeof(float2) * M,
+                        cudaMemcpyHostToDevice));
+    return SFD_OK;
+}
+
+}  // namespace
+
+// ---- C ABI -------------------------------------------------------------------------------------
+extern "C" {
+
+int sfd_host_tables(int N, double lambda, double p1, double p2, double z, double off, double *pre,
+                    double *post, double *H) {
+    if (!pre || !post || !H || log2_exact(N) < 0 || N < 2) return SFD_EINVAL;
+    if (check_view(lambda, p1, p2, z, off, 0.0) != SFD_OK) return SFD_EINVAL;
+    std::vector<cd> a(N), b(N), h(2 * (size_t)N);
+    axis_tables(N, lambda, p1, p2, z, off, a.data(), b.data());
+    kernel_spectrum(N, lambda, p1, p2, z, h.data());
+    std::memcpy(pre, a.data(), sizeof(cd) * N);
+    std::memcpy(post, b.data(), sizeof(cd) * N);
+    std::memcpy(H, h.data(), sizeof(cd) * 2 * N);
+    return SFD_OK;
+}
+
+int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const double *p1,
+                    const double *p2, const double *z, const double *Ox, const double *Oy,
+                    int in_dtype) {
+    if (!out) return SFD_EINVAL;
+    *out = nullptr;
+    if (!p1 || !p2 || !z || !Ox || !Oy) return SFD_EINVAL;
+    const int l2 = log2_exact(N);
+    if (l2 < 6 || l2 > 11 || n_views < 1) return SFD_EINVAL;
+    if (in_dtype != SFD_U8 && in_dtype != SFD_F32) return SFD_EINVAL;
+    for (int v = 0; v < n_views; ++v)
+        if (check_view(lambda, p1[v], p2[v], z[v], Ox[v], Oy[v]) != SFD_OK) return SFD_EINVAL;
+
+    if (!g_init.load()) {
+        SFD_CUDA(sfd_kernels_init());
+        g_init.store(true);
+    }
+    sfd_plan *p = new (std::nothrow) sfd_plan;
+    if (!p) return SFD_ENOMEM;
+    p->d.N = N;
+    p->d.M = 2 * N;
+    p->d.log2M = l2 + 1;
+    p->d.V = n_views;
+    p->d.in_dtype = in_dtype;
+    p->lambda = lambda;
+    p->p1.assign(p1, p1 + n_views);
+    p->p2.assign(p2, p2 + n_views);
+    p->z.assign(z, z + n_views);
+    p->Ox.assign(Ox, Ox + n_views);
+    p->Oy.assign(Oy, Oy + n_views);
+
+    int rc = SFD_OK;
+    auto fail = [&](int code) {
+        sfd_plan_destroy(p);
+        return code;
+    };
+    if (cudaGetDevice(&p->device) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaGetDevice"));
+    const size_t V = n_views, M = 2 * (size_t)N, nn = (size_t)N * N;
+    const size_t n_tab = V * (4 * (size_t)N + M) + M;  // complex64 elements
+    cudaError_t e;
+    if ((e = cudaMalloc(&p->table_alloc, n_tab * sizeof(float2))) != cudaSuccess)
+        return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc tables"));
+    float2 *t = (float2 *)p->table_alloc;
+    p->d.pre_y = t;
+    p->d.post_y = t + V * N;
+    p->d.pre_x = t + 2 * V * N;
+    p->d.post_x = t + 3 * V * N;
+    p->d.H = t + 4 * V * N;
+    p->d.tw = p->d.H + V * M;
+    if ((e = cudaMalloc((void **)&p->d.B, V * nn * sizeof(float2))) != cudaSuccess)
+        return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc B"));
+    if ((e = cudaMalloc((void **)&p->d.inten_ws, V * nn * sizeof(float))) != cudaSuccess)
+        return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc I"));
+    if ((e = cudaMalloc((void **)&p->d.vmax, V * sizeof(unsigned int))) != cudaSuccess)
+        return fail(cuda_fail(e, "cudaMalloc vmax"));
+    p->device_bytes = (long long)(n_tab * sizeof(float2) + V * nn * 12 + V * 4);
+
+    {   // FFT twiddles exp(-2 pi i x / M)
+        std::vector<float2> tw(M);
+        for (size_t x = 0; x < M; ++x) {
+            const cd w = cis_cycles(-(ld)x / (ld)M);
+            tw[x] = make_float2((float)w.real(), (float)w.imag());
+        }
+        if ((e = cudaMemcpy(p->d.tw, tw.data(), M * sizeof(float2), cudaMemcpyHostToDevice)) !=
+            cudaSuccess)
+            return fail(cuda_fail(e, "cudaMemcpy tw"));
+    }
+    for (int v = 0; v < n_views; ++v)
+        if ((rc = upload_view(p, v)) != SFD_OK) return fail(rc);
+    for (int i = 0; i < 4; ++i)
+        if ((e = cudaEventCreate(&p->ev[i])) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
+    *out = p;
+    return SFD_OK;
+}
+
+int sfd_plan_update_view(sfd_plan *p, int view, double p1, double p2, double z, double Ox,
+                         double Oy) {
+    if (!p || view < 0 || view >= p->d.V) return SFD_EINVAL;
+    if (check_view(p->lambda, p1, p2, z, Ox, Oy) != SFD_OK) return SFD_EINVAL;
+    p->p1[view] = p1;
+    p->p2[view] = p2;
+    p->z[view] = z;
+    p->Ox[view] = Ox;
+    p->Oy[view] = Oy;
+    return upload_view(p, view);
+}
+
+int sfd_execute(sfd_plan *p, const void *hologram_dev, void *field_dev, float *intensity_dev,
+                void *stream) {
+    if (!p || !hologram_dev || (!field_dev && !intensity_dev)) return SFD_EINVAL;
+    SFD_CUDA(sfd_launch(p, hologram_dev, (float2 *)field_dev, intensity_dev, nullptr,
+                        (cudaStream_t)stream));
+    return SFD_OK;
+}
+
+int sfd_execute_u8(sfd_plan *p, const void *hologram_dev, unsigned char *intensity_u8_dev,
+                   void *stream) {
+    if (!p || !hologram_dev || !intensity_u8_dev) return SFD_EINVAL;
+    SFD_CUDA(sfd_launch(p, hologram_dev, nullptr, nullptr, intensity_u8_dev, (cudaStream_t)stream));
+    return SFD_OK;
+}
+
+int sfd_stream_run(sfd_plan *p, const void *holograms_pinned, int n_frames,
+                   unsigned char *out_pinned, double *seconds) {
+    if (!p || !holograms_pinned || !out_pinned || n_frames < 0) return SFD_EINVAL;
+    if (seconds) *seconds = 0.0;
+    if (n_frames == 0) return SFD_OK;
+    int rc = stream_state_make(p);
+    if (rc != SFD_OK) return rc;
+    sfd_stream_state *s = p->ss;
+    const size_t nn = (size_t)p->d.N * p->d.N;
+    const size_t in_bytes = nn * (p->d.in_dtype == SFD_U8 ? 1 : 4);
+    const size_t out_bytes = nn * p->d.V;
+    const bool timing = p->timing;
+    p->timing = false;  // the per-kernel events belong to sfd_execute*
+    SFD_CUDA(cudaEventRecord(s->e_t0, s->s_in));
+    for (int f = 0; f < n_frames; ++f) {
+        const int b = f & 1;
+        // (i) H2D of frame f into input buffer b, once the compute of frame f-2 has read it
+        if (f >= 2) SFD_CUDA(cudaStreamWaitEvent(s->s_in, s->e_comp[b], 0));
+        SFD_CUDA(cudaMemcpyAsync(s->d_holo[b], (const char *)holograms_pinned + (size_t)f * in_bytes,
+                                 in_bytes, cudaMemcpyHostToDevice, s->s_in));
+        SFD_CUDA(cudaEventRecord(s->e_in[b], s->s_in));
+        // (ii)-(x) + quantise, once the D2H of frame f-2 has drained output buffer b
+        SFD_CUDA(cudaStreamWaitEvent(s->s_comp, s->e_in[b], 0));
+        if (f >= 2) SFD_CUDA(cudaStreamWaitEvent(s->s_comp, s->e_out[b], 0));
+        SFD_CUDA(sfd_launch(p, s->d_holo[b], nullptr, nullptr, s->d_out[b], s->s_comp));
+        SFD_CUDA(cudaEventRecord(s->e_comp[b], s->s_comp));
+        // (xi) D2H of the 8-bit views
+        SFD_CUDA(cudaStreamWaitEvent(s->s_out, s->e_comp[b], 0));
+        SFD_CUDA(cudaMemcpyAsync(out_pinned + (size_t)f * out_bytes, s->d_out[b], out_bytes,
+                                 cudaMemcpyDeviceToHost, s->s_out));
+        SFD_CUDA(cudaEventRecord(s->e_out[b], s->s_out));
+    }
+    SFD_CUDA(cudaEventRecord(s->e_t1, s->s_out));
+    p->timing = timing;
+    SFD_CUDA(cudaEventSynchronize(s->e_t1));
+    SFD_CUDA(cudaStreamSynchronize(s->s_in));
+    SFD_CUDA(cudaStreamSynchronize(s->s_comp));
+    float ms = 0.f;
+    SFD_CUDA(cudaEventElapsedTime(&ms, s->e_t0, s->e_t1));
+    if (seconds) *seconds = (double)ms * 1e-3;
+    return SFD_OK;
+}
+
+int sfd_plan_destroy(sfd_plan *p) {
+    if (!p) return SFD_OK;
+    stream_state_free(p->ss);
+    if (p->table_alloc) cudaFree(p->table_alloc);
+    if (p->d.B) cudaFree(p->d.B);
+    if (p->d.inten_ws) cudaFree(p->d.inten_ws);
+    if (p->d.vmax) cudaFree(p->d.vmax);
+    for (int i = 0; i < 4; ++i)
+        if (p->ev[i]) cudaEventDestroy(p->ev[i]);
+    delete p;
+    return SFD_OK;
+}
+
+int sfd_plan_get_n(const sfd_plan *p) { return p ? p->d.N : SFD_EINVAL; }
+int sfd_plan_get_views(const sfd_plan *p) { return p ? p->d.V : SFD_EINVAL; }
+int sfd_plan_get_m(const sfd_plan *p) { return p ? p->d.M : SFD_EINVAL; }
+long long sfd_plan_device_bytes(const sfd_plan *p) { return p ? p->device_bytes : SFD_EINVAL; }
+
+int sfd_plan_set_timing(sfd_plan *p, int enable) {
+    if (!p) return SFD_EINVAL;
+    p->timing = enable != 0;
+    if (!p->timing) p->ev_valid = p->ev_quant = false;
+    return SFD_OK;
+}
+
+int sfd_plan_last_kernel_ms(sfd_plan *p, float ms[3]) {
+    if (!p || !ms) return SFD_EINVAL;
+    ms[0] = ms[1] = ms[2] = 0.f;
+    if (!p->ev_valid) return SFD_EINVAL;
+    SFD_CUDA(cudaEventSynchronize(p->ev[p->ev_quant ? 3 : 2]));
+    SFD_CUDA(cudaEventElapsedTime(&ms[0], p->ev[0], p->ev[1]));
+    SFD_CUDA(cudaEventElapsedTime(&ms[1], p->ev[1], p->ev[2]));
+    if (p->ev_quant) SFD_CUDA(cudaEventElapsedTime(&ms[2], p->ev[2], p->ev[3]));
+    return SFD_OK;
+}
+
+long long sfd_launch_count(void) { return sfd_launch_count_impl(); }
+
+const char *sfd_error_string(int code) {
+    switch (code) {
+        case SFD_OK: return "success";
+        case SFD_EINVAL: return "invalid argument";
+        case SFD_ENOMEM: return "out of memory";
+        case SFD_ECUDA: return "CUDA runtime error (see sfd_last_cuda_error)";
+        case SFD_EUNSUPPORTED: return "unsupported request";
+    }
+    return "unknown error code";
+}
+
+const char *sfd_last_cuda_error(void) { return g_cuda_err; }
+
+const char *sfd_version(void) { return "sfd 0.1 sm_100a"; }
+
+}  // extern "C"

@@ -1,0 +1,93 @@
+"""CPU-only checks of the C-ABI library: it loads, exports every symbol include/sfd.h declares,
+rejects bad arguments before touching CUDA, fails loudly without a GPU, and its float64 host table
+builder (Eq. 2-4) agrees with the oracle's independently written tables."""
+import ctypes
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import shifted_fresnel as O
+from paper_1001_4309_b200 import build as sfd_build
+from paper_1001_4309_b200 import workloads as W
+
+sfd_build.build()
+from paper_1001_4309_b200 import binding as B  # noqa: E402
+
+
+def test_library_exports_every_declared_symbol():
+    names = B.declared_symbols()
+    assert len(names) >= 17 and "sfd_plan_create" in names and "sfd_stream_run" in names
+    lib = ctypes.CDLL(str(B.LIB_PATH))
+    for n in names:
+        assert hasattr(lib, n), f"libsfd.so does not export {n}"
+    # and the binding has a function of the same name for each
+    for n in names:
+        assert callable(getattr(B, n)), f"binding lacks {n}"
+
+
+def test_version_and_error_strings():
+    assert "sm_100a" in B.sfd_version()
+    assert B.sfd_error_string(0) == "success"
+    assert "invalid" in B.sfd_error_string(B.SFD_EINVAL)
+    assert B.sfd_launch_count() == 0 or torch.cuda.is_available()
+
+
+@pytest.mark.parametrize("bad", [
+    dict(N=100), dict(N=32), dict(N=4096), dict(n_views=0), dict(lam=0.0), dict(lam=-1e-6),
+    dict(p1=[0.0]), dict(p2=[-1e-6]), dict(z=[0.0]), dict(z=[float("nan")]), dict(z=[float("inf")]),
+    dict(Ox=[float("nan")]), dict(in_dtype=7),
+])
+def test_plan_create_rejects_bad_arguments(bad):
+    kw = dict(N=64, n_views=1, lam=W.LAMBDA, p1=[W.PITCH], p2=[W.PITCH], z=[0.05], Ox=[0.0],
+              Oy=[0.0], in_dtype=B.SFD_F32)
+    kw.update(bad)
+    with pytest.raises(B.SfdError) as e:
+        B.sfd_plan_create(kw["N"], kw["n_views"], kw["lam"], kw["p1"], kw["p2"], kw["z"], kw["Ox"],
+                          kw["Oy"], kw["in_dtype"])
+    assert e.value.code == B.SFD_EINVAL
+
+
+def test_null_arguments_are_einval():
+    assert B._lib.sfd_execute(None, None, None, None, None) == B.SFD_EINVAL
+    assert B._lib.sfd_execute_u8(None, None, None, None) == B.SFD_EINVAL
+    assert B._lib.sfd_stream_run(None, None, 1, None, None) == B.SFD_EINVAL
+    assert B._lib.sfd_plan_destroy(None) == B.SFD_OK
+    assert B._lib.sfd_plan_create(None, 64, 1, 1e-6, None, None, None, None, None, 0) == B.SFD_EINVAL
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
+def test_no_gpu_fails_loudly_not_silently():
+    """The product has no CPU fallback: without a device a valid plan request is SFD_ECUDA."""
+    with pytest.raises(B.SfdError) as e:
+        B.sfd_plan_create(64, 1, W.LAMBDA, [W.PITCH], [W.PITCH], [0.05], [0.0], [0.0], B.SFD_F32)
+    assert e.value.code == B.SFD_ECUDA
+    assert "cuda" in str(e.value).lower()
+
+
+@pytest.mark.parametrize("N,p2,z,off", [
+    (64, 4.65e-6, 0.05, 0.0),
+    (256, 2.0e-6, 0.08, 0.4e-3),
+    (1024, 1.0e-6, 0.08, -0.6e-3),
+    (1024, 4.65e-6, -0.06, 0.0),
+    (2048, 4.65e-6, 0.02, 0.9e-3),       # aliased chirp, S*N = 3.5 (reading 16)
+])
+def test_host_tables_match_oracle_tables(N, p2, z, off):
+    """Host logic pin: the plan's float64 tables (own C++ code, long double phases, own FFT) against
+    the oracle's Eq.(2)-(4) factors (NumPy, scipy.fft)."""
+    lam, p1 = W.LAMBDA, W.PITCH
+    pre, post, H = B.sfd_host_tables(N, lam, p1, p2, z, off)
+    pre_o = O.pre_chirp(N, lam, z, p1, p2, 0.0, off)
+    post_o = O.post_chirp(N, lam, z, p1, p2, 0.0, off)
+    h = O.chirp_kernel(N, 2 * N, O.scale_factor(lam, z, p1, p2))
+    H_o = np.fft.fft(h) / (2 * N)
+    assert np.max(np.abs(pre - pre_o)) < 2e-11
+    assert np.max(np.abs(post - post_o)) < 2e-11
+    assert np.max(np.abs(H - H_o)) < 1e-12 * max(1.0, np.max(np.abs(H_o)) * 2 * N)
+
+
+def test_host_tables_reject_bad_arguments():
+    with pytest.raises(B.SfdError):
+        B.sfd_host_tables(100, W.LAMBDA, W.PITCH, W.PITCH, 0.05, 0.0)
+    with pytest.raises(B.SfdError):
+        B.sfd_host_tables(64, W.LAMBDA, W.PITCH, W.PITCH, 0.0, 0.0)

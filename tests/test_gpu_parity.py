@@ -1,0 +1,242 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle, element by element.
+
+Tolerances are the north_star's (BASELINE.json): per view, relative L2 error <= 2e-5 and
+max|du| <= 1e-4 max|u|; the same bounds are applied to the intensity."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import shifted_fresnel as O
+from paper_1001_4309_b200 import build as sfd_build
+from paper_1001_4309_b200 import workloads as W
+
+sfd_build.build()
+from paper_1001_4309_b200 import binding as B  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+REL_L2 = 2e-5
+REL_MAX = 1e-4
+
+
+def _dev():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (no CPU fallback exists)"
+    return torch.device("cuda:0")
+
+
+def _assert_close(got, want, what):
+    got = np.asarray(got)
+    want = np.asarray(want)
+    assert got.shape == want.shape
+    for v in range(want.shape[0]):
+        d = got[v].astype(want.dtype) - want[v]
+        l2 = np.linalg.norm(d) / np.linalg.norm(want[v])
+        mx = np.max(np.abs(d)) / np.max(np.abs(want[v]))
+        assert l2 <= REL_L2, f"{what} view {v}: rel-L2 {l2:.3e} > {REL_L2}"
+        assert mx <= REL_MAX, f"{what} view {v}: max err {mx:.3e} > {REL_MAX}"
+
+
+def _run(wl, holo=None, **kw):
+    holo = wl.hologram() if holo is None else holo
+    with B.Plan(wl) as plan:
+        f, I = plan.execute(torch.from_numpy(holo).to(_dev()), **kw)
+        torch.cuda.synchronize()
+        return holo, (None if f is None else f.cpu().numpy()), (None if I is None else I.cpu().numpy())
+
+
+def test_config0_tiny_against_the_definition():
+    """Config 0: 64x64 float32, 1 view; oracle form D (direct O(N^4) double sum) and form B."""
+    wl = W.config(0)
+    holo, f, I = _run(wl)
+    fD, ID = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, form="D")
+    fB, _ = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, form="B")
+    _assert_close(f, fD, "field vs form D")
+    _assert_close(f, fB, "field vs form B")
+    _assert_close(I, ID, "intensity vs form D")
+
+
+def test_small_multiview_all_forms():
+    """256^2 uint8, 3 views with mixed sign of z: several CTAs per pass, several views."""
+    wl = W.small_multiview()
+    holo, f, I = _run(wl)
+    fB, IB = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, form="B")
+    fM, _ = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, form="M")
+    _assert_close(f, fB, "field vs form B")
+    _assert_close(f, fM, "field vs form M")
+    _assert_close(I, IB, "intensity")
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_configs_1024_full(cfg):
+    """Configs 1 and 2 at full size, every output element, in the launch configuration bench.py
+    times (same plan parameters, uint8 hologram from the same generator)."""
+    wl = W.config(cfg)
+    holo, f, I = _run(wl)
+    fB, IB = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, form="B")
+    _assert_close(f, fB, f"config {cfg} field")
+    _assert_close(I, IB, f"config {cfg} intensity")
+
+
+def test_config4_scale_stress_full():
+    """Config 4: 2048^2, 16 views (4096-point FFTs), contains aliased views (reading 16)."""
+    wl = W.config(4)
+    holo, f, I = _run(wl)
+    fB, IB = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, form="B")
+    _assert_close(f, fB, "config 4 field")
+    _assert_close(I, IB, "config 4 intensity")
+
+
+@pytest.mark.parametrize("N", [64, 128, 256, 512, 1024, 2048])
+def test_every_size_float_input(N):
+    """Every supported N (each has its own radix schedule), float32 input, two views (z<0 too)."""
+    rng = np.random.default_rng(N)
+    holo = rng.random((N, N), dtype=np.float32)
+    wl = W.Workload(f"rand{N}", N, W.LAMBDA, np.full(2, W.PITCH), np.array([3.1e-6, 4.65e-6]),
+                    np.array([0.07, -0.04]), np.array([0.2e-3, 0.0]), np.array([-0.1e-3, 0.0]),
+                    W.IN_F32)
+    _, f, I = _run(wl, holo)
+    fB, IB = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, form="B")
+    _assert_close(f, fB, f"N={N} field")
+    _assert_close(I, IB, f"N={N} intensity")
+
+
+def test_delta_closed_form_on_gpu_output():
+    """Pin P4 applied to the GPU result itself: a single bright sample reconstructs to the pure
+    chirp c0 exp(i pi [(x1-x0*)^2 + (y1-y0*)^2]/(lambda z)) (Eq. 1 with one term)."""
+    N, lam, p1, p2, z, Ox, Oy = 256, W.LAMBDA, W.PITCH, 2.3e-6, 0.04, 0.15e-3, -0.25e-3
+    holo = np.zeros((N, N), np.float32)
+    n0, m0 = 37, 201
+    holo[n0, m0] = 1.0
+    wl = W.Workload("delta", N, lam, np.array([p1]), np.array([p2]), np.array([z]), np.array([Ox]),
+                    np.array([Oy]), W.IN_F32)
+    _, f, I = _run(wl, holo)
+    x0 = (m0 - N / 2) * p1
+    y0 = (n0 - N / 2) * p1
+    x1 = (np.arange(N) - N / 2) * p2 + Ox
+    y1 = (np.arange(N) - N / 2) * p2 + Oy
+    ph = ((x1[None, :] - x0) ** 2 + (y1[:, None] - y0) ** 2) / (2 * lam * z)
+    zl = z / lam
+    want = p1 * p1 * np.exp(2j * np.pi * (zl - np.rint(zl))) / (1j * lam * z) * np.exp(
+        2j * np.pi * (ph - np.rint(ph)))
+    _assert_close(f, want[None], "delta field")
+    assert np.allclose(I[0], (p1 * p1 / (lam * abs(z))) ** 2, rtol=2e-4)
+
+
+def test_outputs_optional_and_consistent():
+    wl = W.small_multiview(N=128, V=2, seed=11)
+    holo, f, I = _run(wl)
+    _, f2, none_i = _run(wl, holo, intensity=False)
+    _, none_f, I2 = _run(wl, holo, field=False)
+    assert none_i is None and none_f is None
+    assert np.array_equal(f, f2) and np.array_equal(I, I2)
+    with B.Plan(wl) as plan:
+        with pytest.raises(B.SfdError) as e:
+            plan.execute(torch.from_numpy(holo).to(_dev()), field=False, intensity=False)
+        assert e.value.code == B.SFD_EINVAL
+
+
+def test_plan_reuse_two_plans_and_side_stream():
+    """One plan executed many times gives the same bits; two live plans do not disturb each other;
+    execution on a non-default stream is ordered by that stream."""
+    dev = _dev()
+    wa, wb = W.small_multiview(N=256, V=2, seed=3), W.small_multiview(N=128, V=3, seed=5)
+    ha, hb = torch.from_numpy(wa.hologram()).to(dev), torch.from_numpy(wb.hologram()).to(dev)
+    with B.Plan(wa) as pa, B.Plan(wb) as pb:
+        fa0, _ = pa.execute(ha)
+        fb0, _ = pb.execute(hb)
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            for _ in range(5):
+                fa, _ = pa.execute(ha)
+                fb, _ = pb.execute(hb)
+        s.synchronize()
+        assert torch.equal(fa, fa0) and torch.equal(fb, fb0)
+    fB, _ = O.reconstruct_views(wa.hologram(), wa.lam, wa.p1, wa.p2, wa.z, wa.Ox, wa.Oy)
+    _assert_close(fa.cpu().numpy(), fB, "reused plan")
+
+
+def test_update_view_rebuilds_tables():
+    wl = W.small_multiview(N=128, V=2, seed=9)
+    holo = wl.hologram()
+    dev = _dev()
+    with B.Plan(wl) as plan:
+        plan.update_view(1, W.PITCH, 1.7e-6, -0.033, 0.05e-3, 0.02e-3)
+        f, _ = plan.execute(torch.from_numpy(holo).to(dev))
+        f = f.cpu().numpy()
+    p2 = wl.p2.copy(); z = wl.z.copy(); Ox = wl.Ox.copy(); Oy = wl.Oy.copy()
+    p2[1], z[1], Ox[1], Oy[1] = 1.7e-6, -0.033, 0.05e-3, 0.02e-3
+    fB, _ = O.reconstruct_views(holo, wl.lam, wl.p1, p2, z, Ox, Oy)
+    _assert_close(f, fB, "updated view")
+
+
+def _u8_check(got, I_oracle, what):
+    """8-bit output (reading 15): equal to the oracle's quantisation except where 255 I/max sits
+    within float32 rounding of a .5 boundary; there +-1 LSB is allowed."""
+    for v in range(I_oracle.shape[0]):
+        want = O.quantise_u8(I_oracle[v]).astype(np.int16)
+        d = np.abs(got[v].astype(np.int16) - want)
+        assert d.max() <= 1, f"{what} view {v}: off by {d.max()} LSB"
+        x = 255.0 * I_oracle[v] / I_oracle[v].max()
+        near = np.abs(x - np.floor(x) - 0.5) < 1e-3 * np.maximum(x, 1.0)
+        assert not np.any((d == 1) & ~near), f"{what} view {v}: 1-LSB error away from a boundary"
+        assert (d == 1).mean() < 5e-3
+
+
+def test_execute_u8_against_oracle_quantisation():
+    wl = W.small_multiview(N=256, V=3, seed=21)
+    holo = wl.hologram()
+    with B.Plan(wl) as plan:
+        out = plan.execute_u8(torch.from_numpy(holo).to(_dev())).cpu().numpy()
+    _, IB = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy)
+    _u8_check(out, IB, "execute_u8")
+    # an all-zero hologram gives all-zero images (degenerate max)
+    with B.Plan(wl) as plan:
+        z = plan.execute_u8(torch.zeros((wl.N, wl.N), dtype=torch.uint8, device=_dev()))
+        assert int(z.max()) == 0
+
+
+def test_stream_run_matches_execute_u8_and_oracle():
+    """Config 3 shape (1024^2, 4 views) on 6 frames: the double-buffered pinned pipeline returns,
+    frame by frame, the same bytes as sfd_execute_u8, and those match the oracle."""
+    wl = W.config(3, n_frames=6)
+    frames = np.stack([wl.hologram(f) for f in range(wl.n_frames)])
+    pinned = torch.from_numpy(frames).pin_memory()
+    dev = _dev()
+    with B.Plan(wl) as plan:
+        out, sec = plan.stream_run(pinned)
+        assert sec > 0
+        for f in range(wl.n_frames):
+            ref = plan.execute_u8(pinned[f].to(dev))
+            assert torch.equal(ref.cpu(), out[f]), f"frame {f}: stream differs from execute_u8"
+        out2, _ = plan.stream_run(pinned)      # the pipeline is reusable
+        assert torch.equal(out, out2)
+    for f in (0, wl.n_frames - 1):
+        _, IB = O.reconstruct_views(frames[f], wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy)
+        _u8_check(out[f].numpy(), IB, f"stream frame {f}")
+
+
+def test_stream_run_edge_cases():
+    wl = W.small_multiview(N=128, V=1, seed=2)
+    with B.Plan(wl) as plan:
+        one = torch.from_numpy(wl.hologram()[None]).pin_memory()
+        out, sec = plan.stream_run(one)                      # a single frame (no overlap partner)
+        ref = plan.execute_u8(one[0].to(_dev())).cpu()
+        assert torch.equal(out[0], ref)
+        assert B.sfd_stream_run(plan.handle, one, 0, out) == 0.0   # zero frames: no work, OK
+
+
+def test_launch_counter_and_kernel_timing():
+    wl = W.small_multiview(N=128, V=2, seed=4)
+    h = torch.from_numpy(wl.hologram()).to(_dev())
+    with B.Plan(wl) as plan:
+        n0 = B.sfd_launch_count()
+        plan.execute(h)
+        assert B.sfd_launch_count() - n0 == 2          # pass y, pass x
+        plan.execute_u8(h)
+        assert B.sfd_launch_count() - n0 == 5          # + pass y, pass x, quantise
+        plan.set_timing(True)
+        plan.execute(h)
+        ms = plan.last_kernel_ms()
+        assert ms[0] > 0 and ms[1] > 0 and ms[2] == 0
+        assert plan.device_bytes > 0 and B.sfd_plan_get_m(plan.handle) == 256
