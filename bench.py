@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--e2e-frames", type=int, default=128)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--kernels", default="auto", choices=["auto", "generic"],
+                    help="generic = force the generic Stockham kernels at N=1024 (A/B timing)")
     ap.add_argument("--intensity-only", action="store_true",
                     help="skip the complex field output (row f1); not the headline configuration")
     return ap.parse_args()
@@ -245,6 +247,8 @@ def run_sfd(args, info):
     intens = [torch.empty((V, N, N), dtype=torch.float32, device=dev) for _ in range(R)]
 
     plan = B.Plan(wl)
+    if args.kernels == "generic":
+        plan.select_kernels(B.SFD_KERNELS_GENERIC)
     stream = torch.cuda.current_stream()
     sampler = ClockSampler(torch.cuda._get_nvml_device_index(dev) if hasattr(
         torch.cuda, "_get_nvml_device_index") else info.local_rank)

@@ -109,6 +109,14 @@ SFD_API int sfd_plan_get_views(const sfd_plan *plan);
 SFD_API int sfd_plan_get_m(const sfd_plan *plan);
 SFD_API long long sfd_plan_device_bytes(const sfd_plan *plan);
 
+/* Kernel selection.  SFD_KERNELS_AUTO (default): N = 1024 runs the one-warp-per-line kernels
+ * (DESIGN.md 5.4), every other size the generic shared-memory Stockham kernels.
+ * SFD_KERNELS_GENERIC forces the generic kernels at every size (tests, A/B timing).  Both compute
+ * the same transform; results differ by fp32 rounding only.  Errors: SFD_EINVAL. */
+#define SFD_KERNELS_AUTO 0
+#define SFD_KERNELS_GENERIC 1
+SFD_API int sfd_plan_select_kernels(sfd_plan *plan, int which);
+
 /* Timing aid for benchmarks: CUDA-event time, in milliseconds, of each of the two hot kernels
  * (pass y, pass x) of the most recent execute call on this plan, recorded on the stream they
  * were launched on.  Synchronises on those events.  ms[0] = pass y, ms[1] = pass x,

@@ -20,6 +20,7 @@ HEADER_PATH = _PKG.parent / "include" / "sfd.h"
 
 SFD_OK, SFD_EINVAL, SFD_ENOMEM, SFD_ECUDA, SFD_EUNSUPPORTED = 0, -1, -2, -3, -4
 SFD_U8, SFD_F32 = 0, 1
+SFD_KERNELS_AUTO, SFD_KERNELS_GENERIC = 0, 1
 
 if not LIB_PATH.exists():
     raise ImportError(
@@ -42,6 +43,7 @@ _sig = {
     "sfd_plan_get_views": (C.c_int, [_vp]),
     "sfd_plan_get_m": (C.c_int, [_vp]),
     "sfd_plan_device_bytes": (C.c_longlong, [_vp]),
+    "sfd_plan_select_kernels": (C.c_int, [_vp, C.c_int]),
     "sfd_plan_set_timing": (C.c_int, [_vp, C.c_int]),
     "sfd_plan_last_kernel_ms": (C.c_int, [_vp, C.POINTER(C.c_float)]),
     "sfd_launch_count": (C.c_longlong, []),
@@ -170,6 +172,10 @@ def sfd_plan_device_bytes(plan):
     return int(_lib.sfd_plan_device_bytes(plan))
 
 
+def sfd_plan_select_kernels(plan, which):
+    _chk(_lib.sfd_plan_select_kernels(plan, int(which)), "sfd_plan_select_kernels")
+
+
 def sfd_plan_set_timing(plan, enable):
     _chk(_lib.sfd_plan_set_timing(plan, int(bool(enable))), "sfd_plan_set_timing")
 
@@ -265,6 +271,9 @@ class Plan:
 
     def update_view(self, view, p1, p2, z, Ox, Oy):
         sfd_plan_update_view(self.handle, view, p1, p2, z, Ox, Oy)
+
+    def select_kernels(self, which):
+        sfd_plan_select_kernels(self.handle, which)
 
     def set_timing(self, enable=True):
         sfd_plan_set_timing(self.handle, enable)

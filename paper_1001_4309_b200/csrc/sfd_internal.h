@@ -2,6 +2,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "sfd.h"
+
 #include <vector>
 
 struct sfd_stream_state;  // pinned double-buffer pipeline (sfd_plan.cpp)
@@ -20,7 +22,13 @@ struct sfd_dev {
     float2 *B = nullptr;           // [V][N][N] intermediate between pass y and pass x
     float *inten_ws = nullptr;     // [V][N][N] intensity scratch of the 8-bit mode
     unsigned int *vmax = nullptr;  // [V] per-view max intensity (float bits)
+    // N = 1024 fast path (sfd_warp1024.cuh); branch b = 0 even bins, 1 odd bins of the 2N-point DFT
+    float2 *w_tabY = nullptr;  // [V][4][N]  pre_y b0 | pre_y b1 | c0 post_y b0 | c0 post_y b1
+    float2 *w_tabX = nullptr;  // [V][4][N]  pre_x b0 | pre_x b1 | post_x b0 | post_x b1
+    float2 *w_H2 = nullptr;    // [V][2][N]  H[2k] | H[2k+1]
+    float2 *w_twl = nullptr;   // [32][32]   exp(-2 pi i lane k / 1024) at [k][lane]
 };
+
 
 struct sfd_plan {
     sfd_dev d;
@@ -28,6 +36,8 @@ struct sfd_plan {
     double lambda = 0;
     std::vector<double> p1, p2, z, Ox, Oy;
     void *table_alloc = nullptr;
+    void *fast_alloc = nullptr;
+    int kernels = SFD_KERNELS_AUTO;
     long long device_bytes = 0;
     bool timing = false;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};

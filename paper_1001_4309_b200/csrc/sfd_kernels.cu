@@ -11,6 +11,7 @@
 
 #include "sfd_fft_core.cuh"
 #include "sfd_internal.h"
+#include "sfd_warp1024.cuh"
 
 namespace {
 
@@ -76,7 +77,94 @@ k_quantise(const float4 *__restrict__ inten, const unsigned int *__restrict__ vm
     }
 }
 
+// ---- N = 1024 fast path (sfd_warp1024.cuh): persistent kernels, one warp per line --------------------
+// k_cols_1024: work item = (view, group of 4 adjacent hologram columns); one CTA (4 warps) per item.
+template <typename TIn>
+__global__ void __launch_bounds__(128, 3)
+k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
+            const float2 *__restrict__ H2, const float2 *__restrict__ twl, float2 *__restrict__ B,
+            unsigned int *vmax, int V) {
+    extern __shared__ float4 smem4[];
+    sfdw::SmemY &sm = *reinterpret_cast<sfdw::SmemY *>(smem4);
+    if (vmax != nullptr && blockIdx.x == 0 && threadIdx.x < V) vmax[threadIdx.x] = 0u;
+    float2 tw[32];
+    sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
+    const int groups = sfdw::N / sfdw::YC, items = V * groups;
+    for (int item = blockIdx.x; item < items; item += gridDim.x) {
+        const int view = item / groups, col0 = (item % groups) * sfdw::YC;
+        sfdw::pass_y_cta<TIn>(sm, holo, tabY + (size_t)view * 4 * sfdw::N,
+                              H2 + (size_t)view * 2 * sfdw::N, tw,
+                              B + (size_t)view * sfdw::N * sfdw::N, col0);
+    }
+}
+
+// k_rows_1024: work item = one row of B (view-major); one warp per item.
+__global__ void __launch_bounds__(128, 3)
+k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
+            const float2 *__restrict__ H2, const float2 *__restrict__ twl,
+            float2 *__restrict__ field, float *__restrict__ inten, unsigned int *vmax, int V) {
+    extern __shared__ float4 smem4[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    sfdw::SmemXWarp &sm = reinterpret_cast<sfdw::SmemXWarp *>(smem4)[warp];
+    float2 tw[32];
+    sfdw::load_twiddles(tw, lane, twl);
+    const int lines = V * sfdw::N;
+    for (int line = blockIdx.x * 4 + warp; line < lines; line += gridDim.x * 4) {
+        const int view = line / sfdw::N;
+        const size_t off = (size_t)line * sfdw::N;
+        float mx = sfdw::pass_x_warp(sm, B + off, tabX + (size_t)view * 4 * sfdw::N,
+                                     H2 + (size_t)view * 2 * sfdw::N, tw,
+                                     field ? field + off : nullptr, inten ? inten + off : nullptr);
+        if (vmax != nullptr) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+            if (lane == 0) atomicMax(vmax + view, __float_as_uint(mx));
+        }
+    }
+}
+
 std::atomic<long long> g_launches{0};
+int g_sms = 0;
+
+cudaError_t launch_warp1024(sfd_plan *p, const void *holo, float2 *field, float *inten,
+                            unsigned char *u8, cudaStream_t st) {
+    const sfd_dev &d = p->d;
+    const int V = d.V;
+    unsigned int *vmax = u8 ? d.vmax : nullptr;
+    if (u8) {
+        field = nullptr;
+        inten = d.inten_ws;
+    }
+    const bool timing = p->timing;
+    if (timing) cudaEventRecord(p->ev[0], st);
+    const int slots = g_sms * 3;
+    const int items_y = V * (sfdw::N / sfdw::YC);
+    const int gy = items_y < slots ? items_y : slots;
+    if (d.in_dtype == 0)
+        k_cols_1024<unsigned char><<<gy, 128, sizeof(sfdw::SmemY), st>>>(
+            (const unsigned char *)holo, d.w_tabY, d.w_H2, d.w_twl, d.B, vmax, V);
+    else
+        k_cols_1024<float><<<gy, 128, sizeof(sfdw::SmemY), st>>>(
+            (const float *)holo, d.w_tabY, d.w_H2, d.w_twl, d.B, vmax, V);
+    if (timing) cudaEventRecord(p->ev[1], st);
+    const int ctas_x = (V * sfdw::N + 3) / 4;
+    const int gx = ctas_x < slots ? ctas_x : slots;
+    k_rows_1024<<<gx, 128, 4 * sizeof(sfdw::SmemXWarp), st>>>(d.B, d.w_tabX, d.w_H2, d.w_twl, field,
+                                                             inten, vmax, V);
+    if (timing) cudaEventRecord(p->ev[2], st);
+    int n = 2;
+    if (u8) {
+        const int quads = sfdw::N * sfdw::N / 4;
+        dim3 gq((quads + 256 * 4 - 1) / (256 * 4), V);
+        k_quantise<<<gq, 256, 0, st>>>((const float4 *)d.inten_ws, d.vmax, (uchar4 *)u8, quads);
+        if (timing) cudaEventRecord(p->ev[3], st);
+        ++n;
+    }
+    p->ev_valid = timing;
+    p->ev_quant = timing && u8 != nullptr;
+    g_launches.fetch_add(n, std::memory_order_relaxed);
+    return cudaGetLastError();
+}
 
 template <int LOG2M, typename TIn> cudaError_t set_attr() {
     cudaError_t e = cudaFuncSetAttribute(k_pass_y<LOG2M, TIn>,
@@ -137,11 +225,24 @@ cudaError_t sfd_kernels_init() {
     if ((e = set_attr<L, float>()) != cudaSuccess) return e;
     SFD_ATTR(7) SFD_ATTR(8) SFD_ATTR(9) SFD_ATTR(10) SFD_ATTR(11) SFD_ATTR(12)
 #undef SFD_ATTR
+    if ((e = cudaFuncSetAttribute(k_cols_1024<unsigned char>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)sizeof(sfdw::SmemY))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_cols_1024<float>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)sizeof(sfdw::SmemY))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_rows_1024, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)(4 * sizeof(sfdw::SmemXWarp)))) != cudaSuccess) return e;
+    int dev = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
     return cudaSuccess;
 }
 
 cudaError_t sfd_launch(sfd_plan *p, const void *holo, float2 *field, float *inten,
                        unsigned char *u8, cudaStream_t st) {
+    // N = 1024: one-warp-per-line kernels (need the 4-byte aligned hologram rows of the uint8 tile load)
+    if (p->d.N == sfdw::N && p->kernels != SFD_KERNELS_GENERIC && p->d.w_twl != nullptr &&
+        (reinterpret_cast<size_t>(holo) & 3) == 0)
+        return launch_warp1024(p, holo, field, inten, u8, st);
     switch (p->d.log2M) {
         case 7: return launch_t<7>(p, holo, field, inten, u8, st);
         case 8: return launch_t<8>(p, holo, field, inten, u8, st);

@@ -36,9 +36,11 @@ def _assert_close(got, want, what):
         assert mx <= REL_MAX, f"{what} view {v}: max err {mx:.3e} > {REL_MAX}"
 
 
-def _run(wl, holo=None, **kw):
+def _run(wl, holo=None, kernels=None, **kw):
     holo = wl.hologram() if holo is None else holo
     with B.Plan(wl) as plan:
+        if kernels is not None:
+            plan.select_kernels(kernels)
         f, I = plan.execute(torch.from_numpy(holo).to(_dev()), **kw)
         torch.cuda.synchronize()
         return holo, (None if f is None else f.cpu().numpy()), (None if I is None else I.cpu().numpy())
@@ -75,6 +77,28 @@ def test_configs_1024_full(cfg):
     fB, IB = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, form="B")
     _assert_close(f, fB, f"config {cfg} field")
     _assert_close(I, IB, f"config {cfg} intensity")
+
+
+@pytest.mark.parametrize("in_dtype", [W.IN_U8, W.IN_F32])
+def test_1024_generic_and_warp_kernels_agree_with_oracle(in_dtype):
+    """N = 1024 has two kernel sets (one warp per line; generic Stockham, 5.3).
+    Both must meet the tolerance against the oracle, for both input types, with a delta in the
+    last row/column so that an indexing slip at the tile edges shows."""
+    wl = W.config(2)
+    if in_dtype == W.IN_F32:
+        holo = np.random.default_rng(5).random((1024, 1024), dtype=np.float32)
+        holo[1023, 1023] = 40.0
+        holo[0, 1021] = 25.0
+        wl = W.Workload("rand1024", 1024, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, W.IN_F32)
+    else:
+        holo = wl.hologram().copy()
+        holo[1023, 1023] = 255
+        holo[0, 1021] = 0
+    fB, IB = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, form="B")
+    for which in (B.SFD_KERNELS_AUTO, B.SFD_KERNELS_GENERIC):
+        _, f, I = _run(wl, holo, kernels=which)
+        _assert_close(f, fB, f"kernels={which} field")
+        _assert_close(I, IB, f"kernels={which} intensity")
 
 
 def test_config4_scale_stress_full():
