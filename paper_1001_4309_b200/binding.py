@@ -9,13 +9,15 @@ raises ``SfdError`` on a non-zero return code."""
 from __future__ import annotations
 
 import ctypes as C
+import os
 import pathlib
 import re
 
 import numpy as np
 
 _PKG = pathlib.Path(__file__).resolve().parent
-LIB_PATH = _PKG / "libsfd.so"
+# SFD_LIBRARY=<path> loads another build of the same library (e.g. an experimental variant)
+LIB_PATH = pathlib.Path(os.environ.get("SFD_LIBRARY", _PKG / "libsfd.so"))
 HEADER_PATH = _PKG.parent / "include" / "sfd.h"
 
 SFD_OK, SFD_EINVAL, SFD_ENOMEM, SFD_ECUDA, SFD_EUNSUPPORTED = 0, -1, -2, -3, -4

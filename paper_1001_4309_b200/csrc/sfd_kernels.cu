@@ -77,50 +77,42 @@ k_quantise(const float4 *__restrict__ inten, const unsigned int *__restrict__ vm
     }
 }
 
-// ---- N = 1024 fast path (sfd_warp1024.cuh): persistent kernels, one warp per line --------------------
-// k_cols_1024: work item = (view, group of 4 adjacent hologram columns); one CTA (4 warps) per item.
+// ---- N = 1024 fast path (sfd_warp1024.cuh): persistent kernels, one warp pair per line --------------
+// One CTA of 8 warps per SM; the register budget (255) holds 32 values, 31 twiddles and a 32-value
+// prefetch vector per thread.
 template <typename TIn>
-__global__ void __launch_bounds__(128, 3)
+__global__ void __launch_bounds__(256, 1)
 k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
             const float2 *__restrict__ H2, const float2 *__restrict__ twl, float2 *__restrict__ B,
             unsigned int *vmax, int V) {
     extern __shared__ float4 smem4[];
-    sfdw::SmemY &sm = *reinterpret_cast<sfdw::SmemY *>(smem4);
+    sfdw::SmemY<TIn> &sm = *reinterpret_cast<sfdw::SmemY<TIn> *>(smem4);
     if (vmax != nullptr && blockIdx.x == 0 && threadIdx.x < V) vmax[threadIdx.x] = 0u;
     float2 tw[32];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
-    const int groups = sfdw::N / sfdw::YC, items = V * groups;
-    for (int item = blockIdx.x; item < items; item += gridDim.x) {
-        const int view = item / groups, col0 = (item % groups) * sfdw::YC;
-        sfdw::pass_y_cta<TIn>(sm, holo, tabY + (size_t)view * 4 * sfdw::N,
-                              H2 + (size_t)view * 2 * sfdw::N, tw,
-                              B + (size_t)view * sfdw::N * sfdw::N, col0);
-    }
+    if (((threadIdx.x >> 5) & 1) == 0)
+        sfdw::pass_y_loop<TIn, 0>(sm, holo, tabY, H2, tw, B, V);
+    else
+        sfdw::pass_y_loop<TIn, 1>(sm, holo, tabY, H2, tw, B, V);
 }
 
-// k_rows_1024: work item = one row of B (view-major); one warp per item.
-__global__ void __launch_bounds__(128, 3)
+__global__ void __launch_bounds__(256, 1)
 k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
             const float2 *__restrict__ H2, const float2 *__restrict__ twl,
             float2 *__restrict__ field, float *__restrict__ inten, unsigned int *vmax, int V) {
     extern __shared__ float4 smem4[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    sfdw::SmemXWarp &sm = reinterpret_cast<sfdw::SmemXWarp *>(smem4)[warp];
-    float2 tw[32];
-    sfdw::load_twiddles(tw, lane, twl);
-    const int lines = V * sfdw::N;
-    for (int line = blockIdx.x * 4 + warp; line < lines; line += gridDim.x * 4) {
-        const int view = line / sfdw::N;
-        const size_t off = (size_t)line * sfdw::N;
-        float mx = sfdw::pass_x_warp(sm, B + off, tabX + (size_t)view * 4 * sfdw::N,
-                                     H2 + (size_t)view * 2 * sfdw::N, tw,
-                                     field ? field + off : nullptr, inten ? inten + off : nullptr);
-        if (vmax != nullptr) {
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-            if (lane == 0) atomicMax(vmax + view, __float_as_uint(mx));
-        }
+    sfdw::SmemX &sm = *reinterpret_cast<sfdw::SmemX *>(smem4);
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < sfdw::XP * 2; ++i) sfdw::mbar_init(&sm.bar[0][0] + i, 1);
+        sfdw::mbar_fence_init();
     }
+    float2 tw[32];
+    sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
+    __syncthreads();
+    if (((threadIdx.x >> 5) & 1) == 0)
+        sfdw::pass_x_loop<0>(sm, B, tabX, H2, tw, field, inten, vmax, V);
+    else
+        sfdw::pass_x_loop<1>(sm, B, tabX, H2, tw, field, inten, vmax, V);
 }
 
 std::atomic<long long> g_launches{0};
@@ -137,20 +129,19 @@ cudaError_t launch_warp1024(sfd_plan *p, const void *holo, float2 *field, float 
     }
     const bool timing = p->timing;
     if (timing) cudaEventRecord(p->ev[0], st);
-    const int slots = g_sms * 3;
     const int items_y = V * (sfdw::N / sfdw::YC);
-    const int gy = items_y < slots ? items_y : slots;
+    const int gy = items_y < g_sms ? items_y : g_sms;
     if (d.in_dtype == 0)
-        k_cols_1024<unsigned char><<<gy, 128, sizeof(sfdw::SmemY), st>>>(
+        k_cols_1024<unsigned char><<<gy, 256, sizeof(sfdw::SmemY<unsigned char>), st>>>(
             (const unsigned char *)holo, d.w_tabY, d.w_H2, d.w_twl, d.B, vmax, V);
     else
-        k_cols_1024<float><<<gy, 128, sizeof(sfdw::SmemY), st>>>(
+        k_cols_1024<float><<<gy, 256, sizeof(sfdw::SmemY<float>), st>>>(
             (const float *)holo, d.w_tabY, d.w_H2, d.w_twl, d.B, vmax, V);
     if (timing) cudaEventRecord(p->ev[1], st);
-    const int ctas_x = (V * sfdw::N + 3) / 4;
-    const int gx = ctas_x < slots ? ctas_x : slots;
-    k_rows_1024<<<gx, 128, 4 * sizeof(sfdw::SmemXWarp), st>>>(d.B, d.w_tabX, d.w_H2, d.w_twl, field,
-                                                             inten, vmax, V);
+    const int ctas_x = (V * sfdw::N + sfdw::XP - 1) / sfdw::XP;
+    const int gx = ctas_x < g_sms ? ctas_x : g_sms;
+    k_rows_1024<<<gx, 256, sizeof(sfdw::SmemX), st>>>(d.B, d.w_tabX, d.w_H2, d.w_twl, field, inten,
+                                                      vmax, V);
     if (timing) cudaEventRecord(p->ev[2], st);
     int n = 2;
     if (u8) {
@@ -226,11 +217,11 @@ cudaError_t sfd_kernels_init() {
     SFD_ATTR(7) SFD_ATTR(8) SFD_ATTR(9) SFD_ATTR(10) SFD_ATTR(11) SFD_ATTR(12)
 #undef SFD_ATTR
     if ((e = cudaFuncSetAttribute(k_cols_1024<unsigned char>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)sizeof(sfdw::SmemY))) != cudaSuccess) return e;
+                                  (int)sizeof(sfdw::SmemY<unsigned char>))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(k_cols_1024<float>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)sizeof(sfdw::SmemY))) != cudaSuccess) return e;
+                                  (int)sizeof(sfdw::SmemY<float>))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(k_rows_1024, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)(4 * sizeof(sfdw::SmemXWarp)))) != cudaSuccess) return e;
+                                  (int)sizeof(sfdw::SmemX))) != cudaSuccess) return e;
     int dev = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
@@ -239,9 +230,10 @@ cudaError_t sfd_kernels_init() {
 
 cudaError_t sfd_launch(sfd_plan *p, const void *holo, float2 *field, float *inten,
                        unsigned char *u8, cudaStream_t st) {
-    // N = 1024: one-warp-per-line kernels (need the 4-byte aligned hologram rows of the uint8 tile load)
+    // N = 1024: warp-pair-per-line kernels (their tile loads read 4 hologram samples at once: the
+    // hologram must be aligned to 4 samples)
     if (p->d.N == sfdw::N && p->kernels != SFD_KERNELS_GENERIC && p->d.w_twl != nullptr &&
-        (reinterpret_cast<size_t>(holo) & 3) == 0)
+        (reinterpret_cast<size_t>(holo) & (p->d.in_dtype == 0 ? 3 : 15)) == 0)
         return launch_warp1024(p, holo, field, inten, u8, st);
     switch (p->d.log2M) {
         case 7: return launch_t<7>(p, holo, field, inten, u8, st);
