@@ -117,6 +117,10 @@ SFD_API long long sfd_plan_device_bytes(const sfd_plan *plan);
 #define SFD_KERNELS_GENERIC 1
 SFD_API int sfd_plan_select_kernels(sfd_plan *plan, int which);
 
+/* 1 if sfd_execute* on this plan currently runs the N = 1024 warp-pair kernels (k_cols_1024,
+ * k_rows_1024), 0 if it runs the generic kernels (k_pass_y, k_pass_x); SFD_EINVAL for NULL. */
+SFD_API int sfd_plan_uses_warp_kernels(const sfd_plan *plan);
+
 /* Timing aid for benchmarks: CUDA-event time, in milliseconds, of each of the two hot kernels
  * (pass y, pass x) of the most recent execute call on this plan, recorded on the stream they
  * were launched on.  Synchronises on those events.  ms[0] = pass y, ms[1] = pass x,

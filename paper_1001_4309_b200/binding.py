@@ -46,6 +46,7 @@ _sig = {
     "sfd_plan_get_m": (C.c_int, [_vp]),
     "sfd_plan_device_bytes": (C.c_longlong, [_vp]),
     "sfd_plan_select_kernels": (C.c_int, [_vp, C.c_int]),
+    "sfd_plan_uses_warp_kernels": (C.c_int, [_vp]),
     "sfd_plan_set_timing": (C.c_int, [_vp, C.c_int]),
     "sfd_plan_last_kernel_ms": (C.c_int, [_vp, C.POINTER(C.c_float)]),
     "sfd_launch_count": (C.c_longlong, []),
@@ -178,6 +179,10 @@ def sfd_plan_select_kernels(plan, which):
     _chk(_lib.sfd_plan_select_kernels(plan, int(which)), "sfd_plan_select_kernels")
 
 
+def sfd_plan_uses_warp_kernels(plan):
+    return int(_lib.sfd_plan_uses_warp_kernels(plan))
+
+
 def sfd_plan_set_timing(plan, enable):
     _chk(_lib.sfd_plan_set_timing(plan, int(bool(enable))), "sfd_plan_set_timing")
 
@@ -276,6 +281,10 @@ class Plan:
 
     def select_kernels(self, which):
         sfd_plan_select_kernels(self.handle, which)
+
+    @property
+    def uses_warp_kernels(self):
+        return bool(sfd_plan_uses_warp_kernels(self.handle))
 
     def set_timing(self, enable=True):
         sfd_plan_set_timing(self.handle, enable)

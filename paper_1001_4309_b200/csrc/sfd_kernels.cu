@@ -6,7 +6,8 @@
 //   k_pass_x : grid (N/RPC, V); per CTA RPC rows of B: x pre_x, FFT, x H, inverse FFT, crop, x post_x
 //              -> field, |.|^2 -> intensity (Eq. 5), optional per-view max
 // plus, in the 8-bit mode (step (xi), reading 15), k_quantise.
-// The per-thread arithmetic lives in sfd_fft_core.cuh.
+// The per-thread arithmetic lives in sfd_fft_core.cuh.  For N = 1024 the same two passes run as the
+// persistent kernels k_cols_1024 / k_rows_1024 (one warp pair per line, sfd_warp1024.cuh).
 #include <atomic>
 
 #include "sfd_fft_core.cuh"

@@ -455,6 +455,11 @@ int sfd_plan_select_kernels(sfd_plan *p, int which) {
     return SFD_OK;
 }
 
+int sfd_plan_uses_warp_kernels(const sfd_plan *p) {
+    if (!p) return SFD_EINVAL;
+    return p->d.N == 1024 && p->kernels != SFD_KERNELS_GENERIC && p->d.w_twl != nullptr ? 1 : 0;
+}
+
 int sfd_plan_set_timing(sfd_plan *p, int enable) {
     if (!p) return SFD_EINVAL;
     p->timing = enable != 0;

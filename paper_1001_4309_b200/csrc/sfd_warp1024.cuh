@@ -1,4 +1,4 @@
-// sfd_warp1024.cuh — the N = 1024 fast path: one warp per line, 32 complex values per thread.
+// sfd_warp1024.cuh — the N = 1024 fast path: one warp pair per line, 32 complex values per thread.
 //
 // The padded 2N-point transforms of PAPER.md steps (ii)-(ix) (L86-93) have a zero upper half on
 // the way in and a discarded upper half on the way out.  Splitting the 2N-point DFT by the parity
@@ -21,8 +21,9 @@
 //
 // A line is worked on by a PAIR of warps, one per branch, which meet once per line at a named
 // barrier to add their partial results (each warp finishes and stores one half of the line).  With
-// 8 warps per SM that is 4 lines in flight per SM: 4096 lines / (148 x 4) = 6.92 rounds, so the last
-// round is 92 % full (one warp per line and 12 warps per SM would give 2.3 rounds).  Every table
+// 8 warps per SM that is 4 lines in flight per SM: the 4096 lines of a 4-view pass take
+// 4096 / (148 x 4) = 6.92 -> 7 rounds, 98.8 % of them filled (one warp per line and 12 warps per SM
+// would take 2.3 -> 3 rounds, 77 % filled).  Every table
 // stream (pre, H, post) is fetched into a 32-value register vector P one phase ahead of its use,
 // and pass x gets its input rows by bulk async copy (TMA) into a double-buffered tile.
 #pragma once
@@ -38,6 +39,60 @@ constexpr int N = 1024;     // line length handled by this path
 constexpr int XS = 34;      // row stride (complex) of the transpose tile: 16-byte aligned rows,
                             // conflict-free for both the 8-byte column writes and 16-byte row reads
 constexpr int XB = 32 * XS;  // complex elements of one warp's transpose tile
+
+// Packed fp32 pairs (sm_100 FADD2): one instruction adds/subtracts both components of a complex
+// number.  The lane-op rate of the FMA pipe is unchanged, but a complex add costs one issue slot
+// instead of two — butterflies are mostly complex adds, so the radix-32 DFT shrinks from 440 to
+// about 310 instructions.
+__device__ __forceinline__ float2 padd(float2 a, float2 b) {
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;"
+        : "=l"(r)
+        : "l"(*reinterpret_cast<unsigned long long *>(&a)),
+          "l"(*reinterpret_cast<unsigned long long *>(&b)));
+    return *reinterpret_cast<float2 *>(&r);
+}
+__device__ __forceinline__ float2 psub(float2 a, float2 b) {
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;"
+        : "=l"(r)
+        : "l"(*reinterpret_cast<unsigned long long *>(&a)),
+          "l"(*reinterpret_cast<unsigned long long *>(&b)));
+    return *reinterpret_cast<float2 *>(&r);
+}
+// a + DIR*i*b and a - DIR*i*b (component swap: scalar adds)
+template <int DIR> __device__ __forceinline__ float2 add_ib(float2 a, float2 b) {
+    return DIR > 0 ? make_float2(a.x - b.y, a.y + b.x) : make_float2(a.x + b.y, a.y - b.x);
+}
+template <int DIR> __device__ __forceinline__ void pdft4(float2 &a0, float2 &a1, float2 &a2, float2 &a3) {
+    const float2 s0 = padd(a0, a2), d0 = psub(a0, a2), s1 = padd(a1, a3), t = psub(a1, a3);
+    a0 = padd(s0, s1);
+    a2 = psub(s0, s1);
+    a1 = add_ib<DIR>(d0, t);
+    a3 = add_ib<-DIR>(d0, t);
+}
+// 16-point DFT, natural order in and out (same factorisation as sfd::dft16)
+template <int DIR> __device__ __forceinline__ void pdft16(float2 (&a)[16]) {
+    using sfd::mul_w16;
+    pdft4<DIR>(a[0], a[4], a[8], a[12]);
+    pdft4<DIR>(a[1], a[5], a[9], a[13]);
+    pdft4<DIR>(a[2], a[6], a[10], a[14]);
+    pdft4<DIR>(a[3], a[7], a[11], a[15]);
+    a[5] = mul_w16<DIR, 1>(a[5]);   a[6] = mul_w16<DIR, 2>(a[6]);   a[7] = mul_w16<DIR, 3>(a[7]);
+    a[9] = mul_w16<DIR, 2>(a[9]);   a[10] = mul_w16<DIR, 4>(a[10]); a[11] = mul_w16<DIR, 6>(a[11]);
+    a[13] = mul_w16<DIR, 3>(a[13]); a[14] = mul_w16<DIR, 6>(a[14]); a[15] = mul_w16<DIR, 9>(a[15]);
+    pdft4<DIR>(a[0], a[1], a[2], a[3]);
+    pdft4<DIR>(a[4], a[5], a[6], a[7]);
+    pdft4<DIR>(a[8], a[9], a[10], a[11]);
+    pdft4<DIR>(a[12], a[13], a[14], a[15]);
+    float2 t;
+    t = a[1];  a[1] = a[4];   a[4] = t;
+    t = a[2];  a[2] = a[8];   a[8] = t;
+    t = a[3];  a[3] = a[12];  a[12] = t;
+    t = a[6];  a[6] = a[9];   a[9] = t;
+    t = a[7];  a[7] = a[13];  a[13] = t;
+    t = a[11]; a[11] = a[14]; a[14] = t;
+}
 
 // a * exp(DIR * 2 pi i * K / 32)
 template <int DIR, int K> __device__ __forceinline__ float2 mul_w32(float2 a) {
@@ -67,13 +122,13 @@ template <int DIR> __device__ __forceinline__ void dft32(float2 (&a)[32]) {
         e[s] = a[2 * s];
         o[s] = a[2 * s + 1];
     }
-    sfd::dft16<DIR, false>(e);
-    sfd::dft16<DIR, false>(o);
+    pdft16<DIR>(e);
+    pdft16<DIR>(o);
 #define SFDW_BF(K)                                   \
     {                                                \
         const float2 t = mul_w32<DIR, K>(o[K]);      \
-        a[K] = cadd(e[K], t);                        \
-        a[K + 16] = csub(e[K], t);                   \
+        a[K] = padd(e[K], t);                        \
+        a[K + 16] = psub(e[K], t);                   \
     }
     SFDW_BF(0) SFDW_BF(1) SFDW_BF(2) SFDW_BF(3) SFDW_BF(4) SFDW_BF(5) SFDW_BF(6) SFDW_BF(7)
     SFDW_BF(8) SFDW_BF(9) SFDW_BF(10) SFDW_BF(11) SFDW_BF(12) SFDW_BF(13) SFDW_BF(14) SFDW_BF(15)
@@ -192,7 +247,7 @@ __device__ __forceinline__ void add_halves(float2 (&v)[32], float2 (*xch)[512], 
     for (int q = 0; q < 16; ++q) xch[1 - B][q * 32 + lane] = v[16 * (1 - B) + q];
     pair_sync(pair);
 #pragma unroll
-    for (int q = 0; q < 16; ++q) v[16 * B + q] = cadd(v[16 * B + q], xch[B][q * 32 + lane]);
+    for (int q = 0; q < 16; ++q) v[16 * B + q] = padd(v[16 * B + q], xch[B][q * 32 + lane]);
 }
 
 // ---- pass y: 4 adjacent hologram columns per CTA, one warp pair per column -----------------------
