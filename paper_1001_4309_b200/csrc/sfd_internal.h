@@ -23,9 +23,9 @@ struct sfd_dev {
     float *inten_ws = nullptr;     // [V][N][N] intensity scratch of the 8-bit mode
     unsigned int *vmax = nullptr;  // [V] per-view max intensity (float bits)
     // N = 1024 fast path (sfd_warp1024.cuh); branch b = 0 even bins, 1 odd bins of the 2N-point DFT
-    float2 *w_tabY = nullptr;  // [V][4][N]  pre_y b0 | pre_y b1 | c0 post_y b0 | c0 post_y b1
-    float2 *w_tabX = nullptr;  // [V][4][N]  pre_x b0 | pre_x b1 | post_x b0 | post_x b1
-    float2 *w_H2 = nullptr;    // [V][2][N]  H[2k] | H[2k+1]
+    // per view and branch b: pre_b | H_b | conj(post_b), H_0[k] = H[2k], H_1[k] = H[2k+1]
+    float2 *w_tabY = nullptr;  // [V][2][3][N]  pre carries 1/255 (uint8 input), post carries c0
+    float2 *w_tabX = nullptr;  // [V][2][3][N]
     float2 *w_twl = nullptr;   // [32][32]   exp(-2 pi i lane k / 1024) at [k][lane]
 };
 

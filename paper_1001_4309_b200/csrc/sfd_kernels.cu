@@ -79,41 +79,53 @@ k_quantise(const float4 *__restrict__ inten, const unsigned int *__restrict__ vm
 }
 
 // ---- N = 1024 fast path (sfd_warp1024.cuh): persistent kernels, one warp pair per line --------------
-// One CTA of 8 warps per SM; the register budget (255) holds 32 values, 31 twiddles and a 32-value
-// prefetch vector per thread.
+// One CTA per SM.  Even warps run branch 0 (even bins), odd warps branch 1.
 template <typename TIn>
-__global__ void __launch_bounds__(256, 1)
+__global__ void __launch_bounds__(sfdw::WY * 32, 1)
 k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
-            const float2 *__restrict__ H2, const float2 *__restrict__ twl, float2 *__restrict__ B,
-            unsigned int *vmax, int V) {
+            const float2 *__restrict__ twl, float2 *__restrict__ B, unsigned int *vmax, int V) {
     extern __shared__ float4 smem4[];
     sfdw::SmemY<TIn> &sm = *reinterpret_cast<sfdw::SmemY<TIn> *>(smem4);
     if (vmax != nullptr && blockIdx.x == 0 && threadIdx.x < V) vmax[threadIdx.x] = 0u;
-    float2 tw[32];
-    sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
-    if (((threadIdx.x >> 5) & 1) == 0)
-        sfdw::pass_y_loop<TIn, 0>(sm, holo, tabY, H2, tw, B, V);
-    else
-        sfdw::pass_y_loop<TIn, 1>(sm, holo, tabY, H2, tw, B, V);
-}
-
-__global__ void __launch_bounds__(256, 1)
-k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
-            const float2 *__restrict__ H2, const float2 *__restrict__ twl,
-            float2 *__restrict__ field, float *__restrict__ inten, unsigned int *vmax, int V) {
-    extern __shared__ float4 smem4[];
-    sfdw::SmemX &sm = *reinterpret_cast<sfdw::SmemX *>(smem4);
     if (threadIdx.x == 0) {
-        for (int i = 0; i < sfdw::XP * 2; ++i) sfdw::mbar_init(&sm.bar[0][0] + i, 1);
+        sfdw::mbar_init(&sm.tbar[0], 1);
+        sfdw::mbar_init(&sm.tbar[1], 1);
+        sfdw::mbar_init(&sm.rdone[0], 4);
+        sfdw::mbar_init(&sm.rdone[1], 4);
         sfdw::mbar_fence_init();
     }
-    float2 tw[32];
+    if (!sfdw::TWR)
+        for (int i = threadIdx.x; i < 1024; i += blockDim.x) sm.tw[i] = __ldg(twl + i);
+    float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
     __syncthreads();
     if (((threadIdx.x >> 5) & 1) == 0)
-        sfdw::pass_x_loop<0>(sm, B, tabX, H2, tw, field, inten, vmax, V);
+        sfdw::pass_y_loop<TIn, 0>(sm, holo, tabY, tw, B, V);
     else
-        sfdw::pass_x_loop<1>(sm, B, tabX, H2, tw, field, inten, vmax, V);
+        sfdw::pass_y_loop<TIn, 1>(sm, holo, tabY, tw, B, V);
+}
+
+__global__ void __launch_bounds__(sfdw::WX * 32, 1)
+k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
+            const float2 *__restrict__ twl, float2 *__restrict__ field, float *__restrict__ inten,
+            unsigned int *vmax, int V) {
+    extern __shared__ float4 smem4[];
+    sfdw::SmemX &sm = *reinterpret_cast<sfdw::SmemX *>(smem4);
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < sfdw::XP; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
+        sfdw::mbar_init(&sm.tbar[0], 1);
+        sfdw::mbar_init(&sm.tbar[1], 1);
+        sfdw::mbar_fence_init();
+    }
+    if (!sfdw::TWR)
+        for (int i = threadIdx.x; i < 1024; i += blockDim.x) sm.tw[i] = __ldg(twl + i);
+    float2 tw[sfdw::TWN];
+    sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
+    __syncthreads();
+    if (((threadIdx.x >> 5) & 1) == 0)
+        sfdw::pass_x_loop<0>(sm, B, tabX, tw, field, inten, vmax, V);
+    else
+        sfdw::pass_x_loop<1>(sm, B, tabX, tw, field, inten, vmax, V);
 }
 
 std::atomic<long long> g_launches{0};
@@ -130,19 +142,19 @@ cudaError_t launch_warp1024(sfd_plan *p, const void *holo, float2 *field, float 
     }
     const bool timing = p->timing;
     if (timing) cudaEventRecord(p->ev[0], st);
-    const int items_y = V * (sfdw::N / sfdw::YC);
-    const int gy = items_y < g_sms ? items_y : g_sms;
+    // one CTA per SM, but at least V CTAs: a CTA's contiguous range of items (rows) then touches at
+    // most two views (the kernels hold two table sets)
+    const int gy = V > g_sms ? V : g_sms;
     if (d.in_dtype == 0)
-        k_cols_1024<unsigned char><<<gy, 256, sizeof(sfdw::SmemY<unsigned char>), st>>>(
-            (const unsigned char *)holo, d.w_tabY, d.w_H2, d.w_twl, d.B, vmax, V);
+        k_cols_1024<unsigned char><<<gy, sfdw::WY * 32, sizeof(sfdw::SmemY<unsigned char>), st>>>(
+            (const unsigned char *)holo, d.w_tabY, d.w_twl, d.B, vmax, V);
     else
-        k_cols_1024<float><<<gy, 256, sizeof(sfdw::SmemY<float>), st>>>(
-            (const float *)holo, d.w_tabY, d.w_H2, d.w_twl, d.B, vmax, V);
+        k_cols_1024<float><<<gy, sfdw::WY * 32, sizeof(sfdw::SmemY<float>), st>>>(
+            (const float *)holo, d.w_tabY, d.w_twl, d.B, vmax, V);
     if (timing) cudaEventRecord(p->ev[1], st);
-    const int ctas_x = (V * sfdw::N + sfdw::XP - 1) / sfdw::XP;
-    const int gx = ctas_x < g_sms ? ctas_x : g_sms;
-    k_rows_1024<<<gx, 256, sizeof(sfdw::SmemX), st>>>(d.B, d.w_tabX, d.w_H2, d.w_twl, field, inten,
-                                                      vmax, V);
+    const int gx = gy;
+    k_rows_1024<<<gx, sfdw::WX * 32, sizeof(sfdw::SmemX), st>>>(d.B, d.w_tabX, d.w_twl, field, inten,
+                                                                vmax, V);
     if (timing) cudaEventRecord(p->ev[2], st);
     int n = 2;
     if (u8) {

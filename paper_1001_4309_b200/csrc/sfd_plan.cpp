@@ -131,41 +131,41 @@ void to_f32(const cd *src, float2 *dst, size_t n, cd scale = cd(1, 0)) {
 // Branch tables of the N = 1024 fast path (sfd_warp1024.cuh) for one axis: the 2N-point DFT split
 // by the parity of the frequency index, w = exp(-2 pi i / 2N):
 //   out[4][N] = pre | pre w^n | post | post w^-n   (each times its scale), formed in float64.
-void branch_tables(int N, const cd *pre, const cd *post, cd pre_scale, cd post_scale, float2 *out) {
+// Fast-path tables of one pass and one view, layout [2][3][N]: for branch b the vectors
+// pre_b, H_b, conj(post_b) (sfd_warp1024.cuh); H = the float32 M-point kernel spectrum.
+void branch_tables(int N, const cd *pre, const cd *post, cd pre_scale, cd post_scale,
+                   const float2 *H, float2 *out) {
     for (int n = 0; n < N; ++n) {
         const cd w = cis_cycles(-(ld)n / (ld)(2 * N));
-        const cd t[4] = {pre[n] * pre_scale, pre[n] * pre_scale * w, post[n] * post_scale,
-                         post[n] * post_scale * std::conj(w)};
-        for (int k = 0; k < 4; ++k)
-            out[(size_t)k * N + n] = make_float2((float)t[k].real(), (float)t[k].imag());
+        const cd t[4] = {pre[n] * pre_scale, pre[n] * pre_scale * w,
+                         std::conj(post[n] * post_scale), std::conj(post[n] * post_scale * std::conj(w))};
+        for (int b = 0; b < 2; ++b) {
+            float2 *o = out + (size_t)b * 3 * N;
+            o[n] = make_float2((float)t[b].real(), (float)t[b].imag());
+            o[N + n] = H[2 * n + b];
+            o[2 * N + n] = make_float2((float)t[2 + b].real(), (float)t[2 + b].imag());
+        }
     }
 }
 
 // float32 tables of one view, host staging layout: pre_y[N] post_y[N] pre_x[N] post_x[N] H[M];
-// `fast` (or NULL) receives tabY[4N] tabX[4N] H2[2N] of the fast path.
+// `fast` (or NULL) receives tabY[6N] tabX[6N] of the fast path.
 void build_view_f32(const sfd_plan *p, int v, float2 *pre_y, float2 *post_y, float2 *pre_x,
                     float2 *post_x, float2 *H, float2 *fast) {
     const int N = p->d.N, M = p->d.M;
     std::vector<cd> a(N), b(N), h(M);
     const double in_scale = p->d.in_dtype == SFD_U8 ? 1.0 / 255.0 : 1.0;
     const cd c0 = c0_factor(p->lambda, p->p1[v], p->z[v]);
+    kernel_spectrum(N, p->lambda, p->p1[v], p->p2[v], p->z[v], h.data());
+    to_f32(h.data(), H, M);
     axis_tables(N, p->lambda, p->p1[v], p->p2[v], p->z[v], p->Oy[v], a.data(), b.data());
     to_f32(a.data(), pre_y, N, cd(in_scale, 0));
     to_f32(b.data(), post_y, N, c0);
-    if (fast) branch_tables(N, a.data(), b.data(), cd(in_scale, 0), c0, fast);
+    if (fast) branch_tables(N, a.data(), b.data(), cd(in_scale, 0), c0, H, fast);
     axis_tables(N, p->lambda, p->p1[v], p->p2[v], p->z[v], p->Ox[v], a.data(), b.data());
     to_f32(a.data(), pre_x, N);
     to_f32(b.data(), post_x, N);
-    if (fast) branch_tables(N, a.data(), b.data(), cd(1, 0), cd(1, 0), fast + 4 * (size_t)N);
-    kernel_spectrum(N, p->lambda, p->p1[v], p->p2[v], p->z[v], h.data());
-    to_f32(h.data(), H, M);
-    if (fast) {
-        float2 *H2 = fast + 8 * (size_t)N;
-        for (int k = 0; k < N; ++k) {
-            H2[k] = H[2 * k];
-            H2[N + k] = H[2 * k + 1];
-        }
-    }
+    if (fast) branch_tables(N, a.data(), b.data(), cd(1, 0), cd(1, 0), H, fast + 6 * (size_t)N);
 }
 
 std::atomic<bool> g_init{false};
@@ -226,16 +226,14 @@ int stream_state_make(sfd_plan *p) {
 int upload_view(sfd_plan *p, int v) {
     const int N = p->d.N, M = p->d.M;
     const bool fast = p->d.w_twl != nullptr;
-    std::vector<float2> st((size_t)4 * N + M + (fast ? 10 * (size_t)N : 0));
+    std::vector<float2> st((size_t)4 * N + M + (fast ? 12 * (size_t)N : 0));
     float2 *fs = fast ? st.data() + 4 * N + M : nullptr;
     build_view_f32(p, v, st.data(), st.data() + N, st.data() + 2 * N, st.data() + 3 * N,
                    st.data() + 4 * N, fs);
     if (fast) {
-        SFD_CUDA(cudaMemcpy(p->d.w_tabY + (size_t)v * 4 * N, fs, 4 * sizeof(float2) * N,
+        SFD_CUDA(cudaMemcpy(p->d.w_tabY + (size_t)v * 6 * N, fs, 6 * sizeof(float2) * N,
                             cudaMemcpyHostToDevice));
-        SFD_CUDA(cudaMemcpy(p->d.w_tabX + (size_t)v * 4 * N, fs + 4 * N, 4 * sizeof(float2) * N,
-                            cudaMemcpyHostToDevice));
-        SFD_CUDA(cudaMemcpy(p->d.w_H2 + (size_t)v * 2 * N, fs + 8 * N, 2 * sizeof(float2) * N,
+        SFD_CUDA(cudaMemcpy(p->d.w_tabX + (size_t)v * 6 * N, fs + 6 * N, 6 * sizeof(float2) * N,
                             cudaMemcpyHostToDevice));
     }
     const size_t nb = sizeof(float2) * N;
@@ -333,14 +331,13 @@ int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const dou
             return fail(cuda_fail(e, "cudaMemcpy tw"));
     }
     if (N == 1024) {   // fast-path tables (sfd_warp1024.cuh)
-        const size_t n_fast = V * 10 * (size_t)N + 32 * 32;
+        const size_t n_fast = V * 12 * (size_t)N + 32 * 32;
         if ((e = cudaMalloc(&p->fast_alloc, n_fast * sizeof(float2))) != cudaSuccess)
             return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc fast tables"));
         float2 *f = (float2 *)p->fast_alloc;
         p->d.w_tabY = f;
-        p->d.w_tabX = f + V * 4 * N;
-        p->d.w_H2 = f + V * 8 * N;
-        p->d.w_twl = f + V * 10 * N;
+        p->d.w_tabX = f + V * 6 * N;
+        p->d.w_twl = f + V * 12 * N;
         p->device_bytes += (long long)(n_fast * sizeof(float2));
         std::vector<float2> twl(32 * 32);
         for (int k = 0; k < 32; ++k)

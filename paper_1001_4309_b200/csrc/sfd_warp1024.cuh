@@ -15,17 +15,17 @@
 // With N = 1024 = 32 x 32 an N-point FFT is two radix-32 register butterflies around ONE 32 x 32
 // transpose, and a warp (32 lanes x 32 values) owns a whole branch: the transpose goes through a
 // private shared-memory tile guarded by __syncwarp only; no CTA barrier exists on the FFT path.
-// Per line this moves 4 x 16 KiB through shared memory instead of 8 x 32 KiB (generic path) and the
-// inter-stage twiddles w1024^(lane * k1) are per-thread constants kept in registers for the whole
-// (persistent) kernel.
 //
-// A line is worked on by a PAIR of warps, one per branch, which meet once per line at a named
-// barrier to add their partial results (each warp finishes and stores one half of the line).  With
-// 8 warps per SM that is 4 lines in flight per SM: the 4096 lines of a 4-view pass take
-// 4096 / (148 x 4) = 6.92 -> 7 rounds, 98.8 % of them filled (one warp per line and 12 warps per SM
-// would take 2.3 -> 3 rounds, 77 % filled).  Every table
-// stream (pre, H, post) is fetched into a 32-value register vector P one phase ahead of its use,
-// and pass x gets its input rows by bulk async copy (TMA) into a double-buffered tile.
+// A line is worked on by a PAIR of warps, one per branch, which meet at a named barrier to add
+// their partial results (each warp finishes and stores one half of the line); the half a warp
+// hands over travels through its own transpose tile, which is idle by then.
+//
+// What bounds these kernels is the plain fp32 pipe (about 2500 lane-cycles per warp and line, most
+// of them butterfly adds), closely followed by the shared-memory data pipe and the issue slots, so
+// everything that is not butterfly arithmetic is kept off the long-latency path: the six table
+// vectors of the current view (pre_b, H_b, conj(post_b)) sit in shared memory (one bulk copy per
+// view change, 48 KiB), pass x receives its rows by bulk async copy issued a line ahead, and a
+// CTA walks a CONTIGUOUS range of lines so that it changes view at most once or twice.
 #pragma once
 #include "sfd_fft_core.cuh"
 
@@ -135,32 +135,38 @@ template <int DIR> __device__ __forceinline__ void dft32(float2 (&a)[32]) {
 #undef SFDW_BF
 }
 
-// 1024-point forward FFT of one warp.  In: v[r] = x[lane + 32 r].  Out: v[r] = X[lane + 32 r].
-// tw[k] = exp(-2 pi i lane k / 1024) (this thread's inter-stage twiddles), xb = the warp's tile.
-// The two radix-32 stages share one copy of the butterfly code (rolled loop): the whole line
-// transform then fits the instruction cache, which an unrolled version (~140 KB of SASS) does not.
-__device__ __forceinline__ void fft1024(float2 (&v)[32], int lane, float2 *xb,
-                                        const float2 (&tw)[32]) {
-#pragma unroll 1
-    for (int stage = 0; stage < 2; ++stage) {
-        dft32<-1>(v);  // stage 0: over n1 for n2 = lane -> v[k1]; stage 1: over n2 for k1 = lane
-        if (stage == 0) {
-#pragma unroll
-            for (int k = 1; k < 32; ++k) v[k] = cmul(v[k], tw[k]);
-#pragma unroll
-            for (int k = 0; k < 32; ++k) xb[k * XS + lane] = v[k];  // (k1 = k, n2 = lane)
-            __syncwarp();
-            const float4 *row = reinterpret_cast<const float4 *>(xb + lane * XS);  // k1 = lane
-#pragma unroll
-            for (int q = 0; q < 16; ++q) {
-                const float4 t = row[q];
-                v[2 * q] = make_float2(t.x, t.y);
-                v[2 * q + 1] = make_float2(t.z, t.w);
-            }
-            __syncwarp();
-        }
-    }
+// ---- build knobs (variants are compared with SFD_LIBRARY=<variant .so> python bench.py) -----------
+#ifndef SFDW_WX
+#define SFDW_WX 8   // warps per CTA in pass x (pairs of them work on a row)
+#endif
+#ifndef SFDW_TWR
+#define SFDW_TWR 1  // 1: inter-stage twiddles live in registers, 0: read from shared memory
+#endif
+#ifndef SFDW_PINGPONG
+#define SFDW_PINGPONG 1  // 1: warps sharing a sub-partition take turns in the butterfly phases (pass x)
+#endif
+#ifndef SFDW_PP_SKEW
+#define SFDW_PP_SKEW 0
+#endif
+#ifndef SFDW_ROLLED
+#define SFDW_ROLLED 1  // 1: the two radix-32 stages / two FFTs of a branch share one copy of the code
+#endif
+#if SFDW_ROLLED
+#define SFDW_LOOP _Pragma("unroll 1")
+#else
+#define SFDW_LOOP _Pragma("unroll")
+#endif
+#ifdef SFDW_TRACE
+__device__ long long *g_trace;  // [cta][warp][line slot][16] clock stamps (experiments only)
+__device__ __forceinline__ void stamp(long long *tr, int i) {
+    if ((threadIdx.x & 31) == 0) tr[i] = clock64();
 }
+#define SFDW_STAMP(i) stamp(tr, i)
+#else
+#define SFDW_STAMP(i)
+#endif
+constexpr bool TWR = SFDW_TWR != 0;
+constexpr int TWN = TWR ? 32 : 1;  // length of the per-thread twiddle register vector
 
 // ---- small PTX helpers ---------------------------------------------------------------------------
 __device__ __forceinline__ unsigned smem_u32(const void *p) {
@@ -174,6 +180,10 @@ __device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
 }
 __device__ __forceinline__ void mbar_fence_init() {
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+// orders this thread's earlier generic-proxy shared-memory accesses before later async-proxy ones
+__device__ __forceinline__ void fence_async_smem() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 // arm `bar` for `bytes` and start a 1-D bulk copy global -> shared that completes on it
 __device__ __forceinline__ void bulk_load(void *dst, const void *src, unsigned bytes,
@@ -200,210 +210,359 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned pari
         : "memory");
 }
 
-__device__ __forceinline__ void load_twiddles(float2 (&tw)[32], int lane,
+__device__ __forceinline__ void load_twiddles(float2 (&tw)[TWN], int lane,
                                               const float2 *__restrict__ twl) {
+    if constexpr (TWR) {
 #pragma unroll
-    for (int k = 0; k < 32; ++k) tw[k] = __ldg(twl + k * 32 + lane);
-}
-// P <- 32 table values of this thread (element lane + 32 r)
-__device__ __forceinline__ void fetch(float2 (&P)[32], const float2 *__restrict__ tab, int lane) {
-#pragma unroll
-    for (int r = 0; r < 32; ++r) P[r] = __ldg(tab + lane + 32 * r);
+        for (int k = 0; k < 32; ++k) tw[k] = __ldg(twl + k * 32 + lane);
+    } else {
+        tw[0] = make_float2(1.f, 0.f);
+    }
 }
 
-// One branch of a line, in place (the caller has applied pre): forward FFT, x H_b, inverse FFT.
-// The inverse is run as conj(FFT(conj(.))) so that both transforms execute the same code; the
-// conjugations are sign flips inside the H multiply and inside the post multiply.
-// On entry P holds H_b; on return P holds post_b and v = post_b * (branch result) — this warp's
-// partial sums for all 1024 outputs of the line.
-__device__ __forceinline__ void branch(float2 (&v)[32], float2 (&P)[32], int lane, float2 *xb,
-                                       const float2 (&tw)[32], const float2 *__restrict__ post) {
-#pragma unroll 1
-    for (int pass = 0; pass < 2; ++pass) {
-        fft1024(v, lane, xb, tw);
-        if (pass == 0) {
+// Tables of one view and one pass as they sit in global memory ([V][2][3][N], plan time) and in
+// shared memory: for branch b the vectors pre_b, H_b, conj(post_b).
+constexpr int TABS = 2 * 3 * N;  // complex elements
+// Turn-taking between the two warps that share an SM sub-partition (warps w and w + 4 of an
+// 8-warp CTA).  The butterfly phases of a line saturate the sub-partition's fp32 pipe, the phases
+// between them (transposes, table and input reads, exchange, stores) use the SM-wide shared-memory
+// pipe; left alone, all warps of an SM drift into the same phase and the two kinds of phase run
+// one after the other instead of side by side.  A warp therefore enters a butterfly phase only
+// when it holds its sub-partition's token (named barrier `mine`, armed by the other warp) and
+// passes the token on (`theirs`) when the phase ends: one warp of each sub-partition is always in
+// butterflies while the other does its memory phase.
+struct Turns {
+    int mine, theirs;  // named-barrier ids
+    bool on;
+};
+__device__ __forceinline__ void turn_begin(const Turns &t) {
+    if (t.on) asm volatile("bar.sync %0, 64;" ::"r"(t.mine) : "memory");
+}
+__device__ __forceinline__ void turn_end(const Turns &t) {
+    if (t.on) asm volatile("bar.arrive %0, 64;" ::"r"(t.theirs) : "memory");
+}
+
+// One branch of a line, in place (the caller has applied pre): forward FFT, x H_b, inverse FFT,
+// x post_b.  The inverse is run as conj(FFT(conj(.))) so that both transforms execute the same code:
+//     v <- conj(FFT(v) H_b);  v <- conj(FFT(v) conj(post_b)) = post_b IFFT(H_b FFT(v)) N
+// (the 1/N sits in H).  t = this thread's first element of H_b; conj(post_b) follows it N later.
+// A 1024-point FFT of a warp is: radix-32 butterflies over n1 (element lane + 32 n1), inter-stage
+// twiddles exp(-2 pi i lane k1 / 1024) (tw[k] in registers or twsm[k * 32 + lane]), a 32 x 32
+// transpose through the warp's tile xb, radix-32 butterflies over n2; in v[r] = x[lane + 32 r],
+// out v[r] = X[lane + 32 r].  The four radix-32 steps of the branch share one copy of the code
+// (rolled loop): the line transform then fits the instruction cache.  Steps 0 | 1, 2 | 3 are the
+// three turns of the line.  On return v = this warp's partial sums for all 1024 outputs.
+__device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
+                                       const float2 (&tw)[TWN], const float2 *twsm,
+                                       const float2 *t, const Turns &turns
+#ifdef SFDW_TRACE
+                                       , long long *tr
+#endif
+) {
+    SFDW_LOOP
+    for (int step = 0; step < 4; ++step) {
+        if (step != 2) turn_begin(turns);
+        SFDW_STAMP(step == 0 ? 10 : step == 1 ? 12 : 14);
+        dft32<-1>(v);
+        if (step & 1) {
 #pragma unroll
-            for (int k = 0; k < 32; ++k) {  // v = conj(v * H)
-                const float2 h = P[k], a = v[k];
+            for (int k = 0; k < 32; ++k) {  // v = conj(v * t)
+                const float2 h = t[(step >> 1) * N + 32 * k], a = v[k];
                 v[k] = make_float2(a.x * h.x - a.y * h.y, -(a.x * h.y) - a.y * h.x);
             }
-            fetch(P, post, lane);  // lands during the second FFT
-        }
-    }
+            SFDW_STAMP(15);
+            if (step != 1) turn_end(turns);
+        } else {
 #pragma unroll
-    for (int k = 0; k < 32; ++k) {  // v = post * conj(v)
-        const float2 p = P[k], w = v[k];
-        v[k] = make_float2(p.x * w.x + p.y * w.y, p.y * w.x - p.x * w.y);
+            for (int k = 1; k < 32; ++k) {
+                if constexpr (TWR)
+                    v[k] = cmul(v[k], tw[k]);
+                else
+                    v[k] = cmul(v[k], twsm[k * 32 + lane]);
+            }
+            SFDW_STAMP(step == 0 ? 11 : 13);
+            turn_end(turns);
+#pragma unroll
+            for (int k = 0; k < 32; ++k) xb[k * XS + lane] = v[k];  // (k1 = k, n2 = lane)
+            __syncwarp();
+            const float4 *row = reinterpret_cast<const float4 *>(xb + lane * XS);  // k1 = lane
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                const float4 w = row[q];
+                v[2 * q] = make_float2(w.x, w.y);
+                v[2 * q + 1] = make_float2(w.z, w.w);
+            }
+            __syncwarp();
+        }
+        SFDW_STAMP(4 + step);
     }
 }
 
 // The two warps of a pair hold partial sums v (branch B) for all 32 x 32 outputs of a line.  Warp B
-// finishes outputs r in [16 B, 16 B + 16) (element lane + 32 r): it hands the other 16 to its
-// partner through xch[1 - B], meets it at the pair's named barrier and adds what it was handed.
-// Afterwards v[16 B + q], q < 16, are final.
+// finishes outputs r in [16 B, 16 B + 16) (element lane + 32 r): it leaves the other 16 in its own
+// transpose tile `mine` (idle by now), meets its partner at the pair's named barrier and adds what
+// the partner left in `theirs`.  Afterwards v[16 B + q], q < 16, are final.  The caller must put a
+// pair barrier (or a CTA barrier) between this and the next write to the tile.
 template <int B>
-__device__ __forceinline__ void add_halves(float2 (&v)[32], float2 (*xch)[512], int lane, int pair) {
+__device__ __forceinline__ void add_halves(float2 (&v)[32], float2 *mine, const float2 *theirs,
+                                           int lane, int pair) {
 #pragma unroll
-    for (int q = 0; q < 16; ++q) xch[1 - B][q * 32 + lane] = v[16 * (1 - B) + q];
+    for (int q = 0; q < 16; ++q) mine[q * 32 + lane] = v[16 * (1 - B) + q];
     pair_sync(pair);
 #pragma unroll
-    for (int q = 0; q < 16; ++q) v[16 * B + q] = padd(v[16 * B + q], xch[B][q * 32 + lane]);
+    for (int q = 0; q < 16; ++q) v[16 * B + q] = padd(v[16 * B + q], theirs[q * 32 + lane]);
 }
 
-// ---- pass y: 4 adjacent hologram columns per CTA, one warp pair per column -----------------------
-constexpr int YC = 4;      // columns per CTA
-constexpr int CS = N + 4;  // stride (complex) between the CTA's column buffers: puts columns c and
-                           // c+2 sixteen banks apart for the transposed read-out
+// ---- pass y: 4 adjacent hologram columns per CTA ---------------------------------------------------
+// The CTA is two independent halves of four warps (half h = warps 4h .. 4h+3 = two warp pairs);
+// half h transforms columns col0 + 2h and col0 + 2h + 1 of the CTA's current item.  Nothing
+// synchronises the two halves with each other except the turn-taking of the warps that share a
+// sub-partition (warps w and w + 4).
+constexpr int WY = 8;  // warps per CTA
+constexpr int YC = 4;  // columns per item
+template <typename TIn> struct TileElem { using type = unsigned short; };  // 2 uint8 columns of a row
+template <> struct TileElem<float> { using type = float2; };               // 2 float columns of a row
 template <typename TIn> struct SmemY {
-    float2 xb[2 * YC][XB];
-    float2 xch[YC][2][512];
-    float2 col[YC][CS];
-    // uint8: tile[buf][n0] = the 4 bytes of columns col0..col0+3 of row n0;
-    // float: tile[buf][c * N + n0]
-    unsigned int tile[2][sizeof(TIn) == 1 ? N : YC * N];
+    float2 xb[WY][XB];
+    float2 tabs[2][TABS];  // tables of the (at most two) views this CTA's items belong to
+    float2 tw[32 * 32];
+    typename TileElem<TIn>::type tile[2][2][N];  // [half][buffer][n0]: the half's two input columns
+    unsigned long long tbar[2];
+    unsigned long long rdone[2];  // per half: the read-out of the previous item has left the tiles
 };
 
-template <typename TIn> struct TileRegs {
-    unsigned int w[4];   // uint8: 4 rows x 4 packed columns
-    float4 f[4];         // float: 4 rows x 4 columns
-};
+template <typename TIn> struct TileRegs { typename TileElem<TIn>::type e[8]; };
 
+// the 128 threads of a half fetch rows ht, ht + 128, .. of columns colh, colh + 1
 template <typename TIn>
-__device__ __forceinline__ void tile_load(TileRegs<TIn> &t, const TIn *__restrict__ holo, int col0) {
+__device__ __forceinline__ void tile_load(TileRegs<TIn> &t, const TIn *__restrict__ holo, int colh,
+                                          int ht) {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const size_t row = threadIdx.x + 256 * i;
-        if constexpr (sizeof(TIn) == 1)
-            t.w[i] = __ldg(reinterpret_cast<const unsigned int *>(holo + row * N + col0));
-        else
-            t.f[i] = __ldg(reinterpret_cast<const float4 *>(holo + row * N + col0));
-    }
+    for (int i = 0; i < 8; ++i)
+        t.e[i] = __ldg(reinterpret_cast<const typename TileElem<TIn>::type *>(
+            holo + (size_t)(ht + 128 * i) * N + colh));
 }
 template <typename TIn>
-__device__ __forceinline__ void tile_store(const TileRegs<TIn> &t, unsigned int *tile) {
+__device__ __forceinline__ void tile_store(const TileRegs<TIn> &t,
+                                           typename TileElem<TIn>::type *tile, int ht) {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int row = threadIdx.x + 256 * i;
-        if constexpr (sizeof(TIn) == 1) {
-            tile[row] = t.w[i];
-        } else {
-            float *f = reinterpret_cast<float *>(tile);
-            f[row] = t.f[i].x;
-            f[N + row] = t.f[i].y;
-            f[2 * N + row] = t.f[i].z;
-            f[3 * N + row] = t.f[i].w;
-        }
-    }
+    for (int i = 0; i < 8; ++i) tile[ht + 128 * i] = t.e[i];
+}
+__device__ __forceinline__ float tile_value(unsigned short e, int c) {
+    return (float)((e >> (8 * c)) & 0xffu);
+}
+__device__ __forceinline__ float tile_value(float2 e, int c) { return c ? e.y : e.x; }
+
+__device__ __forceinline__ void half_sync(int half) {  // named barrier of the four warps of a half
+    asm volatile("bar.sync %0, 128;" ::"r"(half + 1) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-// Persistent CTA of 256 threads: work item = (view, group of 4 columns).
-// tabY: [V][4][N] = pre b0 | pre b1 | c0 post b0 | c0 post b1;  H2: [V][2][N];  Bout: [V][N][N].
+// Persistent CTA of 256 threads: work item = (view, group of 4 columns); a CTA takes a contiguous
+// range of items (at most two views: the launcher sizes the grid accordingly).
+// tabY: [V][2][3][N] (post carries c0, pre the 1/255 of uint8 input); Bout: [V][N][N].
+// A warp leaves the partial sums of its branch for all 1024 outputs of its column in its own
+// transpose tile (idle by then); after the half's barrier the 128 threads of the half add the two
+// branches and write 16-byte row chunks B[n1][colh .. colh+1].
 template <typename TIn, int B>
 __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restrict__ holo,
                                             const float2 *__restrict__ tabY,
-                                            const float2 *__restrict__ H2,
-                                            const float2 (&tw)[32], float2 *__restrict__ Bout, int V) {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, c = warp >> 1;
+                                            const float2 (&tw)[TWN], float2 *__restrict__ Bout,
+                                            int V) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int half = warp >> 2, c = (warp >> 1) & 1, ht = threadIdx.x & 127;
     constexpr int groups = N / YC;
     const int items = V * groups;
-    int item = blockIdx.x;
-    if (item >= items) return;
+    const int i0 = (int)((long long)items * blockIdx.x / gridDim.x);
+    const int i1 = (int)((long long)items * (blockIdx.x + 1) / gridDim.x);
+    if (i0 >= i1) return;  // CTA-uniform
     float2 *xb = sm.xb[warp];
-    float2 P[32];
+    const int view0 = i0 / groups;
+    if (threadIdx.x == 0) {
+        bulk_load(sm.tabs[0], tabY + (size_t)view0 * TABS, TABS * sizeof(float2), &sm.tbar[0]);
+        if ((i1 - 1) / groups != view0)
+            bulk_load(sm.tabs[1], tabY + (size_t)(view0 + 1) * TABS, TABS * sizeof(float2),
+                      &sm.tbar[1]);
+    }
     {
         TileRegs<TIn> t;
-        tile_load<TIn>(t, holo, (item % groups) * YC);
-        fetch(P, tabY + (size_t)(item / groups) * 4 * N + B * N, lane);
-        tile_store<TIn>(t, sm.tile[0]);
+        tile_load<TIn>(t, holo, (i0 % groups) * YC + 2 * half, ht);
+        tile_store<TIn>(t, sm.tile[half][0], ht);
     }
-    __syncthreads();
-    int tb = 0;
-    for (; item < items; item += gridDim.x) {
-        const int view = item / groups, col0 = (item % groups) * YC;
-        const int next = item + gridDim.x;
-        const bool has_next = next < items;
+    half_sync(half);
+    constexpr bool PP = SFDW_PINGPONG != 0;
+    const Turns turns{3 + 2 * (warp & 3) + half, 3 + 2 * (warp & 3) + 1 - half, PP};
+    if (PP && half == 1) turn_end(turns);  // the first turn belongs to warps 0..3
+    const float2 *tb_pre = nullptr;
+    int cur_view = -1;
+    for (int item = i0; item < i1; ++item) {
+        const int it = item - i0, tb = it & 1;
+        const int view = item / groups, colh = (item % groups) * YC + 2 * half;
+        if (view != cur_view) {
+            mbar_wait(&sm.tbar[view - view0], 0);
+            tb_pre = sm.tabs[view - view0] + B * 3 * N + lane;
+            cur_view = view;
+        }
+        const bool has_next = item + 1 < i1;
+#ifdef SFDW_TRACE
+        long long *tr = g_trace + (((size_t)blockIdx.x * WY + warp) * 16 + it) * 16;
+#endif
+        SFDW_STAMP(0);
         TileRegs<TIn> t;
-        if (has_next) tile_load<TIn>(t, holo, (next % groups) * YC);
+        if (has_next) tile_load<TIn>(t, holo, ((item + 1) % groups) * YC + 2 * half, ht);
         float2 v[32];
 #pragma unroll
         for (int r = 0; r < 32; ++r) {
-            const int n0 = lane + 32 * r;
-            float a;
-            if constexpr (sizeof(TIn) == 1)
-                a = (float)((sm.tile[tb][n0] >> (8 * c)) & 0xffu);
-            else
-                a = reinterpret_cast<const float *>(sm.tile[tb])[c * N + n0];
-            v[r] = make_float2(a * P[r].x, a * P[r].y);
+            const float a = tile_value(sm.tile[half][tb][lane + 32 * r], c);
+            const float2 p = tb_pre[32 * r];
+            v[r] = make_float2(a * p.x, a * p.y);
         }
-        fetch(P, H2 + (size_t)view * 2 * N + B * N, lane);
-        branch(v, P, lane, xb, tw, tabY + (size_t)view * 4 * N + 2 * N + B * N);
-        if (has_next) fetch(P, tabY + (size_t)(next / groups) * 4 * N + B * N, lane);
-        add_halves<B>(v, sm.xch[c], lane, c);
+        // the previous item's read-out must have left the transpose tiles before they are written
+        SFDW_STAMP(1);
+        if (it > 0) mbar_wait(&sm.rdone[half], (it - 1) & 1);
+        SFDW_STAMP(2);
+#ifdef SFDW_TRACE
+        branch(v, lane, xb, tw, sm.tw, tb_pre + N, turns, tr);
+#else
+        branch(v, lane, xb, tw, sm.tw, tb_pre + N, turns);
+#endif
 #pragma unroll
-        for (int q = 0; q < 16; ++q) sm.col[c][lane + 32 * (16 * B + q)] = v[16 * B + q];
-        if (has_next) tile_store<TIn>(t, sm.tile[tb ^ 1]);
-        __syncthreads();
-        // transposed read-out: 32-byte row chunks B[n1][col0..col0+3], two lanes per row
-        float2 *Bv = Bout + (size_t)view * N * N;
+        for (int r = 0; r < 32; ++r) xb[r * 32 + lane] = v[r];  // element n1 = lane + 32 r at n1
+        if (has_next) tile_store<TIn>(t, sm.tile[half][tb ^ 1], ht);
+        SFDW_STAMP(8);
+        half_sync(half);  // partial sums complete, next input tile visible
+        SFDW_STAMP(9);
+        const float4 *s00 = reinterpret_cast<const float4 *>(sm.xb[4 * half + 0]);
+        const float4 *s01 = reinterpret_cast<const float4 *>(sm.xb[4 * half + 1]);
+        const float4 *s10 = reinterpret_cast<const float4 *>(sm.xb[4 * half + 2]);
+        const float4 *s11 = reinterpret_cast<const float4 *>(sm.xb[4 * half + 3]);
+        float2 *Bv = Bout + (size_t)view * N * N + colh;
 #pragma unroll
-        for (int i = 0; i < 2 * N / 256; ++i) {
-            const int idx = threadIdx.x + 256 * i, n1 = idx >> 1, h = idx & 1;
-            const float2 a = sm.col[2 * h][n1], d = sm.col[2 * h + 1][n1];
-            *reinterpret_cast<float4 *>(Bv + (size_t)n1 * N + col0 + 2 * h) =
-                make_float4(a.x, a.y, d.x, d.y);
+        for (int j = 0; j < 4; ++j) {
+            const int rp = ht + 128 * j;  // rows 2 rp, 2 rp + 1
+            const float4 a0 = s00[rp], a1 = s01[rp], b0 = s10[rp], b1 = s11[rp];
+            const float2 p0 = padd(make_float2(a0.x, a0.y), make_float2(a1.x, a1.y));
+            const float2 q0 = padd(make_float2(b0.x, b0.y), make_float2(b1.x, b1.y));
+            const float2 p1 = padd(make_float2(a0.z, a0.w), make_float2(a1.z, a1.w));
+            const float2 q1 = padd(make_float2(b0.z, b0.w), make_float2(b1.z, b1.w));
+            *reinterpret_cast<float4 *>(Bv + (size_t)(2 * rp) * N) = make_float4(p0.x, p0.y, q0.x, q0.y);
+            *reinterpret_cast<float4 *>(Bv + (size_t)(2 * rp + 1) * N) =
+                make_float4(p1.x, p1.y, q1.x, q1.y);
         }
-        __syncthreads();  // col / xch reusable, next tile visible
-        tb ^= 1;
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&sm.rdone[half]);
+        SFDW_STAMP(3);
     }
+    if (PP && half == 0) turn_begin(turns);  // absorbs the last token
 }
 
 // ---- pass x: one row of B per warp pair -----------------------------------------------------------
-constexpr int XP = 4;  // pairs per CTA
+constexpr int WX = SFDW_WX;  // warps per CTA
+constexpr int XP = WX / 2;   // pairs per CTA = rows in flight per CTA
 struct SmemX {
-    float2 xb[2 * XP][XB];
-    float2 xch[XP][2][2][512];   // [pair][line parity][destination warp][16 x 32]
-    float2 inb[XP][2][N];        // [pair][line parity] input row (bulk async copy destination)
-    unsigned long long bar[XP][2];
+    float2 xb[WX][XB];
+    float2 tabs[2][TABS];  // tables of the (at most two) views this CTA's rows belong to
+    float2 tw[32 * 32];
+    float2 inb[XP][N];  // input row of each pair (bulk async copy destination)
+    unsigned long long ibar[XP];
+    unsigned long long tbar[2];
 };
 
-// tabX: [V][4][N] = pre b0 | pre b1 | post b0 | post b1;  H2: [V][2][N].
+// Work unit = (view, group of XP adjacent rows); a CTA takes a contiguous range of units, so all
+// its pairs are always in the same view.  tabX: [V][2][3][N].
 template <int B>
 __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict__ Bin,
                                             const float2 *__restrict__ tabX,
-                                            const float2 *__restrict__ H2, const float2 (&tw)[32],
-                                            float2 *__restrict__ field, float *__restrict__ inten,
-                                            unsigned int *vmax, int V) {
+                                            const float2 (&tw)[TWN], float2 *__restrict__ field,
+                                            float *__restrict__ inten, unsigned int *vmax, int V) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, pair = warp >> 1;
-    const int lines = V * N, G = gridDim.x * XP;
-    int line = blockIdx.x * XP + pair;
-    if (line >= lines) return;
+    constexpr int gpv = (N + XP - 1) / XP;  // units per view
+    const int units = V * gpv;
+    const int u0 = (int)((long long)units * blockIdx.x / gridDim.x);
+    const int u1 = (int)((long long)units * (blockIdx.x + 1) / gridDim.x);
+    if (u0 >= u1) return;  // CTA-uniform
     float2 *xb = sm.xb[warp];
+    const float2 *xbp = sm.xb[warp ^ 1];
+    const float2 *in = sm.inb[pair] + lane;
     const bool issuer = B == 0 && lane == 0;
-    if (issuer) bulk_load(sm.inb[pair][0], Bin + (size_t)line * N, N * sizeof(float2), &sm.bar[pair][0]);
-    float2 P[32];
-    fetch(P, tabX + (size_t)(line / N) * 4 * N + B * N, lane);
-    for (int it = 0; line < lines; line += G, ++it) {
-        const int buf = it & 1, view = line / N, next = line + G;
-        const bool has_next = next < lines;
-        if (has_next && issuer)
-            bulk_load(sm.inb[pair][buf ^ 1], Bin + (size_t)next * N, N * sizeof(float2),
-                      &sm.bar[pair][buf ^ 1]);
-        mbar_wait(&sm.bar[pair][buf], (it >> 1) & 1);
+    // The launcher sizes the grid so that a CTA's rows lie in at most two views: both table sets
+    // are requested up front and a warp waits for a set the first time it needs it; no CTA-wide
+    // barrier exists in this kernel.
+    const int view0 = u0 / gpv;
+    if (threadIdx.x == 0) {
+        bulk_load(sm.tabs[0], tabX + (size_t)view0 * TABS, TABS * sizeof(float2), &sm.tbar[0]);
+        if ((u1 - 1) / gpv != view0)
+            bulk_load(sm.tabs[1], tabX + (size_t)(view0 + 1) * TABS, TABS * sizeof(float2),
+                      &sm.tbar[1]);
+    }
+    const float2 *tb_pre = nullptr;
+    int cur_view = -1;
+    unsigned iphase = 0;
+    bool pending = false;  // the pair's input row is already on its way
+    // turn-taking of warps w and w + 4 (needs every warp of the CTA to run the same number of
+    // lines: XP divides N); barrier ids 0 = CTA, 1..XP = pairs, then two per sub-partition
+    constexpr bool PP = SFDW_PINGPONG != 0 && WX == 8;
+    const Turns turns{XP + 1 + 2 * (warp & 3) + (warp >> 2), XP + 1 + 2 * (warp & 3) + 1 - (warp >> 2), PP};
+    // The first turn belongs to warps 0..3, and warps 4..7 pass on their first one: this puts the
+    // long memory phase of a warp (exchange, stores, next input, between its turns 3 and 1) beside
+    // the other warp's double turn 2 and the two short ones (transposes) beside turns 3 and 1.
+    if (PP && (warp >> 2) == 1) {
+        turn_end(turns);
+#if SFDW_PP_SKEW
+        turn_begin(turns);
+        turn_end(turns);
+#endif
+    }
+    for (int u = u0; u < u1; ++u) {
+        const int view = u / gpv, line = (u % gpv) * XP + pair;
+        if (line >= N) continue;  // pair-uniform (ragged last group of a view when XP does not divide N)
+        if (view != cur_view) {
+            mbar_wait(&sm.tbar[view - view0], 0);
+            tb_pre = sm.tabs[view - view0] + B * 3 * N + lane;
+            cur_view = view;
+        }
+        const size_t row = (size_t)view * N + line;
+#ifdef SFDW_TRACE
+        long long *tr = g_trace + (((size_t)blockIdx.x * WX + warp) * 16 + (u - u0)) * 16;
+#endif
+        SFDW_STAMP(0);
+        if (!pending && issuer)
+            bulk_load(sm.inb[pair], Bin + row * N, N * sizeof(float2), &sm.ibar[pair]);
+        const int nu = u + 1, nline = (nu % gpv) * XP + pair;
+        const bool has_next = nu < u1 && nline < N;
+        mbar_wait(&sm.ibar[pair], iphase);
+        iphase ^= 1;
+        SFDW_STAMP(1);
         float2 v[32];
 #pragma unroll
-        for (int r = 0; r < 32; ++r) v[r] = cmul(sm.inb[pair][buf][lane + 32 * r], P[r]);
-        fetch(P, H2 + (size_t)view * 2 * N + B * N, lane);
-        branch(v, P, lane, xb, tw, tabX + (size_t)view * 4 * N + 2 * N + B * N);
-        if (has_next) fetch(P, tabX + (size_t)(next / N) * 4 * N + B * N, lane);
-        add_halves<B>(v, sm.xch[pair][buf], lane, pair);
+        for (int r = 0; r < 32; ++r) v[r] = cmul(in[32 * r], tb_pre[32 * r]);
+        SFDW_STAMP(2);
+        // both warps have consumed the input row and finished with each other's transpose tile
+        pair_sync(pair);
+        SFDW_STAMP(3);
+        if (has_next && issuer) {
+            fence_async_smem();
+            bulk_load(sm.inb[pair], Bin + ((size_t)(nu / gpv) * N + nline) * N, N * sizeof(float2),
+                      &sm.ibar[pair]);
+        }
+        pending = has_next;
+#ifdef SFDW_TRACE
+        branch(v, lane, xb, tw, sm.tw, tb_pre + N, turns, tr);
+#else
+        branch(v, lane, xb, tw, sm.tw, tb_pre + N, turns);
+#endif
+        add_halves<B>(v, xb, xbp, lane, pair);
+        SFDW_STAMP(8);
         float mx = 0.f;
-        const size_t off = (size_t)line * N;
+        const size_t off = row * N;
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
             const int m1 = lane + 32 * (16 * B + q);
-            const float2 u = v[16 * B + q];
-            if (field) field[off + m1] = u;
-            const float I = u.x * u.x + u.y * u.y;
+            const float2 w = v[16 * B + q];
+            if (field) field[off + m1] = w;
+            const float I = w.x * w.x + w.y * w.y;
             if (inten) inten[off + m1] = I;
             mx = fmaxf(mx, I);
         }
@@ -413,6 +572,14 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
             // intensities are >= 0, so their float bit patterns order like unsigned integers
             if (lane == 0) atomicMax(vmax + view, __float_as_uint(mx));
         }
+        SFDW_STAMP(9);
+    }
+    if (PP && (warp >> 2) == 0) {  // absorb the tokens still in flight
+        turn_begin(turns);
+#if SFDW_PP_SKEW
+        turn_end(turns);
+        turn_begin(turns);
+#endif
     }
 }
 
