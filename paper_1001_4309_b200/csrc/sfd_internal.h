@@ -43,6 +43,8 @@ struct sfd_plan {
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     bool ev_valid = false, ev_quant = false;
     sfd_stream_state *ss = nullptr;
+    // CUtensorMap of B (bulk stores of the N = 1024 pass y), built by sfd_make_tensormaps
+    alignas(64) unsigned char tmapB[128] = {};
 };
 
 // Enqueue the kernels of one reconstruction on `st` (sfd_kernels.cu).  `u8` non-NULL selects the
@@ -52,3 +54,5 @@ cudaError_t sfd_launch(sfd_plan *p, const void *holo, float2 *field, float *inte
 // One-time per-process kernel attribute set-up (dynamic shared memory opt-in).
 cudaError_t sfd_kernels_init();
 void sfd_count_launch(int n);
+// Builds the plan's tensor maps (after B is allocated; no-op when the fast path is not in use).
+cudaError_t sfd_make_tensormaps(sfd_plan *p);

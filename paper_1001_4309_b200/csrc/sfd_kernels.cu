@@ -8,6 +8,8 @@
 // plus, in the 8-bit mode (step (xi), reading 15), k_quantise.
 // The per-thread arithmetic lives in sfd_fft_core.cuh.  For N = 1024 the same two passes run as the
 // persistent kernels k_cols_1024 / k_rows_1024 (one warp pair per line, sfd_warp1024.cuh).
+#include <cuda.h>  // CUtensorMap (types only: the encoder is fetched through the runtime)
+
 #include <atomic>
 
 #include "sfd_fft_core.cuh"
@@ -83,15 +85,15 @@ k_quantise(const float4 *__restrict__ inten, const unsigned int *__restrict__ vm
 template <typename TIn>
 __global__ void __launch_bounds__(sfdw::WY * 32, 1)
 k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
-            const float2 *__restrict__ twl, float2 *__restrict__ B, unsigned int *vmax, int V) {
+            const float2 *__restrict__ twl, const __grid_constant__ CUtensorMap tmB,
+            unsigned int *vmax, int V) {
     extern __shared__ float4 smem4[];
     sfdw::SmemY<TIn> &sm = *reinterpret_cast<sfdw::SmemY<TIn> *>(smem4);
     if (vmax != nullptr && blockIdx.x == 0 && threadIdx.x < V) vmax[threadIdx.x] = 0u;
     if (threadIdx.x == 0) {
         sfdw::mbar_init(&sm.tbar[0], 1);
         sfdw::mbar_init(&sm.tbar[1], 1);
-        sfdw::mbar_init(&sm.rdone[0], 4);
-        sfdw::mbar_init(&sm.rdone[1], 4);
+        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], 1);
         sfdw::mbar_fence_init();
     }
     if (!sfdw::TWR)
@@ -100,9 +102,9 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
     __syncthreads();
     if (((threadIdx.x >> 5) & 1) == 0)
-        sfdw::pass_y_loop<TIn, 0>(sm, holo, tabY, tw, B, V);
+        sfdw::pass_y_loop<TIn, 0>(sm, holo, tabY, tw, &tmB, V);
     else
-        sfdw::pass_y_loop<TIn, 1>(sm, holo, tabY, tw, B, V);
+        sfdw::pass_y_loop<TIn, 1>(sm, holo, tabY, tw, &tmB, V);
 }
 
 __global__ void __launch_bounds__(sfdw::WX * 32, 1)
@@ -115,6 +117,7 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
         for (int i = 0; i < sfdw::XP; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
         sfdw::mbar_init(&sm.tbar[0], 1);
         sfdw::mbar_init(&sm.tbar[1], 1);
+        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], 1);
         sfdw::mbar_fence_init();
     }
     if (!sfdw::TWR)
@@ -145,12 +148,13 @@ cudaError_t launch_warp1024(sfd_plan *p, const void *holo, float2 *field, float 
     // one CTA per SM, but at least V CTAs: a CTA's contiguous range of items (rows) then touches at
     // most two views (the kernels hold two table sets)
     const int gy = V > g_sms ? V : g_sms;
+    const CUtensorMap &tmB = *reinterpret_cast<const CUtensorMap *>(p->tmapB);
     if (d.in_dtype == 0)
         k_cols_1024<unsigned char><<<gy, sfdw::WY * 32, sizeof(sfdw::SmemY<unsigned char>), st>>>(
-            (const unsigned char *)holo, d.w_tabY, d.w_twl, d.B, vmax, V);
+            (const unsigned char *)holo, d.w_tabY, d.w_twl, tmB, vmax, V);
     else
         k_cols_1024<float><<<gy, sfdw::WY * 32, sizeof(sfdw::SmemY<float>), st>>>(
-            (const float *)holo, d.w_tabY, d.w_twl, d.B, vmax, V);
+            (const float *)holo, d.w_tabY, d.w_twl, tmB, vmax, V);
     if (timing) cudaEventRecord(p->ev[1], st);
     const int gx = gy;
     k_rows_1024<<<gx, sfdw::WX * 32, sizeof(sfdw::SmemX), st>>>(d.B, d.w_tabX, d.w_twl, field, inten,
@@ -219,6 +223,32 @@ cudaError_t launch_t(sfd_plan *p, const void *holo, float2 *field, float *inten,
 
 }  // namespace
 
+// Tensor map of the intermediate B for the bulk stores of k_cols_1024: B as float [V * N][2 N],
+// box = 4 floats (two complex columns) x YBOX rows, no swizzle.  The encoder is a driver entry
+// point; it is fetched through the runtime so that the library does not link libcuda.
+cudaError_t sfd_make_tensormaps(sfd_plan *p) {
+    static_assert(sizeof(CUtensorMap) <= sizeof(p->tmapB), "tensor map storage");
+    if (p->d.N != sfdw::N || p->d.w_twl == nullptr) return cudaSuccess;
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
+                                  const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                  const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
+    if (e != cudaSuccess) return e;
+    if (fn == nullptr || qr != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+    const cuuint64_t dims[2] = {2ull * sfdw::N, (cuuint64_t)p->d.V * sfdw::N};
+    const cuuint64_t strides[1] = {2ull * sfdw::N * sizeof(float)};
+    const cuuint32_t box[2] = {4, sfdw::YBOX};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = ((encode_fn)fn)(
+        reinterpret_cast<CUtensorMap *>(p->tmapB), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, p->d.B, dims,
+        strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+        CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
 void sfd_count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 long long sfd_launch_count_impl() { return g_launches.load(std::memory_order_relaxed); }
 
@@ -243,10 +273,10 @@ cudaError_t sfd_kernels_init() {
 
 cudaError_t sfd_launch(sfd_plan *p, const void *holo, float2 *field, float *inten,
                        unsigned char *u8, cudaStream_t st) {
-    // N = 1024: warp-pair-per-line kernels (their tile loads read 4 hologram samples at once: the
-    // hologram must be aligned to 4 samples)
+    // N = 1024: warp-pair-per-line kernels (their slab loads read 8 bytes of a hologram row at once:
+    // the hologram must be aligned accordingly)
     if (p->d.N == sfdw::N && p->kernels != SFD_KERNELS_GENERIC && p->d.w_twl != nullptr &&
-        (reinterpret_cast<size_t>(holo) & (p->d.in_dtype == 0 ? 3 : 15)) == 0)
+        (reinterpret_cast<size_t>(holo) & (p->d.in_dtype == 0 ? 7 : 15)) == 0)
         return launch_warp1024(p, holo, field, inten, u8, st);
     switch (p->d.log2M) {
         case 7: return launch_t<7>(p, holo, field, inten, u8, st);

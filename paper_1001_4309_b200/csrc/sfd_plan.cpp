@@ -351,6 +351,7 @@ int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const dou
     }
     for (int v = 0; v < n_views; ++v)
         if ((rc = upload_view(p, v)) != SFD_OK) return fail(rc);
+    if ((e = sfd_make_tensormaps(p)) != cudaSuccess) return fail(cuda_fail(e, "cuTensorMapEncodeTiled"));
     for (int i = 0; i < 4; ++i)
         if ((e = cudaEventCreate(&p->ev[i])) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
     *out = p;

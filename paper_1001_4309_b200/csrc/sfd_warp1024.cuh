@@ -145,9 +145,6 @@ template <int DIR> __device__ __forceinline__ void dft32(float2 (&a)[32]) {
 #ifndef SFDW_PINGPONG
 #define SFDW_PINGPONG 1  // 1: warps sharing a sub-partition take turns in the butterfly phases (pass x)
 #endif
-#ifndef SFDW_PP_SKEW
-#define SFDW_PP_SKEW 0
-#endif
 #ifndef SFDW_ROLLED
 #define SFDW_ROLLED 1  // 1: the two radix-32 stages / two FFTs of a branch share one copy of the code
 #endif
@@ -157,7 +154,8 @@ template <int DIR> __device__ __forceinline__ void dft32(float2 (&a)[32]) {
 #define SFDW_LOOP _Pragma("unroll")
 #endif
 #ifdef SFDW_TRACE
-__device__ long long *g_trace;  // [cta][warp][line slot][16] clock stamps (experiments only)
+__device__ long long *g_trace;  // [pass][cta][warp][16 line slots][32] clock stamps (experiments only)
+constexpr size_t TRACE_PASS = (size_t)148 * 8 * 16 * 32;
 __device__ __forceinline__ void stamp(long long *tr, int i) {
     if ((threadIdx.x & 31) == 0) tr[i] = clock64();
 }
@@ -228,18 +226,60 @@ constexpr int TABS = 2 * 3 * N;  // complex elements
 // between them (transposes, table and input reads, exchange, stores) use the SM-wide shared-memory
 // pipe; left alone, all warps of an SM drift into the same phase and the two kinds of phase run
 // one after the other instead of side by side.  A warp therefore enters a butterfly phase only
-// when it holds its sub-partition's token (named barrier `mine`, armed by the other warp) and
-// passes the token on (`theirs`) when the phase ends: one warp of each sub-partition is always in
-// butterflies while the other does its memory phase.
+// when it holds its sub-partition's token and passes the token on when the phase ends: one warp
+// of each sub-partition is in butterflies while the other does its memory phase.
+// The token is a pair of mbarriers (count 1): `mine` completes a phase when the other warp ends
+// its turn, `theirs` is the other warp's.  (bar.arrive / bar.sync on a named barrier with a count
+// of 64 does NOT do this on sm_100: measured, the syncing warp is released at once.)
 struct Turns {
-    int mine, theirs;  // named-barrier ids
+    unsigned mine, theirs;  // shared-memory addresses of the two mbarriers
+    unsigned phase;         // parity of the next completion of `mine` this warp waits for
     bool on;
 };
-__device__ __forceinline__ void turn_begin(const Turns &t) {
-    if (t.on) asm volatile("bar.sync %0, 64;" ::"r"(t.mine) : "memory");
+__device__ __forceinline__ void turn_begin(Turns &t) {
+    if (t.on) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "W_%=:\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+            "@p bra D_%=;\n"
+            "bra W_%=;\n"
+            "D_%=:\n"
+            "}\n" ::"r"(t.mine),
+            "r"(t.phase)
+            : "memory");
+        t.phase ^= 1u;
+    }
 }
 __device__ __forceinline__ void turn_end(const Turns &t) {
-    if (t.on) asm volatile("bar.arrive %0, 64;" ::"r"(t.theirs) : "memory");
+    if (t.on) {
+        __syncwarp();
+        if ((threadIdx.x & 31) == 0)
+            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(t.theirs) : "memory");
+    }
+}
+// Warps 0..3 own the first turn; warps 4..7 pass on their first one and warps 0..3 add one after
+// their last line, so that both warps of a sub-partition take the same number of turns.  The
+// passed turn shifts the two by one: the long memory phase of a warp (exchange, stores, next
+// input, between its turns 3 and 1) lies beside the other warp's double turn 2, the two short
+// ones (transposes) beside turns 3 and 1.
+__device__ __forceinline__ Turns turns_make(unsigned long long *bars, int warp, bool on) {
+    const int sp = warp & 3, up = warp >> 2;
+    return Turns{smem_u32(bars + 2 * sp + up), smem_u32(bars + 2 * sp + 1 - up), 0u, on};
+}
+__device__ __forceinline__ void turns_open(Turns &t, int warp) {
+    if ((warp >> 2) == 1) {
+        turn_end(t);
+        turn_begin(t);
+        turn_end(t);
+    }
+}
+__device__ __forceinline__ void turns_close(Turns &t, int warp) {
+    if ((warp >> 2) == 0) {
+        turn_begin(t);
+        turn_end(t);
+    }
 }
 
 // One branch of a line, in place (the caller has applied pre): forward FFT, x H_b, inverse FFT,
@@ -254,15 +294,16 @@ __device__ __forceinline__ void turn_end(const Turns &t) {
 // three turns of the line.  On return v = this warp's partial sums for all 1024 outputs.
 __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
                                        const float2 (&tw)[TWN], const float2 *twsm,
-                                       const float2 *t, const Turns &turns
+                                       const float2 *t, Turns &turns
 #ifdef SFDW_TRACE
                                        , long long *tr
 #endif
 ) {
     SFDW_LOOP
     for (int step = 0; step < 4; ++step) {
+        SFDW_STAMP(16 + 4 * step + 3);
         if (step != 2) turn_begin(turns);
-        SFDW_STAMP(step == 0 ? 10 : step == 1 ? 12 : 14);
+        SFDW_STAMP(16 + 4 * step);
         dft32<-1>(v);
         if (step & 1) {
 #pragma unroll
@@ -270,7 +311,7 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
                 const float2 h = t[(step >> 1) * N + 32 * k], a = v[k];
                 v[k] = make_float2(a.x * h.x - a.y * h.y, -(a.x * h.y) - a.y * h.x);
             }
-            SFDW_STAMP(15);
+            SFDW_STAMP(16 + 4 * step + 1);
             if (step != 1) turn_end(turns);
         } else {
 #pragma unroll
@@ -280,7 +321,7 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
                 else
                     v[k] = cmul(v[k], twsm[k * 32 + lane]);
             }
-            SFDW_STAMP(step == 0 ? 11 : 13);
+            SFDW_STAMP(16 + 4 * step + 1);
             turn_end(turns);
 #pragma unroll
             for (int k = 0; k < 32; ++k) xb[k * XS + lane] = v[k];  // (k1 = k, n2 = lane)
@@ -294,7 +335,7 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
             }
             __syncwarp();
         }
-        SFDW_STAMP(4 + step);
+        SFDW_STAMP(16 + 4 * step + 2);
     }
 }
 
@@ -318,35 +359,64 @@ __device__ __forceinline__ void add_halves(float2 (&v)[32], float2 *mine, const 
 // half h transforms columns col0 + 2h and col0 + 2h + 1 of the CTA's current item.  Nothing
 // synchronises the two halves with each other except the turn-taking of the warps that share a
 // sub-partition (warps w and w + 4).
+//
+// Write-out.  B is [n1][m0] and a column's outputs are one element per row: written by the LSU
+// that is one 128-byte wavefront per row and store instruction (the v5 profile: 28 % of the
+// data-pipe time of this kernel).  Instead the warps of a half put their final sums into a dense
+// staging tile [n1][2 columns] (16 bytes per row) and one thread hands the tile to the TMA unit
+// (cp.async.bulk.tensor, shared -> global, four boxes of 256 rows x 16 bytes): the scatter costs the
+// LSU pipe nothing and runs beside the next item's butterflies.
 constexpr int WY = 8;  // warps per CTA
 constexpr int YC = 4;  // columns per item
-template <typename TIn> struct TileElem { using type = unsigned short; };  // 2 uint8 columns of a row
-template <> struct TileElem<float> { using type = float2; };               // 2 float columns of a row
+constexpr int YBOX = 256;  // rows of one TMA store box (the tensor map is built with this box)
+// Input slab of a half: SLAB_BYTES = 8 bytes of every hologram row = 2 columns x IPS items.  Half h
+// of item (slab s, k) transforms columns YC IPS s + 2 IPS h + 2 k + {0, 1}: the half reads its slab
+// once per IPS items with one 8-byte load per row (a 2-byte load per row and item costs the LSU one
+// wavefront per row just the same) and keeps it in shared memory as [k][n0] column pairs.
+template <typename TIn> struct TileElem {            // uint8: 4 items per slab
+    using type = unsigned short;                     // 2 uint8 columns of a row
+    using slab = uint2;
+    static constexpr int IPS = 4;
+};
+template <> struct TileElem<float> {                 // float: 1 item per slab
+    using type = float2;                             // 2 float columns of a row
+    using slab = float2;
+    static constexpr int IPS = 1;
+};
 template <typename TIn> struct SmemY {
     float2 xb[WY][XB];
     float2 tabs[2][TABS];  // tables of the (at most two) views this CTA's items belong to
-    float2 tw[32 * 32];
-    typename TileElem<TIn>::type tile[2][2][N];  // [half][buffer][n0]: the half's two input columns
+    alignas(128) float2 stage[2][N][2];  // [half][n1][column of the half]: final sums, TMA store source
+    float2 tw[TWR ? 1 : 32 * 32];
+    typename TileElem<TIn>::type tile[2][TileElem<TIn>::IPS][N];  // [half][k][n0]: the half's slab
     unsigned long long tbar[2];
-    unsigned long long rdone[2];  // per half: the read-out of the previous item has left the tiles
+    unsigned long long turn[8];
 };
 
-template <typename TIn> struct TileRegs { typename TileElem<TIn>::type e[8]; };
+template <typename TIn> struct TileRegs { typename TileElem<TIn>::slab e[8]; };
 
-// the 128 threads of a half fetch rows ht, ht + 128, .. of columns colh, colh + 1
+// the 128 threads of a half fetch rows ht, ht + 128, .. of the slab that starts at column col
 template <typename TIn>
-__device__ __forceinline__ void tile_load(TileRegs<TIn> &t, const TIn *__restrict__ holo, int colh,
+__device__ __forceinline__ void tile_load(TileRegs<TIn> &t, const TIn *__restrict__ holo, int col,
                                           int ht) {
 #pragma unroll
     for (int i = 0; i < 8; ++i)
-        t.e[i] = __ldg(reinterpret_cast<const typename TileElem<TIn>::type *>(
-            holo + (size_t)(ht + 128 * i) * N + colh));
+        t.e[i] = __ldg(reinterpret_cast<const typename TileElem<TIn>::slab *>(
+            holo + (size_t)(ht + 128 * i) * N + col));
 }
-template <typename TIn>
-__device__ __forceinline__ void tile_store(const TileRegs<TIn> &t,
-                                           typename TileElem<TIn>::type *tile, int ht) {
+__device__ __forceinline__ void tile_store(const TileRegs<unsigned char> &t,
+                                           unsigned short (*tile)[N], int ht) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) tile[ht + 128 * i] = t.e[i];
+    for (int i = 0; i < 8; ++i) {
+        tile[0][ht + 128 * i] = (unsigned short)(t.e[i].x & 0xffffu);
+        tile[1][ht + 128 * i] = (unsigned short)(t.e[i].x >> 16);
+        tile[2][ht + 128 * i] = (unsigned short)(t.e[i].y & 0xffffu);
+        tile[3][ht + 128 * i] = (unsigned short)(t.e[i].y >> 16);
+    }
+}
+__device__ __forceinline__ void tile_store(const TileRegs<float> &t, float2 (*tile)[N], int ht) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) tile[0][ht + 128 * i] = t.e[i];
 }
 __device__ __forceinline__ float tile_value(unsigned short e, int c) {
     return (float)((e >> (8 * c)) & 0xffu);
@@ -356,21 +426,31 @@ __device__ __forceinline__ float tile_value(float2 e, int c) { return c ? e.y : 
 __device__ __forceinline__ void half_sync(int half) {  // named barrier of the four warps of a half
     asm volatile("bar.sync %0, 128;" ::"r"(half + 1) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(unsigned long long *bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+// 2-D tiled bulk store shared -> global through tensor map `tm` (box fixed by the map); c0 = float
+// index within the row of B, c1 = row of B (view * N + n1)
+__device__ __forceinline__ void tma_store_2d(const void *tm, const void *src, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(tm),
+        "r"(smem_u32(src)), "r"(c0), "r"(c1)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// all earlier bulk stores of this thread have finished READING shared memory
+__device__ __forceinline__ void bulk_wait_read() {
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
 // Persistent CTA of 256 threads: work item = (view, group of 4 columns); a CTA takes a contiguous
 // range of items (at most two views: the launcher sizes the grid accordingly).
-// tabY: [V][2][3][N] (post carries c0, pre the 1/255 of uint8 input); Bout: [V][N][N].
-// A warp leaves the partial sums of its branch for all 1024 outputs of its column in its own
-// transpose tile (idle by then); after the half's barrier the 128 threads of the half add the two
-// branches and write 16-byte row chunks B[n1][colh .. colh+1].
+// tabY: [V][2][3][N] (post carries c0, pre the 1/255 of uint8 input); tmB: tensor map of B seen as
+// float [V * N][2 N] with box 4 x YBOX.
+// Per item a warp (column c of its half, branch B) transforms its column, hands the half of the
+// outputs it does not finish to its partner through its own transpose tile (idle by then), adds
+// what the partner left for it and writes 16 final values per thread into the staging tile.
 template <typename TIn, int B>
 __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restrict__ holo,
                                             const float2 *__restrict__ tabY,
-                                            const float2 (&tw)[TWN], float2 *__restrict__ Bout,
-                                            int V) {
+                                            const float2 (&tw)[TWN], const void *tmB, int V) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int half = warp >> 2, c = (warp >> 1) & 1, ht = threadIdx.x & 127;
     constexpr int groups = N / YC;
@@ -379,6 +459,9 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
     const int i1 = (int)((long long)items * (blockIdx.x + 1) / gridDim.x);
     if (i0 >= i1) return;  // CTA-uniform
     float2 *xb = sm.xb[warp];
+    const float2 *xbp = sm.xb[warp ^ 1];
+    float2 *stg = &sm.stage[half][0][0];
+    const bool leader = ht == 0;  // issues and retires the half's bulk stores
     const int view0 = i0 / groups;
     if (threadIdx.x == 0) {
         bulk_load(sm.tabs[0], tabY + (size_t)view0 * TABS, TABS * sizeof(float2), &sm.tbar[0]);
@@ -386,76 +469,73 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
             bulk_load(sm.tabs[1], tabY + (size_t)(view0 + 1) * TABS, TABS * sizeof(float2),
                       &sm.tbar[1]);
     }
+    constexpr int IPS = TileElem<TIn>::IPS;
+    static_assert(groups % IPS == 0, "a slab never straddles two views");
     {
         TileRegs<TIn> t;
-        tile_load<TIn>(t, holo, (i0 % groups) * YC + 2 * half, ht);
-        tile_store<TIn>(t, sm.tile[half][0], ht);
+        tile_load<TIn>(t, holo, (i0 % groups) / IPS * (YC * IPS) + 2 * IPS * half, ht);
+        tile_store(t, sm.tile[half], ht);
     }
     half_sync(half);
     constexpr bool PP = SFDW_PINGPONG != 0;
-    const Turns turns{3 + 2 * (warp & 3) + half, 3 + 2 * (warp & 3) + 1 - half, PP};
-    if (PP && half == 1) turn_end(turns);  // the first turn belongs to warps 0..3
+    Turns turns = turns_make(sm.turn, warp, PP);
+    turns_open(turns, warp);
     const float2 *tb_pre = nullptr;
     int cur_view = -1;
     for (int item = i0; item < i1; ++item) {
-        const int it = item - i0, tb = it & 1;
-        const int view = item / groups, colh = (item % groups) * YC + 2 * half;
+        const int view = item / groups, g = item % groups, k = g % IPS;
+        const int colh = g / IPS * (YC * IPS) + 2 * IPS * half + 2 * k;
         if (view != cur_view) {
             mbar_wait(&sm.tbar[view - view0], 0);
             tb_pre = sm.tabs[view - view0] + B * 3 * N + lane;
             cur_view = view;
         }
-        const bool has_next = item + 1 < i1;
+        const bool has_next = item + 1 < i1 && k == IPS - 1;  // the next item opens a new slab
 #ifdef SFDW_TRACE
-        long long *tr = g_trace + (((size_t)blockIdx.x * WY + warp) * 16 + it) * 16;
+        long long *tr = g_trace + (((size_t)blockIdx.x * WY + warp) * 16 + (item - i0)) * 32;
 #endif
         SFDW_STAMP(0);
         TileRegs<TIn> t;
-        if (has_next) tile_load<TIn>(t, holo, ((item + 1) % groups) * YC + 2 * half, ht);
+        if (has_next)
+            tile_load<TIn>(t, holo, ((item + 1) % groups) / IPS * (YC * IPS) + 2 * IPS * half, ht);
         float2 v[32];
 #pragma unroll
         for (int r = 0; r < 32; ++r) {
-            const float a = tile_value(sm.tile[half][tb][lane + 32 * r], c);
+            const float a = tile_value(sm.tile[half][k][lane + 32 * r], c);
             const float2 p = tb_pre[32 * r];
             v[r] = make_float2(a * p.x, a * p.y);
         }
-        // the previous item's read-out must have left the transpose tiles before they are written
         SFDW_STAMP(1);
-        if (it > 0) mbar_wait(&sm.rdone[half], (it - 1) & 1);
-        SFDW_STAMP(2);
 #ifdef SFDW_TRACE
         branch(v, lane, xb, tw, sm.tw, tb_pre + N, turns, tr);
 #else
         branch(v, lane, xb, tw, sm.tw, tb_pre + N, turns);
 #endif
-#pragma unroll
-        for (int r = 0; r < 32; ++r) xb[r * 32 + lane] = v[r];  // element n1 = lane + 32 r at n1
-        if (has_next) tile_store<TIn>(t, sm.tile[half][tb ^ 1], ht);
         SFDW_STAMP(8);
-        half_sync(half);  // partial sums complete, next input tile visible
-        SFDW_STAMP(9);
-        const float4 *s00 = reinterpret_cast<const float4 *>(sm.xb[4 * half + 0]);
-        const float4 *s01 = reinterpret_cast<const float4 *>(sm.xb[4 * half + 1]);
-        const float4 *s10 = reinterpret_cast<const float4 *>(sm.xb[4 * half + 2]);
-        const float4 *s11 = reinterpret_cast<const float4 *>(sm.xb[4 * half + 3]);
-        float2 *Bv = Bout + (size_t)view * N * N + colh;
+        // the previous item's bulk stores must have left the staging tile before it is rewritten
+        if (leader) bulk_wait_read();
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const int rp = ht + 128 * j;  // rows 2 rp, 2 rp + 1
-            const float4 a0 = s00[rp], a1 = s01[rp], b0 = s10[rp], b1 = s11[rp];
-            const float2 p0 = padd(make_float2(a0.x, a0.y), make_float2(a1.x, a1.y));
-            const float2 q0 = padd(make_float2(b0.x, b0.y), make_float2(b1.x, b1.y));
-            const float2 p1 = padd(make_float2(a0.z, a0.w), make_float2(a1.z, a1.w));
-            const float2 q1 = padd(make_float2(b0.z, b0.w), make_float2(b1.z, b1.w));
-            *reinterpret_cast<float4 *>(Bv + (size_t)(2 * rp) * N) = make_float4(p0.x, p0.y, q0.x, q0.y);
-            *reinterpret_cast<float4 *>(Bv + (size_t)(2 * rp + 1) * N) =
-                make_float4(p1.x, p1.y, q1.x, q1.y);
+        for (int q = 0; q < 16; ++q) xb[q * 32 + lane] = v[16 * (1 - B) + q];
+        half_sync(half);  // partner's hand-over visible; staging tile and input tile free
+        SFDW_STAMP(9);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const float2 w = padd(v[16 * B + q], xbp[q * 32 + lane]);
+            stg[(lane + 32 * (16 * B + q)) * 2 + c] = w;
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&sm.rdone[half]);
+        if (has_next) tile_store(t, sm.tile[half], ht);
+        fence_async_smem();  // staging writes -> async proxy
+        half_sync(half);     // staging tile complete, next input tile visible, hand-over tiles free
+        if (leader) {
+#pragma unroll
+            for (int j = 0; j < N / YBOX; ++j)
+                tma_store_2d(tmB, stg + j * YBOX * 2, 2 * colh, view * N + j * YBOX);
+            bulk_commit();
+        }
         SFDW_STAMP(3);
     }
-    if (PP && half == 0) turn_begin(turns);  // absorbs the last token
+    if (leader) bulk_wait_read();  // shared memory must outlive the last store's reads
+    turns_close(turns, warp);
 }
 
 // ---- pass x: one row of B per warp pair -----------------------------------------------------------
@@ -468,6 +548,7 @@ struct SmemX {
     float2 inb[XP][N];  // input row of each pair (bulk async copy destination)
     unsigned long long ibar[XP];
     unsigned long long tbar[2];
+    unsigned long long turn[8];
 };
 
 // Work unit = (view, group of XP adjacent rows); a CTA takes a contiguous range of units, so all
@@ -502,19 +583,10 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
     unsigned iphase = 0;
     bool pending = false;  // the pair's input row is already on its way
     // turn-taking of warps w and w + 4 (needs every warp of the CTA to run the same number of
-    // lines: XP divides N); barrier ids 0 = CTA, 1..XP = pairs, then two per sub-partition
-    constexpr bool PP = SFDW_PINGPONG != 0 && WX == 8;
-    const Turns turns{XP + 1 + 2 * (warp & 3) + (warp >> 2), XP + 1 + 2 * (warp & 3) + 1 - (warp >> 2), PP};
-    // The first turn belongs to warps 0..3, and warps 4..7 pass on their first one: this puts the
-    // long memory phase of a warp (exchange, stores, next input, between its turns 3 and 1) beside
-    // the other warp's double turn 2 and the two short ones (transposes) beside turns 3 and 1.
-    if (PP && (warp >> 2) == 1) {
-        turn_end(turns);
-#if SFDW_PP_SKEW
-        turn_begin(turns);
-        turn_end(turns);
-#endif
-    }
+    // lines: XP divides N)
+    constexpr bool PP = SFDW_PINGPONG != 0 && WX == 8 && N % XP == 0;
+    Turns turns = turns_make(sm.turn, warp, PP);
+    turns_open(turns, warp);
     for (int u = u0; u < u1; ++u) {
         const int view = u / gpv, line = (u % gpv) * XP + pair;
         if (line >= N) continue;  // pair-uniform (ragged last group of a view when XP does not divide N)
@@ -525,7 +597,7 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
         }
         const size_t row = (size_t)view * N + line;
 #ifdef SFDW_TRACE
-        long long *tr = g_trace + (((size_t)blockIdx.x * WX + warp) * 16 + (u - u0)) * 16;
+        long long *tr = g_trace + TRACE_PASS + (((size_t)blockIdx.x * WX + warp) * 16 + ((u - u0) & 15)) * 32;
 #endif
         SFDW_STAMP(0);
         if (!pending && issuer)
@@ -574,13 +646,7 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
         }
         SFDW_STAMP(9);
     }
-    if (PP && (warp >> 2) == 0) {  // absorb the tokens still in flight
-        turn_begin(turns);
-#if SFDW_PP_SKEW
-        turn_end(turns);
-        turn_begin(turns);
-#endif
-    }
+    turns_close(turns, warp);
 }
 
 }  // namespace sfdw
