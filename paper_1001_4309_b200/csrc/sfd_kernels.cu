@@ -93,7 +93,7 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
     if (threadIdx.x == 0) {
         sfdw::mbar_init(&sm.tbar[0], 1);
         sfdw::mbar_init(&sm.tbar[1], 1);
-        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], 1);
+        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
         sfdw::mbar_fence_init();
     }
     if (!sfdw::TWR)
@@ -117,7 +117,7 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
         for (int i = 0; i < sfdw::XP; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
         sfdw::mbar_init(&sm.tbar[0], 1);
         sfdw::mbar_init(&sm.tbar[1], 1);
-        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], 1);
+        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
         sfdw::mbar_fence_init();
     }
     if (!sfdw::TWR)

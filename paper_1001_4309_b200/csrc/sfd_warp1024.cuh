@@ -143,7 +143,10 @@ template <int DIR> __device__ __forceinline__ void dft32(float2 (&a)[32]) {
 #define SFDW_TWR 1  // 1: inter-stage twiddles live in registers, 0: read from shared memory
 #endif
 #ifndef SFDW_PINGPONG
-#define SFDW_PINGPONG 1  // 1: warps sharing a sub-partition take turns in the butterfly phases (pass x)
+// coupling of the two warps that share a sub-partition (see Turns below); measured on config 2
+// (reconstructions/s): 0 none 48.1k, 1 strict alternation (mbarrier tokens) 46.5k, 2 rendezvous
+// before every butterfly phase (mbarrier) 43.5k, 3 named-barrier hand-off 50.9k
+#define SFDW_PINGPONG 3
 #endif
 #ifndef SFDW_ROLLED
 #define SFDW_ROLLED 1  // 1: the two radix-32 stages / two FFTs of a branch share one copy of the code
@@ -221,23 +224,40 @@ __device__ __forceinline__ void load_twiddles(float2 (&tw)[TWN], int lane,
 // Tables of one view and one pass as they sit in global memory ([V][2][3][N], plan time) and in
 // shared memory: for branch b the vectors pre_b, H_b, conj(post_b).
 constexpr int TABS = 2 * 3 * N;  // complex elements
-// Turn-taking between the two warps that share an SM sub-partition (warps w and w + 4 of an
-// 8-warp CTA).  The butterfly phases of a line saturate the sub-partition's fp32 pipe, the phases
-// between them (transposes, table and input reads, exchange, stores) use the SM-wide shared-memory
-// pipe; left alone, all warps of an SM drift into the same phase and the two kinds of phase run
-// one after the other instead of side by side.  A warp therefore enters a butterfly phase only
-// when it holds its sub-partition's token and passes the token on when the phase ends: one warp
-// of each sub-partition is in butterflies while the other does its memory phase.
-// The token is a pair of mbarriers (count 1): `mine` completes a phase when the other warp ends
-// its turn, `theirs` is the other warp's.  (bar.arrive / bar.sync on a named barrier with a count
-// of 64 does NOT do this on sm_100: measured, the syncing warp is released at once.)
+// Coupling of the two warps that share an SM sub-partition (warps w and w + 4 of an 8-warp CTA).
+// The butterfly phases of a line load the sub-partition's fp32 pipe, the phases between them
+// (transposes, table and input reads, exchange, stores) the SM-wide shared-memory pipe; left alone
+// the warps of an SM drift into the same phase and the shared-memory pipe sees bursts.  Four
+// policies are kept as a build knob (SFDW_PINGPONG), a butterfly phase being bracketed by
+// turn_begin / turn_end:
+//   1  a token per sub-partition (two mbarriers, count 1): strictly alternating, exclusive turns.
+//      Verified exclusive with clock stamps - and slower than no coupling: the memory phases of a
+//      line (about 3700 cycles) are longer than the partner's turns (about 3300), so the fp32 pipe
+//      idles while both warps are in memory phases.
+//   2  both warps meet (one mbarrier, count 2) before every turn: slower still.
+//   3  bar.arrive on the partner's named barrier at turn_end, bar.sync on one's own at turn_begin,
+//      both with a thread count of 64.  Measured with clock stamps this does NOT exclude anything
+//      (a warp waits about 45 cycles per turn on average; the butterfly phases of the two warps
+//      overlap freely); it bounds how far the two warps drift apart and is the fastest of the
+//      four.  It is the default for that reason only.
+//   0  no coupling.
 struct Turns {
     unsigned mine, theirs;  // shared-memory addresses of the two mbarriers
     unsigned phase;         // parity of the next completion of `mine` this warp waits for
     bool on;
 };
 __device__ __forceinline__ void turn_begin(Turns &t) {
+#if SFDW_PINGPONG == 3
+    if (t.on) asm volatile("bar.sync %0, 64;" ::"r"(t.mine) : "memory");
+    return;
+#endif
     if (t.on) {
+#if SFDW_PINGPONG == 2
+        // rendezvous: both warps of the sub-partition start their k-th turn together
+        __syncwarp();
+        if ((threadIdx.x & 31) == 0)
+            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(t.mine) : "memory");
+#endif
         asm volatile(
             "{\n"
             ".reg .pred p;\n"
@@ -253,7 +273,11 @@ __device__ __forceinline__ void turn_begin(Turns &t) {
     }
 }
 __device__ __forceinline__ void turn_end(const Turns &t) {
-    if (t.on) {
+#if SFDW_PINGPONG == 3
+    if (t.on) asm volatile("bar.arrive %0, 64;" ::"r"(t.theirs) : "memory");
+    return;
+#endif
+    if (t.on && SFDW_PINGPONG != 2) {
         __syncwarp();
         if ((threadIdx.x & 31) == 0)
             asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(t.theirs) : "memory");
@@ -266,19 +290,31 @@ __device__ __forceinline__ void turn_end(const Turns &t) {
 // ones (transposes) beside turns 3 and 1.
 __device__ __forceinline__ Turns turns_make(unsigned long long *bars, int warp, bool on) {
     const int sp = warp & 3, up = warp >> 2;
+#if SFDW_PINGPONG == 3
+    return Turns{5u + 2 * sp + up, 5u + 2 * sp + 1 - up, 0u, on};  // named barriers 5..12
+#elif SFDW_PINGPONG == 2
+    return Turns{smem_u32(bars + 2 * sp), smem_u32(bars + 2 * sp), 0u, on};
+#else
     return Turns{smem_u32(bars + 2 * sp + up), smem_u32(bars + 2 * sp + 1 - up), 0u, on};
+#endif
 }
 __device__ __forceinline__ void turns_open(Turns &t, int warp) {
     if ((warp >> 2) == 1) {
+#if SFDW_PINGPONG == 3
         turn_end(t);
+#else
+#if SFDW_PINGPONG != 2
+        turn_end(t);
+#endif
         turn_begin(t);
         turn_end(t);
+#endif
     }
 }
 __device__ __forceinline__ void turns_close(Turns &t, int warp) {
     if ((warp >> 2) == 0) {
         turn_begin(t);
-        turn_end(t);
+        if (SFDW_PINGPONG != 3) turn_end(t);
     }
 }
 
