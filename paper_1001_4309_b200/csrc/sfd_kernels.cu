@@ -91,8 +91,6 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
     sfdw::SmemY<TIn> &sm = *reinterpret_cast<sfdw::SmemY<TIn> *>(smem4);
     if (vmax != nullptr && blockIdx.x == 0 && threadIdx.x < V) vmax[threadIdx.x] = 0u;
     if (threadIdx.x == 0) {
-        sfdw::mbar_init(&sm.tbar[0], 1);
-        sfdw::mbar_init(&sm.tbar[1], 1);
         for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
         sfdw::mbar_fence_init();
     }
@@ -100,11 +98,14 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
         for (int i = threadIdx.x; i < 1024; i += blockDim.x) sm.tw[i] = __ldg(twl + i);
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
-    __syncthreads();
+    // tables of this CTA's view(s) -> tensor memory (the barriers inside also publish the mbarriers)
+    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabY, V * (sfdw::N / sfdw::YC), sfdw::N / sfdw::YC);
+    const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     if (((threadIdx.x >> 5) & 1) == 0)
-        sfdw::pass_y_loop<TIn, 0>(sm, holo, tabY, tw, &tmB, V);
+        sfdw::pass_y_loop<TIn, 0>(sm, holo, tq, tw, &tmB, V);
     else
-        sfdw::pass_y_loop<TIn, 1>(sm, holo, tabY, tw, &tmB, V);
+        sfdw::pass_y_loop<TIn, 1>(sm, holo, tq, tw, &tmB, V);
+    sfdw::tm_finish(tbase);
 }
 
 __global__ void __launch_bounds__(sfdw::WX * 32, 1)
@@ -115,8 +116,6 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
     sfdw::SmemX &sm = *reinterpret_cast<sfdw::SmemX *>(smem4);
     if (threadIdx.x == 0) {
         for (int i = 0; i < sfdw::XP; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
-        sfdw::mbar_init(&sm.tbar[0], 1);
-        sfdw::mbar_init(&sm.tbar[1], 1);
         for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
         sfdw::mbar_fence_init();
     }
@@ -124,11 +123,14 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
         for (int i = threadIdx.x; i < 1024; i += blockDim.x) sm.tw[i] = __ldg(twl + i);
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
-    __syncthreads();
+    constexpr int gpv = (sfdw::N + sfdw::XP - 1) / sfdw::XP;  // units per view, as in pass_x_loop
+    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabX, V * gpv, gpv);
+    const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     if (((threadIdx.x >> 5) & 1) == 0)
-        sfdw::pass_x_loop<0>(sm, B, tabX, tw, field, inten, vmax, V);
+        sfdw::pass_x_loop<0>(sm, B, tq, tw, field, inten, vmax, V);
     else
-        sfdw::pass_x_loop<1>(sm, B, tabX, tw, field, inten, vmax, V);
+        sfdw::pass_x_loop<1>(sm, B, tq, tw, field, inten, vmax, V);
+    sfdw::tm_finish(tbase);
 }
 
 std::atomic<long long> g_launches{0};

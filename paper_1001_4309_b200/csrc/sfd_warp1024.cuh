@@ -224,6 +224,127 @@ __device__ __forceinline__ void load_twiddles(float2 (&tw)[TWN], int lane,
 // Tables of one view and one pass as they sit in global memory ([V][2][3][N], plan time) and in
 // shared memory: for branch b the vectors pre_b, H_b, conj(post_b).
 constexpr int TABS = 2 * 3 * N;  // complex elements
+
+// ---- tables in tensor memory --------------------------------------------------------------------
+// The three table vectors of a branch are read once per line and thread (96 complex values): from
+// shared memory that is a third of all shared-memory wavefronts of a line, on the pipe that also
+// carries the transposes.  Tensor memory (256 KB per SM, 128 lanes x 512 columns of 32 bits, unused
+// here otherwise: there is no MMA on this path) has its own read path into the register file
+// (tcgen05.ld, 64 B/clk per sub-partition measured, no contention between sub-partitions), and its
+// shape fits: a warp may touch only the 32 lanes of its sub-partition, lane l of warp w holds what
+// thread l needs.  Both warps of a sub-partition (w, w + 4) run the same branch b = w & 1, so each
+// lane quarter holds, per view set s (a CTA's lines lie in at most two views), 192 columns:
+//     column 192 s + 64 t + 2 r + {0, 1} = re, im of table t (pre_b, H_b, conj(post_b)) at lane + 32 r
+// A chunk is 16 columns = 8 complex values; tcgen05.wait::ld waits for every load in flight, so
+// the loops below wait for chunk j, start chunk j + 1 and then use chunk j.
+constexpr int TM_COLS = 512;      // allocated columns (all of it: one CTA per SM)
+constexpr int TM_SET = 192;       // columns of one view set
+constexpr int TM_TAB = 64;        // columns of one table
+struct TChunk { unsigned w[16]; };
+#define SFDW_O16(c) "=r"(c.w[0]), "=r"(c.w[1]), "=r"(c.w[2]), "=r"(c.w[3]), "=r"(c.w[4]), "=r"(c.w[5]), \
+    "=r"(c.w[6]), "=r"(c.w[7]), "=r"(c.w[8]), "=r"(c.w[9]), "=r"(c.w[10]), "=r"(c.w[11]), "=r"(c.w[12]), \
+    "=r"(c.w[13]), "=r"(c.w[14]), "=r"(c.w[15])
+#define SFDW_IO16(c) "+r"(c.w[0]), "+r"(c.w[1]), "+r"(c.w[2]), "+r"(c.w[3]), "+r"(c.w[4]), "+r"(c.w[5]), \
+    "+r"(c.w[6]), "+r"(c.w[7]), "+r"(c.w[8]), "+r"(c.w[9]), "+r"(c.w[10]), "+r"(c.w[11]), "+r"(c.w[12]), \
+    "+r"(c.w[13]), "+r"(c.w[14]), "+r"(c.w[15])
+#define SFDW_I16(c) "r"(c.w[0]), "r"(c.w[1]), "r"(c.w[2]), "r"(c.w[3]), "r"(c.w[4]), "r"(c.w[5]), \
+    "r"(c.w[6]), "r"(c.w[7]), "r"(c.w[8]), "r"(c.w[9]), "r"(c.w[10]), "r"(c.w[11]), "r"(c.w[12]), \
+    "r"(c.w[13]), "r"(c.w[14]), "r"(c.w[15])
+// same, tied to `dep` so that the load is issued before anything that consumes dep afterwards
+__device__ __forceinline__ void tm_ld_before(TChunk &c, unsigned taddr, float &dep) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%17];"
+        : SFDW_O16(c), "+f"(dep)
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tm_ld(TChunk &c, unsigned taddr) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : SFDW_O16(c)
+        : "r"(taddr));
+}
+// the registers of `c` are valid afterwards (they are operands so that no use moves above the wait)
+__device__ __forceinline__ void tm_wait(TChunk &c) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;" : SFDW_IO16(c));
+}
+__device__ __forceinline__ void tm_st(const TChunk &c, unsigned taddr) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%16], "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15};" ::SFDW_I16(c),
+        "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ float2 tm_val(const TChunk &c, int i) {
+    return make_float2(__uint_as_float(c.w[2 * i]), __uint_as_float(c.w[2 * i + 1]));
+}
+// warp 0 allocates all columns and publishes the base address in *slot
+__device__ __forceinline__ void tm_alloc(unsigned *slot) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                     smem_u32(slot)),
+                 "n"(TM_COLS)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tm_free(unsigned base) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(base), "n"(TM_COLS)
+                 : "memory");
+}
+__device__ __forceinline__ void tm_sync_cta() {  // makes tcgen05.st of other warps visible
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+}
+// this warp's lane quarter
+__device__ __forceinline__ unsigned tm_quarter(unsigned base, int warp) {
+    return base + ((unsigned)(32 * (warp & 3)) << 16);
+}
+// The two warps of a sub-partition copy the tables of `view`, branch warp & 1, into set `set` of
+// their quarter: warp w the chunks 0..5 (pre_b and half of H_b), warp w + 4 the chunks 6..11.  All
+// 48 loads of a thread are issued before the first store: one trip to L2 per set.
+// tab: [V][2][3][N] in global memory
+__device__ __forceinline__ void tm_fill(unsigned quarter, int set, const float2 *__restrict__ tab,
+                                        int view, int warp, int lane) {
+    const float2 *src = tab + (size_t)view * TABS + (size_t)(warp & 1) * 3 * N + lane;
+    const int ch0 = 6 * (warp >> 2);  // first chunk of this warp; chunk = 8 values, 4 chunks per table
+    TChunk c[6];
+#pragma unroll
+    for (int j = 0; j < 6; ++j)
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const float2 x = __ldg(src + 32 * (8 * (ch0 + j) + i));  // table t = chunk / 4 starts at t * N
+            c[j].w[2 * i] = __float_as_uint(x.x);
+            c[j].w[2 * i + 1] = __float_as_uint(x.y);
+        }
+#pragma unroll
+    for (int j = 0; j < 6; ++j) tm_st(c[j], quarter + set * TM_SET + 16 * (ch0 + j));
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+// Kernel prologue (all threads): allocate, fill the one or two view sets this CTA's contiguous
+// range [total b / g, total (b + 1) / g) of work units touches (per_view units per view), make
+// them visible.  Returns the base address; tm_finish releases it at the end of the kernel.
+__device__ __forceinline__ unsigned tm_setup(unsigned *slot, const float2 *__restrict__ tab,
+                                             int total, int per_view) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (warp == 0) tm_alloc(slot);
+    tm_sync_cta();
+    const unsigned base = *reinterpret_cast<volatile unsigned *>(slot);
+    const int a0 = (int)((long long)total * blockIdx.x / gridDim.x);
+    const int a1 = (int)((long long)total * (blockIdx.x + 1) / gridDim.x);
+    if (a0 < a1) {
+        const int view0 = a0 / per_view;
+        const unsigned q = tm_quarter(base, warp);
+        tm_fill(q, 0, tab, view0, warp, lane);
+        if ((a1 - 1) / per_view != view0) tm_fill(q, 1, tab, view0 + 1, warp, lane);
+    }
+    tm_sync_cta();
+    return base;
+}
+__device__ __forceinline__ void tm_finish(unsigned base) {
+    tm_sync_cta();
+    if ((threadIdx.x >> 5) == 0) tm_free(base);
+}
 // Coupling of the two warps that share an SM sub-partition (warps w and w + 4 of an 8-warp CTA).
 // The butterfly phases of a line load the sub-partition's fp32 pipe, the phases between them
 // (transposes, table and input reads, exchange, stores) the SM-wide shared-memory pipe; left alone
@@ -321,7 +442,7 @@ __device__ __forceinline__ void turns_close(Turns &t, int warp) {
 // One branch of a line, in place (the caller has applied pre): forward FFT, x H_b, inverse FFT,
 // x post_b.  The inverse is run as conj(FFT(conj(.))) so that both transforms execute the same code:
 //     v <- conj(FFT(v) H_b);  v <- conj(FFT(v) conj(post_b)) = post_b IFFT(H_b FFT(v)) N
-// (the 1/N sits in H).  t = this thread's first element of H_b; conj(post_b) follows it N later.
+// (the 1/N sits in H).  t = tensor-memory address of H_b in this warp's quarter; conj(post_b) follows it.
 // A 1024-point FFT of a warp is: radix-32 butterflies over n1 (element lane + 32 n1), inter-stage
 // twiddles exp(-2 pi i lane k1 / 1024) (tw[k] in registers or twsm[k * 32 + lane]), a 32 x 32
 // transpose through the warp's tile xb, radix-32 butterflies over n2; in v[r] = x[lane + 32 r],
@@ -330,7 +451,7 @@ __device__ __forceinline__ void turns_close(Turns &t, int warp) {
 // three turns of the line.  On return v = this warp's partial sums for all 1024 outputs.
 __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
                                        const float2 (&tw)[TWN], const float2 *twsm,
-                                       const float2 *t, Turns &turns
+                                       unsigned t, Turns &turns
 #ifdef SFDW_TRACE
                                        , long long *tr
 #endif
@@ -340,12 +461,21 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
         SFDW_STAMP(16 + 4 * step + 3);
         if (step != 2) turn_begin(turns);
         SFDW_STAMP(16 + 4 * step);
+        TChunk c0, c1;
+        const unsigned ta = t + (step >> 1) * TM_TAB;
+        if (step & 1) tm_ld_before(c0, ta, v[0].x);  // in flight during the butterflies
         dft32<-1>(v);
         if (step & 1) {
 #pragma unroll
-            for (int k = 0; k < 32; ++k) {  // v = conj(v * t)
-                const float2 h = t[(step >> 1) * N + 32 * k], a = v[k];
-                v[k] = make_float2(a.x * h.x - a.y * h.y, -(a.x * h.y) - a.y * h.x);
+            for (int j = 0; j < 4; ++j) {  // v = conj(v * t)
+                TChunk &c = (j & 1) ? c1 : c0;
+                tm_wait(c);
+                if (j < 3) tm_ld((j & 1) ? c0 : c1, ta + 16 * (j + 1));
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const float2 h = tm_val(c, i), a = v[8 * j + i];
+                    v[8 * j + i] = make_float2(a.x * h.x - a.y * h.y, -(a.x * h.y) - a.y * h.x);
+                }
             }
             SFDW_STAMP(16 + 4 * step + 1);
             if (step != 1) turn_end(turns);
@@ -421,12 +551,11 @@ template <> struct TileElem<float> {                 // float: 1 item per slab
 };
 template <typename TIn> struct SmemY {
     float2 xb[WY][XB];
-    float2 tabs[2][TABS];  // tables of the (at most two) views this CTA's items belong to
     alignas(128) float2 stage[2][N][2];  // [half][n1][column of the half]: final sums, TMA store source
     float2 tw[TWR ? 1 : 32 * 32];
     typename TileElem<TIn>::type tile[2][TileElem<TIn>::IPS][N];  // [half][k][n0]: the half's slab
-    unsigned long long tbar[2];
     unsigned long long turn[8];
+    unsigned tmem;  // base address of the tensor-memory allocation
 };
 
 template <typename TIn> struct TileRegs { typename TileElem<TIn>::slab e[8]; };
@@ -485,8 +614,8 @@ __device__ __forceinline__ void bulk_wait_read() {
 // what the partner left for it and writes 16 final values per thread into the staging tile.
 template <typename TIn, int B>
 __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restrict__ holo,
-                                            const float2 *__restrict__ tabY,
-                                            const float2 (&tw)[TWN], const void *tmB, int V) {
+                                            unsigned tq, const float2 (&tw)[TWN],
+                                            const void *tmB, int V) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int half = warp >> 2, c = (warp >> 1) & 1, ht = threadIdx.x & 127;
     constexpr int groups = N / YC;
@@ -499,12 +628,6 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
     float2 *stg = &sm.stage[half][0][0];
     const bool leader = ht == 0;  // issues and retires the half's bulk stores
     const int view0 = i0 / groups;
-    if (threadIdx.x == 0) {
-        bulk_load(sm.tabs[0], tabY + (size_t)view0 * TABS, TABS * sizeof(float2), &sm.tbar[0]);
-        if ((i1 - 1) / groups != view0)
-            bulk_load(sm.tabs[1], tabY + (size_t)(view0 + 1) * TABS, TABS * sizeof(float2),
-                      &sm.tbar[1]);
-    }
     constexpr int IPS = TileElem<TIn>::IPS;
     static_assert(groups % IPS == 0, "a slab never straddles two views");
     {
@@ -516,16 +639,10 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
     constexpr bool PP = SFDW_PINGPONG != 0;
     Turns turns = turns_make(sm.turn, warp, PP);
     turns_open(turns, warp);
-    const float2 *tb_pre = nullptr;
-    int cur_view = -1;
     for (int item = i0; item < i1; ++item) {
         const int view = item / groups, g = item % groups, k = g % IPS;
         const int colh = g / IPS * (YC * IPS) + 2 * IPS * half + 2 * k;
-        if (view != cur_view) {
-            mbar_wait(&sm.tbar[view - view0], 0);
-            tb_pre = sm.tabs[view - view0] + B * 3 * N + lane;
-            cur_view = view;
-        }
+        const unsigned tpre = tq + (view - view0) * TM_SET;  // pre_b | H_b | conj(post_b)
         const bool has_next = item + 1 < i1 && k == IPS - 1;  // the next item opens a new slab
 #ifdef SFDW_TRACE
         long long *tr = g_trace + (((size_t)blockIdx.x * WY + warp) * 16 + (item - i0)) * 32;
@@ -535,17 +652,27 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
         if (has_next)
             tile_load<TIn>(t, holo, ((item + 1) % groups) / IPS * (YC * IPS) + 2 * IPS * half, ht);
         float2 v[32];
+        {
+            TChunk c0, c1;
+            tm_ld(c0, tpre);
 #pragma unroll
-        for (int r = 0; r < 32; ++r) {
-            const float a = tile_value(sm.tile[half][k][lane + 32 * r], c);
-            const float2 p = tb_pre[32 * r];
-            v[r] = make_float2(a * p.x, a * p.y);
+            for (int j = 0; j < 4; ++j) {
+                TChunk &ch = (j & 1) ? c1 : c0;
+                tm_wait(ch);
+                if (j < 3) tm_ld((j & 1) ? c0 : c1, tpre + 16 * (j + 1));
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const float a = tile_value(sm.tile[half][k][lane + 32 * (8 * j + i)], c);
+                    const float2 p = tm_val(ch, i);
+                    v[8 * j + i] = make_float2(a * p.x, a * p.y);
+                }
+            }
         }
         SFDW_STAMP(1);
 #ifdef SFDW_TRACE
-        branch(v, lane, xb, tw, sm.tw, tb_pre + N, turns, tr);
+        branch(v, lane, xb, tw, sm.tw, tpre + TM_TAB, turns, tr);
 #else
-        branch(v, lane, xb, tw, sm.tw, tb_pre + N, turns);
+        branch(v, lane, xb, tw, sm.tw, tpre + TM_TAB, turns);
 #endif
         SFDW_STAMP(8);
         // the previous item's bulk stores must have left the staging tile before it is rewritten
@@ -579,19 +706,18 @@ constexpr int WX = SFDW_WX;  // warps per CTA
 constexpr int XP = WX / 2;   // pairs per CTA = rows in flight per CTA
 struct SmemX {
     float2 xb[WX][XB];
-    float2 tabs[2][TABS];  // tables of the (at most two) views this CTA's rows belong to
     float2 tw[32 * 32];
     float2 inb[XP][N];  // input row of each pair (bulk async copy destination)
     unsigned long long ibar[XP];
-    unsigned long long tbar[2];
     unsigned long long turn[8];
+    unsigned tmem;  // base address of the tensor-memory allocation
 };
 
 // Work unit = (view, group of XP adjacent rows); a CTA takes a contiguous range of units, so all
 // its pairs are always in the same view.  tabX: [V][2][3][N].
 template <int B>
 __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict__ Bin,
-                                            const float2 *__restrict__ tabX,
+                                            unsigned tq,
                                             const float2 (&tw)[TWN], float2 *__restrict__ field,
                                             float *__restrict__ inten, unsigned int *vmax, int V) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, pair = warp >> 1;
@@ -604,18 +730,7 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
     const float2 *xbp = sm.xb[warp ^ 1];
     const float2 *in = sm.inb[pair] + lane;
     const bool issuer = B == 0 && lane == 0;
-    // The launcher sizes the grid so that a CTA's rows lie in at most two views: both table sets
-    // are requested up front and a warp waits for a set the first time it needs it; no CTA-wide
-    // barrier exists in this kernel.
     const int view0 = u0 / gpv;
-    if (threadIdx.x == 0) {
-        bulk_load(sm.tabs[0], tabX + (size_t)view0 * TABS, TABS * sizeof(float2), &sm.tbar[0]);
-        if ((u1 - 1) / gpv != view0)
-            bulk_load(sm.tabs[1], tabX + (size_t)(view0 + 1) * TABS, TABS * sizeof(float2),
-                      &sm.tbar[1]);
-    }
-    const float2 *tb_pre = nullptr;
-    int cur_view = -1;
     unsigned iphase = 0;
     bool pending = false;  // the pair's input row is already on its way
     // turn-taking of warps w and w + 4 (needs every warp of the CTA to run the same number of
@@ -626,11 +741,7 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
     for (int u = u0; u < u1; ++u) {
         const int view = u / gpv, line = (u % gpv) * XP + pair;
         if (line >= N) continue;  // pair-uniform (ragged last group of a view when XP does not divide N)
-        if (view != cur_view) {
-            mbar_wait(&sm.tbar[view - view0], 0);
-            tb_pre = sm.tabs[view - view0] + B * 3 * N + lane;
-            cur_view = view;
-        }
+        const unsigned tpre = tq + (view - view0) * TM_SET;  // pre_b | H_b | conj(post_b)
         const size_t row = (size_t)view * N + line;
 #ifdef SFDW_TRACE
         long long *tr = g_trace + TRACE_PASS + (((size_t)blockIdx.x * WX + warp) * 16 + ((u - u0) & 15)) * 32;
@@ -644,8 +755,19 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
         iphase ^= 1;
         SFDW_STAMP(1);
         float2 v[32];
+        {
+            TChunk c0, c1;
+            tm_ld(c0, tpre);
 #pragma unroll
-        for (int r = 0; r < 32; ++r) v[r] = cmul(in[32 * r], tb_pre[32 * r]);
+            for (int j = 0; j < 4; ++j) {
+                TChunk &ch = (j & 1) ? c1 : c0;
+                tm_wait(ch);
+                if (j < 3) tm_ld((j & 1) ? c0 : c1, tpre + 16 * (j + 1));
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+                    v[8 * j + i] = cmul(in[32 * (8 * j + i)], tm_val(ch, i));
+            }
+        }
         SFDW_STAMP(2);
         // both warps have consumed the input row and finished with each other's transpose tile
         pair_sync(pair);
@@ -657,9 +779,9 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
         }
         pending = has_next;
 #ifdef SFDW_TRACE
-        branch(v, lane, xb, tw, sm.tw, tb_pre + N, turns, tr);
+        branch(v, lane, xb, tw, sm.tw, tpre + TM_TAB, turns, tr);
 #else
-        branch(v, lane, xb, tw, sm.tw, tb_pre + N, turns);
+        branch(v, lane, xb, tw, sm.tw, tpre + TM_TAB, turns);
 #endif
         add_halves<B>(v, xb, xbp, lane, pair);
         SFDW_STAMP(8);
