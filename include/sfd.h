@@ -100,6 +100,22 @@ SFD_API int sfd_stream_run(sfd_plan *plan, const void *holograms_pinned, int n_f
 SFD_API int sfd_plan_update_view(sfd_plan *plan, int view, double p1, double p2, double z, double Ox,
                          double Oy);
 
+/* General geometry (Eq.(2)-(4) L58-65 and the definitions L67 keep
+ * separate x and y sampling pitches, hence S_x = p1x p2x/(lambda z) != S_y = p1y p2y/(lambda z), and
+ * offsets (O_x0, O_y0) of the hologram window next to (O_x1, O_y1) of the reconstruction window).
+ * Physical coordinates (reading 1 of DESIGN.md): x0 = (m0 - N/2) p1x + O0x, y0 = (n0 - N/2) p1y + O0y,
+ * x1 = (m1 - N/2) p2x + O1x, y1 = (n1 - N/2) p2y + O1y, all lengths in metres, arrays [n_views] on
+ * the host.  sfd_plan_create is this call with p1x = p1y, p2x = p2y, O0 = 0.  The grid stays N x N.
+ * Each axis gets its own chirp tables and its own cached kernel spectrum.  Same errors. */
+SFD_API int sfd_plan_create_general(sfd_plan **out, int N, int n_views, double lambda,
+                                    const double *p1x, const double *p1y, const double *p2x,
+                                    const double *p2y, const double *z, const double *O0x,
+                                    const double *O0y, const double *O1x, const double *O1y,
+                                    int in_dtype);
+SFD_API int sfd_plan_update_view_general(sfd_plan *plan, int view, double p1x, double p1y,
+                                         double p2x, double p2y, double z, double O0x, double O0y,
+                                         double O1x, double O1y);
+
 /* Destroy a plan and free everything it owns.  NULL is accepted. */
 SFD_API int sfd_plan_destroy(sfd_plan *plan);
 
@@ -137,6 +153,10 @@ SFD_API long long sfd_launch_count(void);
  * arrays of 2N, 2N and 4N doubles.  `off` is the window shift along that axis.  N: power of two. */
 SFD_API int sfd_host_tables(int N, double lambda, double p1, double p2, double z, double off, double *pre,
                     double *post, double *H);
+
+/* The same for a hologram window shifted by off0 along that axis (general geometry). */
+SFD_API int sfd_host_tables_general(int N, double lambda, double p1, double p2, double z, double off0,
+                                    double off, double *pre, double *post, double *H);
 
 /* Static description of an error code / of the last CUDA error seen by this thread. */
 SFD_API const char *sfd_error_string(int code);

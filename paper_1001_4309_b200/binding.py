@@ -36,6 +36,10 @@ _vp = C.c_void_p
 _sig = {
     "sfd_plan_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_double, _dp, _dp, _dp, _dp,
                                   _dp, C.c_int]),
+    "sfd_plan_create_general": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_double] + [_dp] * 9
+                                + [C.c_int]),
+    "sfd_plan_update_view_general": (C.c_int, [_vp, C.c_int] + [C.c_double] * 9),
+    "sfd_host_tables_general": (C.c_int, [C.c_int] + [C.c_double] * 6 + [_dp, _dp, _dp]),
     "sfd_execute": (C.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "sfd_execute_u8": (C.c_int, [_vp, _vp, _vp, _vp]),
     "sfd_stream_run": (C.c_int, [_vp, _vp, C.c_int, _vp, _dp]),
@@ -132,6 +136,23 @@ def sfd_plan_create(N, n_views, lam, p1, p2, z, Ox, Oy, in_dtype=SFD_U8):
     return h.value
 
 
+def sfd_plan_create_general(N, n_views, lam, p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y,
+                            in_dtype=SFD_U8):
+    """General geometry: separate x/y pitches and hologram-window offsets (include/sfd.h)."""
+    arrs = [_darr(a, n_views) for a in (p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y)]
+    h = _vp()
+    _chk(_lib.sfd_plan_create_general(C.byref(h), int(N), int(n_views), float(lam),
+                                      *[a.ctypes.data_as(_dp) for a in arrs], int(in_dtype)),
+         "sfd_plan_create_general")
+    return h.value
+
+
+def sfd_plan_update_view_general(plan, view, p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y):
+    _chk(_lib.sfd_plan_update_view_general(plan, int(view), *map(float, (p1x, p1y, p2x, p2y, z, O0x,
+                                                                         O0y, O1x, O1y))),
+         "sfd_plan_update_view_general")
+
+
 def sfd_execute(plan, hologram_dev, field_dev, intensity_dev, stream=None):
     _chk(_lib.sfd_execute(plan, _ptr(hologram_dev), _ptr(field_dev), _ptr(intensity_dev),
                           _stream(stream)), "sfd_execute")
@@ -204,6 +225,18 @@ def sfd_host_tables(N, lam, p1, p2, z, off):
     return pre, post, H
 
 
+def sfd_host_tables_general(N, lam, p1, p2, z, off0, off):
+    """The same with the hologram window shifted by ``off0`` along the axis."""
+    pre = np.empty(N, np.complex128)
+    post = np.empty(N, np.complex128)
+    H = np.empty(2 * N, np.complex128)
+    _chk(_lib.sfd_host_tables_general(int(N), float(lam), float(p1), float(p2), float(z),
+                                      float(off0), float(off), pre.ctypes.data_as(_dp),
+                                      post.ctypes.data_as(_dp), H.ctypes.data_as(_dp)),
+         "sfd_host_tables_general")
+    return pre, post, H
+
+
 # ---- convenience wrapper: owns the handle, allocates outputs with torch --------------------------
 class Plan:
     """``Plan(workload)`` or ``Plan(N=..., lam=..., p1=..., p2=..., z=..., Ox=..., Oy=...,
@@ -216,8 +249,13 @@ class Plan:
         self.N = int(kw["N"])
         self.V = len(np.atleast_1d(kw["z"]))
         self.in_dtype = int(kw.get("in_dtype", SFD_U8))
-        self.handle = sfd_plan_create(self.N, self.V, kw["lam"], kw["p1"], kw["p2"], kw["z"],
-                                      kw["Ox"], kw["Oy"], self.in_dtype)
+        if "p1x" in kw:     # general geometry: p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y
+            self.handle = sfd_plan_create_general(
+                self.N, self.V, kw["lam"], kw["p1x"], kw["p1y"], kw["p2x"], kw["p2y"], kw["z"],
+                kw["O0x"], kw["O0y"], kw["O1x"], kw["O1y"], self.in_dtype)
+        else:
+            self.handle = sfd_plan_create(self.N, self.V, kw["lam"], kw["p1"], kw["p2"], kw["z"],
+                                          kw["Ox"], kw["Oy"], self.in_dtype)
 
     def close(self):
         if self.handle:
@@ -275,6 +313,9 @@ class Plan:
             out_pinned = torch.empty((F, self.V, self.N, self.N), dtype=torch.uint8).pin_memory()
         sec = sfd_stream_run(self.handle, holograms_pinned, F, out_pinned)
         return out_pinned, sec
+
+    def update_view_general(self, view, p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y):
+        sfd_plan_update_view_general(self.handle, view, p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y)
 
     def update_view(self, view, p1, p2, z, Ox, Oy):
         sfd_plan_update_view(self.handle, view, p1, p2, z, Ox, Oy)

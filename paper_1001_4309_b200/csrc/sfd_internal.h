@@ -16,7 +16,8 @@ struct sfd_dev {
     float2 *post_y = nullptr;  // [V][N]  Eq.(2) y-part x c0
     float2 *pre_x = nullptr;   // [V][N]  Eq.(3) x-part
     float2 *post_x = nullptr;  // [V][N]  Eq.(2) x-part
-    float2 *H = nullptr;       // [V][M]  FFT_M(h)/M, h of Eq.(4) wrapped (S_x = S_y: one per view)
+    float2 *H = nullptr;       // [V][M]  y axis: FFT_M(h)/M, h of Eq.(4) wrapped, S = S_y
+    float2 *Hx = nullptr;      // [V][M]  x axis: the same with S = S_x
     float2 *tw = nullptr;      // [M]     exp(-2 pi i x / M)
     // workspace
     float2 *B = nullptr;           // [V][N][N] intermediate between pass y and pass x
@@ -34,7 +35,8 @@ struct sfd_plan {
     sfd_dev d;
     int device = 0;
     double lambda = 0;
-    std::vector<double> p1, p2, z, Ox, Oy;
+    // per view; p1, p2, Ox, Oy are the x-axis values (and the y-axis ones in the square API)
+    std::vector<double> p1, p2, z, Ox, Oy, p1y, p2y, O0x, O0y;
     void *table_alloc = nullptr;
     void *fast_alloc = nullptr;
     int kernels = SFD_KERNELS_AUTO;

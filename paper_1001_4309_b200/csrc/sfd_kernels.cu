@@ -94,12 +94,12 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
         for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
         sfdw::mbar_fence_init();
     }
-    if (!sfdw::TWR)
+    if (SFDW_TWR == 0)
         for (int i = threadIdx.x; i < 1024; i += blockDim.x) sm.tw[i] = __ldg(twl + i);
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
     // tables of this CTA's view(s) -> tensor memory (the barriers inside also publish the mbarriers)
-    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabY, V * (sfdw::N / sfdw::YC), sfdw::N / sfdw::YC);
+    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabY, twl, V * (sfdw::N / sfdw::YC), sfdw::N / sfdw::YC);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     if (((threadIdx.x >> 5) & 1) == 0)
         sfdw::pass_y_loop<TIn, 0>(sm, holo, tq, tw, &tmB, V);
@@ -119,12 +119,12 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
         for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
         sfdw::mbar_fence_init();
     }
-    if (!sfdw::TWR)
+    if (SFDW_TWR == 0)
         for (int i = threadIdx.x; i < 1024; i += blockDim.x) sm.tw[i] = __ldg(twl + i);
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
     constexpr int gpv = (sfdw::N + sfdw::XP - 1) / sfdw::XP;  // units per view, as in pass_x_loop
-    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabX, V * gpv, gpv);
+    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabX, twl, V * gpv, gpv);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     if (((threadIdx.x >> 5) & 1) == 0)
         sfdw::pass_x_loop<0>(sm, B, tq, tw, field, inten, vmax, V);
@@ -206,7 +206,7 @@ cudaError_t launch_t(sfd_plan *p, const void *holo, float2 *field, float *inten,
         k_pass_y<LOG2M, float><<<gy, TL::THREADS_Y, TL::SMEM_Y, st>>>(
             (const float *)holo, d.pre_y, d.H, d.post_y, d.tw, d.B, vmax);
     if (timing) cudaEventRecord(p->ev[1], st);
-    k_pass_x<LOG2M><<<gx, TL::THREADS_X, TL::SMEM_X, st>>>(d.B, d.pre_x, d.H, d.post_x, d.tw, field,
+    k_pass_x<LOG2M><<<gx, TL::THREADS_X, TL::SMEM_X, st>>>(d.B, d.pre_x, d.Hx, d.post_x, d.tw, field,
                                                            inten, vmax);
     if (timing) cudaEventRecord(p->ev[2], st);
     int n = 2;

@@ -68,15 +68,17 @@ void fft_host(std::vector<cd> &a) {
     }
 }
 
-// One axis of one view.  `off` is the shift of the reconstruction window along this axis.
+// One axis of one view.  `off` is the shift of the reconstruction window along this axis, `off0`
+// the shift of the hologram window (O_x0 / O_y0 of Eq.(2)-(3), L58-62; 0 in the square API).
 //   pre[m]  = exp(i pi x0^2/(lambda z)) exp(-i 2 pi m p1 a1/(lambda z)) exp(-i pi S m^2)   Eq.(3)
 //   post[m] = exp(i pi x1^2/(lambda z)) exp(-i 2 pi a0 x1/(lambda z)) exp(-i pi S m^2)     Eq.(2)
-// with x0 = a0 + m p1, a0 = -N/2 p1, x1 = a1 + m p2, a1 = -N/2 p2 + off, S = p1 p2/(lambda z).
+// with x0 = a0 + m p1, a0 = -N/2 p1 + off0, x1 = a1 + m p2, a1 = -N/2 p2 + off,
+// S = p1 p2/(lambda z).
 void axis_tables(int N, double lambda, double p1, double p2, double z, double off, cd *pre,
-                 cd *post) {
+                 cd *post, double off0 = 0.0) {
     const ld lz = (ld)lambda * (ld)z;
     const ld S = (ld)p1 * (ld)p2 / lz;
-    const ld a0 = -(ld)N / 2 * (ld)p1;
+    const ld a0 = -(ld)N / 2 * (ld)p1 + (ld)off0;
     const ld a1 = -(ld)N / 2 * (ld)p2 + (ld)off;
     for (int m = 0; m < N; ++m) {
         const ld x0 = a0 + (ld)m * p1, x1 = a1 + (ld)m * p2;
@@ -100,10 +102,10 @@ void kernel_spectrum(int N, double lambda, double p1, double p2, double z, cd *H
     for (int k = 0; k < M; ++k) H[k] = h[k] / (double)M;
 }
 
-// c0 = p1^2 exp(i 2 pi z/lambda) / (i lambda z)   (constant of Eq.(2) times the area element)
-cd c0_factor(double lambda, double p1, double z) {
+// c0 = p1x p1y exp(i 2 pi z/lambda) / (i lambda z)   (constant of Eq.(2) times the area element)
+cd c0_factor(double lambda, double p1x, double p1y, double z) {
     const cd e = cis_cycles((ld)z / (ld)lambda);
-    return (p1 * p1) * e / (cd(0, 1) * (lambda * z));
+    return (p1x * p1y) * e / (cd(0, 1) * (lambda * z));
 }
 
 bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
@@ -148,24 +150,27 @@ void branch_tables(int N, const cd *pre, const cd *post, cd pre_scale, cd post_s
     }
 }
 
-// float32 tables of one view, host staging layout: pre_y[N] post_y[N] pre_x[N] post_x[N] H[M];
-// `fast` (or NULL) receives tabY[6N] tabX[6N] of the fast path.
+// float32 tables of one view, host staging layout: pre_y[N] post_y[N] pre_x[N] post_x[N] Hy[M]
+// Hx[M]; `fast` (or NULL) receives tabY[6N] tabX[6N] of the fast path.  The y axis uses
+// (p1y, p2y, O0y, Oy), the x axis (p1, p2, O0x, Ox): S_x and S_y may differ (Eq.(2)-(4), L58-67).
 void build_view_f32(const sfd_plan *p, int v, float2 *pre_y, float2 *post_y, float2 *pre_x,
-                    float2 *post_x, float2 *H, float2 *fast) {
+                    float2 *post_x, float2 *Hy, float2 *Hx, float2 *fast) {
     const int N = p->d.N, M = p->d.M;
     std::vector<cd> a(N), b(N), h(M);
     const double in_scale = p->d.in_dtype == SFD_U8 ? 1.0 / 255.0 : 1.0;
-    const cd c0 = c0_factor(p->lambda, p->p1[v], p->z[v]);
-    kernel_spectrum(N, p->lambda, p->p1[v], p->p2[v], p->z[v], h.data());
-    to_f32(h.data(), H, M);
-    axis_tables(N, p->lambda, p->p1[v], p->p2[v], p->z[v], p->Oy[v], a.data(), b.data());
+    const cd c0 = c0_factor(p->lambda, p->p1[v], p->p1y[v], p->z[v]);
+    kernel_spectrum(N, p->lambda, p->p1y[v], p->p2y[v], p->z[v], h.data());
+    to_f32(h.data(), Hy, M);
+    axis_tables(N, p->lambda, p->p1y[v], p->p2y[v], p->z[v], p->Oy[v], a.data(), b.data(), p->O0y[v]);
     to_f32(a.data(), pre_y, N, cd(in_scale, 0));
     to_f32(b.data(), post_y, N, c0);
-    if (fast) branch_tables(N, a.data(), b.data(), cd(in_scale, 0), c0, H, fast);
-    axis_tables(N, p->lambda, p->p1[v], p->p2[v], p->z[v], p->Ox[v], a.data(), b.data());
+    if (fast) branch_tables(N, a.data(), b.data(), cd(in_scale, 0), c0, Hy, fast);
+    kernel_spectrum(N, p->lambda, p->p1[v], p->p2[v], p->z[v], h.data());
+    to_f32(h.data(), Hx, M);
+    axis_tables(N, p->lambda, p->p1[v], p->p2[v], p->z[v], p->Ox[v], a.data(), b.data(), p->O0x[v]);
     to_f32(a.data(), pre_x, N);
     to_f32(b.data(), post_x, N);
-    if (fast) branch_tables(N, a.data(), b.data(), cd(1, 0), cd(1, 0), H, fast + 6 * (size_t)N);
+    if (fast) branch_tables(N, a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, fast + 6 * (size_t)N);
 }
 
 std::atomic<bool> g_init{false};
@@ -226,10 +231,10 @@ int stream_state_make(sfd_plan *p) {
 int upload_view(sfd_plan *p, int v) {
     const int N = p->d.N, M = p->d.M;
     const bool fast = p->d.w_twl != nullptr;
-    std::vector<float2> st((size_t)4 * N + M + (fast ? 12 * (size_t)N : 0));
-    float2 *fs = fast ? st.data() + 4 * N + M : nullptr;
+    std::vector<float2> st((size_t)4 * N + 2 * M + (fast ? 12 * (size_t)N : 0));
+    float2 *fs = fast ? st.data() + 4 * N + 2 * M : nullptr;
     build_view_f32(p, v, st.data(), st.data() + N, st.data() + 2 * N, st.data() + 3 * N,
-                   st.data() + 4 * N, fs);
+                   st.data() + 4 * N, st.data() + 4 * N + M, fs);
     if (fast) {
         SFD_CUDA(cudaMemcpy(p->d.w_tabY + (size_t)v * 6 * N, fs, 6 * sizeof(float2) * N,
                             cudaMemcpyHostToDevice));
@@ -243,6 +248,8 @@ int upload_view(sfd_plan *p, int v) {
     SFD_CUDA(cudaMemcpy(p->d.post_x + (size_t)v * N, st.data() + 3 * N, nb, cudaMemcpyHostToDevice));
     SFD_CUDA(cudaMemcpy(p->d.H + (size_t)v * M, st.data() + 4 * N, sizeof(float2) * M,
                         cudaMemcpyHostToDevice));
+    SFD_CUDA(cudaMemcpy(p->d.Hx + (size_t)v * M, st.data() + 4 * N + M, sizeof(float2) * M,
+                        cudaMemcpyHostToDevice));
     return SFD_OK;
 }
 
@@ -253,10 +260,15 @@ extern "C" {
 
 int sfd_host_tables(int N, double lambda, double p1, double p2, double z, double off, double *pre,
                     double *post, double *H) {
+    return sfd_host_tables_general(N, lambda, p1, p2, z, 0.0, off, pre, post, H);
+}
+
+int sfd_host_tables_general(int N, double lambda, double p1, double p2, double z, double off0,
+                            double off, double *pre, double *post, double *H) {
     if (!pre || !post || !H || log2_exact(N) < 0 || N < 2) return SFD_EINVAL;
-    if (check_view(lambda, p1, p2, z, off, 0.0) != SFD_OK) return SFD_EINVAL;
+    if (check_view(lambda, p1, p2, z, off, off0) != SFD_OK) return SFD_EINVAL;
     std::vector<cd> a(N), b(N), h(2 * (size_t)N);
-    axis_tables(N, lambda, p1, p2, z, off, a.data(), b.data());
+    axis_tables(N, lambda, p1, p2, z, off, a.data(), b.data(), off0);
     kernel_spectrum(N, lambda, p1, p2, z, h.data());
     std::memcpy(pre, a.data(), sizeof(cd) * N);
     std::memcpy(post, b.data(), sizeof(cd) * N);
@@ -269,12 +281,27 @@ int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const dou
                     int in_dtype) {
     if (!out) return SFD_EINVAL;
     *out = nullptr;
-    if (!p1 || !p2 || !z || !Ox || !Oy) return SFD_EINVAL;
+    if (!p1 || !p2 || !z || !Ox || !Oy || n_views < 1) return SFD_EINVAL;
+    const std::vector<double> zero(n_views, 0.0);
+    return sfd_plan_create_general(out, N, n_views, lambda, p1, p1, p2, p2, z, zero.data(),
+                                   zero.data(), Ox, Oy, in_dtype);
+}
+
+int sfd_plan_create_general(sfd_plan **out, int N, int n_views, double lambda, const double *p1x,
+                            const double *p1y, const double *p2x, const double *p2y,
+                            const double *z, const double *O0x, const double *O0y,
+                            const double *O1x, const double *O1y, int in_dtype) {
+    if (!out) return SFD_EINVAL;
+    *out = nullptr;
+    if (!p1x || !p1y || !p2x || !p2y || !z || !O0x || !O0y || !O1x || !O1y) return SFD_EINVAL;
     const int l2 = log2_exact(N);
     if (l2 < 6 || l2 > 11 || n_views < 1) return SFD_EINVAL;
     if (in_dtype != SFD_U8 && in_dtype != SFD_F32) return SFD_EINVAL;
-    for (int v = 0; v < n_views; ++v)
-        if (check_view(lambda, p1[v], p2[v], z[v], Ox[v], Oy[v]) != SFD_OK) return SFD_EINVAL;
+    for (int v = 0; v < n_views; ++v) {
+        if (check_view(lambda, p1x[v], p2x[v], z[v], O1x[v], O0x[v]) != SFD_OK) return SFD_EINVAL;
+        if (check_view(lambda, p1y[v], p2y[v], z[v], O1y[v], O0y[v]) != SFD_OK) return SFD_EINVAL;
+    }
+    const double *p1 = p1x, *p2 = p2x, *Ox = O1x, *Oy = O1y;
 
     if (!g_init.load()) {
         SFD_CUDA(sfd_kernels_init());
@@ -293,6 +320,10 @@ int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const dou
     p->z.assign(z, z + n_views);
     p->Ox.assign(Ox, Ox + n_views);
     p->Oy.assign(Oy, Oy + n_views);
+    p->p1y.assign(p1y, p1y + n_views);
+    p->p2y.assign(p2y, p2y + n_views);
+    p->O0x.assign(O0x, O0x + n_views);
+    p->O0y.assign(O0y, O0y + n_views);
 
     int rc = SFD_OK;
     auto fail = [&](int code) {
@@ -301,7 +332,7 @@ int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const dou
     };
     if (cudaGetDevice(&p->device) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaGetDevice"));
     const size_t V = n_views, M = 2 * (size_t)N, nn = (size_t)N * N;
-    const size_t n_tab = V * (4 * (size_t)N + M) + M;  // complex64 elements
+    const size_t n_tab = V * (4 * (size_t)N + 2 * M) + M;  // complex64 elements
     cudaError_t e;
     if ((e = cudaMalloc(&p->table_alloc, n_tab * sizeof(float2))) != cudaSuccess)
         return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc tables"));
@@ -311,7 +342,8 @@ int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const dou
     p->d.pre_x = t + 2 * V * N;
     p->d.post_x = t + 3 * V * N;
     p->d.H = t + 4 * V * N;
-    p->d.tw = p->d.H + V * M;
+    p->d.Hx = p->d.H + V * M;
+    p->d.tw = p->d.Hx + V * M;
     if ((e = cudaMalloc((void **)&p->d.B, V * nn * sizeof(float2))) != cudaSuccess)
         return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc B"));
     if ((e = cudaMalloc((void **)&p->d.inten_ws, V * nn * sizeof(float))) != cudaSuccess)
@@ -362,11 +394,30 @@ int sfd_plan_update_view(sfd_plan *p, int view, double p1, double p2, double z, 
                          double Oy) {
     if (!p || view < 0 || view >= p->d.V) return SFD_EINVAL;
     if (check_view(p->lambda, p1, p2, z, Ox, Oy) != SFD_OK) return SFD_EINVAL;
-    p->p1[view] = p1;
-    p->p2[view] = p2;
+    p->p1[view] = p->p1y[view] = p1;
+    p->p2[view] = p->p2y[view] = p2;
     p->z[view] = z;
     p->Ox[view] = Ox;
     p->Oy[view] = Oy;
+    p->O0x[view] = p->O0y[view] = 0.0;
+    return upload_view(p, view);
+}
+
+int sfd_plan_update_view_general(sfd_plan *p, int view, double p1x, double p1y, double p2x,
+                                 double p2y, double z, double O0x, double O0y, double O1x,
+                                 double O1y) {
+    if (!p || view < 0 || view >= p->d.V) return SFD_EINVAL;
+    if (check_view(p->lambda, p1x, p2x, z, O1x, O0x) != SFD_OK) return SFD_EINVAL;
+    if (check_view(p->lambda, p1y, p2y, z, O1y, O0y) != SFD_OK) return SFD_EINVAL;
+    p->p1[view] = p1x;
+    p->p1y[view] = p1y;
+    p->p2[view] = p2x;
+    p->p2y[view] = p2y;
+    p->z[view] = z;
+    p->Ox[view] = O1x;
+    p->Oy[view] = O1y;
+    p->O0x[view] = O0x;
+    p->O0y[view] = O0y;
     return upload_view(p, view);
 }
 

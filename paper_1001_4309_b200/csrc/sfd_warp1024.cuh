@@ -116,6 +116,9 @@ template <int DIR, int K> __device__ __forceinline__ float2 mul_w32(float2 a) {
 // X[k] = E[k] + W^k O[k], X[k+16] = E[k] - W^k O[k] with E/O the 16-point DFTs of the even/odd
 // inputs.
 template <int DIR> __device__ __forceinline__ void dft32(float2 (&a)[32]) {
+#ifdef SFDW_NOFFT  // timing experiment only: the butterflies vanish, everything else stays
+    return;
+#endif
     float2 e[16], o[16];
 #pragma unroll
     for (int s = 0; s < 16; ++s) {
@@ -140,7 +143,7 @@ template <int DIR> __device__ __forceinline__ void dft32(float2 (&a)[32]) {
 #define SFDW_WX 8   // warps per CTA in pass x (pairs of them work on a row)
 #endif
 #ifndef SFDW_TWR
-#define SFDW_TWR 1  // 1: inter-stage twiddles live in registers, 0: read from shared memory
+#define SFDW_TWR 1  // inter-stage twiddles: 1 in registers, 0 from shared memory, 2 from tensor memory
 #endif
 #ifndef SFDW_PINGPONG
 // coupling of the two warps that share a sub-partition (see Turns below); measured on config 2
@@ -166,7 +169,8 @@ __device__ __forceinline__ void stamp(long long *tr, int i) {
 #else
 #define SFDW_STAMP(i)
 #endif
-constexpr bool TWR = SFDW_TWR != 0;
+constexpr bool TWR = SFDW_TWR == 1;
+constexpr bool TWT = SFDW_TWR == 2;
 constexpr int TWN = TWR ? 32 : 1;  // length of the per-thread twiddle register vector
 
 // ---- small PTX helpers ---------------------------------------------------------------------------
@@ -240,6 +244,7 @@ constexpr int TABS = 2 * 3 * N;  // complex elements
 constexpr int TM_COLS = 512;      // allocated columns (all of it: one CTA per SM)
 constexpr int TM_SET = 192;       // columns of one view set
 constexpr int TM_TAB = 64;        // columns of one table
+constexpr int TM_TW = 2 * TM_SET;  // first of the 64 twiddle columns (SFDW_TWR == 2)
 struct TChunk { unsigned w[16]; };
 #define SFDW_O16(c) "=r"(c.w[0]), "=r"(c.w[1]), "=r"(c.w[2]), "=r"(c.w[3]), "=r"(c.w[4]), "=r"(c.w[5]), \
     "=r"(c.w[6]), "=r"(c.w[7]), "=r"(c.w[8]), "=r"(c.w[9]), "=r"(c.w[10]), "=r"(c.w[11]), "=r"(c.w[12]), \
@@ -325,7 +330,8 @@ __device__ __forceinline__ void tm_fill(unsigned quarter, int set, const float2 
 // range [total b / g, total (b + 1) / g) of work units touches (per_view units per view), make
 // them visible.  Returns the base address; tm_finish releases it at the end of the kernel.
 __device__ __forceinline__ unsigned tm_setup(unsigned *slot, const float2 *__restrict__ tab,
-                                             int total, int per_view) {
+                                             const float2 *__restrict__ twl, int total,
+                                             int per_view) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (warp == 0) tm_alloc(slot);
     tm_sync_cta();
@@ -337,6 +343,20 @@ __device__ __forceinline__ unsigned tm_setup(unsigned *slot, const float2 *__res
         const unsigned q = tm_quarter(base, warp);
         tm_fill(q, 0, tab, view0, warp, lane);
         if ((a1 - 1) / per_view != view0) tm_fill(q, 1, tab, view0 + 1, warp, lane);
+    }
+    if (TWT && warp < 4) {  // twiddles exp(-2 pi i lane k / 1024), k = 0..31, twl: [k][lane]
+#pragma unroll 1
+        for (int j = 0; j < 4; ++j) {
+            TChunk c;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const float2 x = __ldg(twl + (8 * j + i) * 32 + lane);
+                c.w[2 * i] = __float_as_uint(x.x);
+                c.w[2 * i + 1] = __float_as_uint(x.y);
+            }
+            tm_st(c, tm_quarter(base, warp) + TM_TW + 16 * j);
+        }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
     tm_sync_cta();
     return base;
@@ -480,12 +500,25 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
             SFDW_STAMP(16 + 4 * step + 1);
             if (step != 1) turn_end(turns);
         } else {
+            if constexpr (TWT) {
+                const unsigned tt = (t & 0xffff0000u) + TM_TW;  // twiddle columns of this quarter
+                tm_ld(c0, tt);
 #pragma unroll
-            for (int k = 1; k < 32; ++k) {
-                if constexpr (TWR)
-                    v[k] = cmul(v[k], tw[k]);
-                else
-                    v[k] = cmul(v[k], twsm[k * 32 + lane]);
+                for (int j = 0; j < 4; ++j) {
+                    TChunk &c = (j & 1) ? c1 : c0;
+                    tm_wait(c);
+                    if (j < 3) tm_ld((j & 1) ? c0 : c1, tt + 16 * (j + 1));
+#pragma unroll
+                    for (int i = (j == 0 ? 1 : 0); i < 8; ++i) v[8 * j + i] = cmul(v[8 * j + i], tm_val(c, i));
+                }
+            } else {
+#pragma unroll
+                for (int k = 1; k < 32; ++k) {
+                    if constexpr (TWR)
+                        v[k] = cmul(v[k], tw[k]);
+                    else
+                        v[k] = cmul(v[k], twsm[k * 32 + lane]);
+                }
             }
             SFDW_STAMP(16 + 4 * step + 1);
             turn_end(turns);
@@ -552,7 +585,7 @@ template <> struct TileElem<float> {                 // float: 1 item per slab
 template <typename TIn> struct SmemY {
     float2 xb[WY][XB];
     alignas(128) float2 stage[2][N][2];  // [half][n1][column of the half]: final sums, TMA store source
-    float2 tw[TWR ? 1 : 32 * 32];
+    float2 tw[SFDW_TWR == 0 ? 32 * 32 : 1];
     typename TileElem<TIn>::type tile[2][TileElem<TIn>::IPS][N];  // [half][k][n0]: the half's slab
     unsigned long long turn[8];
     unsigned tmem;  // base address of the tensor-memory allocation

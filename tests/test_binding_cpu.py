@@ -91,3 +91,23 @@ def test_host_tables_reject_bad_arguments():
         B.sfd_host_tables(100, W.LAMBDA, W.PITCH, W.PITCH, 0.05, 0.0)
     with pytest.raises(B.SfdError):
         B.sfd_host_tables(64, W.LAMBDA, W.PITCH, W.PITCH, 0.0, 0.0)
+
+
+@pytest.mark.parametrize("N,p1,p2,z,off0,off", [
+    (64, 4.65e-6, 3.0e-6, 0.05, 0.1e-3, -0.2e-3),
+    (1024, 6.0e-6, 1.5e-6, 0.08, -0.3e-3, 0.5e-3),
+    (1024, 4.65e-6, 4.65e-6, -0.07, 0.25e-3, 0.0),
+])
+def test_host_tables_general_match_oracle_tables(N, p1, p2, z, off0, off):
+    """General geometry (row f3): hologram-window offset O_0 of Eq.(2)-(3), L58-62, and a hologram
+    pitch different from the default; the plan's float64 tables against the oracle's factors."""
+    lam = W.LAMBDA
+    pre, post, H = B.sfd_host_tables_general(N, lam, p1, p2, z, off0, off)
+    assert np.max(np.abs(pre - O.pre_chirp(N, lam, z, p1, p2, off0, off))) < 2e-11
+    assert np.max(np.abs(post - O.post_chirp(N, lam, z, p1, p2, off0, off))) < 2e-11
+    H_o = np.fft.fft(O.chirp_kernel(N, 2 * N, O.scale_factor(lam, z, p1, p2))) / (2 * N)
+    assert np.max(np.abs(H - H_o)) < 1e-12 * max(1.0, np.max(np.abs(H_o)) * 2 * N)
+    # off0 = 0 is the square entry point
+    a, b, c = B.sfd_host_tables_general(N, lam, p1, p2, z, 0.0, off)
+    a2, b2, c2 = B.sfd_host_tables(N, lam, p1, p2, z, off)
+    assert np.array_equal(a, a2) and np.array_equal(b, b2) and np.array_equal(c, c2)
