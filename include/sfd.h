@@ -84,6 +84,19 @@ SFD_API int sfd_execute(sfd_plan *plan, const void *hologram_dev, void *field_de
 SFD_API int sfd_execute_u8(sfd_plan *plan, const void *hologram_dev, unsigned char *intensity_u8_dev,
                    void *stream);
 
+/* Depth stacks / focus sweep ("different depths along the depth direction",
+ * PAPER.md L33 and Fig. 1): a plan whose views differ only in z is a depth stack of one hologram.
+ * This call runs the same two passes and, fused into the last one, reduces every view to its first
+ * two intensity moments
+ *     moments_dev[2 v] = sum over the N x N window of I,   moments_dev[2 v + 1] = sum of I^2
+ * (device array of 2 n_views doubles; per-thread partial sums in float32, accumulation across warps
+ * in float64 with atomics: the last bits depend on the order of arrival).  The paper defines no
+ * focus measure (reading 21); any variance-type measure follows from the two moments,
+ * e.g. the normalised variance N^2 sum I^2 / (sum I)^2 - 1.  intensity_dev ([n_views][N][N] float32)
+ * may be NULL: nothing but the moments is then written.  Asynchronous on `stream`. */
+SFD_API int sfd_execute_focus(sfd_plan *plan, const void *hologram_dev, double *moments_dev,
+                              float *intensity_dev, void *stream);
+
 /* Real-time stream (steps (i)-(xi) repeated, L83-97): reconstruct n_frames holograms that sit in
  * page-locked host memory, double-buffering the H2D copies against compute and the D2H copies of
  * the 8-bit results, on three internal streams.  Blocking: returns when out_pinned is complete.

@@ -97,6 +97,20 @@ def intensity(u1):
     return u1.real * u1.real + u1.imag * u1.imag
 
 
+def focus_moments(I):
+    """Row f2 (depth stacks, PAPER.md L33 / Fig. 1): per view the first two moments of the intensity
+    of Eq.(5) over the N x N window, ``(sum I, sum I^2)``, in float64.  ``I`` is ``[V, N, N]``.
+    The paper defines no focus measure; ``normalised_variance`` is the usual one built on them."""
+    I = np.asarray(I, dtype=np.float64)
+    return np.stack([I.sum(axis=(-2, -1)), (I * I).sum(axis=(-2, -1))], axis=-1)
+
+
+def normalised_variance(moments, n_pixels):
+    """``var(I) / mean(I)^2 = P sum I^2 / (sum I)^2 - 1`` from ``focus_moments`` (P pixels)."""
+    m = np.asarray(moments, dtype=np.float64)
+    return n_pixels * m[..., 1] / (m[..., 0] * m[..., 0]) - 1.0
+
+
 def quantise_u8(I):
     """Real-time mode output (step xi L95, reading 15): per image,
     ``I8 = round_half_even(255 I / max I)`` as uint8; an all-zero image maps to zeros."""

@@ -42,6 +42,7 @@ _sig = {
     "sfd_host_tables_general": (C.c_int, [C.c_int] + [C.c_double] * 6 + [_dp, _dp, _dp]),
     "sfd_execute": (C.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "sfd_execute_u8": (C.c_int, [_vp, _vp, _vp, _vp]),
+    "sfd_execute_focus": (C.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "sfd_stream_run": (C.c_int, [_vp, _vp, C.c_int, _vp, _dp]),
     "sfd_plan_update_view": (C.c_int, [_vp, C.c_int] + [C.c_double] * 5),
     "sfd_plan_destroy": (C.c_int, [_vp]),
@@ -156,6 +157,11 @@ def sfd_plan_update_view_general(plan, view, p1x, p1y, p2x, p2y, z, O0x, O0y, O1
 def sfd_execute(plan, hologram_dev, field_dev, intensity_dev, stream=None):
     _chk(_lib.sfd_execute(plan, _ptr(hologram_dev), _ptr(field_dev), _ptr(intensity_dev),
                           _stream(stream)), "sfd_execute")
+
+
+def sfd_execute_focus(plan, hologram_dev, moments_dev, intensity_dev=None, stream=None):
+    _chk(_lib.sfd_execute_focus(plan, _ptr(hologram_dev), _ptr(moments_dev), _ptr(intensity_dev),
+                                _stream(stream)), "sfd_execute_focus")
 
 
 def sfd_execute_u8(plan, hologram_dev, intensity_u8_dev, stream=None):
@@ -293,6 +299,17 @@ class Plan:
             intensity = None
         sfd_execute(self.handle, hologram, field, intensity, stream)
         return field, intensity
+
+    def execute_focus(self, hologram, intensity=False, stream=None):
+        """Depth stack / focus sweep: returns ``(moments[V, 2] float64 = (sum I, sum I^2),
+        intensity[V, N, N] or None)`` as device tensors."""
+        import torch
+        self._check_holo(hologram)
+        mom = torch.empty((self.V, 2), dtype=torch.float64, device=hologram.device)
+        I = (torch.empty((self.V, self.N, self.N), dtype=torch.float32, device=hologram.device)
+             if intensity else None)
+        sfd_execute_focus(self.handle, hologram, mom, I, stream)
+        return mom, I
 
     def execute_u8(self, hologram, out=None, stream=None):
         import torch

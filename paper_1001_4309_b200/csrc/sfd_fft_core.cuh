@@ -284,7 +284,8 @@ template <int LOG2M, int RPC, class SyncF>
 SFD_HD float pass_x_body(int tid, int tile, int view, float2 *smem, const float2 *__restrict__ B,
                          const float2 *__restrict__ pre_x, const float2 *__restrict__ Hx,
                          const float2 *__restrict__ post_x, const float2 *__restrict__ tw,
-                         float2 *__restrict__ field, float *__restrict__ inten, SyncF sync) {
+                         float2 *__restrict__ field, float *__restrict__ inten, SyncF sync,
+                         float &s1, float &s2) {
     using S = Sched<LOG2M>;
     constexpr int N = S::N, T = S::T;
     const int l = tid / T, j = tid % T;
@@ -310,6 +311,8 @@ SFD_HD float pass_x_body(int tid, int tile, int view, float2 *smem, const float2
         const float I = u.x * u.x + u.y * u.y;
         if (inten) inten[row * N + m1] = I;
         mx = I > mx ? I : mx;
+        s1 += I;        // this thread's share of sum I and sum I^2 (focus moments, row f2)
+        s2 += I * I;
     }
     return mx;
 }

@@ -51,8 +51,10 @@ struct sfd_plan {
 
 // Enqueue the kernels of one reconstruction on `st` (sfd_kernels.cu).  `u8` non-NULL selects the
 // 8-bit mode (intensity into the plan's scratch, per-view max, quantise).  Returns a cudaError_t.
+// `mom` non-NULL: [V][2] doubles on the device receive sum I and sum I^2 of every view (focus
+// moments); field and inten may then both be NULL.
 cudaError_t sfd_launch(sfd_plan *p, const void *holo, float2 *field, float *inten,
-                       unsigned char *u8, cudaStream_t st);
+                       unsigned char *u8, cudaStream_t st, double *mom = nullptr);
 // One-time per-process kernel attribute set-up (dynamic shared memory opt-in).
 cudaError_t sfd_kernels_init();
 void sfd_count_launch(int n);

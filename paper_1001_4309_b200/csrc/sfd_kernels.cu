@@ -35,9 +35,10 @@ template <int LOG2M, typename TIn>
 __global__ void __launch_bounds__(Tile<LOG2M>::THREADS_Y)
 k_pass_y(const TIn *__restrict__ holo, const float2 *__restrict__ pre_y,
          const float2 *__restrict__ H, const float2 *__restrict__ post_y,
-         const float2 *__restrict__ tw, float2 *__restrict__ B, unsigned int *vmax) {
+         const float2 *__restrict__ tw, float2 *__restrict__ B, unsigned int *vmax, double *mom) {
     extern __shared__ float2 smem[];
     if (vmax != nullptr && blockIdx.x == 0 && threadIdx.x == 0) vmax[blockIdx.y] = 0u;
+    if (mom != nullptr && blockIdx.x == 0 && threadIdx.x < 2) mom[2 * blockIdx.y + threadIdx.x] = 0.0;
     pass_y_body<LOG2M, Tile<LOG2M>::C, TIn>(threadIdx.x, blockIdx.x, blockIdx.y, smem, holo, pre_y,
                                             H, post_y, tw, B, [] { __syncthreads(); });
 }
@@ -47,11 +48,23 @@ __global__ void __launch_bounds__(Tile<LOG2M>::THREADS_X)
 k_pass_x(const float2 *__restrict__ B, const float2 *__restrict__ pre_x,
          const float2 *__restrict__ H, const float2 *__restrict__ post_x,
          const float2 *__restrict__ tw, float2 *__restrict__ field, float *__restrict__ inten,
-         unsigned int *vmax) {
+         unsigned int *vmax, double *mom) {
     extern __shared__ float2 smem[];
+    float s1 = 0.f, s2 = 0.f;
     float mx = pass_x_body<LOG2M, Tile<LOG2M>::RPC>(threadIdx.x, blockIdx.x, blockIdx.y, smem, B,
                                                     pre_x, H, post_x, tw, field, inten,
-                                                    [] { __syncthreads(); });
+                                                    [] { __syncthreads(); }, s1, s2);
+    if (mom != nullptr) {  // focus moments: warp sums in float, accumulation across warps in double
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+            s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+        }
+        if ((threadIdx.x & 31) == 0) {
+            atomicAdd(mom + 2 * blockIdx.y, (double)s1);
+            atomicAdd(mom + 2 * blockIdx.y + 1, (double)s2);
+        }
+    }
     if (vmax != nullptr) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
@@ -86,10 +99,13 @@ template <typename TIn>
 __global__ void __launch_bounds__(sfdw::WY * 32, 1)
 k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
             const float2 *__restrict__ twl, const __grid_constant__ CUtensorMap tmB,
-            unsigned int *vmax, int V) {
+            unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
     sfdw::SmemY<TIn> &sm = *reinterpret_cast<sfdw::SmemY<TIn> *>(smem4);
-    if (vmax != nullptr && blockIdx.x == 0 && threadIdx.x < V) vmax[threadIdx.x] = 0u;
+    if (vmax != nullptr && blockIdx.x == 0)
+        for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
+    if (mom != nullptr && blockIdx.x == 0)
+        for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
     if (threadIdx.x == 0) {
         for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
         sfdw::mbar_fence_init();
@@ -111,7 +127,7 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
 __global__ void __launch_bounds__(sfdw::WX * 32, 1)
 k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
             const float2 *__restrict__ twl, float2 *__restrict__ field, float *__restrict__ inten,
-            unsigned int *vmax, int V) {
+            unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
     sfdw::SmemX &sm = *reinterpret_cast<sfdw::SmemX *>(smem4);
     if (threadIdx.x == 0) {
@@ -127,9 +143,9 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
     const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabX, twl, V * gpv, gpv);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     if (((threadIdx.x >> 5) & 1) == 0)
-        sfdw::pass_x_loop<0>(sm, B, tq, tw, field, inten, vmax, V);
+        sfdw::pass_x_loop<0>(sm, B, tq, tw, field, inten, vmax, mom, V);
     else
-        sfdw::pass_x_loop<1>(sm, B, tq, tw, field, inten, vmax, V);
+        sfdw::pass_x_loop<1>(sm, B, tq, tw, field, inten, vmax, mom, V);
     sfdw::tm_finish(tbase);
 }
 
@@ -137,7 +153,7 @@ std::atomic<long long> g_launches{0};
 int g_sms = 0;
 
 cudaError_t launch_warp1024(sfd_plan *p, const void *holo, float2 *field, float *inten,
-                            unsigned char *u8, cudaStream_t st) {
+                            unsigned char *u8, double *mom, cudaStream_t st) {
     const sfd_dev &d = p->d;
     const int V = d.V;
     unsigned int *vmax = u8 ? d.vmax : nullptr;
@@ -153,14 +169,14 @@ cudaError_t launch_warp1024(sfd_plan *p, const void *holo, float2 *field, float 
     const CUtensorMap &tmB = *reinterpret_cast<const CUtensorMap *>(p->tmapB);
     if (d.in_dtype == 0)
         k_cols_1024<unsigned char><<<gy, sfdw::WY * 32, sizeof(sfdw::SmemY<unsigned char>), st>>>(
-            (const unsigned char *)holo, d.w_tabY, d.w_twl, tmB, vmax, V);
+            (const unsigned char *)holo, d.w_tabY, d.w_twl, tmB, vmax, mom, V);
     else
         k_cols_1024<float><<<gy, sfdw::WY * 32, sizeof(sfdw::SmemY<float>), st>>>(
-            (const float *)holo, d.w_tabY, d.w_twl, tmB, vmax, V);
+            (const float *)holo, d.w_tabY, d.w_twl, tmB, vmax, mom, V);
     if (timing) cudaEventRecord(p->ev[1], st);
     const int gx = gy;
     k_rows_1024<<<gx, sfdw::WX * 32, sizeof(sfdw::SmemX), st>>>(d.B, d.w_tabX, d.w_twl, field, inten,
-                                                                vmax, V);
+                                                                vmax, mom, V);
     if (timing) cudaEventRecord(p->ev[2], st);
     int n = 2;
     if (u8) {
@@ -187,7 +203,7 @@ template <int LOG2M, typename TIn> cudaError_t set_attr() {
 
 template <int LOG2M>
 cudaError_t launch_t(sfd_plan *p, const void *holo, float2 *field, float *inten,
-                     unsigned char *u8, cudaStream_t st) {
+                     unsigned char *u8, double *mom, cudaStream_t st) {
     using TL = Tile<LOG2M>;
     const sfd_dev &d = p->d;
     const int N = d.N, V = d.V;
@@ -201,13 +217,13 @@ cudaError_t launch_t(sfd_plan *p, const void *holo, float2 *field, float *inten,
     dim3 gy(N / TL::C, V), gx(N / TL::RPC, V);
     if (d.in_dtype == 0)
         k_pass_y<LOG2M, unsigned char><<<gy, TL::THREADS_Y, TL::SMEM_Y, st>>>(
-            (const unsigned char *)holo, d.pre_y, d.H, d.post_y, d.tw, d.B, vmax);
+            (const unsigned char *)holo, d.pre_y, d.H, d.post_y, d.tw, d.B, vmax, mom);
     else
         k_pass_y<LOG2M, float><<<gy, TL::THREADS_Y, TL::SMEM_Y, st>>>(
-            (const float *)holo, d.pre_y, d.H, d.post_y, d.tw, d.B, vmax);
+            (const float *)holo, d.pre_y, d.H, d.post_y, d.tw, d.B, vmax, mom);
     if (timing) cudaEventRecord(p->ev[1], st);
     k_pass_x<LOG2M><<<gx, TL::THREADS_X, TL::SMEM_X, st>>>(d.B, d.pre_x, d.Hx, d.post_x, d.tw, field,
-                                                           inten, vmax);
+                                                           inten, vmax, mom);
     if (timing) cudaEventRecord(p->ev[2], st);
     int n = 2;
     if (u8) {
@@ -274,19 +290,19 @@ cudaError_t sfd_kernels_init() {
 }
 
 cudaError_t sfd_launch(sfd_plan *p, const void *holo, float2 *field, float *inten,
-                       unsigned char *u8, cudaStream_t st) {
+                       unsigned char *u8, cudaStream_t st, double *mom) {
     // N = 1024: warp-pair-per-line kernels (their slab loads read 8 bytes of a hologram row at once:
     // the hologram must be aligned accordingly)
     if (p->d.N == sfdw::N && p->kernels != SFD_KERNELS_GENERIC && p->d.w_twl != nullptr &&
         (reinterpret_cast<size_t>(holo) & (p->d.in_dtype == 0 ? 7 : 15)) == 0)
-        return launch_warp1024(p, holo, field, inten, u8, st);
+        return launch_warp1024(p, holo, field, inten, u8, mom, st);
     switch (p->d.log2M) {
-        case 7: return launch_t<7>(p, holo, field, inten, u8, st);
-        case 8: return launch_t<8>(p, holo, field, inten, u8, st);
-        case 9: return launch_t<9>(p, holo, field, inten, u8, st);
-        case 10: return launch_t<10>(p, holo, field, inten, u8, st);
-        case 11: return launch_t<11>(p, holo, field, inten, u8, st);
-        case 12: return launch_t<12>(p, holo, field, inten, u8, st);
+        case 7: return launch_t<7>(p, holo, field, inten, u8, mom, st);
+        case 8: return launch_t<8>(p, holo, field, inten, u8, mom, st);
+        case 9: return launch_t<9>(p, holo, field, inten, u8, mom, st);
+        case 10: return launch_t<10>(p, holo, field, inten, u8, mom, st);
+        case 11: return launch_t<11>(p, holo, field, inten, u8, mom, st);
+        case 12: return launch_t<12>(p, holo, field, inten, u8, mom, st);
     }
     return cudaErrorInvalidValue;
 }

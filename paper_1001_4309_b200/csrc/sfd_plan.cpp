@@ -429,6 +429,14 @@ int sfd_execute(sfd_plan *p, const void *hologram_dev, void *field_dev, float *i
     return SFD_OK;
 }
 
+int sfd_execute_focus(sfd_plan *p, const void *hologram_dev, double *moments_dev,
+                      float *intensity_dev, void *stream) {
+    if (!p || !hologram_dev || !moments_dev) return SFD_EINVAL;
+    SFD_CUDA(sfd_launch(p, hologram_dev, nullptr, intensity_dev, nullptr, (cudaStream_t)stream,
+                        moments_dev));
+    return SFD_OK;
+}
+
 int sfd_execute_u8(sfd_plan *p, const void *hologram_dev, unsigned char *intensity_u8_dev,
                    void *stream) {
     if (!p || !hologram_dev || !intensity_u8_dev) return SFD_EINVAL;

@@ -752,7 +752,8 @@ template <int B>
 __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict__ Bin,
                                             unsigned tq,
                                             const float2 (&tw)[TWN], float2 *__restrict__ field,
-                                            float *__restrict__ inten, unsigned int *vmax, int V) {
+                                            float *__restrict__ inten, unsigned int *vmax,
+                                            double *mom, int V) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, pair = warp >> 1;
     constexpr int gpv = (N + XP - 1) / XP;  // units per view
     const int units = V * gpv;
@@ -818,7 +819,7 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
 #endif
         add_halves<B>(v, xb, xbp, lane, pair);
         SFDW_STAMP(8);
-        float mx = 0.f;
+        float mx = 0.f, s1 = 0.f, s2 = 0.f;
         const size_t off = row * N;
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
@@ -828,6 +829,24 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
             const float I = w.x * w.x + w.y * w.y;
             if (inten) inten[off + m1] = I;
             mx = fmaxf(mx, I);
+        }
+        if (mom != nullptr) {  // focus moments (row f2): sum I, sum I^2 of the view
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                const float2 w = v[16 * B + q];
+                const float I = w.x * w.x + w.y * w.y;
+                s1 += I;
+                s2 = fmaf(I, I, s2);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+                s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+            }
+            if (lane == 0) {
+                atomicAdd(mom + 2 * view, (double)s1);
+                atomicAdd(mom + 2 * view + 1, (double)s2);
+            }
         }
         if (vmax != nullptr) {
 #pragma unroll

@@ -177,6 +177,15 @@ def small_multiview(N=256, V=3, seed=7):
                     O[:, 1].copy(), IN_U8, z_obj=0.05, seed=seed)
 
 
+def depth_stack(N=1024, V=16, z0=0.04, z1=0.12, p2=PITCH, seed=1, z_obj=0.08):
+    """Row f2: one Gabor hologram (object at ``z_obj``), V views that differ only in z (linear sweep
+    z0..z1), no shift — the focus sweep a user of the microscope runs to find the object plane."""
+    z = np.linspace(z0, z1, V)
+    zero = np.zeros(V)
+    return Workload(f"depth_stack_{N}x{V}", N, LAMBDA, np.full(V, PITCH), np.full(V, p2), z, zero,
+                    zero.copy(), IN_U8, z_obj=z_obj, seed=seed)
+
+
 # --------------------------------------------------------------------------------------
 # host-side sharding for --gpus N (views and frames are independent: no collective)
 # --------------------------------------------------------------------------------------

@@ -346,3 +346,47 @@ def test_round_trip_on_gpu_at_unit_SN():
     rec = fr[0].cpu().numpy().astype(np.complex128) + 1j * fi[0].cpu().numpy().astype(np.complex128)
     err = np.linalg.norm(rec - u0) / np.linalg.norm(u0)
     assert err < 5e-6, f"round trip rel-L2 {err:.3e}"
+
+
+# ---- depth stacks / focus moments ------------------------------------------
+@pytest.mark.parametrize("N,V", [(256, 5), (1024, 6)])
+def test_focus_moments_of_a_depth_stack(N, V):
+    """sfd_execute_focus: per-view (sum I, sum I^2) fused into pass x, against the oracle's moments of
+    form B; the intensity written next to them must be the ordinary one; NULL intensity allowed.
+    Tolerance: fp32 intensities (rel 1e-6 each, random sign) summed over N^2 pixels, partial sums of
+    16-32 pixels in fp32 -> 1e-5 relative is generous."""
+    wl = W.depth_stack(N=N, V=V, z0=0.05, z1=0.11)
+    holo = wl.hologram()
+    h = torch.from_numpy(holo).to(_dev())
+    with B.Plan(wl) as plan:
+        mom, I = plan.execute_focus(h, intensity=True)
+        mom2, none = plan.execute_focus(h)
+        _, I_ref = plan.execute(h, field=False)
+        torch.cuda.synchronize()
+    assert none is None
+    assert torch.equal(I, I_ref)
+    _, I_or = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, form="B")
+    want = O.focus_moments(I_or)
+    for got in (mom.cpu().numpy(), mom2.cpu().numpy()):
+        assert got.shape == (V, 2)
+        assert np.max(np.abs(got / want - 1.0)) < 1e-5
+    nv_gpu = O.normalised_variance(mom.cpu().numpy(), N * N)
+    nv_or = O.normalised_variance(want, N * N)
+    assert np.max(np.abs(nv_gpu - nv_or)) < 1e-4 * np.max(np.abs(nv_or)) + 1e-7
+    assert int(np.argmax(nv_gpu)) == int(np.argmax(nv_or)) or np.isclose(np.max(nv_or), np.sort(nv_or)[-2], rtol=1e-4)
+
+
+def test_focus_moments_delta_closed_form_on_gpu():
+    """P4 on the CUDA path: a delta gives constant modulus, so sum I = N^2 c^2, sum I^2 = N^2 c^4."""
+    N = 128
+    u0 = np.zeros((N, N), dtype=np.float32)
+    u0[40, 77] = 1.0
+    zs = np.array([0.03, 0.06, -0.09])
+    with B.Plan(N=N, lam=W.LAMBDA, p1=np.full(3, W.PITCH), p2=np.full(3, 2.0e-6), z=zs, Ox=np.zeros(3),
+                Oy=np.zeros(3), in_dtype=B.SFD_F32) as plan:
+        mom, _ = plan.execute_focus(torch.from_numpy(u0).to(_dev()))
+        torch.cuda.synchronize()
+    c2 = (W.PITCH ** 2 / (W.LAMBDA * np.abs(zs))) ** 2
+    m = mom.cpu().numpy()
+    assert np.allclose(m[:, 0], N * N * c2, rtol=2e-6)
+    assert np.allclose(m[:, 1], N * N * c2 * c2, rtol=4e-6)

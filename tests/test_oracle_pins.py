@@ -299,3 +299,32 @@ def test_reconstruct_views_front_end():
     assert fb.shape == (2, 16, 16) and ib.shape == (2, 16, 16)
     assert rel_l2(fb, fd) < 1e-12
     assert np.allclose(ib, np.abs(fd) ** 2, rtol=1e-10)
+
+
+# ---- row f2: focus moments of a depth stack ---------------------------------------------------
+def test_focus_moments_closed_forms():
+    """``focus_moments`` against values fixed without it: (a) a delta reconstructs to constant
+    modulus p0^2/(lambda |z|) (P4), so sum I = N^2 c^2, sum I^2 = N^2 c^4 and the normalised
+    variance is 0 at every depth; (b) at S = 1/N the map is unitary (P8): sum I p1^2 = sum |u0|^2 p0^2;
+    (c) two-valued image: moments by counting."""
+    N = 32
+    u0 = np.zeros((N, N))
+    u0[7, 20] = 1.0
+    zs = [0.03, 0.05, -0.08]
+    I = np.stack([O.intensity(O.bluestein_fft(u0, LAM, z, P, 2.0e-6, (0.1e-3, 0.0))) for z in zs])
+    m = O.focus_moments(I)
+    c2 = np.array([(P * P / (LAM * abs(z))) ** 2 for z in zs])
+    assert np.allclose(m[:, 0], N * N * c2, rtol=1e-11)
+    assert np.allclose(m[:, 1], N * N * c2 * c2, rtol=1e-11)
+    assert np.all(np.abs(O.normalised_variance(m, N * N)) < 1e-10)
+    rng = np.random.default_rng(21)
+    p1 = 3.3e-6
+    z = N * P * p1 / LAM
+    u = rng.random((N, N))
+    m = O.focus_moments(O.intensity(O.bluestein_fft(u, LAM, z, P, p1))[None])
+    assert np.isclose(m[0, 0] * p1 * p1, np.sum(u * u) * P * P, rtol=1e-11)
+    img = np.full((1, 4, 4), 2.0)
+    img[0, :2] = 3.0                       # 8 pixels of 3, 8 pixels of 2
+    m = O.focus_moments(img)
+    assert m[0, 0] == 40.0 and m[0, 1] == 8 * 9 + 8 * 4
+    assert np.isclose(O.normalised_variance(m, 16)[0], 16 * 104 / 1600 - 1)
