@@ -102,10 +102,7 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
             unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
     sfdw::SmemY<TIn> &sm = *reinterpret_cast<sfdw::SmemY<TIn> *>(smem4);
-    if (vmax != nullptr && blockIdx.x == 0)
-        for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
-    if (mom != nullptr && blockIdx.x == 0)
-        for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
+    sfdw::pdl_launch_dependents();
     if (threadIdx.x == 0) {
         for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
         sfdw::mbar_fence_init();
@@ -117,6 +114,13 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
     // tables of this CTA's view(s) -> tensor memory (the barriers inside also publish the mbarriers)
     const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabY, twl, V * (sfdw::N / sfdw::YC), sfdw::N / sfdw::YC);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
+    // everything above touches plan constants only; the hologram, B, vmax and mom belong to the
+    // kernels before this one in the stream
+    sfdw::pdl_wait();
+    if (vmax != nullptr && blockIdx.x == 0)
+        for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
+    if (mom != nullptr && blockIdx.x == 0)
+        for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
     if (((threadIdx.x >> 5) & 1) == 0)
         sfdw::pass_y_loop<TIn, 0>(sm, holo, tq, tw, &tmB, V);
     else
@@ -130,6 +134,7 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
             unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
     sfdw::SmemX &sm = *reinterpret_cast<sfdw::SmemX *>(smem4);
+    sfdw::pdl_launch_dependents();
     if (threadIdx.x == 0) {
         for (int i = 0; i < sfdw::XP; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
         for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
@@ -142,6 +147,7 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
     constexpr int gpv = (sfdw::N + sfdw::XP - 1) / sfdw::XP;  // units per view, as in pass_x_loop
     const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabX, twl, V * gpv, gpv);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
+    sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
     if (((threadIdx.x >> 5) & 1) == 0)
         sfdw::pass_x_loop<0>(sm, B, tq, tw, field, inten, vmax, mom, V);
     else
@@ -167,16 +173,35 @@ cudaError_t launch_warp1024(sfd_plan *p, const void *holo, float2 *field, float 
     // most two views (the kernels hold two table sets)
     const int gy = V > g_sms ? V : g_sms;
     const CUtensorMap &tmB = *reinterpret_cast<const CUtensorMap *>(p->tmapB);
-    if (d.in_dtype == 0)
-        k_cols_1024<unsigned char><<<gy, sfdw::WY * 32, sizeof(sfdw::SmemY<unsigned char>), st>>>(
-            (const unsigned char *)holo, d.w_tabY, d.w_twl, tmB, vmax, mom, V);
-    else
-        k_cols_1024<float><<<gy, sfdw::WY * 32, sizeof(sfdw::SmemY<float>), st>>>(
-            (const float *)holo, d.w_tabY, d.w_twl, tmB, vmax, mom, V);
+    // Programmatic dependent launch: a kernel may start on an SM as soon as the kernel before it in
+    // the stream has left that SM, runs its prologue (barriers, twiddles, tensor-memory tables) and
+    // waits (griddepcontrol.wait) for the whole predecessor before touching its data.
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(gy);
+    cfg.blockDim = dim3(sfdw::WY * 32);
+    cfg.stream = st;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    cudaError_t le;
+    if (d.in_dtype == 0) {
+        cfg.dynamicSmemBytes = sizeof(sfdw::SmemY<unsigned char>);
+        le = cudaLaunchKernelEx(&cfg, k_cols_1024<unsigned char>, (const unsigned char *)holo,
+                                (const float2 *)d.w_tabY, (const float2 *)d.w_twl, tmB, vmax, mom, V);
+    } else {
+        cfg.dynamicSmemBytes = sizeof(sfdw::SmemY<float>);
+        le = cudaLaunchKernelEx(&cfg, k_cols_1024<float>, (const float *)holo,
+                                (const float2 *)d.w_tabY, (const float2 *)d.w_twl, tmB, vmax, mom, V);
+    }
+    if (le != cudaSuccess) return le;
     if (timing) cudaEventRecord(p->ev[1], st);
-    const int gx = gy;
-    k_rows_1024<<<gx, sfdw::WX * 32, sizeof(sfdw::SmemX), st>>>(d.B, d.w_tabX, d.w_twl, field, inten,
-                                                                vmax, mom, V);
+    cfg.blockDim = dim3(sfdw::WX * 32);
+    cfg.dynamicSmemBytes = sizeof(sfdw::SmemX);
+    le = cudaLaunchKernelEx(&cfg, k_rows_1024, (const float2 *)d.B, (const float2 *)d.w_tabX,
+                            (const float2 *)d.w_twl, field, inten, vmax, mom, V);
+    if (le != cudaSuccess) return le;
     if (timing) cudaEventRecord(p->ev[2], st);
     int n = 2;
     if (u8) {

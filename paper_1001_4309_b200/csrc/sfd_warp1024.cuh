@@ -174,6 +174,12 @@ constexpr bool TWT = SFDW_TWR == 2;
 constexpr int TWN = TWR ? 32 : 1;  // length of the per-thread twiddle register vector
 
 // ---- small PTX helpers ---------------------------------------------------------------------------
+// programmatic dependent launch: let the next kernel of the stream start early / wait until the
+// kernels before this one have completed and their writes are visible
+__device__ __forceinline__ void pdl_launch_dependents() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ unsigned smem_u32(const void *p) {
     return (unsigned)__cvta_generic_to_shared(p);
 }
