@@ -280,7 +280,7 @@ SFD_HD void pass_y_body(int tid, int tile, int view, float2 *smem, const TIn *__
 // Pass x (steps (ii)-(x) along x): a CTA takes RPC adjacent rows of one view; thread (l, j), j
 // fastest, works on row row0 + l.  in = B[n1][m0] * pre_x[m0], out * post_x[m1] is the field
 // u1[n1][m1]; intensity = |u1|^2 (Eq. 5).  Returns the largest intensity this thread produced.
-template <int LOG2M, int RPC, class SyncF>
+template <int LOG2M, int RPC, bool MOM, class SyncF>
 SFD_HD float pass_x_body(int tid, int tile, int view, float2 *smem, const float2 *__restrict__ B,
                          const float2 *__restrict__ pre_x, const float2 *__restrict__ Hx,
                          const float2 *__restrict__ post_x, const float2 *__restrict__ tw,
@@ -311,8 +311,10 @@ SFD_HD float pass_x_body(int tid, int tile, int view, float2 *smem, const float2
         const float I = u.x * u.x + u.y * u.y;
         if (inten) inten[row * N + m1] = I;
         mx = I > mx ? I : mx;
-        s1 += I;        // this thread's share of sum I and sum I^2 (focus moments, row f2)
-        s2 += I * I;
+        if (MOM) {      // this thread's share of sum I and sum I^2 (focus moments, row f2)
+            s1 += I;
+            s2 += I * I;
+        }
     }
     return mx;
 }

@@ -43,7 +43,7 @@ k_pass_y(const TIn *__restrict__ holo, const float2 *__restrict__ pre_y,
                                             H, post_y, tw, B, [] { __syncthreads(); });
 }
 
-template <int LOG2M>
+template <int LOG2M, bool MOM>
 __global__ void __launch_bounds__(Tile<LOG2M>::THREADS_X)
 k_pass_x(const float2 *__restrict__ B, const float2 *__restrict__ pre_x,
          const float2 *__restrict__ H, const float2 *__restrict__ post_x,
@@ -51,10 +51,10 @@ k_pass_x(const float2 *__restrict__ B, const float2 *__restrict__ pre_x,
          unsigned int *vmax, double *mom) {
     extern __shared__ float2 smem[];
     float s1 = 0.f, s2 = 0.f;
-    float mx = pass_x_body<LOG2M, Tile<LOG2M>::RPC>(threadIdx.x, blockIdx.x, blockIdx.y, smem, B,
+    float mx = pass_x_body<LOG2M, Tile<LOG2M>::RPC, MOM>(threadIdx.x, blockIdx.x, blockIdx.y, smem, B,
                                                     pre_x, H, post_x, tw, field, inten,
                                                     [] { __syncthreads(); }, s1, s2);
-    if (mom != nullptr) {  // focus moments: warp sums in float, accumulation across warps in double
+    if (MOM) {  // focus moments: warp sums in float, accumulation across warps in double
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             s1 += __shfl_xor_sync(0xffffffffu, s1, o);
@@ -222,7 +222,10 @@ template <int LOG2M, typename TIn> cudaError_t set_attr() {
                                          cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)Tile<LOG2M>::SMEM_Y);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_pass_x<LOG2M>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    e = cudaFuncSetAttribute(k_pass_x<LOG2M, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)Tile<LOG2M>::SMEM_X);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_pass_x<LOG2M, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 (int)Tile<LOG2M>::SMEM_X);
 }
 
@@ -247,8 +250,12 @@ cudaError_t launch_t(sfd_plan *p, const void *holo, float2 *field, float *inten,
         k_pass_y<LOG2M, float><<<gy, TL::THREADS_Y, TL::SMEM_Y, st>>>(
             (const float *)holo, d.pre_y, d.H, d.post_y, d.tw, d.B, vmax, mom);
     if (timing) cudaEventRecord(p->ev[1], st);
-    k_pass_x<LOG2M><<<gx, TL::THREADS_X, TL::SMEM_X, st>>>(d.B, d.pre_x, d.Hx, d.post_x, d.tw, field,
-                                                           inten, vmax, mom);
+    if (mom == nullptr)
+        k_pass_x<LOG2M, false><<<gx, TL::THREADS_X, TL::SMEM_X, st>>>(d.B, d.pre_x, d.Hx, d.post_x,
+                                                                      d.tw, field, inten, vmax, mom);
+    else
+        k_pass_x<LOG2M, true><<<gx, TL::THREADS_X, TL::SMEM_X, st>>>(d.B, d.pre_x, d.Hx, d.post_x,
+                                                                     d.tw, field, inten, vmax, mom);
     if (timing) cudaEventRecord(p->ev[2], st);
     int n = 2;
     if (u8) {
