@@ -385,9 +385,9 @@ def run_sfd(args, info):
 # ncu `--set full` DRAM traffic per launch (bytes), copied from profiles/ by hand after each capture;
 # key = (workload name, kernel).  Absent = null in the JSON line.
 NCU_TRAFFIC = {
-    # profiles/r01_v6_launches.md / r01_v6_traffic.json (v6 kernels, config 2)
-    ("paper_4view_1024", "k_cols_1024"): 16353792 + 15067392,
-    ("paper_4view_1024", "k_rows_1024"): 33803520 + 3132672,
+    # profiles/r01_v8_launches.md / r01_v8_traffic.json (v8 kernels, config 2)
+    ("paper_4view_1024", "k_cols_1024"): 16610048 + 15330560,
+    ("paper_4view_1024", "k_rows_1024"): 33810432 + 3081984,
 }
 
 
