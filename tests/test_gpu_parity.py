@@ -390,3 +390,47 @@ def test_focus_moments_delta_closed_form_on_gpu():
     m = mom.cpu().numpy()
     assert np.allclose(m[:, 0], N * N * c2, rtol=2e-6)
     assert np.allclose(m[:, 1], N * N * c2 * c2, rtol=4e-6)
+
+
+# ---- edges of the N = 1024 kernels -------------------------------------------------------------------
+def test_1024_many_views_more_than_sms():
+    """V = 150 views at N = 1024: more views than SMs, so the grid grows to V CTAs (a CTA's range then
+    lies in at most two views) and CTAs run in waves; B, field and intensity are 1.2 + 1.2 + 0.6 GB.
+    The oracle checks a sample of views; all views that share parameters must agree bit for bit."""
+    V = 150
+    rng = np.random.default_rng(77)
+    base = W.config(2)
+    pick = rng.integers(0, 4, V)                      # every view is one of config 2's four
+    kw = dict(N=1024, lam=base.lam, p1=base.p1[pick], p2=base.p2[pick], z=base.z[pick], Ox=base.Ox[pick],
+              Oy=base.Oy[pick], in_dtype=base.in_dtype)
+    holo = base.hologram()
+    with B.Plan(**kw) as plan:
+        assert plan.uses_warp_kernels
+        f, I = plan.execute(torch.from_numpy(holo).to(_dev()))
+        torch.cuda.synchronize()
+    want, _ = O.reconstruct_views(holo, base.lam, base.p1, base.p2, base.z, base.Ox, base.Oy, form="B")
+    first = {int(k): int(np.flatnonzero(pick == k)[0]) for k in np.unique(pick)}
+    for k, v0 in first.items():
+        _assert_close(f[v0:v0 + 1].cpu().numpy(), want[k:k + 1], f"view {v0} (= config 2 view {k})")
+    for v in (0, 1, 73, 148, 149):
+        assert torch.equal(f[v], f[first[int(pick[v])]]), f"view {v} differs from its twin"
+        assert torch.equal(I[v], I[first[int(pick[v])]])
+
+
+def test_1024_unaligned_hologram_falls_back_to_generic_kernels():
+    """The N = 1024 kernels read 8 bytes of a hologram row at once; a hologram that does not start on an
+    8-byte boundary silently takes the generic kernels (same numbers to rounding)."""
+    wl = W.config(1)
+    holo = wl.hologram()
+    buf = torch.empty(holo.size + 16, dtype=torch.uint8, device=_dev())
+    off = 1 if buf.data_ptr() % 8 == 0 else (9 - buf.data_ptr() % 8)
+    view = buf[off:off + holo.size].view(1024, 1024)
+    assert view.data_ptr() % 8 != 0
+    view.copy_(torch.from_numpy(holo))
+    with B.Plan(wl) as plan:
+        n0 = B.sfd_launch_count()
+        f, _ = plan.execute(view)
+        torch.cuda.synchronize()
+        assert B.sfd_launch_count() - n0 == 2
+    fB, _ = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, form="B")
+    _assert_close(f.cpu().numpy(), fB, "unaligned hologram")
