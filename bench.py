@@ -293,7 +293,7 @@ def run_sfd(args, info):
     peak, peak_src = measured_peaks()
     keys = ["k_pass_y", "k_pass_x"]                    # rows of algorithmic()
     # the kernels that actually ran: N = 1024 has its own pair (sfd_plan_uses_warp_kernels)
-    names = ["k_cols_1024", "k_rows_1024"] if plan.uses_warp_kernels else keys
+    names = [f"k_cols_{wl.N}", f"k_rows_{wl.N}"] if plan.uses_warp_kernels else keys
     dom = int(np.argmax(kms[:2]))
     per_kernel = {}
     for k, name in enumerate(names):

@@ -138,16 +138,17 @@ SFD_API int sfd_plan_get_views(const sfd_plan *plan);
 SFD_API int sfd_plan_get_m(const sfd_plan *plan);
 SFD_API long long sfd_plan_device_bytes(const sfd_plan *plan);
 
-/* Kernel selection.  SFD_KERNELS_AUTO (default): N = 1024 runs the one-warp-per-line kernels
- * (DESIGN.md 5.4), every other size the generic shared-memory Stockham kernels.
+/* Kernel selection.  SFD_KERNELS_AUTO (default): N = 1024 and N = 2048 run the warp-per-branch
+ * kernels, every other size the generic shared-memory Stockham kernels.
  * SFD_KERNELS_GENERIC forces the generic kernels at every size (tests, A/B timing).  Both compute
  * the same transform; results differ by fp32 rounding only.  Errors: SFD_EINVAL. */
 #define SFD_KERNELS_AUTO 0
 #define SFD_KERNELS_GENERIC 1
 SFD_API int sfd_plan_select_kernels(sfd_plan *plan, int which);
 
-/* 1 if sfd_execute* on this plan currently runs the N = 1024 warp-pair kernels (k_cols_1024,
- * k_rows_1024), 0 if it runs the generic kernels (k_pass_y, k_pass_x); SFD_EINVAL for NULL. */
+/* 1 if sfd_execute* on this plan currently runs the warp-per-branch kernels (k_cols_1024 /
+ * k_rows_1024 or k_cols_2048 / k_rows_2048), 0 if it runs the generic kernels (k_pass_y, k_pass_x);
+ * SFD_EINVAL for NULL. */
 SFD_API int sfd_plan_uses_warp_kernels(const sfd_plan *plan);
 
 /* Timing aid for benchmarks: CUDA-event time, in milliseconds, of each of the two hot kernels

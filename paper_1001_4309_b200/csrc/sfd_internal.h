@@ -25,6 +25,7 @@ struct sfd_dev {
     unsigned int *vmax = nullptr;  // [V] per-view max intensity (float bits)
     // N = 1024 fast path (sfd_warp1024.cuh); branch b = 0 even bins, 1 odd bins of the 2N-point DFT
     // per view and branch b: pre_b | H_b | conj(post_b), H_0[k] = H[2k], H_1[k] = H[2k+1]
+    // (N = 2048, sfd_warp2048.cuh: four branches, [V][4][5][1024]: preA_b | preB_b | H_b | postA_b | postB_b)
     float2 *w_tabY = nullptr;  // [V][2][3][N]  pre carries 1/255 (uint8 input), post carries c0
     float2 *w_tabX = nullptr;  // [V][2][3][N]
     float2 *w_twl = nullptr;   // [32][32]   exp(-2 pi i lane k / 1024) at [k][lane]

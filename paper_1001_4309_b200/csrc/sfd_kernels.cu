@@ -15,6 +15,7 @@
 #include "sfd_fft_core.cuh"
 #include "sfd_internal.h"
 #include "sfd_warp1024.cuh"
+#include "sfd_warp2048.cuh"
 
 namespace {
 
@@ -155,6 +156,57 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
     sfdw::tm_finish(tbase);
 }
 
+// ---- N = 2048 (sfd_warp2048.cuh): four branches per line, a quad of warps per line ------------------
+// grid = V * cpv CTAs: CTA c works on view c / cpv.  tab: [V][4][5][1024].
+template <typename TIn>
+__global__ void __launch_bounds__(256, 1)
+k_cols_2048(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
+            const float2 *__restrict__ twl, const __grid_constant__ CUtensorMap tmB,
+            unsigned int *vmax, double *mom, int V, int cpv) {
+    extern __shared__ float4 smem4[];
+    sfdq::SmemYQ<TIn> &sm = *reinterpret_cast<sfdq::SmemYQ<TIn> *>(smem4);
+    sfdw::pdl_launch_dependents();
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
+        sfdw::mbar_fence_init();
+    }
+    float2 tw[sfdw::TWN];
+    sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
+    const sfdq::Range rg = sfdq::cta_range(cpv);
+    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabY, rg.view);
+    const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
+    sfdw::pdl_wait();
+    if (vmax != nullptr && blockIdx.x == 0)
+        for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
+    if (mom != nullptr && blockIdx.x == 0)
+        for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
+    sfdq::pass_y_quad<TIn>(sm, holo, tq, tw, &tmB, rg);
+    sfdw::tm_finish(tbase);
+}
+
+__global__ void __launch_bounds__(256, 1)
+k_rows_2048(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
+            const float2 *__restrict__ twl, float2 *__restrict__ field, float *__restrict__ inten,
+            unsigned int *vmax, double *mom, int cpv) {
+    extern __shared__ float4 smem4[];
+    sfdq::SmemXQ &sm = *reinterpret_cast<sfdq::SmemXQ *>(smem4);
+    sfdw::pdl_launch_dependents();
+    if (threadIdx.x == 0) {
+        sfdw::mbar_init(&sm.ibar[0], 1);
+        sfdw::mbar_init(&sm.ibar[1], 1);
+        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
+        sfdw::mbar_fence_init();
+    }
+    float2 tw[sfdw::TWN];
+    sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
+    const sfdq::Range rg = sfdq::cta_range(cpv);
+    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabX, rg.view);
+    const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
+    sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
+    sfdq::pass_x_quad(sm, B, tq, tw, field, inten, vmax, mom, rg);
+    sfdw::tm_finish(tbase);
+}
+
 std::atomic<long long> g_launches{0};
 int g_sms = 0;
 
@@ -206,6 +258,61 @@ cudaError_t launch_warp1024(sfd_plan *p, const void *holo, float2 *field, float 
     int n = 2;
     if (u8) {
         const int quads = sfdw::N * sfdw::N / 4;
+        dim3 gq((quads + 256 * 4 - 1) / (256 * 4), V);
+        k_quantise<<<gq, 256, 0, st>>>((const float4 *)d.inten_ws, d.vmax, (uchar4 *)u8, quads);
+        if (timing) cudaEventRecord(p->ev[3], st);
+        ++n;
+    }
+    p->ev_valid = timing;
+    p->ev_quant = timing && u8 != nullptr;
+    g_launches.fetch_add(n, std::memory_order_relaxed);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_warp2048(sfd_plan *p, const void *holo, float2 *field, float *inten,
+                            unsigned char *u8, double *mom, cudaStream_t st) {
+    const sfd_dev &d = p->d;
+    const int V = d.V;
+    unsigned int *vmax = u8 ? d.vmax : nullptr;
+    if (u8) {
+        field = nullptr;
+        inten = d.inten_ws;
+    }
+    const bool timing = p->timing;
+    if (timing) cudaEventRecord(p->ev[0], st);
+    const int cpv = g_sms / V > 0 ? g_sms / V : 1;  // CTAs per view: a CTA works inside one view
+    const CUtensorMap &tmB = *reinterpret_cast<const CUtensorMap *>(p->tmapB);
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(V * cpv);
+    cfg.blockDim = dim3(256);
+    cfg.stream = st;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    cudaError_t le;
+    if (d.in_dtype == 0) {
+        cfg.dynamicSmemBytes = sizeof(sfdq::SmemYQ<unsigned char>);
+        le = cudaLaunchKernelEx(&cfg, k_cols_2048<unsigned char>, (const unsigned char *)holo,
+                                (const float2 *)d.w_tabY, (const float2 *)d.w_twl, tmB, vmax, mom, V,
+                                cpv);
+    } else {
+        cfg.dynamicSmemBytes = sizeof(sfdq::SmemYQ<float>);
+        le = cudaLaunchKernelEx(&cfg, k_cols_2048<float>, (const float *)holo,
+                                (const float2 *)d.w_tabY, (const float2 *)d.w_twl, tmB, vmax, mom, V,
+                                cpv);
+    }
+    if (le != cudaSuccess) return le;
+    if (timing) cudaEventRecord(p->ev[1], st);
+    cfg.dynamicSmemBytes = sizeof(sfdq::SmemXQ);
+    le = cudaLaunchKernelEx(&cfg, k_rows_2048, (const float2 *)d.B, (const float2 *)d.w_tabX,
+                            (const float2 *)d.w_twl, field, inten, vmax, mom, cpv);
+    if (le != cudaSuccess) return le;
+    if (timing) cudaEventRecord(p->ev[2], st);
+    int n = 2;
+    if (u8) {
+        const int quads = sfdq::NL * sfdq::NL / 4;
         dim3 gq((quads + 256 * 4 - 1) / (256 * 4), V);
         k_quantise<<<gq, 256, 0, st>>>((const float4 *)d.inten_ws, d.vmax, (uchar4 *)u8, quads);
         if (timing) cudaEventRecord(p->ev[3], st);
@@ -278,7 +385,8 @@ cudaError_t launch_t(sfd_plan *p, const void *holo, float2 *field, float *inten,
 // point; it is fetched through the runtime so that the library does not link libcuda.
 cudaError_t sfd_make_tensormaps(sfd_plan *p) {
     static_assert(sizeof(CUtensorMap) <= sizeof(p->tmapB), "tensor map storage");
-    if (p->d.N != sfdw::N || p->d.w_twl == nullptr) return cudaSuccess;
+    if ((p->d.N != sfdw::N && p->d.N != sfdq::NL) || p->d.w_twl == nullptr) return cudaSuccess;
+    const cuuint64_t n = (cuuint64_t)p->d.N;
     typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
                                   const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
                                   const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -288,8 +396,8 @@ cudaError_t sfd_make_tensormaps(sfd_plan *p) {
     cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
     if (e != cudaSuccess) return e;
     if (fn == nullptr || qr != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
-    const cuuint64_t dims[2] = {2ull * sfdw::N, (cuuint64_t)p->d.V * sfdw::N};
-    const cuuint64_t strides[1] = {2ull * sfdw::N * sizeof(float)};
+    const cuuint64_t dims[2] = {2 * n, (cuuint64_t)p->d.V * n};
+    const cuuint64_t strides[1] = {2 * n * sizeof(float)};
     const cuuint32_t box[2] = {4, sfdw::YBOX};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = ((encode_fn)fn)(
@@ -315,6 +423,12 @@ cudaError_t sfd_kernels_init() {
                                   (int)sizeof(sfdw::SmemY<float>))) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(k_rows_1024, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                   (int)sizeof(sfdw::SmemX))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_cols_2048<unsigned char>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)sizeof(sfdq::SmemYQ<unsigned char>))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_cols_2048<float>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)sizeof(sfdq::SmemYQ<float>))) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_rows_2048, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)sizeof(sfdq::SmemXQ))) != cudaSuccess) return e;
     int dev = 0;
     if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
     if ((e = cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
@@ -328,6 +442,9 @@ cudaError_t sfd_launch(sfd_plan *p, const void *holo, float2 *field, float *inte
     if (p->d.N == sfdw::N && p->kernels != SFD_KERNELS_GENERIC && p->d.w_twl != nullptr &&
         (reinterpret_cast<size_t>(holo) & (p->d.in_dtype == 0 ? 7 : 15)) == 0)
         return launch_warp1024(p, holo, field, inten, u8, mom, st);
+    if (p->d.N == sfdq::NL && p->kernels != SFD_KERNELS_GENERIC && p->d.w_twl != nullptr &&
+        (reinterpret_cast<size_t>(holo) & (p->d.in_dtype == 0 ? 7 : 15)) == 0)
+        return launch_warp2048(p, holo, field, inten, u8, mom, st);
     switch (p->d.log2M) {
         case 7: return launch_t<7>(p, holo, field, inten, u8, mom, st);
         case 8: return launch_t<8>(p, holo, field, inten, u8, mom, st);

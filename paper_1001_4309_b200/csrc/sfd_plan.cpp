@@ -150,6 +150,27 @@ void branch_tables(int N, const cd *pre, const cd *post, cd pre_scale, cd post_s
     }
 }
 
+// Tables of the N = 2048 kernels (sfd_warp2048.cuh) for one axis: the 4096-point DFT split by the
+// frequency index modulo 4, w = exp(-2 pi i / 4096); layout [4][5][1024]: for branch b the vectors
+//   preA_b = pre[n] w^(b n), preB_b = pre[n+1024] w^(b (n+1024)), H_b[k] = H[4k+b],
+//   postA_b = post[n] w^(-b n), postB_b = post[n+1024] w^(-b (n+1024))            (n, k < 1024)
+void branch_tables4(const cd *pre, const cd *post, cd pre_scale, cd post_scale, const float2 *H,
+                    float2 *out) {
+    const int Nb = 1024;
+    for (int b = 0; b < 4; ++b)
+        for (int n = 0; n < Nb; ++n) {
+            float2 *o = out + (size_t)b * 5 * Nb + n;
+            for (int half = 0; half < 2; ++half) {
+                const int m = n + half * Nb;
+                const cd w = cis_cycles(-(ld)((long long)b * m) / (ld)4096);
+                const cd a = pre[m] * pre_scale * w, c = post[m] * post_scale * std::conj(w);
+                o[(size_t)half * Nb] = make_float2((float)a.real(), (float)a.imag());
+                o[(size_t)(3 + half) * Nb] = make_float2((float)c.real(), (float)c.imag());
+            }
+            o[(size_t)2 * Nb] = H[4 * n + b];
+        }
+}
+
 // float32 tables of one view, host staging layout: pre_y[N] post_y[N] pre_x[N] post_x[N] Hy[M]
 // Hx[M]; `fast` (or NULL) receives tabY[6N] tabX[6N] of the fast path.  The y axis uses
 // (p1y, p2y, O0y, Oy), the x axis (p1, p2, O0x, Ox): S_x and S_y may differ (Eq.(2)-(4), L58-67).
@@ -164,13 +185,15 @@ void build_view_f32(const sfd_plan *p, int v, float2 *pre_y, float2 *post_y, flo
     axis_tables(N, p->lambda, p->p1y[v], p->p2y[v], p->z[v], p->Oy[v], a.data(), b.data(), p->O0y[v]);
     to_f32(a.data(), pre_y, N, cd(in_scale, 0));
     to_f32(b.data(), post_y, N, c0);
-    if (fast) branch_tables(N, a.data(), b.data(), cd(in_scale, 0), c0, Hy, fast);
+    if (fast && N == 1024) branch_tables(N, a.data(), b.data(), cd(in_scale, 0), c0, Hy, fast);
+    if (fast && N == 2048) branch_tables4(a.data(), b.data(), cd(in_scale, 0), c0, Hy, fast);
     kernel_spectrum(N, p->lambda, p->p1[v], p->p2[v], p->z[v], h.data());
     to_f32(h.data(), Hx, M);
     axis_tables(N, p->lambda, p->p1[v], p->p2[v], p->z[v], p->Ox[v], a.data(), b.data(), p->O0x[v]);
     to_f32(a.data(), pre_x, N);
     to_f32(b.data(), post_x, N);
-    if (fast) branch_tables(N, a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, fast + 6 * (size_t)N);
+    if (fast && N == 1024) branch_tables(N, a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, fast + 6 * (size_t)N);
+    if (fast && N == 2048) branch_tables4(a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, fast + 20 * 1024);
 }
 
 std::atomic<bool> g_init{false};
@@ -231,14 +254,16 @@ int stream_state_make(sfd_plan *p) {
 int upload_view(sfd_plan *p, int v) {
     const int N = p->d.N, M = p->d.M;
     const bool fast = p->d.w_twl != nullptr;
-    std::vector<float2> st((size_t)4 * N + 2 * M + (fast ? 12 * (size_t)N : 0));
+    // fast-path tables of one view and one pass: N = 1024: [2][3][1024], N = 2048: [4][5][1024]
+    const size_t fpass = !fast ? 0 : N == 1024 ? 6 * (size_t)1024 : 20 * (size_t)1024;
+    std::vector<float2> st((size_t)4 * N + 2 * M + 2 * fpass);
     float2 *fs = fast ? st.data() + 4 * N + 2 * M : nullptr;
     build_view_f32(p, v, st.data(), st.data() + N, st.data() + 2 * N, st.data() + 3 * N,
                    st.data() + 4 * N, st.data() + 4 * N + M, fs);
     if (fast) {
-        SFD_CUDA(cudaMemcpy(p->d.w_tabY + (size_t)v * 6 * N, fs, 6 * sizeof(float2) * N,
+        SFD_CUDA(cudaMemcpy(p->d.w_tabY + (size_t)v * fpass, fs, fpass * sizeof(float2),
                             cudaMemcpyHostToDevice));
-        SFD_CUDA(cudaMemcpy(p->d.w_tabX + (size_t)v * 6 * N, fs + 6 * N, 6 * sizeof(float2) * N,
+        SFD_CUDA(cudaMemcpy(p->d.w_tabX + (size_t)v * fpass, fs + fpass, fpass * sizeof(float2),
                             cudaMemcpyHostToDevice));
     }
     const size_t nb = sizeof(float2) * N;
@@ -362,14 +387,15 @@ int sfd_plan_create_general(sfd_plan **out, int N, int n_views, double lambda, c
             cudaSuccess)
             return fail(cuda_fail(e, "cudaMemcpy tw"));
     }
-    if (N == 1024) {   // fast-path tables (sfd_warp1024.cuh)
-        const size_t n_fast = V * 12 * (size_t)N + 32 * 32;
+    if (N == 1024 || N == 2048) {   // fast-path tables (sfd_warp1024.cuh, sfd_warp2048.cuh)
+        const size_t fpass = N == 1024 ? 6 * (size_t)1024 : 20 * (size_t)1024;
+        const size_t n_fast = V * 2 * fpass + 32 * 32;
         if ((e = cudaMalloc(&p->fast_alloc, n_fast * sizeof(float2))) != cudaSuccess)
             return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc fast tables"));
         float2 *f = (float2 *)p->fast_alloc;
         p->d.w_tabY = f;
-        p->d.w_tabX = f + V * 6 * N;
-        p->d.w_twl = f + V * 12 * N;
+        p->d.w_tabX = f + V * fpass;
+        p->d.w_twl = f + V * 2 * fpass;
         p->device_bytes += (long long)(n_fast * sizeof(float2));
         std::vector<float2> twl(32 * 32);
         for (int k = 0; k < 32; ++k)
@@ -514,7 +540,10 @@ int sfd_plan_select_kernels(sfd_plan *p, int which) {
 
 int sfd_plan_uses_warp_kernels(const sfd_plan *p) {
     if (!p) return SFD_EINVAL;
-    return p->d.N == 1024 && p->kernels != SFD_KERNELS_GENERIC && p->d.w_twl != nullptr ? 1 : 0;
+    return (p->d.N == 1024 || p->d.N == 2048) && p->kernels != SFD_KERNELS_GENERIC &&
+                   p->d.w_twl != nullptr
+               ? 1
+               : 0;
 }
 
 int sfd_plan_set_timing(sfd_plan *p, int enable) {

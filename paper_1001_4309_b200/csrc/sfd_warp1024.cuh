@@ -475,6 +475,9 @@ __device__ __forceinline__ void turns_close(Turns &t, int warp) {
 // out v[r] = X[lane + 32 r].  The four radix-32 steps of the branch share one copy of the code
 // (rolled loop): the line transform then fits the instruction cache.  Steps 0 | 1, 2 | 3 are the
 // three turns of the line.  On return v = this warp's partial sums for all 1024 outputs.
+// POST = false (N = 2048 kernels, sfd_warp2048.cuh): the last multiply is left to the caller, on
+// return v = IFFT(H_b FFT(v)) N.
+template <bool POST = true>
 __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
                                        const float2 (&tw)[TWN], const float2 *twsm,
                                        unsigned t, Turns &turns
@@ -489,9 +492,15 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
         SFDW_STAMP(16 + 4 * step);
         TChunk c0, c1;
         const unsigned ta = t + (step >> 1) * TM_TAB;
-        if (step & 1) tm_ld_before(c0, ta, v[0].x);  // in flight during the butterflies
+        const bool mul = POST || step == 1;
+        if ((step & 1) && mul) tm_ld_before(c0, ta, v[0].x);  // in flight during the butterflies
         dft32<-1>(v);
-        if (step & 1) {
+        if ((step & 1) && !mul) {
+#pragma unroll
+            for (int k = 0; k < 32; ++k) v[k].y = -v[k].y;
+            SFDW_STAMP(16 + 4 * step + 1);
+            turn_end(turns);
+        } else if (step & 1) {
 #pragma unroll
             for (int j = 0; j < 4; ++j) {  // v = conj(v * t)
                 TChunk &c = (j & 1) ? c1 : c0;

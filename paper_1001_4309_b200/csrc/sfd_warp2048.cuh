@@ -1,0 +1,331 @@
+// sfd_warp2048.cuh — the N = 2048 kernels: the warp-per-branch scheme of sfd_warp1024.cuh with four
+// branches per line.
+//
+// The padded transform of a 2048-point line has length L = 4096.  Splitting its DFT by the
+// frequency index modulo 4 (one radix-4 step with the zero half skipped on the way in and the
+// discarded half skipped on the way out, w = exp(-2 pi i / L)) gives four independent branches
+// b = 0..3 of 1024-point transforms (n' < 1024):
+//
+//     forward:  X[4k+b] = FFT_1024(y_b)[k],   y_b[n'] = x[n'] w^(b n') + x[n'+1024] w^(b (n'+1024))
+//     inverse:  y[n]    = sum_b w^(-b n) g_b[n mod 1024],   g_b = IFFT_1024(H[4k+b] X[4k+b]) 1024
+//
+// so with the plan-time tables (x = in pre, out = post y)
+//     preA_b = pre[n'] w^(b n'),  preB_b = pre[n'+1024] w^(b (n'+1024)),  H_b[k] = H[4k+b],
+//     postA_b = post[n'] w^(-b n'),  postB_b = post[n'+1024] w^(-b (n'+1024))
+// a line is   out[n'] = sum_b postA_b g_b,  out[n'+1024] = sum_b postB_b g_b,
+//             g_b = IFFT(H_b FFT(in[n'] preA_b + in[n'+1024] preB_b)).
+// A warp owns a branch exactly as in the N = 1024 kernels (same `branch()`, same transpose tile,
+// same twiddles); four warps (a quad) work on a line, a CTA of 8 warps on two lines.  Warp b of a
+// quad finishes output quarter b (n in [512 b, 512 b + 512)): the other three quarters of its
+// partial sums go to the exchange area, one quad barrier later it adds what the others left for it.
+// The five tables of a branch sit in the tensor-memory quarter of its sub-partition (320 columns,
+// one view: a CTA works inside one view, the launcher gives every view floor(SMs / V) CTAs).
+#pragma once
+#include "sfd_warp1024.cuh"
+
+namespace sfdq {
+
+using namespace sfdw;  // N = 1024 is the branch length here
+
+constexpr int NL = 2048;            // line length
+constexpr int NBR = 4;              // branches per line
+constexpr int QTABS = NBR * 5 * N;  // complex elements of one view's tables of one pass: [4][5][N]
+// tensor-memory columns of the five tables of a branch
+constexpr int TQ_PREA = 0, TQ_PREB = 64, TQ_H = 128, TQ_POSTA = 192, TQ_POSTB = 256;
+constexpr int QU = NL / 2;          // work units per view: 2 lines (pass x) / 2 columns (pass y)
+
+__device__ __forceinline__ void quad_sync(int quad) {  // named barrier of the four warps of a quad
+    asm volatile("bar.sync %0, 128;" ::"r"(quad + 1) : "memory");
+}
+__device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "memory"); }
+
+// The two warps of a sub-partition copy the 20 chunks (5 tables x 4 chunks of 8 values) of
+// `view`, branch warp & 3, into their quarter: warp w chunks 0..9, warp w + 4 chunks 10..19, five
+// chunks (40 loads per thread) in flight at a time.  tab: [V][4][5][N] in global memory.
+__device__ __forceinline__ void tmq_fill(unsigned quarter, const float2 *__restrict__ tab, int view,
+                                         int warp, int lane) {
+    const float2 *src = tab + (size_t)view * QTABS + (size_t)(warp & 3) * 5 * N + lane;
+#pragma unroll 1
+    for (int h = 0; h < 2; ++h) {
+        const int ch0 = 10 * (warp >> 2) + 5 * h;
+        TChunk c[5];
+#pragma unroll
+        for (int j = 0; j < 5; ++j)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const float2 x = __ldg(src + 32 * (8 * (ch0 + j) + i));
+                c[j].w[2 * i] = __float_as_uint(x.x);
+                c[j].w[2 * i + 1] = __float_as_uint(x.y);
+            }
+#pragma unroll
+        for (int j = 0; j < 5; ++j) tm_st(c[j], quarter + 16 * (ch0 + j));
+    }
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ unsigned tmq_setup(unsigned *slot, const float2 *__restrict__ tab,
+                                              int view) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (warp == 0) tm_alloc(slot);
+    tm_sync_cta();
+    const unsigned base = *reinterpret_cast<volatile unsigned *>(slot);
+    tmq_fill(tm_quarter(base, warp), tab, view, warp, lane);
+    tm_sync_cta();
+    return base;
+}
+
+// This CTA's view and its contiguous range of the view's QU work units (cpv CTAs per view).
+struct Range { int view, u0, u1; };
+__device__ __forceinline__ Range cta_range(int cpv) {
+    const int view = blockIdx.x / cpv, idx = blockIdx.x % cpv;
+    return Range{view, (int)((long long)QU * idx / cpv), (int)((long long)QU * (idx + 1) / cpv)};
+}
+
+// Exchange area: ex[warp][slot][i][lane], slot = target quarter with the source's own skipped.
+struct Exch { float2 v[8][3][16][32]; };
+
+// g = this warp's branch result for n' = lane + 32 r.  Multiplies it by postA_b / postB_b, keeps
+// output quarter b in `mine` (final after quad_collect) and leaves the other three quarters in
+// the exchange area.  Output quarter oq covers n = lane + 32 (16 oq + i): oq < 2 uses postA and
+// g[16 oq + i], oq >= 2 uses postB and g[16 (oq - 2) + i].
+__device__ __forceinline__ void quad_scatter(const float2 (&g)[32], float2 (&mine)[16], unsigned tq,
+                                             int b, int lane, Exch &ex, int warp) {
+    TChunk c0, c1;
+    tm_ld(c0, tq + TQ_POSTA);
+#pragma unroll
+    for (int oq = 0; oq < 4; ++oq) {
+        const unsigned tab = tq + (oq < 2 ? TQ_POSTA : TQ_POSTB) + 32 * (oq & 1);
+        float2 *dst = &ex.v[warp][oq < b ? oq : oq - 1][0][lane];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            TChunk &c = j ? c1 : c0;
+            tm_wait(c);
+            if (j == 0)
+                tm_ld(c1, tab + 16);
+            else if (oq < 3)
+                tm_ld(c0, tq + (oq + 1 < 2 ? TQ_POSTA : TQ_POSTB) + 32 * ((oq + 1) & 1));
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const float2 w = cmul(g[16 * (oq & 1) + 8 * j + i], tm_val(c, i));
+                if (oq == b)
+                    mine[8 * j + i] = w;
+                else
+                    dst[(8 * j + i) * 32] = w;
+            }
+        }
+    }
+}
+// after the quad barrier: add what the other three warps of the quad left for quarter b
+__device__ __forceinline__ void quad_collect(float2 (&mine)[16], int b, int lane, const Exch &ex,
+                                             int warp) {
+#pragma unroll
+    for (int d = 1; d < 4; ++d) {
+        const int bo = (b + d) & 3;  // the other branch
+        const float2 *src = &ex.v[(warp & 4) | bo][b < bo ? b : b - 1][0][lane];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) mine[i] = padd(mine[i], src[i * 32]);
+    }
+}
+
+// ---- pass x: two rows of B per CTA ------------------------------------------------------------------
+struct SmemXQ {
+    float2 xb[8][XB];
+    Exch ex;
+    float2 inb[2][NL];  // input row of each quad (bulk async copy destination)
+    unsigned long long ibar[2];
+    unsigned long long turn[8];
+    unsigned tmem;
+};
+
+__device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *__restrict__ Bin, unsigned tq,
+                                            const float2 (&tw)[TWN], float2 *__restrict__ field,
+                                            float *__restrict__ inten, unsigned int *vmax,
+                                            double *mom, Range rg) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, quad = warp >> 2, b = warp & 3;
+    float2 *xb = sm.xb[warp];
+    const float2 *in = sm.inb[quad] + lane;
+    const bool issuer = b == 0 && lane == 0;
+    unsigned iphase = 0;
+    bool pending = false;
+    Turns turns = turns_make(sm.turn, warp, SFDW_PINGPONG != 0);
+    turns_open(turns, warp);
+    for (int u = rg.u0; u < rg.u1; ++u) {
+        const size_t row = (size_t)rg.view * NL + 2 * u + quad;
+        if (!pending && issuer)
+            bulk_load(sm.inb[quad], Bin + row * NL, NL * sizeof(float2), &sm.ibar[quad]);
+        const bool has_next = u + 1 < rg.u1;
+        mbar_wait(&sm.ibar[quad], iphase);
+        iphase ^= 1;
+        float2 v[32];
+        {   // v = in[n'] preA_b + in[n' + 1024] preB_b
+            TChunk ca, cb;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                tm_ld(ca, tq + TQ_PREA + 16 * j);
+                tm_ld(cb, tq + TQ_PREB + 16 * j);
+                tm_wait(ca);
+                tm_wait(cb);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int r = 8 * j + i;
+                    v[r] = padd(cmul(in[32 * r], tm_val(ca, i)), cmul(in[32 * r + N], tm_val(cb, i)));
+                }
+            }
+        }
+        // all four warps have consumed the row and read the previous line's exchange area
+        quad_sync(quad);
+        if (has_next && issuer) {
+            fence_async_smem();
+            bulk_load(sm.inb[quad], Bin + (row + 2) * NL, NL * sizeof(float2), &sm.ibar[quad]);
+        }
+        pending = has_next;
+#ifdef SFDW_TRACE
+        long long *tr = g_trace;
+        branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns, tr);
+#else
+        branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns);
+#endif
+        float2 mine[16];
+        quad_scatter(v, mine, tq, b, lane, sm.ex, warp);
+        quad_sync(quad);
+        quad_collect(mine, b, lane, sm.ex, warp);
+        float mx = 0.f, s1 = 0.f, s2 = 0.f;
+        const size_t off = row * NL;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int m1 = lane + 32 * (16 * b + i);
+            const float2 w = mine[i];
+            if (field) field[off + m1] = w;
+            const float I = w.x * w.x + w.y * w.y;
+            if (inten) inten[off + m1] = I;
+            mx = fmaxf(mx, I);
+            if (mom != nullptr) {
+                s1 += I;
+                s2 = fmaf(I, I, s2);
+            }
+        }
+        if (mom != nullptr) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+                s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+            }
+            if (lane == 0) {
+                atomicAdd(mom + 2 * rg.view, (double)s1);
+                atomicAdd(mom + 2 * rg.view + 1, (double)s2);
+            }
+        }
+        if (vmax != nullptr) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+            if (lane == 0) atomicMax(vmax + rg.view, __float_as_uint(mx));
+        }
+    }
+    turns_close(turns, warp);
+}
+
+// ---- pass y: two adjacent hologram columns per CTA --------------------------------------------------
+template <typename TIn> struct SmemYQ {
+    float2 xb[8][XB];
+    Exch ex;
+    alignas(128) float2 stage[NL][2];  // [n1][column]: final sums, TMA store source
+    typename TileElem<TIn>::type tile[TileElem<TIn>::IPS][NL];  // [k][n0]: slab of 8 bytes per row
+    unsigned long long turn[8];
+    unsigned tmem;
+};
+
+// the 256 threads fetch rows tid, tid + 256, .. of the slab that starts at column col
+template <typename TIn>
+__device__ __forceinline__ void slab_load(TileRegs<TIn> &t, const TIn *__restrict__ holo, int col) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+        t.e[i] = __ldg(reinterpret_cast<const typename TileElem<TIn>::slab *>(
+            holo + (size_t)(threadIdx.x + 256 * i) * NL + col));
+}
+__device__ __forceinline__ void slab_store(const TileRegs<unsigned char> &t, unsigned short (*tile)[NL]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int n0 = threadIdx.x + 256 * i;
+        tile[0][n0] = (unsigned short)(t.e[i].x & 0xffffu);
+        tile[1][n0] = (unsigned short)(t.e[i].x >> 16);
+        tile[2][n0] = (unsigned short)(t.e[i].y & 0xffffu);
+        tile[3][n0] = (unsigned short)(t.e[i].y >> 16);
+    }
+}
+__device__ __forceinline__ void slab_store(const TileRegs<float> &t, float2 (*tile)[NL]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) tile[0][threadIdx.x + 256 * i] = t.e[i];
+}
+
+// Work unit g of the view = columns 2 g, 2 g + 1 (quad q takes column 2 g + q); a slab holds IPS
+// units.  tmB: tensor map of B seen as float [V * NL][2 NL] with box 4 x YBOX.
+template <typename TIn>
+__device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *__restrict__ holo,
+                                            unsigned tq, const float2 (&tw)[TWN], const void *tmB,
+                                            Range rg) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, quad = warp >> 2, b = warp & 3;
+    constexpr int IPS = TileElem<TIn>::IPS;
+    if (rg.u0 >= rg.u1) return;  // CTA-uniform
+    float2 *xb = sm.xb[warp];
+    float2 *stg = &sm.stage[0][0];
+    const bool leader = threadIdx.x == 0;  // issues and retires the bulk stores
+    {
+        TileRegs<TIn> t;
+        slab_load<TIn>(t, holo, rg.u0 / IPS * (2 * IPS));
+        slab_store(t, sm.tile);
+    }
+    cta_sync();
+    Turns turns = turns_make(sm.turn, warp, SFDW_PINGPONG != 0);
+    turns_open(turns, warp);
+    for (int g = rg.u0; g < rg.u1; ++g) {
+        const int k = g % IPS;
+        const bool next_slab = g + 1 < rg.u1 && k == IPS - 1;
+        TileRegs<TIn> t;
+        if (next_slab) slab_load<TIn>(t, holo, (g + 1) / IPS * (2 * IPS));
+        float2 v[32];
+        {   // v = a[n'] preA_b + a[n' + 1024] preB_b (a real)
+            TChunk ca, cb;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                tm_ld(ca, tq + TQ_PREA + 16 * j);
+                tm_ld(cb, tq + TQ_PREB + 16 * j);
+                tm_wait(ca);
+                tm_wait(cb);
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int r = 8 * j + i;
+                    const float a0 = tile_value(sm.tile[k][lane + 32 * r], quad);
+                    const float a1 = tile_value(sm.tile[k][lane + 32 * r + N], quad);
+                    const float2 pa = tm_val(ca, i), pb = tm_val(cb, i);
+                    v[r] = make_float2(fmaf(a1, pb.x, a0 * pa.x), fmaf(a1, pb.y, a0 * pa.y));
+                }
+            }
+        }
+#ifdef SFDW_TRACE
+        long long *tr = g_trace;
+        branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns, tr);
+#else
+        branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns);
+#endif
+        // the previous item's bulk stores must have left the staging tile before it is rewritten
+        if (leader) bulk_wait_read();
+        float2 mine[16];
+        quad_scatter(v, mine, tq, b, lane, sm.ex, warp);
+        cta_sync();  // exchange area complete; staging tile and slab free
+        quad_collect(mine, b, lane, sm.ex, warp);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) stg[(lane + 32 * (16 * b + i)) * 2 + quad] = mine[i];
+        if (next_slab) slab_store(t, sm.tile);
+        fence_async_smem();  // staging writes -> async proxy
+        cta_sync();          // staging tile complete, next slab visible, exchange area free
+        if (leader) {
+#pragma unroll
+            for (int j = 0; j < NL / YBOX; ++j)
+                tma_store_2d(tmB, stg + j * YBOX * 2, 4 * g, rg.view * NL + j * YBOX);
+            bulk_commit();
+        }
+    }
+    if (leader) bulk_wait_read();  // shared memory must outlive the last store's reads
+    turns_close(turns, warp);
+}
+
+}  // namespace sfdq

@@ -434,3 +434,40 @@ def test_1024_unaligned_hologram_falls_back_to_generic_kernels():
         assert B.sfd_launch_count() - n0 == 2
     fB, _ = O.reconstruct_views(holo, wl.lam, wl.p1, wl.p2, wl.z, wl.Ox, wl.Oy, form="B")
     _assert_close(f.cpu().numpy(), fB, "unaligned hologram")
+
+
+# ---- the N = 2048 warp kernels (four branches per line, sfd_warp2048.cuh) -----------------------------
+@pytest.mark.parametrize("in_dtype", [B.SFD_U8, B.SFD_F32])
+def test_2048_warp_and_generic_kernels_general_geometry(in_dtype):
+    """N = 2048 has two kernel sets as well.  Both against the oracle on anisotropic, shifted views
+    (z < 0 included), with marked samples in the last row/column and at the 1024 fold; then the 8-bit
+    mode and the focus moments through the warp kernels."""
+    N = 2048
+    rng = np.random.default_rng(91)
+    if in_dtype == B.SFD_F32:
+        holo = rng.random((N, N), dtype=np.float32)
+        holo[N - 1, N - 1] = 40.0
+        holo[1024, 1023] = 25.0
+    else:
+        holo = rng.integers(0, 256, (N, N), dtype=np.uint8)
+        holo[N - 1, N - 1] = 255
+        holo[1024, 1023] = 0
+    want = _general_oracle(holo, _GENERAL, "B")
+    h = torch.from_numpy(holo).to(_dev())
+    with B.Plan(N=N, lam=W.LAMBDA, in_dtype=in_dtype, **_GENERAL) as plan:
+        assert plan.uses_warp_kernels
+        f, I = plan.execute(h)
+        mom, _ = plan.execute_focus(h)
+        u8 = plan.execute_u8(h) if in_dtype == B.SFD_U8 else None
+        plan.select_kernels(B.SFD_KERNELS_GENERIC)
+        assert not plan.uses_warp_kernels
+        fg, _ = plan.execute(h)
+        torch.cuda.synchronize()
+    _assert_close(f.cpu().numpy(), want, "N=2048 warp kernels field")
+    _assert_close(I.cpu().numpy(), O.intensity(want), "N=2048 warp kernels intensity")
+    _assert_close(fg.cpu().numpy(), want, "N=2048 generic kernels field")
+    assert np.max(np.abs(mom.cpu().numpy() / O.focus_moments(O.intensity(want)) - 1.0)) < 1e-5
+    if u8 is not None:
+        for v in range(3):
+            d = np.abs(u8[v].cpu().numpy().astype(int) - O.quantise_u8(O.intensity(want[v])).astype(int))
+            assert d.max() <= 1 and (d > 0).mean() < 1e-3
