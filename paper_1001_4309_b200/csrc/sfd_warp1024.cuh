@@ -631,8 +631,10 @@ __device__ __forceinline__ void tile_store(const TileRegs<float> &t, float2 (*ti
 #pragma unroll
     for (int i = 0; i < 8; ++i) tile[0][ht + 128 * i] = t.e[i];
 }
+// uint8 -> float without the conversion unit (I2F shares the MIO queue with shared memory and is
+// quarter rate): one byte permute drops the sample into the mantissa of 2^23, one add removes 2^23
 __device__ __forceinline__ float tile_value(unsigned short e, int c) {
-    return (float)((e >> (8 * c)) & 0xffu);
+    return __uint_as_float(__byte_perm((unsigned)e, 0x4B000000u, c ? 0x7651u : 0x7650u)) - 8388608.f;
 }
 __device__ __forceinline__ float tile_value(float2 e, int c) { return c ? e.y : e.x; }
 

@@ -228,7 +228,9 @@ template <typename TIn> struct SmemYQ {
     float2 xb[8][XB];
     Exch ex;
     alignas(128) float2 stage[NL][2];  // [n1][column]: final sums, TMA store source
-    typename TileElem<TIn>::type tile[TileElem<TIn>::IPS][NL];  // [k][n0]: slab of 8 bytes per row
+    // slab of 8 bytes per row as column pairs: [k][n'][h] = rows n' and n' + 1024 side by side, so
+    // that one 4-byte (uint8) / 16-byte (float) read gives both samples a thread folds together
+    typename TileElem<TIn>::type tile[TileElem<TIn>::IPS][N][2];
     unsigned long long turn[8];
     unsigned tmem;
 };
@@ -241,19 +243,34 @@ __device__ __forceinline__ void slab_load(TileRegs<TIn> &t, const TIn *__restric
         t.e[i] = __ldg(reinterpret_cast<const typename TileElem<TIn>::slab *>(
             holo + (size_t)(threadIdx.x + 256 * i) * NL + col));
 }
-__device__ __forceinline__ void slab_store(const TileRegs<unsigned char> &t, unsigned short (*tile)[NL]) {
+__device__ __forceinline__ void slab_store(const TileRegs<unsigned char> &t,
+                                           unsigned short (*tile)[N][2]) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int n0 = threadIdx.x + 256 * i, n = n0 & (N - 1), h = n0 >> 10;
+        tile[0][n][h] = (unsigned short)(t.e[i].x & 0xffffu);
+        tile[1][n][h] = (unsigned short)(t.e[i].x >> 16);
+        tile[2][n][h] = (unsigned short)(t.e[i].y & 0xffffu);
+        tile[3][n][h] = (unsigned short)(t.e[i].y >> 16);
+    }
+}
+__device__ __forceinline__ void slab_store(const TileRegs<float> &t, float2 (*tile)[N][2]) {
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
         const int n0 = threadIdx.x + 256 * i;
-        tile[0][n0] = (unsigned short)(t.e[i].x & 0xffffu);
-        tile[1][n0] = (unsigned short)(t.e[i].x >> 16);
-        tile[2][n0] = (unsigned short)(t.e[i].y & 0xffffu);
-        tile[3][n0] = (unsigned short)(t.e[i].y >> 16);
+        tile[0][n0 & (N - 1)][n0 >> 10] = t.e[i];
     }
 }
-__device__ __forceinline__ void slab_store(const TileRegs<float> &t, float2 (*tile)[NL]) {
-#pragma unroll
-    for (int i = 0; i < 8; ++i) tile[0][threadIdx.x + 256 * i] = t.e[i];
+// both samples (rows n' and n' + 1024) of column c of the pair
+__device__ __forceinline__ float2 fold_values(const unsigned short (&e)[2], int c) {
+    const unsigned w = *reinterpret_cast<const unsigned *>(e);  // [n'] low half, [n' + 1024] high half
+    return make_float2(
+        __uint_as_float(__byte_perm(w, 0x4B000000u, c ? 0x7651u : 0x7650u)) - 8388608.f,
+        __uint_as_float(__byte_perm(w, 0x4B000000u, c ? 0x7653u : 0x7652u)) - 8388608.f);
+}
+__device__ __forceinline__ float2 fold_values(const float2 (&e)[2], int c) {
+    const float4 w = *reinterpret_cast<const float4 *>(e);
+    return c ? make_float2(w.y, w.w) : make_float2(w.x, w.z);
 }
 
 // Work unit g of the view = columns 2 g, 2 g + 1 (quad q takes column 2 g + q); a slab holds IPS
@@ -280,7 +297,6 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *__restri
         const int k = g % IPS;
         const bool next_slab = g + 1 < rg.u1 && k == IPS - 1;
         TileRegs<TIn> t;
-        if (next_slab) slab_load<TIn>(t, holo, (g + 1) / IPS * (2 * IPS));
         float2 v[32];
         {   // v = a[n'] preA_b + a[n' + 1024] preB_b (a real)
             TChunk ca, cb;
@@ -293,13 +309,15 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *__restri
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
                     const int r = 8 * j + i;
-                    const float a0 = tile_value(sm.tile[k][lane + 32 * r], quad);
-                    const float a1 = tile_value(sm.tile[k][lane + 32 * r + N], quad);
+                    const float2 a = fold_values(sm.tile[k][lane + 32 * r], quad);
                     const float2 pa = tm_val(ca, i), pb = tm_val(cb, i);
-                    v[r] = make_float2(fmaf(a1, pb.x, a0 * pa.x), fmaf(a1, pb.y, a0 * pa.y));
+                    v[r] = make_float2(fmaf(a.y, pb.x, a.x * pa.x), fmaf(a.y, pb.y, a.x * pa.y));
                 }
             }
         }
+        // the slab of the next items is fetched behind the tile reads: its loads touch one row per
+        // lane (32 wavefronts each) and would hold up everything queued after them
+        if (next_slab) slab_load<TIn>(t, holo, (g + 1) / IPS * (2 * IPS));
 #ifdef SFDW_TRACE
         long long *tr = g_trace;
         branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns, tr);
