@@ -172,7 +172,7 @@ k_cols_2048(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
     }
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
-    const sfdq::Range rg = sfdq::cta_range(cpv);
+    const sfdq::Range rg = sfdq::cta_range(cpv, sfdq::QUY);
     const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabY, rg.view);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     sfdw::pdl_wait();
@@ -199,7 +199,7 @@ k_rows_2048(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
     }
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
-    const sfdq::Range rg = sfdq::cta_range(cpv);
+    const sfdq::Range rg = sfdq::cta_range(cpv, sfdq::QUX);
     const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabX, rg.view);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
@@ -381,7 +381,7 @@ cudaError_t launch_t(sfd_plan *p, const void *holo, float2 *field, float *inten,
 }  // namespace
 
 // Tensor map of the intermediate B for the bulk stores of k_cols_1024: B as float [V * N][2 N],
-// box = 4 floats (two complex columns) x YBOX rows, no swizzle.  The encoder is a driver entry
+// box = 4 floats (two complex columns; N = 2048: 8 floats, four columns) x YBOX rows, no swizzle.  The encoder is a driver entry
 // point; it is fetched through the runtime so that the library does not link libcuda.
 cudaError_t sfd_make_tensormaps(sfd_plan *p) {
     static_assert(sizeof(CUtensorMap) <= sizeof(p->tmapB), "tensor map storage");
@@ -398,7 +398,7 @@ cudaError_t sfd_make_tensormaps(sfd_plan *p) {
     if (fn == nullptr || qr != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
     const cuuint64_t dims[2] = {2 * n, (cuuint64_t)p->d.V * n};
     const cuuint64_t strides[1] = {2 * n * sizeof(float)};
-    const cuuint32_t box[2] = {4, sfdw::YBOX};
+    const cuuint32_t box[2] = {p->d.N == sfdq::NL ? (cuuint32_t)sfdq::YBOXW : 4u, sfdw::YBOX};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = ((encode_fn)fn)(
         reinterpret_cast<CUtensorMap *>(p->tmapB), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, p->d.B, dims,

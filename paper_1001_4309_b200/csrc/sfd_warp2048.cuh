@@ -32,7 +32,8 @@ constexpr int NBR = 4;              // branches per line
 constexpr int QTABS = NBR * 5 * N;  // complex elements of one view's tables of one pass: [4][5][N]
 // tensor-memory columns of the five tables of a branch
 constexpr int TQ_PREA = 0, TQ_PREB = 64, TQ_H = 128, TQ_POSTA = 192, TQ_POSTB = 256;
-constexpr int QU = NL / 2;          // work units per view: 2 lines (pass x) / 2 columns (pass y)
+constexpr int QUX = NL / 2;         // work units per view, pass x: 2 rows
+constexpr int QUY = NL / 4;         // work units per view, pass y: 4 columns (2 per quad)
 
 __device__ __forceinline__ void quad_sync(int quad) {  // named barrier of the four warps of a quad
     asm volatile("bar.sync %0, 128;" ::"r"(quad + 1) : "memory");
@@ -73,28 +74,33 @@ __device__ __forceinline__ unsigned tmq_setup(unsigned *slot, const float2 *__re
     return base;
 }
 
-// This CTA's view and its contiguous range of the view's QU work units (cpv CTAs per view).
+// This CTA's view and its contiguous range of the view's `units` work units (cpv CTAs per view).
 struct Range { int view, u0, u1; };
-__device__ __forceinline__ Range cta_range(int cpv) {
+__device__ __forceinline__ Range cta_range(int cpv, int units) {
     const int view = blockIdx.x / cpv, idx = blockIdx.x % cpv;
-    return Range{view, (int)((long long)QU * idx / cpv), (int)((long long)QU * (idx + 1) / cpv)};
+    return Range{view, (int)((long long)units * idx / cpv), (int)((long long)units * (idx + 1) / cpv)};
 }
 
-// Exchange area: ex[warp][slot][i][lane], slot = target quarter with the source's own skipped.
-struct Exch { float2 v[8][3][16][32]; };
+// Exchange area of a warp: three quarters of 16 x 32 values for the other three warps of the quad
+// (slot = target quarter with the source's own skipped).  Slots 0 and 1 live in the warp's transpose
+// tile, which is idle between two branch() calls, slot 2 in ex.v[warp].
+struct Exch { float2 v[8][16 * 32]; };
+__device__ __forceinline__ float2 *exch_slot(float2 (*xb)[XB], Exch &ex, int warp, int slot) {
+    return slot < 2 ? xb[warp] + slot * (16 * 32) : ex.v[warp];
+}
 
 // g = this warp's branch result for n' = lane + 32 r.  Multiplies it by postA_b / postB_b, keeps
 // output quarter b in `mine` (final after quad_collect) and leaves the other three quarters in
 // the exchange area.  Output quarter oq covers n = lane + 32 (16 oq + i): oq < 2 uses postA and
 // g[16 oq + i], oq >= 2 uses postB and g[16 (oq - 2) + i].
 __device__ __forceinline__ void quad_scatter(const float2 (&g)[32], float2 (&mine)[16], unsigned tq,
-                                             int b, int lane, Exch &ex, int warp) {
+                                             int b, int lane, float2 (*xb)[XB], Exch &ex, int warp) {
     TChunk c0, c1;
     tm_ld(c0, tq + TQ_POSTA);
 #pragma unroll
     for (int oq = 0; oq < 4; ++oq) {
         const unsigned tab = tq + (oq < 2 ? TQ_POSTA : TQ_POSTB) + 32 * (oq & 1);
-        float2 *dst = &ex.v[warp][oq < b ? oq : oq - 1][0][lane];
+        float2 *dst = exch_slot(xb, ex, warp, oq < b ? oq : oq > 0 ? oq - 1 : 0) + lane;
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
             TChunk &c = j ? c1 : c0;
@@ -115,12 +121,12 @@ __device__ __forceinline__ void quad_scatter(const float2 (&g)[32], float2 (&min
     }
 }
 // after the quad barrier: add what the other three warps of the quad left for quarter b
-__device__ __forceinline__ void quad_collect(float2 (&mine)[16], int b, int lane, const Exch &ex,
-                                             int warp) {
+__device__ __forceinline__ void quad_collect(float2 (&mine)[16], int b, int lane, float2 (*xb)[XB],
+                                             Exch &ex, int warp) {
 #pragma unroll
     for (int d = 1; d < 4; ++d) {
         const int bo = (b + d) & 3;  // the other branch
-        const float2 *src = &ex.v[(warp & 4) | bo][b < bo ? b : b - 1][0][lane];
+        const float2 *src = exch_slot(xb, ex, (warp & 4) | bo, b < bo ? b : b - 1) + lane;
 #pragma unroll
         for (int i = 0; i < 16; ++i) mine[i] = padd(mine[i], src[i * 32]);
     }
@@ -185,9 +191,9 @@ __device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *__restrict
         branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns);
 #endif
         float2 mine[16];
-        quad_scatter(v, mine, tq, b, lane, sm.ex, warp);
+        quad_scatter(v, mine, tq, b, lane, sm.xb, sm.ex, warp);
         quad_sync(quad);
-        quad_collect(mine, b, lane, sm.ex, warp);
+        quad_collect(mine, b, lane, sm.xb, sm.ex, warp);
         float mx = 0.f, s1 = 0.f, s2 = 0.f;
         const size_t off = row * NL;
 #pragma unroll
@@ -223,41 +229,60 @@ __device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *__restrict
     turns_close(turns, warp);
 }
 
-// ---- pass y: two adjacent hologram columns per CTA --------------------------------------------------
+// ---- pass y: four adjacent hologram columns per CTA, two per quad -------------------------------------
+// Work unit u of a view = columns 4 u .. 4 u + 3; quad q transforms columns 4 u + 2 q and
+// 4 u + 2 q + 1 one after the other.  The final sums of all four columns meet in one staging tile
+// [n1][4] that one thread hands to the TMA unit: 32 bytes = one full sector per row of B.  (With
+// 16-byte rows B, which at this size does not fit L2, cost 1.2 GB of DRAM traffic per launch for
+// 0.5 GB of payload: half-written sectors are read back and merged.)
+// A quad reads its hologram samples as a slab of 8 bytes per row: uint8 = the 8 columns of two
+// units (its own are bytes 4 k + 2 q + c, k = u % 2), float = its 2 columns of one unit, and keeps
+// them in shared memory as [k][n'][h] column pairs with rows n' and n' + 1024 side by side (one
+// read gives both samples a thread folds together).
+template <typename TIn> struct SubSlab {  // uint8
+    using elem = uint2;
+    static constexpr int IPS = 2;
+    __device__ static int col(int u, int q) { return 8 * (u / 2); }
+};
+template <> struct SubSlab<float> {
+    using elem = float2;
+    static constexpr int IPS = 1;
+    __device__ static int col(int u, int q) { return 4 * u + 2 * q; }
+};
+constexpr int YBOXW = 8;  // floats per row of a TMA store box of pass y (4 complex columns)
 template <typename TIn> struct SmemYQ {
     float2 xb[8][XB];
     Exch ex;
-    alignas(128) float2 stage[NL][2];  // [n1][column]: final sums, TMA store source
-    // slab of 8 bytes per row as column pairs: [k][n'][h] = rows n' and n' + 1024 side by side, so
-    // that one 4-byte (uint8) / 16-byte (float) read gives both samples a thread folds together
-    typename TileElem<TIn>::type tile[TileElem<TIn>::IPS][N][2];
+    alignas(128) float2 stage[NL][4];  // [n1][column of the unit]: final sums, TMA store source
+    typename TileElem<TIn>::type tile[2][SubSlab<TIn>::IPS][N][2];  // [quad][k][n'][h]
     unsigned long long turn[8];
     unsigned tmem;
 };
+template <typename TIn> struct SubRegs { typename SubSlab<TIn>::elem e[16]; };
 
-// the 256 threads fetch rows tid, tid + 256, .. of the slab that starts at column col
+// the 128 threads of a quad fetch rows qt, qt + 128, .. of the slab that starts at column col
 template <typename TIn>
-__device__ __forceinline__ void slab_load(TileRegs<TIn> &t, const TIn *__restrict__ holo, int col) {
+__device__ __forceinline__ void sub_load(SubRegs<TIn> &t, const TIn *__restrict__ holo, int col,
+                                         int qt) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
-        t.e[i] = __ldg(reinterpret_cast<const typename TileElem<TIn>::slab *>(
-            holo + (size_t)(threadIdx.x + 256 * i) * NL + col));
+    for (int i = 0; i < 16; ++i)
+        t.e[i] = __ldg(reinterpret_cast<const typename SubSlab<TIn>::elem *>(
+            holo + (size_t)(qt + 128 * i) * NL + col));
 }
-__device__ __forceinline__ void slab_store(const TileRegs<unsigned char> &t,
-                                           unsigned short (*tile)[N][2]) {
+__device__ __forceinline__ void sub_store(const SubRegs<unsigned char> &t,
+                                          unsigned short (*tile)[N][2], int qt, int quad) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const int n0 = threadIdx.x + 256 * i, n = n0 & (N - 1), h = n0 >> 10;
-        tile[0][n][h] = (unsigned short)(t.e[i].x & 0xffffu);
-        tile[1][n][h] = (unsigned short)(t.e[i].x >> 16);
-        tile[2][n][h] = (unsigned short)(t.e[i].y & 0xffffu);
-        tile[3][n][h] = (unsigned short)(t.e[i].y >> 16);
+    for (int i = 0; i < 16; ++i) {
+        const int n0 = qt + 128 * i, n = n0 & (N - 1), h = n0 >> 10;
+        tile[0][n][h] = (unsigned short)(t.e[i].x >> (16 * quad));
+        tile[1][n][h] = (unsigned short)(t.e[i].y >> (16 * quad));
     }
 }
-__device__ __forceinline__ void slab_store(const TileRegs<float> &t, float2 (*tile)[N][2]) {
+__device__ __forceinline__ void sub_store(const SubRegs<float> &t, float2 (*tile)[N][2], int qt,
+                                          int quad) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const int n0 = threadIdx.x + 256 * i;
+    for (int i = 0; i < 16; ++i) {
+        const int n0 = qt + 128 * i;
         tile[0][n0 & (N - 1)][n0 >> 10] = t.e[i];
     }
 }
@@ -273,73 +298,82 @@ __device__ __forceinline__ float2 fold_values(const float2 (&e)[2], int c) {
     return c ? make_float2(w.y, w.w) : make_float2(w.x, w.z);
 }
 
-// Work unit g of the view = columns 2 g, 2 g + 1 (quad q takes column 2 g + q); a slab holds IPS
-// units.  tmB: tensor map of B seen as float [V * NL][2 NL] with box 4 x YBOX.
+// tmB: tensor map of B seen as float [V * NL][2 NL] with box YBOXW x YBOX.
 template <typename TIn>
 __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *__restrict__ holo,
                                             unsigned tq, const float2 (&tw)[TWN], const void *tmB,
                                             Range rg) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, quad = warp >> 2, b = warp & 3;
-    constexpr int IPS = TileElem<TIn>::IPS;
+    const int qt = threadIdx.x & 127;
+    constexpr int IPS = SubSlab<TIn>::IPS;
     if (rg.u0 >= rg.u1) return;  // CTA-uniform
     float2 *xb = sm.xb[warp];
     float2 *stg = &sm.stage[0][0];
     const bool leader = threadIdx.x == 0;  // issues and retires the bulk stores
     {
-        TileRegs<TIn> t;
-        slab_load<TIn>(t, holo, rg.u0 / IPS * (2 * IPS));
-        slab_store(t, sm.tile);
+        SubRegs<TIn> t;
+        sub_load<TIn>(t, holo, SubSlab<TIn>::col(rg.u0, quad), qt);
+        sub_store(t, sm.tile[quad], qt, quad);
     }
-    cta_sync();
+    quad_sync(quad);
     Turns turns = turns_make(sm.turn, warp, SFDW_PINGPONG != 0);
     turns_open(turns, warp);
-    for (int g = rg.u0; g < rg.u1; ++g) {
-        const int k = g % IPS;
-        const bool next_slab = g + 1 < rg.u1 && k == IPS - 1;
-        TileRegs<TIn> t;
-        float2 v[32];
-        {   // v = a[n'] preA_b + a[n' + 1024] preB_b (a real)
-            TChunk ca, cb;
+    for (int u = rg.u0; u < rg.u1; ++u) {
+        const int k = u % IPS;
+        const bool next_slab = u + 1 < rg.u1 && k == IPS - 1;
+        SubRegs<TIn> t;
+#pragma unroll 1
+        for (int cc = 0; cc < 2; ++cc) {  // the quad's two columns, one after the other
+            float2 v[32];
+            {   // v = a[n'] preA_b + a[n' + 1024] preB_b (a real)
+                TChunk ca, cb;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                tm_ld(ca, tq + TQ_PREA + 16 * j);
-                tm_ld(cb, tq + TQ_PREB + 16 * j);
-                tm_wait(ca);
-                tm_wait(cb);
+                for (int j = 0; j < 4; ++j) {
+                    tm_ld(ca, tq + TQ_PREA + 16 * j);
+                    tm_ld(cb, tq + TQ_PREB + 16 * j);
+                    tm_wait(ca);
+                    tm_wait(cb);
 #pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    const int r = 8 * j + i;
-                    const float2 a = fold_values(sm.tile[k][lane + 32 * r], quad);
-                    const float2 pa = tm_val(ca, i), pb = tm_val(cb, i);
-                    v[r] = make_float2(fmaf(a.y, pb.x, a.x * pa.x), fmaf(a.y, pb.y, a.x * pa.y));
+                    for (int i = 0; i < 8; ++i) {
+                        const int r = 8 * j + i;
+                        const float2 a = fold_values(sm.tile[quad][k][lane + 32 * r], cc);
+                        const float2 pa = tm_val(ca, i), pb = tm_val(cb, i);
+                        v[r] = make_float2(fmaf(a.y, pb.x, a.x * pa.x), fmaf(a.y, pb.y, a.x * pa.y));
+                    }
                 }
             }
-        }
-        // the slab of the next items is fetched behind the tile reads: its loads touch one row per
-        // lane (32 wavefronts each) and would hold up everything queued after them
-        if (next_slab) slab_load<TIn>(t, holo, (g + 1) / IPS * (2 * IPS));
+            // the next sub-slab is fetched behind the tile reads of the unit's last column: its
+            // loads touch one row per lane (32 wavefronts each)
+            if (cc == 1 && next_slab) sub_load<TIn>(t, holo, SubSlab<TIn>::col(u + 1, quad), qt);
+            quad_sync(quad);  // the previous column's exchange area has been read by all four warps
 #ifdef SFDW_TRACE
-        long long *tr = g_trace;
-        branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns, tr);
+            long long *tr = g_trace;
+            branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns, tr);
 #else
-        branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns);
+            branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns);
 #endif
-        // the previous item's bulk stores must have left the staging tile before it is rewritten
-        if (leader) bulk_wait_read();
-        float2 mine[16];
-        quad_scatter(v, mine, tq, b, lane, sm.ex, warp);
-        cta_sync();  // exchange area complete; staging tile and slab free
-        quad_collect(mine, b, lane, sm.ex, warp);
+            // the previous unit's bulk stores must have left the staging tile before it is rewritten
+            if (cc == 0 && leader) bulk_wait_read();
+            float2 mine[16];
+            quad_scatter(v, mine, tq, b, lane, sm.xb, sm.ex, warp);
+            if (cc == 0)
+                cta_sync();  // also: the staging tile is free (the leader sits in quad 0)
+            else
+                quad_sync(quad);
+            quad_collect(mine, b, lane, sm.xb, sm.ex, warp);
 #pragma unroll
-        for (int i = 0; i < 16; ++i) stg[(lane + 32 * (16 * b + i)) * 2 + quad] = mine[i];
-        if (next_slab) slab_store(t, sm.tile);
-        fence_async_smem();  // staging writes -> async proxy
-        cta_sync();          // staging tile complete, next slab visible, exchange area free
-        if (leader) {
+            for (int i = 0; i < 16; ++i) stg[(lane + 32 * (16 * b + i)) * 4 + 2 * quad + cc] = mine[i];
+            if (cc == 1) {
+                if (next_slab) sub_store(t, sm.tile[quad], qt, quad);  // the tile was last read before this column's first barrier
+                fence_async_smem();  // staging writes -> async proxy
+                cta_sync();          // staging tile complete (both quads), next slab visible
+                if (leader) {
 #pragma unroll
-            for (int j = 0; j < NL / YBOX; ++j)
-                tma_store_2d(tmB, stg + j * YBOX * 2, 4 * g, rg.view * NL + j * YBOX);
-            bulk_commit();
+                    for (int j = 0; j < NL / YBOX; ++j)
+                        tma_store_2d(tmB, stg + j * YBOX * 4, 8 * u, rg.view * NL + j * YBOX);
+                    bulk_commit();
+                }
+            }
         }
     }
     if (leader) bulk_wait_read();  // shared memory must outlive the last store's reads
