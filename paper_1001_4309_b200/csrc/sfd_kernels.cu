@@ -6,8 +6,9 @@
 //   k_pass_x : grid (N/RPC, V); per CTA RPC rows of B: x pre_x, FFT, x H, inverse FFT, crop, x post_x
 //              -> field, |.|^2 -> intensity (Eq. 5), optional per-view max
 // plus, in the 8-bit mode (step (xi), reading 15), k_quantise.
-// The per-thread arithmetic lives in sfd_fft_core.cuh.  For N = 1024 the same two passes run as the
-// persistent kernels k_cols_1024 / k_rows_1024 (one warp pair per line, sfd_warp1024.cuh).
+// The per-thread arithmetic lives in sfd_fft_core.cuh.  For N = 1024 and N = 2048 the same two passes
+// run as the persistent warp-per-branch kernels k_cols_1024 / k_rows_1024 (a warp pair per line,
+// sfd_warp1024.cuh) and k_cols_2048 / k_rows_2048 (a quad of warps per line, sfd_warp2048.cuh).
 #include <cuda.h>  // CUtensorMap (types only: the encoder is fetched through the runtime)
 
 #include <atomic>

@@ -20,12 +20,16 @@
 // their partial results (each warp finishes and stores one half of the line); the half a warp
 // hands over travels through its own transpose tile, which is idle by then.
 //
-// What bounds these kernels is the plain fp32 pipe (about 2500 lane-cycles per warp and line, most
-// of them butterfly adds), closely followed by the shared-memory data pipe and the issue slots, so
-// everything that is not butterfly arithmetic is kept off the long-latency path: the six table
-// vectors of the current view (pre_b, H_b, conj(post_b)) sit in shared memory (one bulk copy per
-// view change, 48 KiB), pass x receives its rows by bulk async copy issued a line ahead, and a
-// CTA walks a CONTIGUOUS range of lines so that it changes view at most once or twice.
+// What bounds these kernels (measured): a single warp saturates its
+// sub-partition's fp32 pipe during a radix-32 butterfly (464 cycles per 32-point DFT, about 2730 per
+// warp and line), and the chain of shared-memory phases of a line (two transposes, exchange, input,
+// stores: 430 wavefronts per warp and line, latency-bound in the in-order LSU pipe) is as long
+// again.  So everything that can leave the LSU pipe has left it: the three table vectors of a branch
+// (pre_b, H_b, conj(post_b)) live in tensor memory and are read with tcgen05.ld, pass x receives
+// its rows by bulk async copy issued a line ahead, pass y hands its output tile to the TMA unit,
+// and a CTA walks a CONTIGUOUS range of lines so that it touches at most two views.  Both kernels
+// are launched with programmatic stream serialization: their prologue (mbarriers, twiddles,
+// tensor-memory tables) overlaps the tail of the kernel before them.
 #pragma once
 #include "sfd_fft_core.cuh"
 
