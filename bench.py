@@ -60,6 +60,11 @@ def parse_args():
     return ap.parse_args()
 
 
+def fp32_floor_us(N, V, sms=148, ghz=1.965):
+    """Time one pass of the warp-per-branch kernels needs if the fp32 pipes never idle (us)."""
+    return V * N * (N // 512) * 2730.0 / (4 * sms) / (ghz * 1e3)
+
+
 def measured_peaks():
     p = ROOT / "MEASURED_PEAKS.json"
     if p.exists():
@@ -329,6 +334,14 @@ def run_sfd(args, info):
                          "gbs": round(step_bytes / (sec_rank / args.steps) / 1e9, 1),
                          "frac": round(step_bytes / (sec_rank / args.steps) / 1e9 / peak, 4)}},
         "kernels": per_kernel,
+        # measured pipe model of the warp-per-branch kernels: a 1024-point
+        # branch of a line costs 2730 fp32-pipe cycles of one of the 4 x 148 sub-partitions
+        "fp32_pipe": ({"floor_us_per_kernel": round(fp32_floor_us(N, V), 2),
+                       "frac": round(fp32_floor_us(N, V) / (1e3 * float(kms[dom])), 4),
+                       "model": "2730 pipe cycles per 1024-point branch and line (4 radix-32 butterflies of "
+                                "464 cycles, 2 twiddle and 3 table multiplies), N/512 branches per line, "
+                                "V N lines per kernel, 592 sub-partitions at 1.965 GHz"}
+                      if plan.uses_warp_kernels else None),
         "timing": f"library CUDA events around each kernel on the launching stream, mean of "
                   f"{ksteps} steps after the timed region (kernel sum "
                   f"{kms[:2].sum():.4f} ms vs {1e3 * sec_rank / args.steps:.4f} ms/step)",

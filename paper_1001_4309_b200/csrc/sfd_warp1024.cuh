@@ -703,8 +703,6 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
 #endif
         SFDW_STAMP(0);
         TileRegs<TIn> t;
-        if (has_next)
-            tile_load<TIn>(t, holo, ((item + 1) % groups) / IPS * (YC * IPS) + 2 * IPS * half, ht);
         float2 v[32];
         {
             TChunk c0, c1;
@@ -723,6 +721,10 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
             }
         }
         SFDW_STAMP(1);
+        // the next slab is fetched behind the tile reads: its loads touch one row per lane (32
+        // wavefronts each) and would hold up everything queued after them
+        if (has_next)
+            tile_load<TIn>(t, holo, ((item + 1) % groups) / IPS * (YC * IPS) + 2 * IPS * half, ht);
 #ifdef SFDW_TRACE
         branch(v, lane, xb, tw, sm.tw, tpre + TM_TAB, turns, tr);
 #else
