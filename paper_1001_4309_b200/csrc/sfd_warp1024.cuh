@@ -317,24 +317,27 @@ __device__ __forceinline__ unsigned tm_quarter(unsigned base, int warp) {
 }
 // The two warps of a sub-partition copy the tables of `view`, branch warp & 1, into set `set` of
 // their quarter: warp w the chunks 0..5 (pre_b and half of H_b), warp w + 4 the chunks 6..11.  All
-// 48 loads of a thread are issued before the first store: one trip to L2 per set.
+// 48 loads of a thread are issued before the first store (and before the allocation): one trip
+// to L2 per set.
 // tab: [V][2][3][N] in global memory
-__device__ __forceinline__ void tm_fill(unsigned quarter, int set, const float2 *__restrict__ tab,
-                                        int view, int warp, int lane) {
+struct TFill { TChunk c[6]; };
+__device__ __forceinline__ void tm_fill_load(TFill &f, const float2 *__restrict__ tab, int view,
+                                             int warp, int lane) {
     const float2 *src = tab + (size_t)view * TABS + (size_t)(warp & 1) * 3 * N + lane;
     const int ch0 = 6 * (warp >> 2);  // first chunk of this warp; chunk = 8 values, 4 chunks per table
-    TChunk c[6];
 #pragma unroll
     for (int j = 0; j < 6; ++j)
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
             const float2 x = __ldg(src + 32 * (8 * (ch0 + j) + i));  // table t = chunk / 4 starts at t * N
-            c[j].w[2 * i] = __float_as_uint(x.x);
-            c[j].w[2 * i + 1] = __float_as_uint(x.y);
+            f.c[j].w[2 * i] = __float_as_uint(x.x);
+            f.c[j].w[2 * i + 1] = __float_as_uint(x.y);
         }
+}
+__device__ __forceinline__ void tm_fill_store(const TFill &f, unsigned quarter, int set, int warp) {
+    const int ch0 = 6 * (warp >> 2);
 #pragma unroll
-    for (int j = 0; j < 6; ++j) tm_st(c[j], quarter + set * TM_SET + 16 * (ch0 + j));
-    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    for (int j = 0; j < 6; ++j) tm_st(f.c[j], quarter + set * TM_SET + 16 * (ch0 + j));
 }
 // Kernel prologue (all threads): allocate, fill the one or two view sets this CTA's contiguous
 // range [total b / g, total (b + 1) / g) of work units touches (per_view units per view), make
@@ -343,16 +346,22 @@ __device__ __forceinline__ unsigned tm_setup(unsigned *slot, const float2 *__res
                                              const float2 *__restrict__ twl, int total,
                                              int per_view) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int a0 = (int)((long long)total * blockIdx.x / gridDim.x);
+    const int a1 = (int)((long long)total * (blockIdx.x + 1) / gridDim.x);
+    const int view0 = a0 < a1 ? a0 / per_view : 0;
+    TFill f;
+    if (a0 < a1) tm_fill_load(f, tab, view0, warp, lane);  // on their way during the allocation
     if (warp == 0) tm_alloc(slot);
     tm_sync_cta();
     const unsigned base = *reinterpret_cast<volatile unsigned *>(slot);
-    const int a0 = (int)((long long)total * blockIdx.x / gridDim.x);
-    const int a1 = (int)((long long)total * (blockIdx.x + 1) / gridDim.x);
     if (a0 < a1) {
-        const int view0 = a0 / per_view;
         const unsigned q = tm_quarter(base, warp);
-        tm_fill(q, 0, tab, view0, warp, lane);
-        if ((a1 - 1) / per_view != view0) tm_fill(q, 1, tab, view0 + 1, warp, lane);
+        tm_fill_store(f, q, 0, warp);
+        if ((a1 - 1) / per_view != view0) {
+            tm_fill_load(f, tab, view0 + 1, warp, lane);
+            tm_fill_store(f, q, 1, warp);
+        }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
     if (TWT && warp < 4) {  // twiddles exp(-2 pi i lane k / 1024), k = 0..31, twl: [k][lane]
 #pragma unroll 1
