@@ -113,6 +113,15 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
         for (int i = threadIdx.x; i < 1024; i += blockDim.x) sm.tw[i] = __ldg(twl + i);
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
+    {   // pull the first slab of this CTA towards L2 while the prologue runs (a prefetch reads nothing:
+        // it may precede griddepcontrol.wait)
+        constexpr int groups = sfdw::N / sfdw::YC, IPS = sfdw::TileElem<TIn>::IPS;
+        const int i0 = (int)((long long)V * groups * blockIdx.x / gridDim.x);
+        const TIn *p0 = holo + (i0 % groups) / IPS * (sfdw::YC * IPS);
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(p0 + (size_t)(threadIdx.x + 256 * i) * sfdw::N));
+    }
     // tables of this CTA's view(s) -> tensor memory (the barriers inside also publish the mbarriers)
     const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabY, twl, V * (sfdw::N / sfdw::YC), sfdw::N / sfdw::YC);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
