@@ -18,6 +18,15 @@
 #include "sfd_warp1024.cuh"
 #include "sfd_warp2048.cuh"
 
+#ifdef SFDW_TRACE
+// kernel-level clock stamps (experiments only): [kernel 0/1][cta][8] behind the per-line stamps
+#define SFD_KSTAMP(kern, i)                                                                      \
+    if (threadIdx.x == 0)                                                                        \
+        sfdw::g_trace[2 * sfdw::TRACE_PASS + ((size_t)(kern) * 148 + blockIdx.x) * 8 + (i)] = clock64();
+#else
+#define SFD_KSTAMP(kern, i)
+#endif
+
 namespace {
 
 using namespace sfd;
@@ -104,6 +113,7 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
             unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
     sfdw::SmemY<TIn> &sm = *reinterpret_cast<sfdw::SmemY<TIn> *>(smem4);
+    SFD_KSTAMP(0, 0);
     sfdw::pdl_launch_dependents();
     if (threadIdx.x == 0) {
         for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
@@ -127,7 +137,9 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     // everything above touches plan constants only; the hologram, B, vmax and mom belong to the
     // kernels before this one in the stream
+    SFD_KSTAMP(0, 1);
     sfdw::pdl_wait();
+    SFD_KSTAMP(0, 2);
     if (vmax != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
     if (mom != nullptr && blockIdx.x == 0)
@@ -136,7 +148,9 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
         sfdw::pass_y_loop<TIn, 0>(sm, holo, tq, tw, &tmB, V);
     else
         sfdw::pass_y_loop<TIn, 1>(sm, holo, tq, tw, &tmB, V);
+    SFD_KSTAMP(0, 3);
     sfdw::tm_finish(tbase);
+    SFD_KSTAMP(0, 4);
 }
 
 __global__ void __launch_bounds__(sfdw::WX * 32, 1)
@@ -145,6 +159,7 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
             unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
     sfdw::SmemX &sm = *reinterpret_cast<sfdw::SmemX *>(smem4);
+    SFD_KSTAMP(1, 0);
     sfdw::pdl_launch_dependents();
     if (threadIdx.x == 0) {
         for (int i = 0; i < sfdw::XP; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
@@ -158,12 +173,16 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
     constexpr int gpv = (sfdw::N + sfdw::XP - 1) / sfdw::XP;  // units per view, as in pass_x_loop
     const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabX, twl, V * gpv, gpv);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
+    SFD_KSTAMP(1, 1);
     sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
+    SFD_KSTAMP(1, 2);
     if (((threadIdx.x >> 5) & 1) == 0)
         sfdw::pass_x_loop<0>(sm, B, tq, tw, field, inten, vmax, mom, V);
     else
         sfdw::pass_x_loop<1>(sm, B, tq, tw, field, inten, vmax, mom, V);
+    SFD_KSTAMP(1, 3);
     sfdw::tm_finish(tbase);
+    SFD_KSTAMP(1, 4);
 }
 
 // ---- N = 2048 (sfd_warp2048.cuh): four branches per line, a quad of warps per line ------------------
