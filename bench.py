@@ -402,9 +402,12 @@ def run_sfd(args, info):
 # ncu `--set full` DRAM traffic per launch (bytes), copied from profiles/ by hand after each capture;
 # key = (workload name, kernel).  Absent = null in the JSON line.
 NCU_TRAFFIC = {
-    # profiles/r01_v8_launches.md / r01_v8_traffic.json (v8 kernels, config 2)
-    ("paper_4view_1024", "k_cols_1024"): 16610048 + 15330560,
-    ("paper_4view_1024", "k_rows_1024"): 33810432 + 3081984,
+    # profiles/r01_final_launches.md (final round-1 kernels, config 2)
+    ("paper_4view_1024", "k_cols_1024"): 16755200 + 15465984,
+    ("paper_4view_1024", "k_rows_1024"): 33810688 + 4168192,
+    # profiles/r01_v9_config4.md (N = 2048 warp kernels, config 4)
+    ("scale_stress_2048", "k_cols_2048"): 10770688 + 533581050,
+    ("scale_stress_2048", "k_rows_2048"): 539547390 + 753424640,
 }
 
 
