@@ -48,6 +48,8 @@ k_pass_y(const TIn *__restrict__ holo, const float2 *__restrict__ pre_y,
          const float2 *__restrict__ H, const float2 *__restrict__ post_y,
          const float2 *__restrict__ tw, float2 *__restrict__ B, unsigned int *vmax, double *mom) {
     extern __shared__ float2 smem[];
+    sfdw::pdl_launch_dependents();
+    sfdw::pdl_wait();  // the hologram, B, vmax and mom belong to the kernels before this one
     if (vmax != nullptr && blockIdx.x == 0 && threadIdx.x == 0) vmax[blockIdx.y] = 0u;
     if (mom != nullptr && blockIdx.x == 0 && threadIdx.x < 2) mom[2 * blockIdx.y + threadIdx.x] = 0.0;
     pass_y_body<LOG2M, Tile<LOG2M>::C, TIn>(threadIdx.x, blockIdx.x, blockIdx.y, smem, holo, pre_y,
@@ -61,6 +63,8 @@ k_pass_x(const float2 *__restrict__ B, const float2 *__restrict__ pre_x,
          const float2 *__restrict__ tw, float2 *__restrict__ field, float *__restrict__ inten,
          unsigned int *vmax, double *mom) {
     extern __shared__ float2 smem[];
+    sfdw::pdl_launch_dependents();
+    sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
     float s1 = 0.f, s2 = 0.f;
     float mx = pass_x_body<LOG2M, Tile<LOG2M>::RPC, MOM>(threadIdx.x, blockIdx.x, blockIdx.y, smem, B,
                                                     pre_x, H, post_x, tw, field, inten,
@@ -378,20 +382,41 @@ cudaError_t launch_t(sfd_plan *p, const void *holo, float2 *field, float *inten,
     }
     const bool timing = p->timing;
     if (timing) cudaEventRecord(p->ev[0], st);
-    dim3 gy(N / TL::C, V), gx(N / TL::RPC, V);
+    // programmatic dependent launch (as for the warp kernels): the launch latency of a kernel
+    // overlaps the tail of the kernel before it; the small sizes are launch-bound
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(N / TL::C, V);
+    cfg.blockDim = dim3(TL::THREADS_Y);
+    cfg.dynamicSmemBytes = TL::SMEM_Y;
+    cfg.stream = st;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    cudaError_t le;
     if (d.in_dtype == 0)
-        k_pass_y<LOG2M, unsigned char><<<gy, TL::THREADS_Y, TL::SMEM_Y, st>>>(
-            (const unsigned char *)holo, d.pre_y, d.H, d.post_y, d.tw, d.B, vmax, mom);
+        le = cudaLaunchKernelEx(&cfg, k_pass_y<LOG2M, unsigned char>, (const unsigned char *)holo,
+                                (const float2 *)d.pre_y, (const float2 *)d.H, (const float2 *)d.post_y,
+                                (const float2 *)d.tw, d.B, vmax, mom);
     else
-        k_pass_y<LOG2M, float><<<gy, TL::THREADS_Y, TL::SMEM_Y, st>>>(
-            (const float *)holo, d.pre_y, d.H, d.post_y, d.tw, d.B, vmax, mom);
+        le = cudaLaunchKernelEx(&cfg, k_pass_y<LOG2M, float>, (const float *)holo,
+                                (const float2 *)d.pre_y, (const float2 *)d.H, (const float2 *)d.post_y,
+                                (const float2 *)d.tw, d.B, vmax, mom);
+    if (le != cudaSuccess) return le;
     if (timing) cudaEventRecord(p->ev[1], st);
+    cfg.gridDim = dim3(N / TL::RPC, V);
+    cfg.blockDim = dim3(TL::THREADS_X);
+    cfg.dynamicSmemBytes = TL::SMEM_X;
     if (mom == nullptr)
-        k_pass_x<LOG2M, false><<<gx, TL::THREADS_X, TL::SMEM_X, st>>>(d.B, d.pre_x, d.Hx, d.post_x,
-                                                                      d.tw, field, inten, vmax, mom);
+        le = cudaLaunchKernelEx(&cfg, k_pass_x<LOG2M, false>, (const float2 *)d.B, (const float2 *)d.pre_x,
+                                (const float2 *)d.Hx, (const float2 *)d.post_x, (const float2 *)d.tw, field,
+                                inten, vmax, mom);
     else
-        k_pass_x<LOG2M, true><<<gx, TL::THREADS_X, TL::SMEM_X, st>>>(d.B, d.pre_x, d.Hx, d.post_x,
-                                                                     d.tw, field, inten, vmax, mom);
+        le = cudaLaunchKernelEx(&cfg, k_pass_x<LOG2M, true>, (const float2 *)d.B, (const float2 *)d.pre_x,
+                                (const float2 *)d.Hx, (const float2 *)d.post_x, (const float2 *)d.tw, field,
+                                inten, vmax, mom);
+    if (le != cudaSuccess) return le;
     if (timing) cudaEventRecord(p->ev[2], st);
     int n = 2;
     if (u8) {
