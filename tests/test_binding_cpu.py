@@ -111,3 +111,27 @@ def test_host_tables_general_match_oracle_tables(N, p1, p2, z, off0, off):
     a, b, c = B.sfd_host_tables_general(N, lam, p1, p2, z, 0.0, off)
     a2, b2, c2 = B.sfd_host_tables(N, lam, p1, p2, z, off)
     assert np.array_equal(a, a2) and np.array_equal(b, b2) and np.array_equal(c, c2)
+
+
+@pytest.mark.parametrize("bad", [
+    dict(N=96), dict(n_views=0), dict(p1y=[0.0]), dict(p2x=[float("nan")]), dict(z=[0.0]),
+    dict(O0x=[float("inf")]), dict(O1y=[float("nan")]), dict(in_dtype=-1),
+])
+def test_general_plan_create_rejects_bad_arguments(bad):
+    kw = dict(N=64, n_views=1, lam=W.LAMBDA, p1x=[W.PITCH], p1y=[W.PITCH], p2x=[2e-6], p2y=[3e-6],
+              z=[0.05], O0x=[0.0], O0y=[0.0], O1x=[0.0], O1y=[0.0], in_dtype=B.SFD_F32)
+    kw.update(bad)
+    with pytest.raises(B.SfdError) as e:
+        B.sfd_plan_create_general(kw["N"], kw["n_views"], kw["lam"], kw["p1x"], kw["p1y"], kw["p2x"],
+                                  kw["p2y"], kw["z"], kw["O0x"], kw["O0y"], kw["O1x"], kw["O1y"],
+                                  kw["in_dtype"])
+    assert e.value.code == B.SFD_EINVAL
+
+
+def test_new_entry_points_reject_null():
+    assert B._lib.sfd_execute_focus(None, None, None, None, None) == B.SFD_EINVAL
+    assert B._lib.sfd_plan_update_view_general(None, 0, 1e-6, 1e-6, 1e-6, 1e-6, 0.1, 0.0, 0.0, 0.0,
+                                               0.0) == B.SFD_EINVAL
+    assert B._lib.sfd_plan_create_general(None, 64, 1, 1e-6, *([None] * 9), 0) == B.SFD_EINVAL
+    with pytest.raises(B.SfdError):
+        B.sfd_host_tables_general(100, W.LAMBDA, W.PITCH, W.PITCH, 0.05, 0.0, 0.0)
