@@ -148,10 +148,7 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
         for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
     if (mom != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
-    if (((threadIdx.x >> 5) & 1) == 0)
-        sfdw::pass_y_loop<TIn, 0>(sm, holo, tq, tw, &tmB, V);
-    else
-        sfdw::pass_y_loop<TIn, 1>(sm, holo, tq, tw, &tmB, V);
+    sfdw::pass_y_loop<TIn>(sm, holo, tq, tw, &tmB, V);
     SFD_KSTAMP(0, 3);
     sfdw::tm_finish(tbase);
     SFD_KSTAMP(0, 4);
@@ -180,10 +177,7 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
     SFD_KSTAMP(1, 1);
     sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
     SFD_KSTAMP(1, 2);
-    if (((threadIdx.x >> 5) & 1) == 0)
-        sfdw::pass_x_loop<0>(sm, B, tq, tw, field, inten, vmax, mom, V);
-    else
-        sfdw::pass_x_loop<1>(sm, B, tq, tw, field, inten, vmax, mom, V);
+    sfdw::pass_x_loop(sm, B, tq, tw, field, inten, vmax, mom, V);
     SFD_KSTAMP(1, 3);
     sfdw::tm_finish(tbase);
     SFD_KSTAMP(1, 4);

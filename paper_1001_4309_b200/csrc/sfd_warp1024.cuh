@@ -675,12 +675,32 @@ __device__ __forceinline__ void bulk_wait_read() {
 // Per item a warp (column c of its half, branch B) transforms its column, hands the half of the
 // outputs it does not finish to its partner through its own transpose tile (idle by then), adds
 // what the partner left for it and writes 16 final values per thread into the staging tile.
-template <typename TIn, int B>
+// The two places of a line that depend on the branch index at compile time (which half of the
+// register vector stays) are small functions instantiated for B = 0, 1 and entered through a
+// warp-uniform branch; everything else is ONE copy of code for all eight warps (half the
+// instruction-cache footprint of two template copies of the whole loop: measured, the
+// no_instruction stalls of the N = 2048 kernels, written this way, are a third of those of two copies).
+template <int B>
+__device__ __forceinline__ void y_hand_over(const float2 (&v)[32], float2 *xb, int lane) {
+#pragma unroll
+    for (int q = 0; q < 16; ++q) xb[q * 32 + lane] = v[16 * (1 - B) + q];
+}
+template <int B>
+__device__ __forceinline__ void y_finish(const float2 (&v)[32], const float2 *xbp, float2 *stg,
+                                         int lane, int c) {
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const float2 w = padd(v[16 * B + q], xbp[q * 32 + lane]);
+        stg[(lane + 32 * (16 * B + q)) * 2 + c] = w;
+    }
+}
+
+template <typename TIn>
 __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restrict__ holo,
                                             unsigned tq, const float2 (&tw)[TWN],
                                             const void *tmB, int V) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int half = warp >> 2, c = (warp >> 1) & 1, ht = threadIdx.x & 127;
+    const int half = warp >> 2, c = (warp >> 1) & 1, ht = threadIdx.x & 127, b = warp & 1;
     constexpr int groups = N / YC;
     const int items = V * groups;
     const int i0 = (int)((long long)items * blockIdx.x / gridDim.x);
@@ -742,15 +762,16 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
         SFDW_STAMP(8);
         // the previous item's bulk stores must have left the staging tile before it is rewritten
         if (leader) bulk_wait_read();
-#pragma unroll
-        for (int q = 0; q < 16; ++q) xb[q * 32 + lane] = v[16 * (1 - B) + q];
+        if (b == 0)
+            y_hand_over<0>(v, xb, lane);
+        else
+            y_hand_over<1>(v, xb, lane);
         half_sync(half);  // partner's hand-over visible; staging tile and input tile free
         SFDW_STAMP(9);
-#pragma unroll
-        for (int q = 0; q < 16; ++q) {
-            const float2 w = padd(v[16 * B + q], xbp[q * 32 + lane]);
-            stg[(lane + 32 * (16 * B + q)) * 2 + c] = w;
-        }
+        if (b == 0)
+            y_finish<0>(v, xbp, stg, lane, c);
+        else
+            y_finish<1>(v, xbp, stg, lane, c);
         if (has_next) tile_store(t, sm.tile[half], ht);
         fence_async_smem();  // staging writes -> async proxy
         half_sync(half);     // staging tile complete, next input tile visible, hand-over tiles free
@@ -780,7 +801,49 @@ struct SmemX {
 
 // Work unit = (view, group of XP adjacent rows); a CTA takes a contiguous range of units, so all
 // its pairs are always in the same view.  tabX: [V][2][3][N].
+// exchange of the halves, stores, reductions of one line for branch B (see y_hand_over)
 template <int B>
+__device__ __forceinline__ void x_finish(float2 (&v)[32], float2 *xb, const float2 *xbp, int lane,
+                                         int pair, float2 *__restrict__ field,
+                                         float *__restrict__ inten, size_t off, double *mom,
+                                         unsigned int *vmax, int view) {
+    add_halves<B>(v, xb, xbp, lane, pair);
+    float mx = 0.f, s1 = 0.f, s2 = 0.f;
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        const int m1 = lane + 32 * (16 * B + q);
+        const float2 w = v[16 * B + q];
+        if (field) field[off + m1] = w;
+        const float I = w.x * w.x + w.y * w.y;
+        if (inten) inten[off + m1] = I;
+        mx = fmaxf(mx, I);
+    }
+    if (mom != nullptr) {  // focus moments (row f2): sum I, sum I^2 of the view
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const float2 w = v[16 * B + q];
+            const float I = w.x * w.x + w.y * w.y;
+            s1 += I;
+            s2 = fmaf(I, I, s2);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+            s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+        }
+        if (lane == 0) {
+            atomicAdd(mom + 2 * view, (double)s1);
+            atomicAdd(mom + 2 * view + 1, (double)s2);
+        }
+    }
+    if (vmax != nullptr) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        // intensities are >= 0, so their float bit patterns order like unsigned integers
+        if (lane == 0) atomicMax(vmax + view, __float_as_uint(mx));
+    }
+}
+
 __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict__ Bin,
                                             unsigned tq,
                                             const float2 (&tw)[TWN], float2 *__restrict__ field,
@@ -795,7 +858,8 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
     float2 *xb = sm.xb[warp];
     const float2 *xbp = sm.xb[warp ^ 1];
     const float2 *in = sm.inb[pair] + lane;
-    const bool issuer = B == 0 && lane == 0;
+    const int b = warp & 1;
+    const bool issuer = b == 0 && lane == 0;
     const int view0 = u0 / gpv;
     unsigned iphase = 0;
     bool pending = false;  // the pair's input row is already on its way
@@ -849,43 +913,10 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
 #else
         branch(v, lane, xb, tw, sm.tw, tpre + TM_TAB, turns);
 #endif
-        add_halves<B>(v, xb, xbp, lane, pair);
-        SFDW_STAMP(8);
-        float mx = 0.f, s1 = 0.f, s2 = 0.f;
-        const size_t off = row * N;
-#pragma unroll
-        for (int q = 0; q < 16; ++q) {
-            const int m1 = lane + 32 * (16 * B + q);
-            const float2 w = v[16 * B + q];
-            if (field) field[off + m1] = w;
-            const float I = w.x * w.x + w.y * w.y;
-            if (inten) inten[off + m1] = I;
-            mx = fmaxf(mx, I);
-        }
-        if (mom != nullptr) {  // focus moments (row f2): sum I, sum I^2 of the view
-#pragma unroll
-            for (int q = 0; q < 16; ++q) {
-                const float2 w = v[16 * B + q];
-                const float I = w.x * w.x + w.y * w.y;
-                s1 += I;
-                s2 = fmaf(I, I, s2);
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                s1 += __shfl_xor_sync(0xffffffffu, s1, o);
-                s2 += __shfl_xor_sync(0xffffffffu, s2, o);
-            }
-            if (lane == 0) {
-                atomicAdd(mom + 2 * view, (double)s1);
-                atomicAdd(mom + 2 * view + 1, (double)s2);
-            }
-        }
-        if (vmax != nullptr) {
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
-            // intensities are >= 0, so their float bit patterns order like unsigned integers
-            if (lane == 0) atomicMax(vmax + view, __float_as_uint(mx));
-        }
+        if (b == 0)
+            x_finish<0>(v, xb, xbp, lane, pair, field, inten, row * N, mom, vmax, view);
+        else
+            x_finish<1>(v, xb, xbp, lane, pair, field, inten, row * N, mom, vmax, view);
         SFDW_STAMP(9);
     }
     turns_close(turns, warp);
