@@ -403,8 +403,8 @@ def run_sfd(args, info):
 # key = (workload name, kernel).  Absent = null in the JSON line.
 NCU_TRAFFIC = {
     # profiles/r01_final_launches.md (final round-1 kernels, config 2)
-    ("paper_4view_1024", "k_cols_1024"): 16755200 + 15465984,
-    ("paper_4view_1024", "k_rows_1024"): 33810688 + 4168192,
+    ("paper_4view_1024", "k_cols_1024"): 16595968 + 15315712,
+    ("paper_4view_1024", "k_rows_1024"): 33795584 + 3237120,
     # profiles/r01_v9_config4.md (N = 2048 warp kernels, config 4)
     ("scale_stress_2048", "k_cols_2048"): 10770688 + 533581050,
     ("scale_stress_2048", "k_rows_2048"): 539547390 + 753424640,
