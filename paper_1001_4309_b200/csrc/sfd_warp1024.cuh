@@ -151,9 +151,10 @@ template <int DIR> __device__ __forceinline__ void dft32(float2 (&a)[32]) {
 #endif
 #ifndef SFDW_PINGPONG
 // coupling of the two warps that share a sub-partition (see Turns below); measured on config 2
-// (reconstructions/s): 0 none 48.1k, 1 strict alternation (mbarrier tokens) 46.5k, 2 rendezvous
-// before every butterfly phase (mbarrier) 43.5k, 3 named-barrier hand-off 50.9k
-#define SFDW_PINGPONG 3
+// (reconstructions/s, final round-1 build): 0 none 57.8k, 1 strict alternation of the butterfly
+// phases (mbarrier tokens) 58.7k, 2 rendezvous before every butterfly phase (mbarrier), 3
+// named-barrier hand-off around the butterfly phases 63.6k, 6 the same around the transposes 64.2k
+#define SFDW_PINGPONG 6
 #endif
 #ifndef SFDW_ROLLED
 #define SFDW_ROLLED 1  // 1: the two radix-32 stages / two FFTs of a branch share one copy of the code
@@ -173,6 +174,7 @@ __device__ __forceinline__ void stamp(long long *tr, int i) {
 #else
 #define SFDW_STAMP(i)
 #endif
+constexpr bool PP_TRANSPOSE = SFDW_PINGPONG == 6;  // the hand-off brackets the transposes
 constexpr bool TWR = SFDW_TWR == 1;
 constexpr bool TWT = SFDW_TWR == 2;
 constexpr int TWN = TWR ? 32 : 1;  // length of the per-thread twiddle register vector
@@ -387,7 +389,7 @@ __device__ __forceinline__ void tm_finish(unsigned base) {
 // Coupling of the two warps that share an SM sub-partition (warps w and w + 4 of an 8-warp CTA).
 // The butterfly phases of a line load the sub-partition's fp32 pipe, the phases between them
 // (transposes, table and input reads, exchange, stores) the SM-wide shared-memory pipe; left alone
-// the warps of an SM drift into the same phase and the shared-memory pipe sees bursts.  Four
+// the warps of an SM drift into the same phase and the shared-memory pipe sees bursts.  Five
 // policies are kept as a build knob (SFDW_PINGPONG), a butterfly phase being bracketed by
 // turn_begin / turn_end:
 //   1  a token per sub-partition (two mbarriers, count 1): strictly alternating, exclusive turns.
@@ -398,8 +400,14 @@ __device__ __forceinline__ void tm_finish(unsigned base) {
 //   3  bar.arrive on the partner's named barrier at turn_end, bar.sync on one's own at turn_begin,
 //      both with a thread count of 64.  Measured with clock stamps this does NOT exclude anything
 //      (a warp waits about 45 cycles per turn on average; the butterfly phases of the two warps
-//      overlap freely); it bounds how far the two warps drift apart and is the fastest of the
-//      four.  It is the default for that reason only.
+//      overlap freely); it bounds how far the two warps drift apart and beats 0, 1 and 2 by 8-10 %
+//      (ncu: fewer math_pipe_throttle and mio_throttle stalls, i.e. fewer collisions of the two
+//      warps in the same kind of phase).
+//   6  the same hand-off, but bracketing the two transposes of a branch (bar.sync before the
+//      stores into the tile, bar.arrive after the loads from it) instead of the butterfly phases:
+//      another 1 % (64.2k against 63.6k reconstructions/s, reproducible to 0.01 %).  The default,
+//      for that reason only; the same hand-off around both kinds of phase, or around one transpose
+//      only, is slower, and so are mbarrier tokens in the same places.
 //   0  no coupling.
 struct Turns {
     unsigned mine, theirs;  // shared-memory addresses of the two mbarriers
@@ -407,7 +415,7 @@ struct Turns {
     bool on;
 };
 __device__ __forceinline__ void turn_begin(Turns &t) {
-#if SFDW_PINGPONG == 3
+#if SFDW_PINGPONG == 3 || SFDW_PINGPONG == 6
     if (t.on) asm volatile("bar.sync %0, 64;" ::"r"(t.mine) : "memory");
     return;
 #endif
@@ -433,7 +441,7 @@ __device__ __forceinline__ void turn_begin(Turns &t) {
     }
 }
 __device__ __forceinline__ void turn_end(const Turns &t) {
-#if SFDW_PINGPONG == 3
+#if SFDW_PINGPONG == 3 || SFDW_PINGPONG == 6
     if (t.on) asm volatile("bar.arrive %0, 64;" ::"r"(t.theirs) : "memory");
     return;
 #endif
@@ -450,7 +458,7 @@ __device__ __forceinline__ void turn_end(const Turns &t) {
 // ones (transposes) beside turns 3 and 1.
 __device__ __forceinline__ Turns turns_make(unsigned long long *bars, int warp, bool on) {
     const int sp = warp & 3, up = warp >> 2;
-#if SFDW_PINGPONG == 3
+#if SFDW_PINGPONG == 3 || SFDW_PINGPONG == 6
     return Turns{5u + 2 * sp + up, 5u + 2 * sp + 1 - up, 0u, on};  // named barriers 5..12
 #elif SFDW_PINGPONG == 2
     return Turns{smem_u32(bars + 2 * sp), smem_u32(bars + 2 * sp), 0u, on};
@@ -460,7 +468,7 @@ __device__ __forceinline__ Turns turns_make(unsigned long long *bars, int warp, 
 }
 __device__ __forceinline__ void turns_open(Turns &t, int warp) {
     if ((warp >> 2) == 1) {
-#if SFDW_PINGPONG == 3
+#if SFDW_PINGPONG == 3 || SFDW_PINGPONG == 6
         turn_end(t);
 #else
 #if SFDW_PINGPONG != 2
@@ -474,7 +482,7 @@ __device__ __forceinline__ void turns_open(Turns &t, int warp) {
 __device__ __forceinline__ void turns_close(Turns &t, int warp) {
     if ((warp >> 2) == 0) {
         turn_begin(t);
-        if (SFDW_PINGPONG != 3) turn_end(t);
+        if (SFDW_PINGPONG != 3 && SFDW_PINGPONG != 6) turn_end(t);
     }
 }
 
@@ -501,7 +509,7 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
     SFDW_LOOP
     for (int step = 0; step < 4; ++step) {
         SFDW_STAMP(16 + 4 * step + 3);
-        if (step != 2) turn_begin(turns);
+        if (step != 2 && !PP_TRANSPOSE) turn_begin(turns);
         SFDW_STAMP(16 + 4 * step);
         TChunk c0, c1;
         const unsigned ta = t + (step >> 1) * TM_TAB;
@@ -512,7 +520,7 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
 #pragma unroll
             for (int k = 0; k < 32; ++k) v[k].y = -v[k].y;
             SFDW_STAMP(16 + 4 * step + 1);
-            turn_end(turns);
+            if (!PP_TRANSPOSE) turn_end(turns);
         } else if (step & 1) {
 #pragma unroll
             for (int j = 0; j < 4; ++j) {  // v = conj(v * t)
@@ -526,7 +534,7 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
                 }
             }
             SFDW_STAMP(16 + 4 * step + 1);
-            if (step != 1) turn_end(turns);
+            if (step != 1 && !PP_TRANSPOSE) turn_end(turns);
         } else {
             if constexpr (TWT) {
                 const unsigned tt = (t & 0xffff0000u) + TM_TW;  // twiddle columns of this quarter
@@ -549,7 +557,7 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
                 }
             }
             SFDW_STAMP(16 + 4 * step + 1);
-            turn_end(turns);
+            if (PP_TRANSPOSE) turn_begin(turns); else turn_end(turns);
 #pragma unroll
             for (int k = 0; k < 32; ++k) xb[k * XS + lane] = v[k];  // (k1 = k, n2 = lane)
             __syncwarp();
@@ -561,6 +569,7 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
                 v[2 * q + 1] = make_float2(w.z, w.w);
             }
             __syncwarp();
+            if (PP_TRANSPOSE) turn_end(turns);
         }
         SFDW_STAMP(16 + 4 * step + 2);
     }
