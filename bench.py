@@ -403,8 +403,8 @@ def run_sfd(args, info):
 # key = (workload name, kernel).  Absent = null in the JSON line.
 NCU_TRAFFIC = {
     # profiles/r01_final_launches.md (final round-1 kernels, config 2)
-    ("paper_4view_1024", "k_cols_1024"): 16595968 + 15315712,
-    ("paper_4view_1024", "k_rows_1024"): 33795584 + 3237120,
+    ("paper_4view_1024", "k_cols_1024"): 16894720 + 15644928,
+    ("paper_4view_1024", "k_rows_1024"): 33795584 + 3111168,
     # profiles/r01_v9_config4.md (N = 2048 warp kernels, config 4)
     ("scale_stress_2048", "k_cols_2048"): 10770688 + 533581050,
     ("scale_stress_2048", "k_rows_2048"): 539547390 + 753424640,
