@@ -74,7 +74,10 @@ SFD_API int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, c
  *   hologram_dev   [N][N] samples of the plan's in_dtype.
  *   field_dev      [n_views][N][N] complex64 (re, im interleaved), or NULL to skip the field.
  *   intensity_dev  [n_views][N][N] float32, or NULL to skip the intensity.
- * At least one output must be non-NULL.  Errors: SFD_EINVAL, SFD_ECUDA. */
+ * At least one output must be non-NULL.  Errors: SFD_EINVAL, SFD_ECUDA.
+ * The call only enqueues kernels on `stream` (no allocation, no host synchronisation), so it may be
+ * captured in a CUDA graph (with per-kernel timing off); the kernels of one call and of consecutive
+ * calls are chained by programmatic dependent launch. */
 SFD_API int sfd_execute(sfd_plan *plan, const void *hologram_dev, void *field_dev, float *intensity_dev,
                 void *stream);
 

@@ -502,3 +502,33 @@ def test_warp_kernels_bit_identical_under_concurrent_load(N, V, in_dtype, iters)
             f, I = plan.execute(holo)
             torch.cuda.synchronize()
             assert torch.equal(f, f0) and torch.equal(I, I0), f"run {it} differs from the first"
+
+
+@pytest.mark.parametrize("N", [128, 1024])
+def test_execute_is_capturable_in_a_cuda_graph(N):
+    """sfd_execute only enqueues kernels on the caller's stream (no allocation, no synchronisation), so a
+    frame loop can be captured in a CUDA graph; the programmatic-dependent-launch edges survive the capture.
+    Replays must reproduce the directly executed field bit for bit."""
+    wl = W.small_multiview(N=N, V=3, seed=11) if N < 1024 else W.config(2)
+    holo = torch.from_numpy(wl.hologram()).to(_dev())
+    with B.Plan(wl) as plan:
+        f, I = plan.execute(holo)
+        torch.cuda.synchronize()
+        f0, I0 = f.clone(), I.clone()
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):                      # warm-up off the default stream, as torch asks
+            plan.execute(holo, field=f, intensity=I)
+        torch.cuda.current_stream().wait_stream(side)
+        n0 = B.sfd_launch_count()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            for _ in range(4):
+                plan.execute(holo, field=f, intensity=I)
+        assert B.sfd_launch_count() - n0 == 8
+        for _ in range(3):
+            f.zero_()
+            I.zero_()
+            graph.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(f, f0) and torch.equal(I, I0)
