@@ -169,7 +169,7 @@ def oracle_view_seconds(holo, wl, v):
     return time.perf_counter() - t0
 
 
-def cpu_baseline(wl, holo, budget_s=15.0, max_views=24):
+def cpu_baseline(wl, holo, budget_s=12.0, max_views=400):
     from oracle import shifted_fresnel as O
     oracle_view_seconds(holo, wl, 0)                 # untimed warm-up (FFT plan cache, page faults)
     done, spent = 0, 0.0
