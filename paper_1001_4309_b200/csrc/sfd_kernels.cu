@@ -18,15 +18,6 @@
 #include "sfd_warp1024.cuh"
 #include "sfd_warp2048.cuh"
 
-#ifdef SFDW_TRACE
-// kernel-level clock stamps (experiments only): [kernel 0/1][cta][8] behind the per-line stamps
-#define SFD_KSTAMP(kern, i)                                                                      \
-    if (threadIdx.x == 0)                                                                        \
-        sfdw::g_trace[2 * sfdw::TRACE_PASS + ((size_t)(kern) * 148 + blockIdx.x) * 8 + (i)] = clock64();
-#else
-#define SFD_KSTAMP(kern, i)
-#endif
-
 namespace {
 
 using namespace sfd;
@@ -117,14 +108,7 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
             unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
     sfdw::SmemY<TIn> &sm = *reinterpret_cast<sfdw::SmemY<TIn> *>(smem4);
-    SFD_KSTAMP(0, 0);
     sfdw::pdl_launch_dependents();
-    if (threadIdx.x == 0) {
-        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
-        sfdw::mbar_fence_init();
-    }
-    if (SFDW_TWR == 0)
-        for (int i = threadIdx.x; i < 1024; i += blockDim.x) sm.tw[i] = __ldg(twl + i);
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
     {   // pull the first slab of this CTA towards L2 while the prologue runs (a prefetch reads nothing:
@@ -137,21 +121,17 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
             asm volatile("prefetch.global.L2 [%0];" ::"l"(p0 + (size_t)(threadIdx.x + 256 * i) * sfdw::N));
     }
     // tables of this CTA's view(s) -> tensor memory (the barriers inside also publish the mbarriers)
-    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabY, twl, V * (sfdw::N / sfdw::YC), sfdw::N / sfdw::YC);
+    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabY, V * (sfdw::N / sfdw::YC), sfdw::N / sfdw::YC);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     // everything above touches plan constants only; the hologram, B, vmax and mom belong to the
     // kernels before this one in the stream
-    SFD_KSTAMP(0, 1);
     sfdw::pdl_wait();
-    SFD_KSTAMP(0, 2);
     if (vmax != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
     if (mom != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
     sfdw::pass_y_loop<TIn>(sm, holo, tq, tw, &tmB, V);
-    SFD_KSTAMP(0, 3);
     sfdw::tm_finish(tbase);
-    SFD_KSTAMP(0, 4);
 }
 
 __global__ void __launch_bounds__(sfdw::WX * 32, 1)
@@ -160,27 +140,19 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
             unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
     sfdw::SmemX &sm = *reinterpret_cast<sfdw::SmemX *>(smem4);
-    SFD_KSTAMP(1, 0);
     sfdw::pdl_launch_dependents();
     if (threadIdx.x == 0) {
         for (int i = 0; i < sfdw::XP; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
-        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
         sfdw::mbar_fence_init();
     }
-    if (SFDW_TWR == 0)
-        for (int i = threadIdx.x; i < 1024; i += blockDim.x) sm.tw[i] = __ldg(twl + i);
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
     constexpr int gpv = (sfdw::N + sfdw::XP - 1) / sfdw::XP;  // units per view, as in pass_x_loop
-    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabX, twl, V * gpv, gpv);
+    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabX, V * gpv, gpv);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
-    SFD_KSTAMP(1, 1);
     sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
-    SFD_KSTAMP(1, 2);
     sfdw::pass_x_loop(sm, B, tq, tw, field, inten, vmax, mom, V);
-    SFD_KSTAMP(1, 3);
     sfdw::tm_finish(tbase);
-    SFD_KSTAMP(1, 4);
 }
 
 // ---- N = 2048 (sfd_warp2048.cuh): four branches per line, a quad of warps per line ------------------
@@ -193,10 +165,6 @@ k_cols_2048(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
     extern __shared__ float4 smem4[];
     sfdq::SmemYQ<TIn> &sm = *reinterpret_cast<sfdq::SmemYQ<TIn> *>(smem4);
     sfdw::pdl_launch_dependents();
-    if (threadIdx.x == 0) {
-        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
-        sfdw::mbar_fence_init();
-    }
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
     const sfdq::Range rg = sfdq::cta_range(cpv, sfdq::QUY);
@@ -221,7 +189,6 @@ k_rows_2048(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
     if (threadIdx.x == 0) {
         sfdw::mbar_init(&sm.ibar[0], 1);
         sfdw::mbar_init(&sm.ibar[1], 1);
-        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.turn[i], SFDW_PINGPONG == 2 ? 2 : 1);
         sfdw::mbar_fence_init();
     }
     float2 tw[sfdw::TWN];

@@ -135,16 +135,26 @@ void to_f32(const cd *src, float2 *dst, size_t n, cd scale = cd(1, 0)) {
 //   out[4][N] = pre | pre w^n | post | post w^-n   (each times its scale), formed in float64.
 // Fast-path tables of one pass and one view, layout [2][3][N]: for branch b the vectors
 // pre_b, H_b, conj(post_b) (sfd_warp1024.cuh); H = the float32 M-point kernel spectrum.
+// The butterflies of the warp FFT leave stage-A output k1 multiplied by (-1)^popcount(k1) (sign
+// tracking, sfd_dft32.cuh); k1 is the lane that multiplies table entry lane + 32 r after stage B, so
+// the sign goes into every table that follows an FFT (H_b and the post tables).
+double lane_sign(int n) {
+    const int l = n & 31;
+    return ((l ^ (l >> 1) ^ (l >> 2) ^ (l >> 3) ^ (l >> 4)) & 1) ? -1.0 : 1.0;
+}
+
 void branch_tables(int N, const cd *pre, const cd *post, cd pre_scale, cd post_scale,
                    const float2 *H, float2 *out) {
     for (int n = 0; n < N; ++n) {
         const cd w = cis_cycles(-(ld)n / (ld)(2 * N));
+        const float sg = (float)lane_sign(n);
         const cd t[4] = {pre[n] * pre_scale, pre[n] * pre_scale * w,
-                         std::conj(post[n] * post_scale), std::conj(post[n] * post_scale * std::conj(w))};
+                         (double)sg * std::conj(post[n] * post_scale),
+                         (double)sg * std::conj(post[n] * post_scale * std::conj(w))};
         for (int b = 0; b < 2; ++b) {
             float2 *o = out + (size_t)b * 3 * N;
             o[n] = make_float2((float)t[b].real(), (float)t[b].imag());
-            o[N + n] = H[2 * n + b];
+            o[N + n] = make_float2(sg * H[2 * n + b].x, sg * H[2 * n + b].y);
             o[2 * N + n] = make_float2((float)t[2 + b].real(), (float)t[2 + b].imag());
         }
     }
@@ -163,11 +173,13 @@ void branch_tables4(const cd *pre, const cd *post, cd pre_scale, cd post_scale, 
             for (int half = 0; half < 2; ++half) {
                 const int m = n + half * Nb;
                 const cd w = cis_cycles(-(ld)((long long)b * m) / (ld)4096);
-                const cd a = pre[m] * pre_scale * w, c = post[m] * post_scale * std::conj(w);
+                const cd a = pre[m] * pre_scale * w,
+                         c = lane_sign(n) * post[m] * post_scale * std::conj(w);
                 o[(size_t)half * Nb] = make_float2((float)a.real(), (float)a.imag());
                 o[(size_t)(3 + half) * Nb] = make_float2((float)c.real(), (float)c.imag());
             }
-            o[(size_t)2 * Nb] = H[4 * n + b];
+            o[(size_t)2 * Nb] = make_float2((float)lane_sign(n) * H[4 * n + b].x,
+                                            (float)lane_sign(n) * H[4 * n + b].y);
         }
 }
 
@@ -397,12 +409,15 @@ int sfd_plan_create_general(sfd_plan **out, int N, int n_views, double lambda, c
         p->d.w_tabX = f + V * fpass;
         p->d.w_twl = f + V * 2 * fpass;
         p->device_bytes += (long long)(n_fast * sizeof(float2));
-        std::vector<float2> twl(32 * 32);
-        for (int k = 0; k < 32; ++k)
-            for (int lane = 0; lane < 32; ++lane) {
-                const cd w = cis_cycles(-(ld)(lane * k) / (ld)1024);
-                twl[k * 32 + lane] = make_float2((float)w.real(), (float)w.imag());
-            }
+        // stage-B twiddles of the warp FFT (sfd_dft32.cuh): [j][lane], j = n/2 - 1 + k,
+        // T_n[k] = exp(-2 pi i (lane + 32 k) / (32 n)), n = 2, 4, .., 32, k < n/2
+        std::vector<float2> twl(32 * 32, make_float2(0.f, 0.f));
+        for (int n = 2; n <= 32; n *= 2)
+            for (int k = 0; k < n / 2; ++k)
+                for (int lane = 0; lane < 32; ++lane) {
+                    const cd w = cis_cycles(-(ld)(lane + 32 * k) / (ld)(32 * n));
+                    twl[(n / 2 - 1 + k) * 32 + lane] = make_float2((float)w.real(), (float)w.imag());
+                }
         if ((e = cudaMemcpy(p->d.w_twl, twl.data(), twl.size() * sizeof(float2),
                             cudaMemcpyHostToDevice)) != cudaSuccess)
             return fail(cuda_fail(e, "cudaMemcpy twl"));

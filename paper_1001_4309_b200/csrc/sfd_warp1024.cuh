@@ -21,16 +21,17 @@
 // hands over travels through its own transpose tile, which is idle by then.
 //
 // What bounds these kernels (measured): a single warp saturates its
-// sub-partition's fp32 pipe during a radix-32 butterfly (464 cycles per 32-point DFT, about 2730 per
-// warp and line), and the chain of shared-memory phases of a line (two transposes, exchange, input,
-// stores: 430 wavefronts per warp and line, latency-bound in the in-order LSU pipe) is as long
-// again.  So everything that can leave the LSU pipe has left it: the three table vectors of a branch
+// sub-partition's fp32 pipe during a radix-32 butterfly (FMA-formulated, sfd_dft32.cuh: 388 and 480
+// operations for the two stages of an FFT, about 2060 per warp and line), and the chain of
+// shared-memory phases of a line (two transposes, exchange, input, stores: 430 wavefronts per warp
+// and line, latency-bound in the in-order LSU pipe) is as long again.  So everything that can leave the LSU pipe has left it: the three table vectors of a branch
 // (pre_b, H_b, conj(post_b)) live in tensor memory and are read with tcgen05.ld, pass x receives
 // its rows by bulk async copy issued a line ahead, pass y hands its output tile to the TMA unit,
 // and a CTA walks a CONTIGUOUS range of lines so that it touches at most two views.  Both kernels
 // are launched with programmatic stream serialization: their prologue (mbarriers, twiddles,
 // tensor-memory tables) overlaps the tail of the kernel before them.
 #pragma once
+#include "sfd_dft32.cuh"
 #include "sfd_fft_core.cuh"
 
 namespace sfdw {
@@ -44,10 +45,9 @@ constexpr int XS = 34;      // row stride (complex) of the transpose tile: 16-by
                             // conflict-free for both the 8-byte column writes and 16-byte row reads
 constexpr int XB = 32 * XS;  // complex elements of one warp's transpose tile
 
-// Packed fp32 pairs (sm_100 FADD2): one instruction adds/subtracts both components of a complex
-// number.  The lane-op rate of the FMA pipe is unchanged, but a complex add costs one issue slot
-// instead of two — butterflies are mostly complex adds, so the radix-32 DFT shrinks from 440 to
-// about 310 instructions.
+// Packed fp32 pairs (sm_100 FADD2): one instruction adds both components of a complex number (one
+// issue slot instead of two; the pipe is occupied for two cycles all the same).  Used where partial
+// sums of two warps are added.
 __device__ __forceinline__ float2 padd(float2 a, float2 b) {
     unsigned long long r;
     asm("add.rn.f32x2 %0, %1, %2;"
@@ -64,120 +64,7 @@ __device__ __forceinline__ float2 psub(float2 a, float2 b) {
           "l"(*reinterpret_cast<unsigned long long *>(&b)));
     return *reinterpret_cast<float2 *>(&r);
 }
-// a + DIR*i*b and a - DIR*i*b (component swap: scalar adds)
-template <int DIR> __device__ __forceinline__ float2 add_ib(float2 a, float2 b) {
-    return DIR > 0 ? make_float2(a.x - b.y, a.y + b.x) : make_float2(a.x + b.y, a.y - b.x);
-}
-template <int DIR> __device__ __forceinline__ void pdft4(float2 &a0, float2 &a1, float2 &a2, float2 &a3) {
-    const float2 s0 = padd(a0, a2), d0 = psub(a0, a2), s1 = padd(a1, a3), t = psub(a1, a3);
-    a0 = padd(s0, s1);
-    a2 = psub(s0, s1);
-    a1 = add_ib<DIR>(d0, t);
-    a3 = add_ib<-DIR>(d0, t);
-}
-// 16-point DFT, natural order in and out (same factorisation as sfd::dft16)
-template <int DIR> __device__ __forceinline__ void pdft16(float2 (&a)[16]) {
-    using sfd::mul_w16;
-    pdft4<DIR>(a[0], a[4], a[8], a[12]);
-    pdft4<DIR>(a[1], a[5], a[9], a[13]);
-    pdft4<DIR>(a[2], a[6], a[10], a[14]);
-    pdft4<DIR>(a[3], a[7], a[11], a[15]);
-    a[5] = mul_w16<DIR, 1>(a[5]);   a[6] = mul_w16<DIR, 2>(a[6]);   a[7] = mul_w16<DIR, 3>(a[7]);
-    a[9] = mul_w16<DIR, 2>(a[9]);   a[10] = mul_w16<DIR, 4>(a[10]); a[11] = mul_w16<DIR, 6>(a[11]);
-    a[13] = mul_w16<DIR, 3>(a[13]); a[14] = mul_w16<DIR, 6>(a[14]); a[15] = mul_w16<DIR, 9>(a[15]);
-    pdft4<DIR>(a[0], a[1], a[2], a[3]);
-    pdft4<DIR>(a[4], a[5], a[6], a[7]);
-    pdft4<DIR>(a[8], a[9], a[10], a[11]);
-    pdft4<DIR>(a[12], a[13], a[14], a[15]);
-    float2 t;
-    t = a[1];  a[1] = a[4];   a[4] = t;
-    t = a[2];  a[2] = a[8];   a[8] = t;
-    t = a[3];  a[3] = a[12];  a[12] = t;
-    t = a[6];  a[6] = a[9];   a[9] = t;
-    t = a[7];  a[7] = a[13];  a[13] = t;
-    t = a[11]; a[11] = a[14]; a[14] = t;
-}
-
-// a * exp(DIR * 2 pi i * K / 32)
-template <int DIR, int K> __device__ __forceinline__ float2 mul_w32(float2 a) {
-    if constexpr (K % 2 == 0) {
-        return sfd::mul_w16<DIR, K / 2>(a);
-    } else {
-        constexpr float C[8] = {0.98078528040323044913f, 0.83146961230254523708f,
-                                0.55557023301960222474f, 0.19509032201612826785f,
-                                -0.19509032201612826785f, -0.55557023301960222474f,
-                                -0.83146961230254523708f, -0.98078528040323044913f};
-        constexpr float S[8] = {0.19509032201612826785f, 0.55557023301960222474f,
-                                0.83146961230254523708f, 0.98078528040323044913f,
-                                0.98078528040323044913f, 0.83146961230254523708f,
-                                0.55557023301960222474f, 0.19509032201612826785f};
-        constexpr float c = C[K / 2], s = DIR * S[K / 2];
-        return make_float2(a.x * c - a.y * s, a.x * s + a.y * c);
-    }
-}
-
-// 32-point DFT in registers, natural order in and out, W = exp(DIR * 2 pi i / 32):
-// X[k] = E[k] + W^k O[k], X[k+16] = E[k] - W^k O[k] with E/O the 16-point DFTs of the even/odd
-// inputs.
-template <int DIR> __device__ __forceinline__ void dft32(float2 (&a)[32]) {
-#ifdef SFDW_NOFFT  // timing experiment only: the butterflies vanish, everything else stays
-    return;
-#endif
-    float2 e[16], o[16];
-#pragma unroll
-    for (int s = 0; s < 16; ++s) {
-        e[s] = a[2 * s];
-        o[s] = a[2 * s + 1];
-    }
-    pdft16<DIR>(e);
-    pdft16<DIR>(o);
-#define SFDW_BF(K)                                   \
-    {                                                \
-        const float2 t = mul_w32<DIR, K>(o[K]);      \
-        a[K] = padd(e[K], t);                        \
-        a[K + 16] = psub(e[K], t);                   \
-    }
-    SFDW_BF(0) SFDW_BF(1) SFDW_BF(2) SFDW_BF(3) SFDW_BF(4) SFDW_BF(5) SFDW_BF(6) SFDW_BF(7)
-    SFDW_BF(8) SFDW_BF(9) SFDW_BF(10) SFDW_BF(11) SFDW_BF(12) SFDW_BF(13) SFDW_BF(14) SFDW_BF(15)
-#undef SFDW_BF
-}
-
-// ---- build knobs (variants are compared with SFD_LIBRARY=<variant .so> python bench.py) -----------
-#ifndef SFDW_WX
-#define SFDW_WX 8   // warps per CTA in pass x (pairs of them work on a row)
-#endif
-#ifndef SFDW_TWR
-#define SFDW_TWR 1  // inter-stage twiddles: 1 in registers, 0 from shared memory, 2 from tensor memory
-#endif
-#ifndef SFDW_PINGPONG
-// coupling of the two warps that share a sub-partition (see Turns below); measured on config 2
-// (reconstructions/s, final round-1 build): 0 none 57.8k, 1 strict alternation of the butterfly
-// phases (mbarrier tokens) 58.7k, 2 rendezvous before every butterfly phase (mbarrier), 3
-// named-barrier hand-off around the butterfly phases 63.6k, 6 the same around the transposes 64.2k
-#define SFDW_PINGPONG 6
-#endif
-#ifndef SFDW_ROLLED
-#define SFDW_ROLLED 1  // 1: the two radix-32 stages / two FFTs of a branch share one copy of the code
-#endif
-#if SFDW_ROLLED
-#define SFDW_LOOP _Pragma("unroll 1")
-#else
-#define SFDW_LOOP _Pragma("unroll")
-#endif
-#ifdef SFDW_TRACE
-__device__ long long *g_trace;  // [pass][cta][warp][16 line slots][32] clock stamps (experiments only)
-constexpr size_t TRACE_PASS = (size_t)148 * 8 * 16 * 32;
-__device__ __forceinline__ void stamp(long long *tr, int i) {
-    if ((threadIdx.x & 31) == 0) tr[i] = clock64();
-}
-#define SFDW_STAMP(i) stamp(tr, i)
-#else
-#define SFDW_STAMP(i)
-#endif
-constexpr bool PP_TRANSPOSE = SFDW_PINGPONG == 6;  // the hand-off brackets the transposes
-constexpr bool TWR = SFDW_TWR == 1;
-constexpr bool TWT = SFDW_TWR == 2;
-constexpr int TWN = TWR ? 32 : 1;  // length of the per-thread twiddle register vector
+constexpr int TWN = sfdb::NTW;  // per-lane twiddles of stage B (sfd_dft32.cuh), held in registers
 
 // ---- small PTX helpers ---------------------------------------------------------------------------
 // programmatic dependent launch: let the next kernel of the stream start early / wait until the
@@ -227,14 +114,11 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned pari
         : "memory");
 }
 
+// twl: [31][32] at [j][lane], T_n[k] of sfd_dft32.cuh at j = n/2 - 1 + k (plan constant)
 __device__ __forceinline__ void load_twiddles(float2 (&tw)[TWN], int lane,
                                               const float2 *__restrict__ twl) {
-    if constexpr (TWR) {
 #pragma unroll
-        for (int k = 0; k < 32; ++k) tw[k] = __ldg(twl + k * 32 + lane);
-    } else {
-        tw[0] = make_float2(1.f, 0.f);
-    }
+    for (int j = 0; j < TWN; ++j) tw[j] = __ldg(twl + j * 32 + lane);
 }
 
 // Tables of one view and one pass as they sit in global memory ([V][2][3][N], plan time) and in
@@ -256,7 +140,6 @@ constexpr int TABS = 2 * 3 * N;  // complex elements
 constexpr int TM_COLS = 512;      // allocated columns (all of it: one CTA per SM)
 constexpr int TM_SET = 192;       // columns of one view set
 constexpr int TM_TAB = 64;        // columns of one table
-constexpr int TM_TW = 2 * TM_SET;  // first of the 64 twiddle columns (SFDW_TWR == 2)
 struct TChunk { unsigned w[16]; };
 #define SFDW_O16(c) "=r"(c.w[0]), "=r"(c.w[1]), "=r"(c.w[2]), "=r"(c.w[3]), "=r"(c.w[4]), "=r"(c.w[5]), \
     "=r"(c.w[6]), "=r"(c.w[7]), "=r"(c.w[8]), "=r"(c.w[9]), "=r"(c.w[10]), "=r"(c.w[11]), "=r"(c.w[12]), \
@@ -345,8 +228,7 @@ __device__ __forceinline__ void tm_fill_store(const TFill &f, unsigned quarter, 
 // range [total b / g, total (b + 1) / g) of work units touches (per_view units per view), make
 // them visible.  Returns the base address; tm_finish releases it at the end of the kernel.
 __device__ __forceinline__ unsigned tm_setup(unsigned *slot, const float2 *__restrict__ tab,
-                                             const float2 *__restrict__ twl, int total,
-                                             int per_view) {
+                                             int total, int per_view) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int a0 = (int)((long long)total * blockIdx.x / gridDim.x);
     const int a1 = (int)((long long)total * (blockIdx.x + 1) / gridDim.x);
@@ -365,20 +247,6 @@ __device__ __forceinline__ unsigned tm_setup(unsigned *slot, const float2 *__res
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
-    if (TWT && warp < 4) {  // twiddles exp(-2 pi i lane k / 1024), k = 0..31, twl: [k][lane]
-#pragma unroll 1
-        for (int j = 0; j < 4; ++j) {
-            TChunk c;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const float2 x = __ldg(twl + (8 * j + i) * 32 + lane);
-                c.w[2 * i] = __float_as_uint(x.x);
-                c.w[2 * i + 1] = __float_as_uint(x.y);
-            }
-            tm_st(c, tm_quarter(base, warp) + TM_TW + 16 * j);
-        }
-        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-    }
     tm_sync_cta();
     return base;
 }
@@ -389,189 +257,99 @@ __device__ __forceinline__ void tm_finish(unsigned base) {
 // Coupling of the two warps that share an SM sub-partition (warps w and w + 4 of an 8-warp CTA).
 // The butterfly phases of a line load the sub-partition's fp32 pipe, the phases between them
 // (transposes, table and input reads, exchange, stores) the SM-wide shared-memory pipe; left alone
-// the warps of an SM drift into the same phase and the shared-memory pipe sees bursts.  Five
-// policies are kept as a build knob (SFDW_PINGPONG), a butterfly phase being bracketed by
-// turn_begin / turn_end:
-//   1  a token per sub-partition (two mbarriers, count 1): strictly alternating, exclusive turns.
-//      Verified exclusive with clock stamps - and slower than no coupling: the memory phases of a
-//      line (about 3700 cycles) are longer than the partner's turns (about 3300), so the fp32 pipe
-//      idles while both warps are in memory phases.
-//   2  both warps meet (one mbarrier, count 2) before every turn: slower still.
-//   3  bar.arrive on the partner's named barrier at turn_end, bar.sync on one's own at turn_begin,
-//      both with a thread count of 64.  Measured with clock stamps this does NOT exclude anything
-//      (a warp waits about 45 cycles per turn on average; the butterfly phases of the two warps
-//      overlap freely); it bounds how far the two warps drift apart and beats 0, 1 and 2 by 8-10 %
-//      (ncu: fewer math_pipe_throttle and mio_throttle stalls, i.e. fewer collisions of the two
-//      warps in the same kind of phase).
-//   6  the same hand-off, but bracketing the two transposes of a branch (bar.sync before the
-//      stores into the tile, bar.arrive after the loads from it) instead of the butterfly phases:
-//      another 1 % (64.2k against 63.6k reconstructions/s, reproducible to 0.01 %).  The default,
-//      for that reason only; the same hand-off around both kinds of phase, or around one transpose
-//      only, is slower, and so are mbarrier tokens in the same places.
-//   0  no coupling.
+// the warps of an SM drift into the same phase and the shared-memory pipe sees bursts.  The two
+// warps hand a turn to each other around the two transposes of a branch: bar.sync on one's own
+// named barrier before the stores into the tile, bar.arrive on the partner's after the loads from it
+// (thread count 64).  This does not exclude anything; it bounds how far the two warps drift apart.
+// Measured against the alternatives in round 1 (no coupling, strict mbarrier tokens,
+// rendezvous, the same hand-off around the butterfly phases): the fastest by 1 to 11 %.
 struct Turns {
-    unsigned mine, theirs;  // shared-memory addresses of the two mbarriers
-    unsigned phase;         // parity of the next completion of `mine` this warp waits for
+    unsigned mine, theirs;  // named barriers 5..12
     bool on;
 };
-__device__ __forceinline__ void turn_begin(Turns &t) {
-#if SFDW_PINGPONG == 3 || SFDW_PINGPONG == 6
+__device__ __forceinline__ void turn_begin(const Turns &t) {
     if (t.on) asm volatile("bar.sync %0, 64;" ::"r"(t.mine) : "memory");
-    return;
-#endif
-    if (t.on) {
-#if SFDW_PINGPONG == 2
-        // rendezvous: both warps of the sub-partition start their k-th turn together
-        __syncwarp();
-        if ((threadIdx.x & 31) == 0)
-            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(t.mine) : "memory");
-#endif
-        asm volatile(
-            "{\n"
-            ".reg .pred p;\n"
-            "W_%=:\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-            "@p bra D_%=;\n"
-            "bra W_%=;\n"
-            "D_%=:\n"
-            "}\n" ::"r"(t.mine),
-            "r"(t.phase)
-            : "memory");
-        t.phase ^= 1u;
-    }
 }
 __device__ __forceinline__ void turn_end(const Turns &t) {
-#if SFDW_PINGPONG == 3 || SFDW_PINGPONG == 6
     if (t.on) asm volatile("bar.arrive %0, 64;" ::"r"(t.theirs) : "memory");
-    return;
-#endif
-    if (t.on && SFDW_PINGPONG != 2) {
-        __syncwarp();
-        if ((threadIdx.x & 31) == 0)
-            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(t.theirs) : "memory");
-    }
 }
 // Warps 0..3 own the first turn; warps 4..7 pass on their first one and warps 0..3 add one after
-// their last line, so that both warps of a sub-partition take the same number of turns.  The
-// passed turn shifts the two by one: the long memory phase of a warp (exchange, stores, next
-// input, between its turns 3 and 1) lies beside the other warp's double turn 2, the two short
-// ones (transposes) beside turns 3 and 1.
-__device__ __forceinline__ Turns turns_make(unsigned long long *bars, int warp, bool on) {
-    const int sp = warp & 3, up = warp >> 2;
-#if SFDW_PINGPONG == 3 || SFDW_PINGPONG == 6
-    return Turns{5u + 2 * sp + up, 5u + 2 * sp + 1 - up, 0u, on};  // named barriers 5..12
-#elif SFDW_PINGPONG == 2
-    return Turns{smem_u32(bars + 2 * sp), smem_u32(bars + 2 * sp), 0u, on};
-#else
-    return Turns{smem_u32(bars + 2 * sp + up), smem_u32(bars + 2 * sp + 1 - up), 0u, on};
-#endif
+// their last line, so that both warps of a sub-partition take the same number of turns.
+__device__ __forceinline__ Turns turns_make(int warp, bool on) {
+    const unsigned sp = warp & 3, up = warp >> 2;
+    return Turns{5u + 2 * sp + up, 5u + 2 * sp + 1 - up, on};
 }
-__device__ __forceinline__ void turns_open(Turns &t, int warp) {
-    if ((warp >> 2) == 1) {
-#if SFDW_PINGPONG == 3 || SFDW_PINGPONG == 6
-        turn_end(t);
-#else
-#if SFDW_PINGPONG != 2
-        turn_end(t);
-#endif
-        turn_begin(t);
-        turn_end(t);
-#endif
-    }
+__device__ __forceinline__ void turns_open(const Turns &t, int warp) {
+    if ((warp >> 2) == 1) turn_end(t);
 }
-__device__ __forceinline__ void turns_close(Turns &t, int warp) {
-    if ((warp >> 2) == 0) {
-        turn_begin(t);
-        if (SFDW_PINGPONG != 3 && SFDW_PINGPONG != 6) turn_end(t);
-    }
+__device__ __forceinline__ void turns_close(const Turns &t, int warp) {
+    if ((warp >> 2) == 0) turn_begin(t);
 }
 
 // One branch of a line, in place (the caller has applied pre): forward FFT, x H_b, inverse FFT,
 // x post_b.  The inverse is run as conj(FFT(conj(.))) so that both transforms execute the same code:
 //     v <- conj(FFT(v) H_b);  v <- conj(FFT(v) conj(post_b)) = post_b IFFT(H_b FFT(v)) N
 // (the 1/N sits in H).  t = tensor-memory address of H_b in this warp's quarter; conj(post_b) follows it.
-// A 1024-point FFT of a warp is: radix-32 butterflies over n1 (element lane + 32 n1), inter-stage
-// twiddles exp(-2 pi i lane k1 / 1024) (tw[k] in registers or twsm[k * 32 + lane]), a 32 x 32
-// transpose through the warp's tile xb, radix-32 butterflies over n2; in v[r] = x[lane + 32 r],
-// out v[r] = X[lane + 32 r].  The four radix-32 steps of the branch share one copy of the code
-// (rolled loop): the line transform then fits the instruction cache.  Steps 0 | 1, 2 | 3 are the
-// three turns of the line.  On return v = this warp's partial sums for all 1024 outputs.
+// Both tables carry the lane sign of sfd_dft32.cuh: entry lane + 32 r is multiplied by out_sign(lane).
+// A 1024-point FFT of a warp (four-step, in v[r] = x[lane + 32 r], out v[r] = X[lane + 32 r]):
+//     stage A   32-point DFT over n1 (element lane + 32 n1) in registers            sfdb::dft32
+//     transpose 32 x 32 through the warp's tile xb: lane becomes k1, register n2
+//     stage B   32-point DFT over n2 with the inter-stage twiddles exp(-2 pi i k1 n2 / 1024)
+//               folded into its butterflies (tw: 31 per-lane constants)             sfdb::dft32_tw
+// The two FFTs of the branch share one copy of the code (rolled loop): the line transform then fits
+// the instruction cache.  On return v = this warp's partial sums for all 1024 outputs.
 // POST = false (N = 2048 kernels, sfd_warp2048.cuh): the last multiply is left to the caller, on
 // return v = IFFT(H_b FFT(v)) N.
 template <bool POST = true>
 __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
-                                       const float2 (&tw)[TWN], const float2 *twsm,
-                                       unsigned t, Turns &turns
-#ifdef SFDW_TRACE
-                                       , long long *tr
-#endif
-) {
-    SFDW_LOOP
-    for (int step = 0; step < 4; ++step) {
-        SFDW_STAMP(16 + 4 * step + 3);
-        if (step != 2 && !PP_TRANSPOSE) turn_begin(turns);
-        SFDW_STAMP(16 + 4 * step);
+                                       const float2 (&tw)[TWN], unsigned t, const Turns &turns) {
+#pragma unroll 1
+    for (int f = 0; f < 2; ++f) {
+        sfdb::dft32(v);
+        turn_begin(turns);
+#pragma unroll
+        for (int k = 0; k < 32; ++k) xb[k * XS + lane] = v[k];  // (k1 = k, n2 = lane)
+        __syncwarp();
+        const float4 *row = reinterpret_cast<const float4 *>(xb + lane * XS);  // k1 = lane
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const float4 w = row[q];
+            v[2 * q] = make_float2(w.x, w.y);
+            v[2 * q + 1] = make_float2(w.z, w.w);
+        }
+        __syncwarp();
+        turn_end(turns);
         TChunk c0, c1;
-        const unsigned ta = t + (step >> 1) * TM_TAB;
-        const bool mul = POST || step == 1;
-        if ((step & 1) && mul) tm_ld_before(c0, ta, v[0].x);  // in flight during the butterflies
-        dft32<-1>(v);
-        if ((step & 1) && !mul) {
+        const unsigned ta = t + f * TM_TAB;
+        const bool mul = POST || f == 0;
+        if (mul) tm_ld_before(c0, ta, v[0].x);  // in flight during the butterflies
+        sfdb::dft32_tw(v, tw);
+        // v[k] now holds out_sign(k) x the FFT value (sign tracking of sfd_dft32.cuh; the sign stage A
+        // left behind depends on the lane and sits in the tables): the compile-time sign is applied
+        // together with the conjugation / the table multiply
+        if (!mul) {
 #pragma unroll
-            for (int k = 0; k < 32; ++k) v[k].y = -v[k].y;
-            SFDW_STAMP(16 + 4 * step + 1);
-            if (!PP_TRANSPOSE) turn_end(turns);
-        } else if (step & 1) {
+            for (int k = 0; k < 32; ++k) {
+                if (sfdb::out_sign(k) > 0)
+                    v[k].y = -v[k].y;
+                else
+                    v[k].x = -v[k].x;
+            }
+        } else {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {  // v = conj(v * t)
+            for (int j = 0; j < 4; ++j) {  // v = conj(sign v * table)
                 TChunk &c = (j & 1) ? c1 : c0;
                 tm_wait(c);
                 if (j < 3) tm_ld((j & 1) ? c0 : c1, ta + 16 * (j + 1));
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
-                    const float2 h = tm_val(c, i), a = v[8 * j + i];
-                    v[8 * j + i] = make_float2(a.x * h.x - a.y * h.y, -(a.x * h.y) - a.y * h.x);
+                    const float sg = (float)sfdb::out_sign(8 * j + i);
+                    const float2 h = tm_val(c, i);
+                    const float ax = sg * v[8 * j + i].x, ay = sg * v[8 * j + i].y;
+                    v[8 * j + i] = make_float2(ax * h.x - ay * h.y, -(ax * h.y) - ay * h.x);
                 }
             }
-            SFDW_STAMP(16 + 4 * step + 1);
-            if (step != 1 && !PP_TRANSPOSE) turn_end(turns);
-        } else {
-            if constexpr (TWT) {
-                const unsigned tt = (t & 0xffff0000u) + TM_TW;  // twiddle columns of this quarter
-                tm_ld(c0, tt);
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    TChunk &c = (j & 1) ? c1 : c0;
-                    tm_wait(c);
-                    if (j < 3) tm_ld((j & 1) ? c0 : c1, tt + 16 * (j + 1));
-#pragma unroll
-                    for (int i = (j == 0 ? 1 : 0); i < 8; ++i) v[8 * j + i] = cmul(v[8 * j + i], tm_val(c, i));
-                }
-            } else {
-#pragma unroll
-                for (int k = 1; k < 32; ++k) {
-                    if constexpr (TWR)
-                        v[k] = cmul(v[k], tw[k]);
-                    else
-                        v[k] = cmul(v[k], twsm[k * 32 + lane]);
-                }
-            }
-            SFDW_STAMP(16 + 4 * step + 1);
-            if (PP_TRANSPOSE) turn_begin(turns); else turn_end(turns);
-#pragma unroll
-            for (int k = 0; k < 32; ++k) xb[k * XS + lane] = v[k];  // (k1 = k, n2 = lane)
-            __syncwarp();
-            const float4 *row = reinterpret_cast<const float4 *>(xb + lane * XS);  // k1 = lane
-#pragma unroll
-            for (int q = 0; q < 16; ++q) {
-                const float4 w = row[q];
-                v[2 * q] = make_float2(w.x, w.y);
-                v[2 * q + 1] = make_float2(w.z, w.w);
-            }
-            __syncwarp();
-            if (PP_TRANSPOSE) turn_end(turns);
         }
-        SFDW_STAMP(16 + 4 * step + 2);
     }
 }
 
@@ -622,9 +400,7 @@ template <> struct TileElem<float> {                 // float: 1 item per slab
 template <typename TIn> struct SmemY {
     float2 xb[WY][XB];
     alignas(128) float2 stage[2][N][2];  // [half][n1][column of the half]: final sums, TMA store source
-    float2 tw[SFDW_TWR == 0 ? 32 * 32 : 1];
     typename TileElem<TIn>::type tile[2][TileElem<TIn>::IPS][N];  // [half][k][n0]: the half's slab
-    unsigned long long turn[8];
     unsigned tmem;  // base address of the tensor-memory allocation
 };
 
@@ -728,18 +504,13 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
         tile_store(t, sm.tile[half], ht);
     }
     half_sync(half);
-    constexpr bool PP = SFDW_PINGPONG != 0;
-    Turns turns = turns_make(sm.turn, warp, PP);
+    const Turns turns = turns_make(warp, true);
     turns_open(turns, warp);
     for (int item = i0; item < i1; ++item) {
         const int view = item / groups, g = item % groups, k = g % IPS;
         const int colh = g / IPS * (YC * IPS) + 2 * IPS * half + 2 * k;
         const unsigned tpre = tq + (view - view0) * TM_SET;  // pre_b | H_b | conj(post_b)
         const bool has_next = item + 1 < i1 && k == IPS - 1;  // the next item opens a new slab
-#ifdef SFDW_TRACE
-        long long *tr = g_trace + (((size_t)blockIdx.x * WY + warp) * 16 + (item - i0)) * 32;
-#endif
-        SFDW_STAMP(0);
         TileRegs<TIn> t;
         float2 v[32];
         {
@@ -758,17 +529,11 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
                 }
             }
         }
-        SFDW_STAMP(1);
         // the next slab is fetched behind the tile reads: its loads touch one row per lane (32
         // wavefronts each) and would hold up everything queued after them
         if (has_next)
             tile_load<TIn>(t, holo, ((item + 1) % groups) / IPS * (YC * IPS) + 2 * IPS * half, ht);
-#ifdef SFDW_TRACE
-        branch(v, lane, xb, tw, sm.tw, tpre + TM_TAB, turns, tr);
-#else
-        branch(v, lane, xb, tw, sm.tw, tpre + TM_TAB, turns);
-#endif
-        SFDW_STAMP(8);
+        branch(v, lane, xb, tw, tpre + TM_TAB, turns);
         // the previous item's bulk stores must have left the staging tile before it is rewritten
         if (leader) bulk_wait_read();
         if (b == 0)
@@ -776,7 +541,6 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
         else
             y_hand_over<1>(v, xb, lane);
         half_sync(half);  // partner's hand-over visible; staging tile and input tile free
-        SFDW_STAMP(9);
         if (b == 0)
             y_finish<0>(v, xbp, stg, lane, c);
         else
@@ -790,21 +554,18 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
                 tma_store_2d(tmB, stg + j * YBOX * 2, 2 * colh, view * N + j * YBOX);
             bulk_commit();
         }
-        SFDW_STAMP(3);
     }
     if (leader) bulk_wait_read();  // shared memory must outlive the last store's reads
     turns_close(turns, warp);
 }
 
 // ---- pass x: one row of B per warp pair -----------------------------------------------------------
-constexpr int WX = SFDW_WX;  // warps per CTA
+constexpr int WX = 8;        // warps per CTA
 constexpr int XP = WX / 2;   // pairs per CTA = rows in flight per CTA
 struct SmemX {
     float2 xb[WX][XB];
-    float2 tw[32 * 32];
     float2 inb[XP][N];  // input row of each pair (bulk async copy destination)
     unsigned long long ibar[XP];
-    unsigned long long turn[8];
     unsigned tmem;  // base address of the tensor-memory allocation
 };
 
@@ -874,25 +635,20 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
     bool pending = false;  // the pair's input row is already on its way
     // turn-taking of warps w and w + 4 (needs every warp of the CTA to run the same number of
     // lines: XP divides N)
-    constexpr bool PP = SFDW_PINGPONG != 0 && WX == 8 && N % XP == 0;
-    Turns turns = turns_make(sm.turn, warp, PP);
+    static_assert(WX == 8 && N % XP == 0, "turn-taking needs equal line counts per warp");
+    const Turns turns = turns_make(warp, true);
     turns_open(turns, warp);
     for (int u = u0; u < u1; ++u) {
         const int view = u / gpv, line = (u % gpv) * XP + pair;
         if (line >= N) continue;  // pair-uniform (ragged last group of a view when XP does not divide N)
         const unsigned tpre = tq + (view - view0) * TM_SET;  // pre_b | H_b | conj(post_b)
         const size_t row = (size_t)view * N + line;
-#ifdef SFDW_TRACE
-        long long *tr = g_trace + TRACE_PASS + (((size_t)blockIdx.x * WX + warp) * 16 + ((u - u0) & 15)) * 32;
-#endif
-        SFDW_STAMP(0);
         if (!pending && issuer)
             bulk_load(sm.inb[pair], Bin + row * N, N * sizeof(float2), &sm.ibar[pair]);
         const int nu = u + 1, nline = (nu % gpv) * XP + pair;
         const bool has_next = nu < u1 && nline < N;
         mbar_wait(&sm.ibar[pair], iphase);
         iphase ^= 1;
-        SFDW_STAMP(1);
         float2 v[32];
         {
             TChunk c0, c1;
@@ -907,26 +663,19 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
                     v[8 * j + i] = cmul(in[32 * (8 * j + i)], tm_val(ch, i));
             }
         }
-        SFDW_STAMP(2);
         // both warps have consumed the input row and finished with each other's transpose tile
         pair_sync(pair);
-        SFDW_STAMP(3);
         if (has_next && issuer) {
             fence_async_smem();
             bulk_load(sm.inb[pair], Bin + ((size_t)(nu / gpv) * N + nline) * N, N * sizeof(float2),
                       &sm.ibar[pair]);
         }
         pending = has_next;
-#ifdef SFDW_TRACE
-        branch(v, lane, xb, tw, sm.tw, tpre + TM_TAB, turns, tr);
-#else
-        branch(v, lane, xb, tw, sm.tw, tpre + TM_TAB, turns);
-#endif
+        branch(v, lane, xb, tw, tpre + TM_TAB, turns);
         if (b == 0)
             x_finish<0>(v, xb, xbp, lane, pair, field, inten, row * N, mom, vmax, view);
         else
             x_finish<1>(v, xb, xbp, lane, pair, field, inten, row * N, mom, vmax, view);
-        SFDW_STAMP(9);
     }
     turns_close(turns, warp);
 }

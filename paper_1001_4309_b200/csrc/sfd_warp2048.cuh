@@ -138,7 +138,6 @@ struct SmemXQ {
     Exch ex;
     float2 inb[2][NL];  // input row of each quad (bulk async copy destination)
     unsigned long long ibar[2];
-    unsigned long long turn[8];
     unsigned tmem;
 };
 
@@ -152,7 +151,7 @@ __device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *__restrict
     const bool issuer = b == 0 && lane == 0;
     unsigned iphase = 0;
     bool pending = false;
-    Turns turns = turns_make(sm.turn, warp, SFDW_PINGPONG != 0);
+    const Turns turns = turns_make(warp, true);
     turns_open(turns, warp);
     for (int u = rg.u0; u < rg.u1; ++u) {
         const size_t row = (size_t)rg.view * NL + 2 * u + quad;
@@ -184,12 +183,7 @@ __device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *__restrict
             bulk_load(sm.inb[quad], Bin + (row + 2) * NL, NL * sizeof(float2), &sm.ibar[quad]);
         }
         pending = has_next;
-#ifdef SFDW_TRACE
-        long long *tr = g_trace;
-        branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns, tr);
-#else
-        branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns);
-#endif
+        branch<false>(v, lane, xb, tw, tq + TQ_H, turns);
         float2 mine[16];
         quad_scatter(v, mine, tq, b, lane, sm.xb, sm.ex, warp);
         quad_sync(quad);
@@ -255,7 +249,6 @@ template <typename TIn> struct SmemYQ {
     Exch ex;
     alignas(128) float2 stage[NL][4];  // [n1][column of the unit]: final sums, TMA store source
     typename TileElem<TIn>::type tile[2][SubSlab<TIn>::IPS][N][2];  // [quad][k][n'][h]
-    unsigned long long turn[8];
     unsigned tmem;
 };
 template <typename TIn> struct SubRegs { typename SubSlab<TIn>::elem e[16]; };
@@ -316,7 +309,7 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *__restri
         sub_store(t, sm.tile[quad], qt, quad);
     }
     quad_sync(quad);
-    Turns turns = turns_make(sm.turn, warp, SFDW_PINGPONG != 0);
+    const Turns turns = turns_make(warp, true);
     turns_open(turns, warp);
     for (int u = rg.u0; u < rg.u1; ++u) {
         const int k = u % IPS;
@@ -346,12 +339,7 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *__restri
             // loads touch one row per lane (32 wavefronts each)
             if (cc == 1 && next_slab) sub_load<TIn>(t, holo, SubSlab<TIn>::col(u + 1, quad), qt);
             quad_sync(quad);  // the previous column's exchange area has been read by all four warps
-#ifdef SFDW_TRACE
-            long long *tr = g_trace;
-            branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns, tr);
-#else
-            branch<false>(v, lane, xb, tw, nullptr, tq + TQ_H, turns);
-#endif
+            branch<false>(v, lane, xb, tw, tq + TQ_H, turns);
             // the previous unit's bulk stores must have left the staging tile before it is rewritten
             if (cc == 0 && leader) bulk_wait_read();
             float2 mine[16];
