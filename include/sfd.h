@@ -46,7 +46,8 @@ typedef struct sfd_plan sfd_plan; /* opaque */
 #define SFD_EINVAL (-1)       /* bad argument (NULL, size, non-finite parameter, z == 0, ...) */
 #define SFD_ENOMEM (-2)       /* host or device allocation failed */
 #define SFD_ECUDA (-3)        /* a CUDA runtime call failed; see sfd_last_cuda_error() */
-#define SFD_EUNSUPPORTED (-4) /* valid request that this build does not implement */
+#define SFD_EUNSUPPORTED (-4) /* valid request that this build does not implement (a grid side that
+                                 is not a power of two in 64..2048; more than 64 devices) */
 
 /* hologram sample types (argument in_dtype) */
 #define SFD_U8 0  /* unsigned 8-bit CCD samples; the method sees value/255 (reading 12) */
@@ -58,13 +59,16 @@ typedef struct sfd_plan sfd_plan; /* opaque */
  * of every frame), uploads them as complex64 and allocates the workspace
  * (n_views * N * N complex64 + n_views * N * N float32).
  *   out      receives the plan; *out = NULL on failure.
- *   N        hologram / output side; a power of two, 64 <= N <= 2048.
+ *   N        hologram / output side >= 1; this build has kernels for powers of two in 64..2048 and
+ *            returns SFD_EUNSUPPORTED for every other size.
  *   n_views  >= 1.
  *   lambda   wavelength > 0.
  *   p1,p2,z,Ox,Oy  host arrays [n_views]: hologram pitch (> 0), reconstruction pitch (> 0), depth
  *            (finite, != 0; negative = conjugate reconstruction), shifts of the output window.
  *   in_dtype SFD_U8 or SFD_F32.
- * Errors: SFD_EINVAL, SFD_ENOMEM, SFD_ECUDA. */
+ * Errors: SFD_EINVAL, SFD_EUNSUPPORTED, SFD_ENOMEM, SFD_ECUDA.
+ * The device current at the call becomes the plan's device; later calls on the plan may be made with
+ * any device current (the library switches to the plan's device and back). */
 SFD_API int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const double *p1,
                     const double *p2, const double *z, const double *Ox, const double *Oy,
                     int in_dtype);
@@ -111,17 +115,32 @@ SFD_API int sfd_stream_run(sfd_plan *plan, const void *holograms_pinned, int n_f
                    unsigned char *out_pinned, double *seconds);
 
 /* Replace the parameters of one view (0 <= view < n_views) and rebuild its tables and cached
- * spectrum (the paper's user steers z, p2, Ox, Oy live: L33, L73, L123).  Synchronises with the
- * device (cudaMemcpy) before returning; do not call while an execute on this plan is in flight. */
+ * spectrum (the paper's user steers z, p2, Ox, Oy live: L33, L73, L123).  Blocking form: the new
+ * tables are on the device when the call returns (ordered on the legacy default stream); do not call
+ * it while an execute of this plan is in flight on a non-blocking stream. */
 SFD_API int sfd_plan_update_view(sfd_plan *plan, int view, double p1, double p2, double z, double Ox,
                          double Oy);
+
+/* Live steering without a host-device synchronisation: the tables of the view are built on the host
+ * (float64, about a millisecond at N = 1024: sfd_plan_last_update_host_ms) into a page-locked staging
+ * block and ONE asynchronous copy is enqueued on `stream`.  Stream order does the rest: executes
+ * enqueued on that stream before the call still see the old view, executes enqueued after it the new
+ * one, and the call is legal while earlier executes are in flight.  Use the stream the executes of
+ * this plan run on.  At most 4 updates are in flight per plan (a fifth waits for the first copy). */
+SFD_API int sfd_plan_update_view_async(sfd_plan *plan, int view, double p1, double p2, double z,
+                                       double Ox, double Oy, void *stream);
+SFD_API int sfd_plan_update_view_general_async(sfd_plan *plan, int view, double p1x, double p1y,
+                                               double p2x, double p2y, double z, double O0x,
+                                               double O0y, double O1x, double O1y, void *stream);
+/* Host time, in milliseconds, the table builder took in the most recent update of this plan. */
+SFD_API double sfd_plan_last_update_host_ms(const sfd_plan *plan);
 
 /* General geometry (Eq.(2)-(4) L58-65 and the definitions L67 keep
  * separate x and y sampling pitches, hence S_x = p1x p2x/(lambda z) != S_y = p1y p2y/(lambda z), and
  * offsets (O_x0, O_y0) of the hologram window next to (O_x1, O_y1) of the reconstruction window).
  * Physical coordinates (reading 1 of DESIGN.md): x0 = (m0 - N/2) p1x + O0x, y0 = (n0 - N/2) p1y + O0y,
  * x1 = (m1 - N/2) p2x + O1x, y1 = (n1 - N/2) p2y + O1y, all lengths in metres, arrays [n_views] on
- * the host.  sfd_plan_create is this call with p1x = p1y, p2x = p2y, O0 = 0.  The grid stays N x N.
+ * the host.  sfd_plan_create is this call with p1x = p1y, p2x = p2y, O0 = 0.
  * Each axis gets its own chirp tables and its own cached kernel spectrum.  Same errors. */
 SFD_API int sfd_plan_create_general(sfd_plan **out, int N, int n_views, double lambda,
                                     const double *p1x, const double *p1y, const double *p2x,
@@ -132,26 +151,54 @@ SFD_API int sfd_plan_update_view_general(sfd_plan *plan, int view, double p1x, d
                                          double p2x, double p2y, double z, double O0x, double O0y,
                                          double O1x, double O1y);
 
+/* Rectangular grids (Eq.(2)-(3), L58-62, carry N_x and N_y separately): the hologram and every
+ * output are [Ny][Nx] (Ny rows along y, Nx samples along x); the optical axis sits at index
+ * (Ny/2, Nx/2).  Pass y runs Nx lines of length Ny, pass x Ny lines of length Nx; each axis picks its
+ * kernels by its own length.  Nx, Ny: powers of two in 64..2048 (else SFD_EUNSUPPORTED).
+ * sfd_plan_create_general is this call with Nx = Ny = N. */
+SFD_API int sfd_plan_create_rect(sfd_plan **out, int Nx, int Ny, int n_views, double lambda,
+                                 const double *p1x, const double *p1y, const double *p2x,
+                                 const double *p2y, const double *z, const double *O0x,
+                                 const double *O0y, const double *O1x, const double *O1y,
+                                 int in_dtype);
+
+/* Hologram window inside a larger frame (the 1 360 x 1 024 CCD frame is cut down to
+ * 1 024 x 1 024; reading 13: a crop, which keeps the 4.65 um pitch the paper then uses, L107).
+ * After this call the hologram_dev argument of sfd_execute* points at the FRAME: rows of
+ * row_stride samples, of which the plan reads the Ny x Nx window whose first sample is
+ * frame[row0][col0] - in place, no copy.  row_stride = 0 restores the dense default (row_stride =
+ * Nx, row0 = col0 = 0).  A physical shift of the window goes into O0x / O0y of the plan (the centred
+ * crop needs none).  The warp-per-branch kernels need the window's first sample and the row stride on
+ * 8-byte boundaries (uint8: col0 and row_stride multiples of 8 on an aligned frame); otherwise the
+ * generic kernels run.  sfd_stream_run always reads dense frames.
+ * Errors: SFD_EINVAL (negative values, row_stride < col0 + Nx). */
+SFD_API int sfd_plan_set_input_window(sfd_plan *plan, long long row_stride, int row0, int col0);
+
 /* Destroy a plan and free everything it owns.  NULL is accepted. */
 SFD_API int sfd_plan_destroy(sfd_plan *plan);
 
-/* Plan queries (host): N, n_views, padded FFT length M = 2N, bytes of device memory owned. */
+/* Plan queries (host): Nx (also as "n"), Ny, n_views, padded FFT length Mx = 2 Nx, the plan's device,
+ * bytes of device memory owned. */
 SFD_API int sfd_plan_get_n(const sfd_plan *plan);
+SFD_API int sfd_plan_get_nx(const sfd_plan *plan);
+SFD_API int sfd_plan_get_ny(const sfd_plan *plan);
+SFD_API int sfd_plan_get_device(const sfd_plan *plan);
 SFD_API int sfd_plan_get_views(const sfd_plan *plan);
 SFD_API int sfd_plan_get_m(const sfd_plan *plan);
 SFD_API long long sfd_plan_device_bytes(const sfd_plan *plan);
 
-/* Kernel selection.  SFD_KERNELS_AUTO (default): N = 1024 and N = 2048 run the warp-per-branch
- * kernels, every other size the generic shared-memory Stockham kernels.
+/* Kernel selection.  SFD_KERNELS_AUTO (default): an axis of length 1024 or 2048 runs the
+ * warp-per-branch kernels, every other length the generic shared-memory Stockham
+ * kernels.
  * SFD_KERNELS_GENERIC forces the generic kernels at every size (tests, A/B timing).  Both compute
  * the same transform; results differ by fp32 rounding only.  Errors: SFD_EINVAL. */
 #define SFD_KERNELS_AUTO 0
 #define SFD_KERNELS_GENERIC 1
 SFD_API int sfd_plan_select_kernels(sfd_plan *plan, int which);
 
-/* 1 if sfd_execute* on this plan currently runs the warp-per-branch kernels (k_cols_1024 /
- * k_rows_1024 or k_cols_2048 / k_rows_2048), 0 if it runs the generic kernels (k_pass_y, k_pass_x);
- * SFD_EINVAL for NULL. */
+/* Which passes of sfd_execute* on this plan currently run the warp-per-branch kernels: bit 0 = pass
+ * y (k_cols_1024 / k_cols_2048; for an aligned hologram), bit 1 = pass x (k_rows_1024 /
+ * k_rows_2048); 0 = both run the generic kernels (k_pass_y, k_pass_x); SFD_EINVAL for NULL. */
 SFD_API int sfd_plan_uses_warp_kernels(const sfd_plan *plan);
 
 /* Timing aid for benchmarks: CUDA-event time, in milliseconds, of each of the two hot kernels
@@ -170,6 +217,20 @@ SFD_API long long sfd_launch_count(void);
  * arrays of 2N, 2N and 4N doubles.  `off` is the window shift along that axis.  N: power of two. */
 SFD_API int sfd_host_tables(int N, double lambda, double p1, double p2, double z, double off, double *pre,
                     double *post, double *H);
+
+/* Host-only diagnostic (no GPU needed): one radix-32 stage of the warp FFT as the kernels compute it
+ * (sfd_dft32.cuh, fp32, FMA-formulated radix-2 butterflies), stepped on the CPU.  in / out: 32 complex
+ * values as interleaved (re, im) floats.  twiddled = 0: out[k] = sum_r in[r] exp(-2 pi i r k / 32)
+ * (stage A); twiddled = 1: out[k] = sum_r in[r] exp(-2 pi i (r lane / 1024 + r k / 32)) (stage B of
+ * lane `lane`, 0..31, inter-stage twiddles folded in). */
+SFD_API int sfd_host_dft32(const float *in, float *out, int lane, int twiddled);
+
+/* Measured pipe rates of the current device, the denominators bench.py reports against:
+ * out[0] plain fp32 FMA throughput of the whole GPU in TFLOP/s (2 flop per FMA), out[1] / out[2]
+ * cycles of one stage-A / stage-B radix-32 butterfly for a warp that has its sub-partition to
+ * itself, out[3] the SM clock during the measurement in GHz.  Runs a few milliseconds of kernels on
+ * the legacy default stream and synchronises.  Errors: SFD_EINVAL, SFD_ECUDA. */
+SFD_API int sfd_measure_pipes(double out[4]);
 
 /* The same for a hologram window shifted by off0 along that axis (general geometry). */
 SFD_API int sfd_host_tables_general(int N, double lambda, double p1, double p2, double z, double off0,

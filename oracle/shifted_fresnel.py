@@ -130,6 +130,23 @@ def input_scale(u0):
     return u0.astype(np.float64)
 
 
+def crop_window(frame, Ny, Nx, row0=None, col0=None):
+    """the 1 360 x 1 024 CCD frame is "resized" to 1 024 x 1 024 before the transform.
+    Reading 13: a crop - the only resize that keeps the 4.65 um sample pitch the paper
+    goes on to use (L107: field of view 4.8 mm = 1 024 x 4.65 um).  Returns the ``Ny x Nx`` window
+    whose first sample is ``frame[row0][col0]``; ``None`` centres the window (168 columns are cut on
+    either side of a 1 360-wide frame).  A centred window keeps the optical axis at index N/2, so no
+    offset O_0 is needed; a window shifted by (dr, dc) samples off centre is the hologram window of
+    Eq.(2)-(3) with ``O_0 = (dc p_x0, dr p_y0)``."""
+    frame = np.asarray(frame)
+    rows, cols = frame.shape
+    row0 = (rows - Ny) // 2 if row0 is None else int(row0)
+    col0 = (cols - Nx) // 2 if col0 is None else int(col0)
+    if row0 < 0 or col0 < 0 or row0 + Ny > rows or col0 + Nx > cols:
+        raise ValueError("window exceeds the frame")
+    return frame[row0:row0 + Ny, col0:col0 + Nx]
+
+
 # --------------------------------------------------------------------------------------
 # form D: the definition, O(N^4)
 # --------------------------------------------------------------------------------------

@@ -9,15 +9,13 @@ raises ``SfdError`` on a non-zero return code."""
 from __future__ import annotations
 
 import ctypes as C
-import os
 import pathlib
 import re
 
 import numpy as np
 
 _PKG = pathlib.Path(__file__).resolve().parent
-# SFD_LIBRARY=<path> loads another build of the same library (e.g. an experimental variant)
-LIB_PATH = pathlib.Path(os.environ.get("SFD_LIBRARY", _PKG / "libsfd.so"))
+LIB_PATH = _PKG / "libsfd.so"        # the in-tree build, nothing else
 HEADER_PATH = _PKG.parent / "include" / "sfd.h"
 
 SFD_OK, SFD_EINVAL, SFD_ENOMEM, SFD_ECUDA, SFD_EUNSUPPORTED = 0, -1, -2, -3, -4
@@ -39,6 +37,17 @@ _sig = {
     "sfd_plan_create_general": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_double] + [_dp] * 9
                                 + [C.c_int]),
     "sfd_plan_update_view_general": (C.c_int, [_vp, C.c_int] + [C.c_double] * 9),
+    "sfd_plan_create_rect": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_double] + [_dp] * 9
+                             + [C.c_int]),
+    "sfd_plan_set_input_window": (C.c_int, [_vp, C.c_longlong, C.c_int, C.c_int]),
+    "sfd_plan_update_view_async": (C.c_int, [_vp, C.c_int] + [C.c_double] * 5 + [_vp]),
+    "sfd_plan_update_view_general_async": (C.c_int, [_vp, C.c_int] + [C.c_double] * 9 + [_vp]),
+    "sfd_plan_last_update_host_ms": (C.c_double, [_vp]),
+    "sfd_plan_get_nx": (C.c_int, [_vp]),
+    "sfd_plan_get_ny": (C.c_int, [_vp]),
+    "sfd_plan_get_device": (C.c_int, [_vp]),
+    "sfd_host_dft32": (C.c_int, [C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_int, C.c_int]),
+    "sfd_measure_pipes": (C.c_int, [_dp]),
     "sfd_host_tables_general": (C.c_int, [C.c_int] + [C.c_double] * 6 + [_dp, _dp, _dp]),
     "sfd_execute": (C.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "sfd_execute_u8": (C.c_int, [_vp, _vp, _vp, _vp]),
@@ -148,6 +157,69 @@ def sfd_plan_create_general(N, n_views, lam, p1x, p1y, p2x, p2y, z, O0x, O0y, O1
     return h.value
 
 
+def sfd_plan_create_rect(Nx, Ny, n_views, lam, p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y,
+                         in_dtype=SFD_U8):
+    """Rectangular grid [Ny][Nx] with the general geometry (include/sfd.h)."""
+    arrs = [_darr(a, n_views) for a in (p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y)]
+    h = _vp()
+    _chk(_lib.sfd_plan_create_rect(C.byref(h), int(Nx), int(Ny), int(n_views), float(lam),
+                                   *[a.ctypes.data_as(_dp) for a in arrs], int(in_dtype)),
+         "sfd_plan_create_rect")
+    return h.value
+
+
+def sfd_plan_set_input_window(plan, row_stride, row0, col0):
+    _chk(_lib.sfd_plan_set_input_window(plan, int(row_stride), int(row0), int(col0)),
+         "sfd_plan_set_input_window")
+
+
+def sfd_plan_update_view_async(plan, view, p1, p2, z, Ox, Oy, stream=None):
+    _chk(_lib.sfd_plan_update_view_async(plan, int(view), float(p1), float(p2), float(z), float(Ox),
+                                         float(Oy), _stream(stream)), "sfd_plan_update_view_async")
+
+
+def sfd_plan_update_view_general_async(plan, view, p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y,
+                                       stream=None):
+    _chk(_lib.sfd_plan_update_view_general_async(
+        plan, int(view), *map(float, (p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y)), _stream(stream)),
+        "sfd_plan_update_view_general_async")
+
+
+def sfd_plan_last_update_host_ms(plan):
+    return float(_lib.sfd_plan_last_update_host_ms(plan))
+
+
+def sfd_plan_get_nx(plan):
+    return int(_lib.sfd_plan_get_nx(plan))
+
+
+def sfd_plan_get_ny(plan):
+    return int(_lib.sfd_plan_get_ny(plan))
+
+
+def sfd_plan_get_device(plan):
+    return int(_lib.sfd_plan_get_device(plan))
+
+
+def sfd_host_dft32(x, lane=0, twiddled=False):
+    """Host-only: one radix-32 stage of the warp FFT stepped on the CPU; x = 32 complex values."""
+    a = np.ascontiguousarray(np.asarray(x, dtype=np.complex64)).view(np.float32)
+    if a.shape != (64,):
+        raise ValueError("expected 32 complex values")
+    out = np.empty(64, np.float32)
+    fp = C.POINTER(C.c_float)
+    _chk(_lib.sfd_host_dft32(a.ctypes.data_as(fp), out.ctypes.data_as(fp), int(lane),
+                             int(bool(twiddled))), "sfd_host_dft32")
+    return out.view(np.complex64)
+
+
+def sfd_measure_pipes():
+    """(fp32 FMA TFLOP/s, cycles per stage-A butterfly, cycles per stage-B butterfly, SM GHz)."""
+    out = np.zeros(4, np.float64)
+    _chk(_lib.sfd_measure_pipes(out.ctypes.data_as(_dp)), "sfd_measure_pipes")
+    return tuple(float(v) for v in out)
+
+
 def sfd_plan_update_view_general(plan, view, p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y):
     _chk(_lib.sfd_plan_update_view_general(plan, int(view), *map(float, (p1x, p1y, p2x, p2y, z, O0x,
                                                                          O0y, O1x, O1y))),
@@ -252,10 +324,17 @@ class Plan:
         if workload is not None:
             kw = dict(N=workload.N, lam=workload.lam, p1=workload.p1, p2=workload.p2,
                       z=workload.z, Ox=workload.Ox, Oy=workload.Oy, in_dtype=workload.in_dtype)
-        self.N = int(kw["N"])
+        self.Nx = int(kw["Nx"] if "Nx" in kw else kw["N"])
+        self.Ny = int(kw["Ny"] if "Ny" in kw else kw["N"])
+        self.N = self.Nx
         self.V = len(np.atleast_1d(kw["z"]))
         self.in_dtype = int(kw.get("in_dtype", SFD_U8))
-        if "p1x" in kw:     # general geometry: p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y
+        self.frame_shape = None      # set by set_input_window: hologram tensors are whole frames
+        if "Nx" in kw:      # rectangular grid [Ny][Nx], general geometry
+            self.handle = sfd_plan_create_rect(
+                self.Nx, self.Ny, self.V, kw["lam"], kw["p1x"], kw["p1y"], kw["p2x"], kw["p2y"],
+                kw["z"], kw["O0x"], kw["O0y"], kw["O1x"], kw["O1y"], self.in_dtype)
+        elif "p1x" in kw:   # general geometry: p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y
             self.handle = sfd_plan_create_general(
                 self.N, self.V, kw["lam"], kw["p1x"], kw["p1y"], kw["p2x"], kw["p2y"], kw["z"],
                 kw["O0x"], kw["O0y"], kw["O1x"], kw["O1y"], self.in_dtype)
@@ -279,16 +358,30 @@ class Plan:
     def _check_holo(self, hologram):
         import torch
         want = torch.uint8 if self.in_dtype == SFD_U8 else torch.float32
-        if (hologram.dtype != want or tuple(hologram.shape) != (self.N, self.N)
+        shape = self.frame_shape or (self.Ny, self.Nx)
+        if (hologram.dtype != want or tuple(hologram.shape) != shape
                 or not hologram.is_cuda or not hologram.is_contiguous()):
-            raise ValueError(f"hologram must be a contiguous CUDA tensor [{self.N},{self.N}] {want}")
+            raise ValueError(f"hologram must be a contiguous CUDA tensor {list(shape)} {want}")
+
+    def set_input_window(self, frame_shape, row0, col0):
+        """Holograms passed to execute* are whole frames ``frame_shape = (rows, row_stride)``; the
+        plan reads its Ny x Nx window at (row0, col0) in place.  ``frame_shape=None`` = dense."""
+        if frame_shape is None:
+            sfd_plan_set_input_window(self.handle, 0, 0, 0)
+            self.frame_shape = None
+            return
+        rows, stride = int(frame_shape[0]), int(frame_shape[1])
+        if row0 + self.Ny > rows:
+            raise ValueError("window exceeds the frame")
+        sfd_plan_set_input_window(self.handle, stride, row0, col0)
+        self.frame_shape = (rows, stride)
 
     def execute(self, hologram, field=True, intensity=True, stream=None):
         """Returns ``(field complex64 [V,N,N] | None, intensity float32 [V,N,N] | None)``.
         ``field`` / ``intensity`` may be ``True`` (allocate), ``False`` (skip) or a tensor."""
         import torch
         self._check_holo(hologram)
-        shape = (self.V, self.N, self.N)
+        shape = (self.V, self.Ny, self.Nx)
         if field is True:
             field = torch.empty(shape, dtype=torch.complex64, device=hologram.device)
         elif field is False:
@@ -306,7 +399,7 @@ class Plan:
         import torch
         self._check_holo(hologram)
         mom = torch.empty((self.V, 2), dtype=torch.float64, device=hologram.device)
-        I = (torch.empty((self.V, self.N, self.N), dtype=torch.float32, device=hologram.device)
+        I = (torch.empty((self.V, self.Ny, self.Nx), dtype=torch.float32, device=hologram.device)
              if intensity else None)
         sfd_execute_focus(self.handle, hologram, mom, I, stream)
         return mom, I
@@ -315,7 +408,7 @@ class Plan:
         import torch
         self._check_holo(hologram)
         if out is None:
-            out = torch.empty((self.V, self.N, self.N), dtype=torch.uint8, device=hologram.device)
+            out = torch.empty((self.V, self.Ny, self.Nx), dtype=torch.uint8, device=hologram.device)
         sfd_execute_u8(self.handle, hologram, out, stream)
         return out
 
@@ -327,7 +420,7 @@ class Plan:
         if not holograms_pinned.is_pinned() or not holograms_pinned.is_contiguous():
             raise ValueError("holograms must be a contiguous pinned CPU tensor")
         if out_pinned is None:
-            out_pinned = torch.empty((F, self.V, self.N, self.N), dtype=torch.uint8).pin_memory()
+            out_pinned = torch.empty((F, self.V, self.Ny, self.Nx), dtype=torch.uint8).pin_memory()
         sec = sfd_stream_run(self.handle, holograms_pinned, F, out_pinned)
         return out_pinned, sec
 
@@ -337,12 +430,24 @@ class Plan:
     def update_view(self, view, p1, p2, z, Ox, Oy):
         sfd_plan_update_view(self.handle, view, p1, p2, z, Ox, Oy)
 
+    def update_view_async(self, view, p1, p2, z, Ox, Oy, stream=None):
+        sfd_plan_update_view_async(self.handle, view, p1, p2, z, Ox, Oy, stream)
+
+    @property
+    def last_update_host_ms(self):
+        return sfd_plan_last_update_host_ms(self.handle)
+
     def select_kernels(self, which):
         sfd_plan_select_kernels(self.handle, which)
 
     @property
     def uses_warp_kernels(self):
-        return bool(sfd_plan_uses_warp_kernels(self.handle))
+        """True when both passes run the warp-per-branch kernels (bit 0 = pass y, bit 1 = pass x)."""
+        return sfd_plan_uses_warp_kernels(self.handle) == 3
+
+    @property
+    def warp_kernel_mask(self):
+        return sfd_plan_uses_warp_kernels(self.handle)
 
     def set_timing(self, enable=True):
         sfd_plan_set_timing(self.handle, enable)

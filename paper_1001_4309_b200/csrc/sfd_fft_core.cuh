@@ -243,28 +243,28 @@ SFD_HD void chirpz_line(float2 (&v)[16], int j, LineSmem<ISTR> sm, const float2 
 }
 
 // ---- the two passes of a reconstruction --------------------------------------------------------
+// The grid is Ny rows by Nx columns; tables and B are already offset to the CTA's view.
 // Pass y (steps (ii)-(ix) along y): a CTA takes C adjacent hologram columns of one view; thread
-// (l, j), l fastest, works on column col0 + l.  in = hologram sample (real) * pre_y[n0] (Eq. 3, the
-// 1/255 of uint8 input folded into the table), out * post_y[n1] (Eq. 2 y-part, times c0) is
-// written to the row-major intermediate B[view][n1][m0] in 8C-byte chunks.
+// (l, j), l fastest, works on column col0 + l; the line length is Ny = Sched<LOG2M>::N.
+// in = hologram sample (real) * pre_y[n0] (Eq. 3, the 1/255 of uint8 input folded into the table),
+// out * post_y[n1] (Eq. 2 y-part, times c0) is written to the row-major intermediate B[n1][m0]
+// (nx columns) in 8C-byte chunks.  hstride = elements between hologram rows.
+// The hologram and B are produced by whatever ran before in the stream (a copy, pass y): they are
+// read with plain loads, not through the non-coherent path.
 template <int LOG2M, int C, typename TIn, class SyncF>
-SFD_HD void pass_y_body(int tid, int tile, int view, float2 *smem, const TIn *__restrict__ holo,
+SFD_HD void pass_y_body(int tid, int tile, float2 *smem, const TIn *holo, long long hstride, int nx,
                         const float2 *__restrict__ pre_y, const float2 *__restrict__ Hy,
                         const float2 *__restrict__ post_y, const float2 *__restrict__ tw,
-                        float2 *__restrict__ B, SyncF sync) {
+                        float2 *B, SyncF sync) {
     using S = Sched<LOG2M>;
-    constexpr int N = S::N, T = S::T;
+    constexpr int T = S::T;
     const int l = tid % C, j = tid / C;
     const int col = tile * C + l;
-    pre_y += (size_t)view * N;
-    post_y += (size_t)view * N;
-    Hy += (size_t)view * S::M;
-    B += (size_t)view * N * N;
     float2 v[16];
 #pragma unroll
     for (int s = 0; s < 8; ++s) {
         const int n0 = j + s * T;
-        const float a = (float)SFD_LDG(holo + (size_t)n0 * N + col);
+        const float a = (float)holo[(size_t)n0 * hstride + col];
         const float2 p = SFD_LDG(pre_y + n0);
         v[s] = make_float2(a * p.x, a * p.y);
     }
@@ -273,15 +273,16 @@ SFD_HD void pass_y_body(int tid, int tile, int view, float2 *smem, const TIn *__
 #pragma unroll
     for (int s = 0; s < 8; ++s) {
         const int n1 = j + s * T;
-        B[(size_t)n1 * N + col] = cmul(v[s], SFD_LDG(post_y + n1));
+        B[(size_t)n1 * nx + col] = cmul(v[s], SFD_LDG(post_y + n1));
     }
 }
 
 // Pass x (steps (ii)-(x) along x): a CTA takes RPC adjacent rows of one view; thread (l, j), j
-// fastest, works on row row0 + l.  in = B[n1][m0] * pre_x[m0], out * post_x[m1] is the field
-// u1[n1][m1]; intensity = |u1|^2 (Eq. 5).  Returns the largest intensity this thread produced.
+// fastest, works on row tile * RPC + l of the view; the line length is Nx = Sched<LOG2M>::N.
+// in = B[n1][m0] * pre_x[m0], out * post_x[m1] is the field u1[n1][m1]; intensity = |u1|^2 (Eq. 5).
+// B, field, inten are offset to the view.  Returns the largest intensity this thread produced.
 template <int LOG2M, int RPC, bool MOM, class SyncF>
-SFD_HD float pass_x_body(int tid, int tile, int view, float2 *smem, const float2 *__restrict__ B,
+SFD_HD float pass_x_body(int tid, int tile, float2 *smem, const float2 *B,
                          const float2 *__restrict__ pre_x, const float2 *__restrict__ Hx,
                          const float2 *__restrict__ post_x, const float2 *__restrict__ tw,
                          float2 *__restrict__ field, float *__restrict__ inten, SyncF sync,
@@ -289,10 +290,7 @@ SFD_HD float pass_x_body(int tid, int tile, int view, float2 *smem, const float2
     using S = Sched<LOG2M>;
     constexpr int N = S::N, T = S::T;
     const int l = tid / T, j = tid % T;
-    const size_t row = (size_t)view * N + (size_t)tile * RPC + l;
-    pre_x += (size_t)view * N;
-    post_x += (size_t)view * N;
-    Hx += (size_t)view * S::M;
+    const size_t row = (size_t)tile * RPC + l;
     const float2 *in = B + row * N;
     float2 v[16];
 #pragma unroll

@@ -12,6 +12,8 @@
 #include <cuda.h>  // CUtensorMap (types only: the encoder is fetched through the runtime)
 
 #include <atomic>
+#include <cmath>
+#include <vector>
 
 #include "sfd_fft_core.cuh"
 #include "sfd_internal.h"
@@ -33,33 +35,45 @@ template <int LOG2M> struct Tile {
     static constexpr size_t SMEM_X = sizeof(float2) * Sched<LOG2M>::PADDED * RPC;
 };
 
+// tables of one axis as the generic kernels see them: view v at base + v * vstride
+struct AxisTabs {
+    const float2 *base;
+    long long vstride;
+    int pre, H, post;  // offsets inside a view's block
+};
+
 template <int LOG2M, typename TIn>
 __global__ void __launch_bounds__(Tile<LOG2M>::THREADS_Y)
-k_pass_y(const TIn *__restrict__ holo, const float2 *__restrict__ pre_y,
-         const float2 *__restrict__ H, const float2 *__restrict__ post_y,
-         const float2 *__restrict__ tw, float2 *__restrict__ B, unsigned int *vmax, double *mom) {
+k_pass_y(const TIn *holo, long long hstride, int nx, AxisTabs t, const float2 *__restrict__ tw,
+         float2 *B, unsigned int *vmax, double *mom) {
     extern __shared__ float2 smem[];
     sfdw::pdl_launch_dependents();
     sfdw::pdl_wait();  // the hologram, B, vmax and mom belong to the kernels before this one
-    if (vmax != nullptr && blockIdx.x == 0 && threadIdx.x == 0) vmax[blockIdx.y] = 0u;
-    if (mom != nullptr && blockIdx.x == 0 && threadIdx.x < 2) mom[2 * blockIdx.y + threadIdx.x] = 0.0;
-    pass_y_body<LOG2M, Tile<LOG2M>::C, TIn>(threadIdx.x, blockIdx.x, blockIdx.y, smem, holo, pre_y,
-                                            H, post_y, tw, B, [] { __syncthreads(); });
+    const int view = blockIdx.y;
+    if (vmax != nullptr && blockIdx.x == 0 && threadIdx.x == 0) vmax[view] = 0u;
+    if (mom != nullptr && blockIdx.x == 0 && threadIdx.x < 2) mom[2 * view + threadIdx.x] = 0.0;
+    const float2 *tv = t.base + (size_t)view * t.vstride;
+    pass_y_body<LOG2M, Tile<LOG2M>::C, TIn>(threadIdx.x, blockIdx.x, smem, holo, hstride, nx,
+                                            tv + t.pre, tv + t.H, tv + t.post, tw,
+                                            B + (size_t)view * Sched<LOG2M>::N * nx,
+                                            [] { __syncthreads(); });
 }
 
 template <int LOG2M, bool MOM>
 __global__ void __launch_bounds__(Tile<LOG2M>::THREADS_X)
-k_pass_x(const float2 *__restrict__ B, const float2 *__restrict__ pre_x,
-         const float2 *__restrict__ H, const float2 *__restrict__ post_x,
-         const float2 *__restrict__ tw, float2 *__restrict__ field, float *__restrict__ inten,
-         unsigned int *vmax, double *mom) {
+k_pass_x(const float2 *B, int ny, AxisTabs t, const float2 *__restrict__ tw,
+         float2 *__restrict__ field, float *__restrict__ inten, unsigned int *vmax, double *mom) {
     extern __shared__ float2 smem[];
     sfdw::pdl_launch_dependents();
     sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
+    const int view = blockIdx.y;
+    const float2 *tv = t.base + (size_t)view * t.vstride;
+    const size_t voff = (size_t)view * ny * Sched<LOG2M>::N;
     float s1 = 0.f, s2 = 0.f;
-    float mx = pass_x_body<LOG2M, Tile<LOG2M>::RPC, MOM>(threadIdx.x, blockIdx.x, blockIdx.y, smem, B,
-                                                    pre_x, H, post_x, tw, field, inten,
-                                                    [] { __syncthreads(); }, s1, s2);
+    float mx = pass_x_body<LOG2M, Tile<LOG2M>::RPC, MOM>(
+        threadIdx.x, blockIdx.x, smem, B + voff, tv + t.pre, tv + t.H, tv + t.post, tw,
+        field ? field + voff : nullptr, inten ? inten + voff : nullptr, [] { __syncthreads(); }, s1,
+        s2);
     if (MOM) {  // focus moments: warp sums in float, accumulation across warps in double
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
@@ -67,29 +81,34 @@ k_pass_x(const float2 *__restrict__ B, const float2 *__restrict__ pre_x,
             s2 += __shfl_xor_sync(0xffffffffu, s2, o);
         }
         if ((threadIdx.x & 31) == 0) {
-            atomicAdd(mom + 2 * blockIdx.y, (double)s1);
-            atomicAdd(mom + 2 * blockIdx.y + 1, (double)s2);
+            atomicAdd(mom + 2 * view, (double)s1);
+            atomicAdd(mom + 2 * view + 1, (double)s2);
         }
     }
     if (vmax != nullptr) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
         // intensities are >= 0, so their float bit patterns order like unsigned integers
-        if ((threadIdx.x & 31) == 0) atomicMax(vmax + blockIdx.y, __float_as_uint(mx));
+        if ((threadIdx.x & 31) == 0) atomicMax(vmax + view, __float_as_uint(mx));
     }
 }
 
-// I8 = round_half_even(255 I / max I) per view (reading 15); 4 pixels per thread.
+// I8 = round_half_even(255 I / max I) per view (reading 15); 4 pixels per thread.  Launched with
+// programmatic stream serialization behind pass x: the per-view maxima are complete only when the
+// whole of pass x is, hence a kernel of its own; the intensities it reads were just written and sit
+// in L2.
 __global__ void __launch_bounds__(256)
-k_quantise(const float4 *__restrict__ inten, const unsigned int *__restrict__ vmax,
-           uchar4 *__restrict__ out, int quads_per_view) {
+k_quantise(const float4 *inten, const unsigned int *vmax, uchar4 *__restrict__ out,
+           int quads_per_view) {
+    sfdw::pdl_launch_dependents();
+    sfdw::pdl_wait();
     const int v = blockIdx.y;
     const float mx = __uint_as_float(vmax[v]);
     const float sc = mx > 0.f ? 255.f / mx : 0.f;
     const size_t base = (size_t)v * quads_per_view;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < quads_per_view;
          i += gridDim.x * blockDim.x) {
-        const float4 I = __ldg(inten + base + i);
+        const float4 I = inten[base + i];
         uchar4 o;
         o.x = (unsigned char)min(__float2int_rn(I.x * sc), 255);
         o.y = (unsigned char)min(__float2int_rn(I.y * sc), 255);
@@ -99,29 +118,31 @@ k_quantise(const float4 *__restrict__ inten, const unsigned int *__restrict__ vm
     }
 }
 
-// ---- N = 1024 fast path (sfd_warp1024.cuh): persistent kernels, one warp pair per line --------------
+// ---- axis length 1024 (sfd_warp1024.cuh): persistent kernels, one warp pair per line ---------------
 // One CTA per SM.  Even warps run branch 0 (even bins), odd warps branch 1.
+// k_cols_1024: Ny = 1024 rows, nx columns (lines).  k_rows_1024: Nx = 1024 columns, ny rows (lines).
 template <typename TIn>
 __global__ void __launch_bounds__(sfdw::WY * 32, 1)
-k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
-            const float2 *__restrict__ twl, const __grid_constant__ CUtensorMap tmB,
-            unsigned int *vmax, double *mom, int V) {
+k_cols_1024(const TIn *holo, long long hstride, int nx, const float2 *__restrict__ tabY,
+            long long vstride, const float2 *__restrict__ twl,
+            const __grid_constant__ CUtensorMap tmB, unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
     sfdw::SmemY<TIn> &sm = *reinterpret_cast<sfdw::SmemY<TIn> *>(smem4);
     sfdw::pdl_launch_dependents();
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
+    const int groups = nx / sfdw::YC;
     {   // pull the first slab of this CTA towards L2 while the prologue runs (a prefetch reads nothing:
         // it may precede griddepcontrol.wait)
-        constexpr int groups = sfdw::N / sfdw::YC, IPS = sfdw::TileElem<TIn>::IPS;
+        constexpr int IPS = sfdw::TileElem<TIn>::IPS;
         const int i0 = (int)((long long)V * groups * blockIdx.x / gridDim.x);
         const TIn *p0 = holo + (i0 % groups) / IPS * (sfdw::YC * IPS);
 #pragma unroll
         for (int i = 0; i < 4; ++i)
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(p0 + (size_t)(threadIdx.x + 256 * i) * sfdw::N));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(p0 + (size_t)(threadIdx.x + 256 * i) * hstride));
     }
-    // tables of this CTA's view(s) -> tensor memory (the barriers inside also publish the mbarriers)
-    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabY, V * (sfdw::N / sfdw::YC), sfdw::N / sfdw::YC);
+    // tables of this CTA's view(s) -> tensor memory
+    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabY, vstride, V * groups, groups);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     // everything above touches plan constants only; the hologram, B, vmax and mom belong to the
     // kernels before this one in the stream
@@ -130,12 +151,12 @@ k_cols_1024(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
         for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
     if (mom != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
-    sfdw::pass_y_loop<TIn>(sm, holo, tq, tw, &tmB, V);
+    sfdw::pass_y_loop<TIn>(sm, holo, hstride, nx, tq, tw, &tmB, V);
     sfdw::tm_finish(tbase);
 }
 
 __global__ void __launch_bounds__(sfdw::WX * 32, 1)
-k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
+k_rows_1024(const float2 *B, int ny, const float2 *__restrict__ tabX, long long vstride,
             const float2 *__restrict__ twl, float2 *__restrict__ field, float *__restrict__ inten,
             unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
@@ -147,40 +168,41 @@ k_rows_1024(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
     }
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
-    constexpr int gpv = (sfdw::N + sfdw::XP - 1) / sfdw::XP;  // units per view, as in pass_x_loop
-    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabX, V * gpv, gpv);
+    const int gpv = ny / sfdw::XP;  // units per view, as in pass_x_loop
+    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabX, vstride, V * gpv, gpv);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
-    sfdw::pass_x_loop(sm, B, tq, tw, field, inten, vmax, mom, V);
+    sfdw::pass_x_loop(sm, B, ny, tq, tw, field, inten, vmax, mom, V);
     sfdw::tm_finish(tbase);
 }
 
-// ---- N = 2048 (sfd_warp2048.cuh): four branches per line, a quad of warps per line ------------------
-// grid = V * cpv CTAs: CTA c works on view c / cpv.  tab: [V][4][5][1024].
+// ---- axis length 2048 (sfd_warp2048.cuh): four branches per line, a quad of warps per line ----------
+// grid = V * cpv CTAs: CTA c works on view c / cpv.  tab: [4][5][1024] per view.
 template <typename TIn>
 __global__ void __launch_bounds__(256, 1)
-k_cols_2048(const TIn *__restrict__ holo, const float2 *__restrict__ tabY,
-            const float2 *__restrict__ twl, const __grid_constant__ CUtensorMap tmB,
-            unsigned int *vmax, double *mom, int V, int cpv) {
+k_cols_2048(const TIn *holo, long long hstride, int nx, const float2 *__restrict__ tabY,
+            long long vstride, const float2 *__restrict__ twl,
+            const __grid_constant__ CUtensorMap tmB, unsigned int *vmax, double *mom, int V,
+            int cpv) {
     extern __shared__ float4 smem4[];
     sfdq::SmemYQ<TIn> &sm = *reinterpret_cast<sfdq::SmemYQ<TIn> *>(smem4);
     sfdw::pdl_launch_dependents();
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
-    const sfdq::Range rg = sfdq::cta_range(cpv, sfdq::QUY);
-    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabY, rg.view);
+    const sfdq::Range rg = sfdq::cta_range(cpv, nx / 4);
+    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabY, vstride, rg.view);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     sfdw::pdl_wait();
     if (vmax != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
     if (mom != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
-    sfdq::pass_y_quad<TIn>(sm, holo, tq, tw, &tmB, rg);
+    sfdq::pass_y_quad<TIn>(sm, holo, hstride, tq, tw, &tmB, rg);
     sfdw::tm_finish(tbase);
 }
 
 __global__ void __launch_bounds__(256, 1)
-k_rows_2048(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
+k_rows_2048(const float2 *B, int ny, const float2 *__restrict__ tabX, long long vstride,
             const float2 *__restrict__ twl, float2 *__restrict__ field, float *__restrict__ inten,
             unsigned int *vmax, double *mom, int cpv) {
     extern __shared__ float4 smem4[];
@@ -193,129 +215,183 @@ k_rows_2048(const float2 *__restrict__ B, const float2 *__restrict__ tabX,
     }
     float2 tw[sfdw::TWN];
     sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
-    const sfdq::Range rg = sfdq::cta_range(cpv, sfdq::QUX);
-    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabX, rg.view);
+    const sfdq::Range rg = sfdq::cta_range(cpv, ny / 2);
+    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabX, vstride, rg.view);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
-    sfdq::pass_x_quad(sm, B, tq, tw, field, inten, vmax, mom, rg);
+    sfdq::pass_x_quad(sm, B, ny, tq, tw, field, inten, vmax, mom, rg);
     sfdw::tm_finish(tbase);
 }
 
-std::atomic<long long> g_launches{0};
-int g_sms = 0;
-
-cudaError_t launch_warp1024(sfd_plan *p, const void *holo, float2 *field, float *inten,
-                            unsigned char *u8, double *mom, cudaStream_t st) {
-    const sfd_dev &d = p->d;
-    const int V = d.V;
-    unsigned int *vmax = u8 ? d.vmax : nullptr;
-    if (u8) {
-        field = nullptr;
-        inten = d.inten_ws;
+// ---- pipe micro-benchmarks (sfd_measure_pipes) -------------------------------------------------------
+// fp32 FMA throughput: 8 independent chains per thread, 16 warps per SM
+__global__ void __launch_bounds__(512) k_peak_ffma(float *out, int iters, float a, float b) {
+    float x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = (float)(threadIdx.x + i);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) x[i] = fmaf(x[i], a, b);
     }
-    const bool timing = p->timing;
-    if (timing) cudaEventRecord(p->ev[0], st);
-    // one CTA per SM, but at least V CTAs: a CTA's contiguous range of items (rows) then touches at
-    // most two views (the kernels hold two table sets)
-    const int gy = V > g_sms ? V : g_sms;
-    const CUtensorMap &tmB = *reinterpret_cast<const CUtensorMap *>(p->tmapB);
-    // Programmatic dependent launch: a kernel may start on an SM as soon as the kernel before it in
-    // the stream has left that SM, runs its prologue (barriers, twiddles, tensor-memory tables) and
-    // waits (griddepcontrol.wait) for the whole predecessor before touching its data.
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(gy);
-    cfg.blockDim = dim3(sfdw::WY * 32);
-    cfg.stream = st;
-    cfg.attrs = at;
-    cfg.numAttrs = 1;
-    cudaError_t le;
-    if (d.in_dtype == 0) {
-        cfg.dynamicSmemBytes = sizeof(sfdw::SmemY<unsigned char>);
-        le = cudaLaunchKernelEx(&cfg, k_cols_1024<unsigned char>, (const unsigned char *)holo,
-                                (const float2 *)d.w_tabY, (const float2 *)d.w_twl, tmB, vmax, mom, V);
-    } else {
-        cfg.dynamicSmemBytes = sizeof(sfdw::SmemY<float>);
-        le = cudaLaunchKernelEx(&cfg, k_cols_1024<float>, (const float *)holo,
-                                (const float2 *)d.w_tabY, (const float2 *)d.w_twl, tmB, vmax, mom, V);
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i];
+    if (s == 12345.678f) out[0] = s;  // never true: keeps the chains alive
+}
+// cycles of one radix-32 stage for a warp that has its sub-partition to itself (4 warps per SM);
+// TW selects stage B (twiddles folded in).  in: 32 x 32 complex values per warp slot.
+template <bool TW>
+__global__ void __launch_bounds__(128, 1)
+k_peak_dft32(const float2 *in, const float2 *__restrict__ twl, float2 *out, long long *cycles,
+             int reps) {
+    const int lane = threadIdx.x & 31;
+    float2 v[32], tw[sfdw::TWN];
+    sfdw::load_twiddles(tw, lane, twl);
+#pragma unroll
+    for (int r = 0; r < 32; ++r) v[r] = in[threadIdx.x + 128 * r];
+    __syncthreads();
+    const long long t0 = clock64();
+    for (int i = 0; i < reps; ++i) {
+        if (TW)
+            sfdb::dft32_tw(v, tw);
+        else
+            sfdb::dft32(v);
+#pragma unroll
+        for (int r = 0; r < 32; ++r) {  // keep the magnitudes bounded: exact scaling, 2 ops per value
+            v[r].x *= 0.125f;
+            v[r].y *= 0.125f;
+        }
     }
-    if (le != cudaSuccess) return le;
-    if (timing) cudaEventRecord(p->ev[1], st);
-    cfg.blockDim = dim3(sfdw::WX * 32);
-    cfg.dynamicSmemBytes = sizeof(sfdw::SmemX);
-    le = cudaLaunchKernelEx(&cfg, k_rows_1024, (const float2 *)d.B, (const float2 *)d.w_tabX,
-                            (const float2 *)d.w_twl, field, inten, vmax, mom, V);
-    if (le != cudaSuccess) return le;
-    if (timing) cudaEventRecord(p->ev[2], st);
-    int n = 2;
-    if (u8) {
-        const int quads = sfdw::N * sfdw::N / 4;
-        dim3 gq((quads + 256 * 4 - 1) / (256 * 4), V);
-        k_quantise<<<gq, 256, 0, st>>>((const float4 *)d.inten_ws, d.vmax, (uchar4 *)u8, quads);
-        if (timing) cudaEventRecord(p->ev[3], st);
-        ++n;
-    }
-    p->ev_valid = timing;
-    p->ev_quant = timing && u8 != nullptr;
-    g_launches.fetch_add(n, std::memory_order_relaxed);
-    return cudaGetLastError();
+    const long long t1 = clock64();
+#pragma unroll
+    for (int r = 0; r < 32; ++r) out[(size_t)blockIdx.x * 4096 + threadIdx.x + 128 * r] = v[r];
+    if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
 }
 
-cudaError_t launch_warp2048(sfd_plan *p, const void *holo, float2 *field, float *inten,
-                            unsigned char *u8, double *mom, cudaStream_t st) {
-    const sfd_dev &d = p->d;
-    const int V = d.V;
-    unsigned int *vmax = u8 ? d.vmax : nullptr;
-    if (u8) {
-        field = nullptr;
-        inten = d.inten_ws;
-    }
-    const bool timing = p->timing;
-    if (timing) cudaEventRecord(p->ev[0], st);
-    const int cpv = g_sms / V > 0 ? g_sms / V : 1;  // CTAs per view: a CTA works inside one view
-    const CUtensorMap &tmB = *reinterpret_cast<const CUtensorMap *>(p->tmapB);
+std::atomic<long long> g_launches{0};
+
+// Launch configuration shared by every kernel of the library: programmatic stream serialization,
+// i.e. a kernel may start on an SM as soon as the kernel before it in the stream has left that SM,
+// runs its prologue (barriers, twiddles, tensor-memory tables: plan constants only) and waits
+// (griddepcontrol.wait) for the whole predecessor before touching its data.
+struct Launch {
     cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(V * cpv);
-    cfg.blockDim = dim3(256);
-    cfg.stream = st;
-    cfg.attrs = at;
-    cfg.numAttrs = 1;
-    cudaError_t le;
-    if (d.in_dtype == 0) {
-        cfg.dynamicSmemBytes = sizeof(sfdq::SmemYQ<unsigned char>);
-        le = cudaLaunchKernelEx(&cfg, k_cols_2048<unsigned char>, (const unsigned char *)holo,
-                                (const float2 *)d.w_tabY, (const float2 *)d.w_twl, tmB, vmax, mom, V,
-                                cpv);
-    } else {
-        cfg.dynamicSmemBytes = sizeof(sfdq::SmemYQ<float>);
-        le = cudaLaunchKernelEx(&cfg, k_cols_2048<float>, (const float *)holo,
-                                (const float2 *)d.w_tabY, (const float2 *)d.w_twl, tmB, vmax, mom, V,
-                                cpv);
+    cudaLaunchConfig_t cfg;
+    Launch(dim3 grid, dim3 block, size_t smem, cudaStream_t st) : cfg{} {
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.gridDim = grid;
+        cfg.blockDim = block;
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
     }
-    if (le != cudaSuccess) return le;
-    if (timing) cudaEventRecord(p->ev[1], st);
-    cfg.dynamicSmemBytes = sizeof(sfdq::SmemXQ);
-    le = cudaLaunchKernelEx(&cfg, k_rows_2048, (const float2 *)d.B, (const float2 *)d.w_tabX,
-                            (const float2 *)d.w_twl, field, inten, vmax, mom, cpv);
-    if (le != cudaSuccess) return le;
-    if (timing) cudaEventRecord(p->ev[2], st);
-    int n = 2;
-    if (u8) {
-        const int quads = sfdq::NL * sfdq::NL / 4;
-        dim3 gq((quads + 256 * 4 - 1) / (256 * 4), V);
-        k_quantise<<<gq, 256, 0, st>>>((const float4 *)d.inten_ws, d.vmax, (uchar4 *)u8, quads);
-        if (timing) cudaEventRecord(p->ev[3], st);
-        ++n;
+};
+
+// the slab loads of the warp kernels read 8 bytes of a hologram row at once
+bool slab_aligned(const sfd_plan *p, const void *holo) {
+    const size_t es = p->d.in_dtype == 0 ? 1 : 4;
+    return (reinterpret_cast<size_t>(holo) & 7) == 0 && ((size_t)p->d.in_stride * es & 7) == 0;
+}
+
+AxisTabs axis_y(const sfd_dev &d) { return AxisTabs{d.tabs, d.vstride, d.off_pre_y, d.off_Hy, d.off_post_y}; }
+AxisTabs axis_x(const sfd_dev &d) { return AxisTabs{d.tabs, d.vstride, d.off_pre_x, d.off_Hx, d.off_post_x}; }
+
+// ---- pass y ---------------------------------------------------------------------------------------
+template <int LOG2M>
+cudaError_t launch_y_generic(const sfd_dev &d, const void *holo, unsigned int *vmax, double *mom,
+                             cudaStream_t st) {
+    using TL = Tile<LOG2M>;
+    Launch l(dim3(d.Nx / TL::C, d.V), dim3(TL::THREADS_Y), TL::SMEM_Y, st);
+    if (d.in_dtype == 0)
+        return cudaLaunchKernelEx(&l.cfg, k_pass_y<LOG2M, unsigned char>, (const unsigned char *)holo,
+                                  d.in_stride, d.Nx, axis_y(d), (const float2 *)d.tw_y, d.B, vmax, mom);
+    return cudaLaunchKernelEx(&l.cfg, k_pass_y<LOG2M, float>, (const float *)holo, d.in_stride, d.Nx,
+                              axis_y(d), (const float2 *)d.tw_y, d.B, vmax, mom);
+}
+
+cudaError_t launch_y(sfd_plan *p, const void *holo, unsigned int *vmax, double *mom,
+                     cudaStream_t st) {
+    const sfd_dev &d = p->d;
+    const CUtensorMap &tmB = *reinterpret_cast<const CUtensorMap *>(p->tmapB);
+    const float2 *tabY = d.tabs + d.off_tabY;
+    if (sfd_uses_warp_y(p, holo) && d.Ny == sfdw::N) {
+        // one CTA per SM, but at least V CTAs: a CTA's contiguous range of items then touches at most
+        // two views (the kernel holds two table sets)
+        const int grid = d.V > d.sms ? d.V : d.sms;
+        if (d.in_dtype == 0) {
+            Launch l(dim3(grid), dim3(sfdw::WY * 32), sizeof(sfdw::SmemY<unsigned char>), st);
+            return cudaLaunchKernelEx(&l.cfg, k_cols_1024<unsigned char>, (const unsigned char *)holo,
+                                      d.in_stride, d.Nx, tabY, d.vstride, (const float2 *)d.w_twl, tmB,
+                                      vmax, mom, d.V);
+        }
+        Launch l(dim3(grid), dim3(sfdw::WY * 32), sizeof(sfdw::SmemY<float>), st);
+        return cudaLaunchKernelEx(&l.cfg, k_cols_1024<float>, (const float *)holo, d.in_stride, d.Nx,
+                                  tabY, d.vstride, (const float2 *)d.w_twl, tmB, vmax, mom, d.V);
     }
-    p->ev_valid = timing;
-    p->ev_quant = timing && u8 != nullptr;
-    g_launches.fetch_add(n, std::memory_order_relaxed);
-    return cudaGetLastError();
+    if (sfd_uses_warp_y(p, holo) && d.Ny == sfdq::NL) {
+        const int cpv = d.sms / d.V > 0 ? d.sms / d.V : 1;  // CTAs per view: a CTA works inside one view
+        if (d.in_dtype == 0) {
+            Launch l(dim3(d.V * cpv), dim3(256), sizeof(sfdq::SmemYQ<unsigned char>), st);
+            return cudaLaunchKernelEx(&l.cfg, k_cols_2048<unsigned char>, (const unsigned char *)holo,
+                                      d.in_stride, d.Nx, tabY, d.vstride, (const float2 *)d.w_twl, tmB,
+                                      vmax, mom, d.V, cpv);
+        }
+        Launch l(dim3(d.V * cpv), dim3(256), sizeof(sfdq::SmemYQ<float>), st);
+        return cudaLaunchKernelEx(&l.cfg, k_cols_2048<float>, (const float *)holo, d.in_stride, d.Nx,
+                                  tabY, d.vstride, (const float2 *)d.w_twl, tmB, vmax, mom, d.V, cpv);
+    }
+    switch (d.log2My) {
+        case 7: return launch_y_generic<7>(d, holo, vmax, mom, st);
+        case 8: return launch_y_generic<8>(d, holo, vmax, mom, st);
+        case 9: return launch_y_generic<9>(d, holo, vmax, mom, st);
+        case 10: return launch_y_generic<10>(d, holo, vmax, mom, st);
+        case 11: return launch_y_generic<11>(d, holo, vmax, mom, st);
+        case 12: return launch_y_generic<12>(d, holo, vmax, mom, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+// ---- pass x ---------------------------------------------------------------------------------------
+template <int LOG2M>
+cudaError_t launch_x_generic(const sfd_dev &d, float2 *field, float *inten, unsigned int *vmax,
+                             double *mom, cudaStream_t st) {
+    using TL = Tile<LOG2M>;
+    Launch l(dim3(d.Ny / TL::RPC, d.V), dim3(TL::THREADS_X), TL::SMEM_X, st);
+    if (mom == nullptr)
+        return cudaLaunchKernelEx(&l.cfg, k_pass_x<LOG2M, false>, (const float2 *)d.B, d.Ny, axis_x(d),
+                                  (const float2 *)d.tw_x, field, inten, vmax, mom);
+    return cudaLaunchKernelEx(&l.cfg, k_pass_x<LOG2M, true>, (const float2 *)d.B, d.Ny, axis_x(d),
+                              (const float2 *)d.tw_x, field, inten, vmax, mom);
+}
+
+cudaError_t launch_x(sfd_plan *p, float2 *field, float *inten, unsigned int *vmax, double *mom,
+                     cudaStream_t st) {
+    const sfd_dev &d = p->d;
+    const float2 *tabX = d.tabs + d.off_tabX;
+    if (sfd_uses_warp_x(p) && d.Nx == sfdw::N) {
+        Launch l(dim3(d.V > d.sms ? d.V : d.sms), dim3(sfdw::WX * 32), sizeof(sfdw::SmemX), st);
+        return cudaLaunchKernelEx(&l.cfg, k_rows_1024, (const float2 *)d.B, d.Ny, tabX, d.vstride,
+                                  (const float2 *)d.w_twl, field, inten, vmax, mom, d.V);
+    }
+    if (sfd_uses_warp_x(p) && d.Nx == sfdq::NL) {
+        const int cpv = d.sms / d.V > 0 ? d.sms / d.V : 1;
+        Launch l(dim3(d.V * cpv), dim3(256), sizeof(sfdq::SmemXQ), st);
+        return cudaLaunchKernelEx(&l.cfg, k_rows_2048, (const float2 *)d.B, d.Ny, tabX, d.vstride,
+                                  (const float2 *)d.w_twl, field, inten, vmax, mom, cpv);
+    }
+    switch (d.log2Mx) {
+        case 7: return launch_x_generic<7>(d, field, inten, vmax, mom, st);
+        case 8: return launch_x_generic<8>(d, field, inten, vmax, mom, st);
+        case 9: return launch_x_generic<9>(d, field, inten, vmax, mom, st);
+        case 10: return launch_x_generic<10>(d, field, inten, vmax, mom, st);
+        case 11: return launch_x_generic<11>(d, field, inten, vmax, mom, st);
+        case 12: return launch_x_generic<12>(d, field, inten, vmax, mom, st);
+    }
+    return cudaErrorInvalidValue;
 }
 
 template <int LOG2M, typename TIn> cudaError_t set_attr() {
@@ -330,78 +406,23 @@ template <int LOG2M, typename TIn> cudaError_t set_attr() {
                                 (int)Tile<LOG2M>::SMEM_X);
 }
 
-template <int LOG2M>
-cudaError_t launch_t(sfd_plan *p, const void *holo, float2 *field, float *inten,
-                     unsigned char *u8, double *mom, cudaStream_t st) {
-    using TL = Tile<LOG2M>;
-    const sfd_dev &d = p->d;
-    const int N = d.N, V = d.V;
-    unsigned int *vmax = u8 ? d.vmax : nullptr;
-    if (u8) {
-        field = nullptr;
-        inten = d.inten_ws;
-    }
-    const bool timing = p->timing;
-    if (timing) cudaEventRecord(p->ev[0], st);
-    // programmatic dependent launch (as for the warp kernels): the launch latency of a kernel
-    // overlaps the tail of the kernel before it; the small sizes are launch-bound
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(N / TL::C, V);
-    cfg.blockDim = dim3(TL::THREADS_Y);
-    cfg.dynamicSmemBytes = TL::SMEM_Y;
-    cfg.stream = st;
-    cfg.attrs = at;
-    cfg.numAttrs = 1;
-    cudaError_t le;
-    if (d.in_dtype == 0)
-        le = cudaLaunchKernelEx(&cfg, k_pass_y<LOG2M, unsigned char>, (const unsigned char *)holo,
-                                (const float2 *)d.pre_y, (const float2 *)d.H, (const float2 *)d.post_y,
-                                (const float2 *)d.tw, d.B, vmax, mom);
-    else
-        le = cudaLaunchKernelEx(&cfg, k_pass_y<LOG2M, float>, (const float *)holo,
-                                (const float2 *)d.pre_y, (const float2 *)d.H, (const float2 *)d.post_y,
-                                (const float2 *)d.tw, d.B, vmax, mom);
-    if (le != cudaSuccess) return le;
-    if (timing) cudaEventRecord(p->ev[1], st);
-    cfg.gridDim = dim3(N / TL::RPC, V);
-    cfg.blockDim = dim3(TL::THREADS_X);
-    cfg.dynamicSmemBytes = TL::SMEM_X;
-    if (mom == nullptr)
-        le = cudaLaunchKernelEx(&cfg, k_pass_x<LOG2M, false>, (const float2 *)d.B, (const float2 *)d.pre_x,
-                                (const float2 *)d.Hx, (const float2 *)d.post_x, (const float2 *)d.tw, field,
-                                inten, vmax, mom);
-    else
-        le = cudaLaunchKernelEx(&cfg, k_pass_x<LOG2M, true>, (const float2 *)d.B, (const float2 *)d.pre_x,
-                                (const float2 *)d.Hx, (const float2 *)d.post_x, (const float2 *)d.tw, field,
-                                inten, vmax, mom);
-    if (le != cudaSuccess) return le;
-    if (timing) cudaEventRecord(p->ev[2], st);
-    int n = 2;
-    if (u8) {
-        const int quads = N * N / 4;
-        dim3 gq((quads + 256 * 4 - 1) / (256 * 4), V);
-        k_quantise<<<gq, 256, 0, st>>>((const float4 *)d.inten_ws, d.vmax, (uchar4 *)u8, quads);
-        if (timing) cudaEventRecord(p->ev[3], st);
-        ++n;
-    }
-    p->ev_valid = timing;
-    p->ev_quant = timing && u8 != nullptr;
-    g_launches.fetch_add(n, std::memory_order_relaxed);
-    return cudaGetLastError();
-}
-
 }  // namespace
 
-// Tensor map of the intermediate B for the bulk stores of k_cols_1024: B as float [V * N][2 N],
-// box = 4 floats (two complex columns; N = 2048: 8 floats, four columns) x YBOX rows, no swizzle.  The encoder is a driver entry
-// point; it is fetched through the runtime so that the library does not link libcuda.
+bool sfd_uses_warp_y(const sfd_plan *p, const void *holo) {
+    return p->kernels != SFD_KERNELS_GENERIC && p->d.off_tabY >= 0 && p->d.Nx % 16 == 0 &&
+           (holo == nullptr || slab_aligned(p, holo));
+}
+bool sfd_uses_warp_x(const sfd_plan *p) {
+    return p->kernels != SFD_KERNELS_GENERIC && p->d.off_tabX >= 0 && p->d.Ny % 4 == 0;
+}
+
+// Tensor map of the intermediate B for the bulk stores of the warp pass y: B as float
+// [V * Ny][2 Nx], box = 4 floats (two complex columns; Ny = 2048: 8 floats, four columns) x YBOX rows,
+// no swizzle.  The encoder is a driver entry point; it is fetched through the runtime so that the
+// library does not link libcuda.
 cudaError_t sfd_make_tensormaps(sfd_plan *p) {
     static_assert(sizeof(CUtensorMap) <= sizeof(p->tmapB), "tensor map storage");
-    if ((p->d.N != sfdw::N && p->d.N != sfdq::NL) || p->d.w_twl == nullptr) return cudaSuccess;
-    const cuuint64_t n = (cuuint64_t)p->d.N;
+    if (p->d.off_tabY < 0) return cudaSuccess;
     typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
                                   const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
                                   const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -411,9 +432,9 @@ cudaError_t sfd_make_tensormaps(sfd_plan *p) {
     cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
     if (e != cudaSuccess) return e;
     if (fn == nullptr || qr != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
-    const cuuint64_t dims[2] = {2 * n, (cuuint64_t)p->d.V * n};
-    const cuuint64_t strides[1] = {2 * n * sizeof(float)};
-    const cuuint32_t box[2] = {p->d.N == sfdq::NL ? (cuuint32_t)sfdq::YBOXW : 4u, sfdw::YBOX};
+    const cuuint64_t dims[2] = {2 * (cuuint64_t)p->d.Nx, (cuuint64_t)p->d.V * p->d.Ny};
+    const cuuint64_t strides[1] = {2 * (cuuint64_t)p->d.Nx * sizeof(float)};
+    const cuuint32_t box[2] = {p->d.Ny == sfdq::NL ? (cuuint32_t)sfdq::YBOXW : 4u, sfdw::YBOX};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = ((encode_fn)fn)(
         reinterpret_cast<CUtensorMap *>(p->tmapB), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, p->d.B, dims,
@@ -425,48 +446,144 @@ cudaError_t sfd_make_tensormaps(sfd_plan *p) {
 void sfd_count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 long long sfd_launch_count_impl() { return g_launches.load(std::memory_order_relaxed); }
 
-cudaError_t sfd_kernels_init() {
+// cudaFuncSetAttribute acts on the current device: called once per device (sfd_plan.cpp)
+cudaError_t sfd_kernels_init(int device, int *sms) {
     cudaError_t e;
 #define SFD_ATTR(L)                                                   \
     if ((e = set_attr<L, unsigned char>()) != cudaSuccess) return e;  \
     if ((e = set_attr<L, float>()) != cudaSuccess) return e;
     SFD_ATTR(7) SFD_ATTR(8) SFD_ATTR(9) SFD_ATTR(10) SFD_ATTR(11) SFD_ATTR(12)
 #undef SFD_ATTR
-    if ((e = cudaFuncSetAttribute(k_cols_1024<unsigned char>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)sizeof(sfdw::SmemY<unsigned char>))) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_cols_1024<float>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)sizeof(sfdw::SmemY<float>))) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_rows_1024, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)sizeof(sfdw::SmemX))) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_cols_2048<unsigned char>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)sizeof(sfdq::SmemYQ<unsigned char>))) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_cols_2048<float>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)sizeof(sfdq::SmemYQ<float>))) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(k_rows_2048, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)sizeof(sfdq::SmemXQ))) != cudaSuccess) return e;
-    int dev = 0;
-    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
-    if ((e = cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
-    return cudaSuccess;
+#define SFD_SMEM(kernel, bytes)                                                               \
+    if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,        \
+                                  (int)(bytes))) != cudaSuccess)                              \
+        return e;
+    SFD_SMEM(k_cols_1024<unsigned char>, sizeof(sfdw::SmemY<unsigned char>))
+    SFD_SMEM(k_cols_1024<float>, sizeof(sfdw::SmemY<float>))
+    SFD_SMEM(k_rows_1024, sizeof(sfdw::SmemX))
+    SFD_SMEM(k_cols_2048<unsigned char>, sizeof(sfdq::SmemYQ<unsigned char>))
+    SFD_SMEM(k_cols_2048<float>, sizeof(sfdq::SmemYQ<float>))
+    SFD_SMEM(k_rows_2048, sizeof(sfdq::SmemXQ))
+#undef SFD_SMEM
+    return cudaDeviceGetAttribute(sms, cudaDevAttrMultiProcessorCount, device);
 }
 
 cudaError_t sfd_launch(sfd_plan *p, const void *holo, float2 *field, float *inten,
                        unsigned char *u8, cudaStream_t st, double *mom) {
-    // N = 1024: warp-pair-per-line kernels (their slab loads read 8 bytes of a hologram row at once:
-    // the hologram must be aligned accordingly)
-    if (p->d.N == sfdw::N && p->kernels != SFD_KERNELS_GENERIC && p->d.w_twl != nullptr &&
-        (reinterpret_cast<size_t>(holo) & (p->d.in_dtype == 0 ? 7 : 15)) == 0)
-        return launch_warp1024(p, holo, field, inten, u8, mom, st);
-    if (p->d.N == sfdq::NL && p->kernels != SFD_KERNELS_GENERIC && p->d.w_twl != nullptr &&
-        (reinterpret_cast<size_t>(holo) & (p->d.in_dtype == 0 ? 7 : 15)) == 0)
-        return launch_warp2048(p, holo, field, inten, u8, mom, st);
-    switch (p->d.log2M) {
-        case 7: return launch_t<7>(p, holo, field, inten, u8, mom, st);
-        case 8: return launch_t<8>(p, holo, field, inten, u8, mom, st);
-        case 9: return launch_t<9>(p, holo, field, inten, u8, mom, st);
-        case 10: return launch_t<10>(p, holo, field, inten, u8, mom, st);
-        case 11: return launch_t<11>(p, holo, field, inten, u8, mom, st);
-        case 12: return launch_t<12>(p, holo, field, inten, u8, mom, st);
+    const sfd_dev &d = p->d;
+    unsigned int *vmax = u8 ? d.vmax : nullptr;
+    if (u8) {
+        field = nullptr;
+        inten = d.inten_ws;
     }
-    return cudaErrorInvalidValue;
+    const bool timing = p->timing;
+    cudaError_t e;
+    if (timing) cudaEventRecord(p->ev[0], st);
+    if ((e = launch_y(p, holo, vmax, mom, st)) != cudaSuccess) return e;
+    if (timing) cudaEventRecord(p->ev[1], st);
+    if ((e = launch_x(p, field, inten, vmax, mom, st)) != cudaSuccess) return e;
+    if (timing) cudaEventRecord(p->ev[2], st);
+    int n = 2;
+    if (u8) {
+        const int quads = d.Nx * d.Ny / 4;
+        Launch l(dim3((quads + 256 * 4 - 1) / (256 * 4), d.V), dim3(256), 0, st);
+        if ((e = cudaLaunchKernelEx(&l.cfg, k_quantise, (const float4 *)d.inten_ws,
+                                    (const unsigned int *)d.vmax, (uchar4 *)u8, quads)) != cudaSuccess)
+            return e;
+        if (timing) cudaEventRecord(p->ev[3], st);
+        ++n;
+    }
+    p->ev_valid = timing;
+    p->ev_quant = timing && u8 != nullptr;
+    g_launches.fetch_add(n, std::memory_order_relaxed);
+    return cudaGetLastError();
+}
+
+// ---- sfd_measure_pipes ------------------------------------------------------------------------------
+// out[0] plain fp32 FMA throughput of the whole GPU (TFLOP/s, 2 flop per FMA), out[1] / out[2] cycles
+// of one stage-A / stage-B radix-32 butterfly (sfd_dft32.cuh) for a warp alone on its sub-partition,
+// out[3] SM clock during the measurement (GHz, from clock64 against CUDA events).
+cudaError_t sfd_measure_pipes_impl(double out[4]) {
+    int dev = 0, sms = 0;
+    cudaError_t e;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    float *dummy = nullptr;
+    float2 *in = nullptr, *res = nullptr, *twl = nullptr;
+    long long *cyc = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    std::vector<float2> hin(4096), htw(32 * 32);
+    for (int i = 0; i < 4096; ++i) hin[i] = make_float2(0.001f * (float)(i % 97), -0.002f * (float)(i % 31));
+    for (int i = 0; i < 1024; ++i) htw[i] = make_float2(cosf(0.001f * (float)i), -sinf(0.001f * (float)i));
+    std::vector<long long> hc(sms);
+    auto cleanup = [&]() {
+        cudaFree(dummy); cudaFree(in); cudaFree(res); cudaFree(twl); cudaFree(cyc);
+        if (e0) cudaEventDestroy(e0);
+        if (e1) cudaEventDestroy(e1);
+    };
+#define SFD_TRY(call) if ((e = (call)) != cudaSuccess) { cleanup(); return e; }
+    SFD_TRY(cudaMalloc((void **)&dummy, 256));
+    SFD_TRY(cudaMalloc((void **)&in, 4096 * sizeof(float2)));
+    SFD_TRY(cudaMalloc((void **)&res, (size_t)sms * 4096 * sizeof(float2)));
+    SFD_TRY(cudaMalloc((void **)&twl, 1024 * sizeof(float2)));
+    SFD_TRY(cudaMalloc((void **)&cyc, sms * sizeof(long long)));
+    SFD_TRY(cudaMemcpy(in, hin.data(), 4096 * sizeof(float2), cudaMemcpyHostToDevice));
+    SFD_TRY(cudaMemcpy(twl, htw.data(), 1024 * sizeof(float2), cudaMemcpyHostToDevice));
+    SFD_TRY(cudaEventCreate(&e0));
+    SFD_TRY(cudaEventCreate(&e1));
+    const int iters = 4096;
+    float ms = 0.f;
+    k_peak_ffma<<<sms * 2, 512>>>(dummy, 64, 1.0001f, 0.5f);  // warm-up
+    SFD_TRY(cudaEventRecord(e0));
+    k_peak_ffma<<<sms * 2, 512>>>(dummy, iters, 1.0001f, 0.5f);
+    SFD_TRY(cudaEventRecord(e1));
+    SFD_TRY(cudaEventSynchronize(e1));
+    SFD_TRY(cudaEventElapsedTime(&ms, e0, e1));
+    out[0] = 2.0 * 64.0 * iters * 512.0 * 2.0 * sms / (ms * 1e-3) / 1e12;
+    const int reps = 2000;
+    for (int tw = 0; tw < 2; ++tw) {
+        for (int pass = 0; pass < 2; ++pass) {  // first pass warms the instruction cache
+            SFD_TRY(cudaEventRecord(e0));
+            if (tw)
+                k_peak_dft32<true><<<sms, 128>>>(in, twl, res, cyc, reps);
+            else
+                k_peak_dft32<false><<<sms, 128>>>(in, twl, res, cyc, reps);
+            SFD_TRY(cudaEventRecord(e1));
+            SFD_TRY(cudaEventSynchronize(e1));
+        }
+        SFD_TRY(cudaEventElapsedTime(&ms, e0, e1));
+        SFD_TRY(cudaMemcpy(hc.data(), cyc, sms * sizeof(long long), cudaMemcpyDeviceToHost));
+        double mean = 0;
+        for (int i = 0; i < sms; ++i) mean += (double)hc[i];
+        mean /= sms;
+        out[1 + tw] = mean / reps - 64.0;  // minus the 64 scaling multiplies of the loop body
+        out[3] = mean / (ms * 1e-3) / 1e9;
+    }
+#undef SFD_TRY
+    cleanup();
+    sfd_count_launch(6);
+    return cudaSuccess;
+}
+
+// host-side step of the butterflies (CPU tests): in / out = 32 interleaved (re, im) pairs; the
+// stored-sign convention of sfd_dft32.cuh is undone here so that out is the plain DFT
+void sfd_host_dft32_impl(const float *in, float *out, int lane, int twiddled) {
+    float2 v[32], t[sfdb::NTW];
+    for (int r = 0; r < 32; ++r) v[r] = make_float2(in[2 * r], in[2 * r + 1]);
+    if (twiddled) {
+        for (int n = 2; n <= 32; n *= 2)
+            for (int k = 0; k < n / 2; ++k) {
+                const long double ph = -6.283185307179586476925286766559005768L * (lane + 32 * k) /
+                                       (32.0L * n);
+                t[n / 2 - 1 + k] = make_float2((float)cosl(ph), (float)sinl(ph));
+            }
+        sfdb::dft32_tw(v, t);
+    } else {
+        sfdb::dft32(v);
+    }
+    for (int r = 0; r < 32; ++r) {
+        const float sg = (float)sfdb::out_sign(r);
+        out[2 * r] = sg * v[r].x;
+        out[2 * r + 1] = sg * v[r].y;
+    }
 }

@@ -1,16 +1,17 @@
 // sfd_plan.cpp — host side of libsfd: argument checking, the float64 table builder, plan life
-// cycle, execute entry points and the pinned double-buffered real-time stream.
+// cycle, execute entry points, live view updates and the pinned double-buffered real-time stream.
 //
 // Tables (Eq.(2)-(4), L58-65, with the readings of DESIGN.md §3): every phase is formed in
 // cycles in extended precision, reduced modulo 1, summed and only then turned into a complex
 // number, so the float32 values that reach the GPU carry one rounding each.
 #include <cuda_runtime.h>
 
-#include <atomic>
+#include <chrono>
 #include <cmath>
 #include <complex>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -38,6 +39,33 @@ int cuda_fail(cudaError_t e, const char *where) {
         if (e_ != cudaSuccess) return cuda_fail(e_, #call);     \
     } while (0)
 
+// Makes the plan's device current for the duration of a call and restores the caller's device.
+class DeviceGuard {
+public:
+    explicit DeviceGuard(int want) {
+        if (cudaGetDevice(&prev_) != cudaSuccess) {
+            prev_ = -1;
+            cudaGetLastError();
+        }
+        if (prev_ != want) {
+            err_ = cudaSetDevice(want);
+            switched_ = err_ == cudaSuccess;
+        }
+    }
+    ~DeviceGuard() {
+        if (switched_ && prev_ >= 0) cudaSetDevice(prev_);
+    }
+    cudaError_t error() const { return err_; }
+
+private:
+    int prev_ = -1;
+    bool switched_ = false;
+    cudaError_t err_ = cudaSuccess;
+};
+#define SFD_ON_DEVICE(p)                                                         \
+    DeviceGuard guard_((p)->device);                                             \
+    if (guard_.error() != cudaSuccess) return cuda_fail(guard_.error(), "cudaSetDevice")
+
 const ld TWO_PI = 6.283185307179586476925286766559005768L;
 
 inline ld frac1(ld c) { return c - rintl(c); }  // cycles -> (-1/2, 1/2]
@@ -46,8 +74,15 @@ inline cd cis_cycles(ld c) {
     return cd((double)cosl(TWO_PI * c), (double)sinl(TWO_PI * c));
 }
 
-// In-place radix-2 FFT, double, forward sign; twiddles evaluated directly (no recurrence).
-void fft_host(std::vector<cd> &a) {
+// exp(-2 pi i k / n), k < n/2, evaluated directly (no recurrence)
+std::vector<cd> fft_twiddles(size_t n) {
+    std::vector<cd> w(n / 2);
+    for (size_t k = 0; k < n / 2; ++k) w[k] = cis_cycles(-(ld)k / (ld)n);
+    return w;
+}
+
+// In-place radix-2 FFT, double, forward sign; w = fft_twiddles(a.size()).
+void fft_host(std::vector<cd> &a, const std::vector<cd> &w) {
     const size_t n = a.size();
     for (size_t i = 1, j = 0; i < n; ++i) {
         size_t bit = n >> 1;
@@ -55,8 +90,6 @@ void fft_host(std::vector<cd> &a) {
         j ^= bit;
         if (i < j) std::swap(a[i], a[j]);
     }
-    std::vector<cd> w(n / 2);
-    for (size_t k = 0; k < n / 2; ++k) w[k] = cis_cycles(-(ld)k / (ld)n);
     for (size_t len = 2; len <= n; len <<= 1) {
         const size_t step = n / len;
         for (size_t i = 0; i < n; i += len)
@@ -90,7 +123,9 @@ void axis_tables(int N, double lambda, double p1, double p2, double z, double of
 
 // Spectrum of the wrapped 1-D chirp kernel of Eq.(4): h[j] = exp(i pi S d^2), d = j (j <= N),
 // d = j - M (j > N), M = 2N; returns FFT_M(h)/M (the 1/M of the inverse FFT folded in, reading 8).
-void kernel_spectrum(int N, double lambda, double p1, double p2, double z, cd *H) {
+// w = fft_twiddles(M).
+void kernel_spectrum(int N, double lambda, double p1, double p2, double z, cd *H,
+                     const std::vector<cd> &w) {
     const int M = 2 * N;
     const ld S = (ld)p1 * (ld)p2 / ((ld)lambda * (ld)z);
     std::vector<cd> h(M);
@@ -98,7 +133,7 @@ void kernel_spectrum(int N, double lambda, double p1, double p2, double z, cd *H
         const ld d = j <= N ? (ld)j : (ld)(j - M);
         h[j] = cis_cycles(S * d * d / 2);
     }
-    fft_host(h);
+    fft_host(h, w);
     for (int k = 0; k < M; ++k) H[k] = h[k] / (double)M;
 }
 
@@ -118,6 +153,7 @@ int check_view(double lambda, double p1, double p2, double z, double Ox, double 
 }
 
 int log2_exact(int n) {
+    if (n < 1) return -1;
     int l = 0;
     while ((1 << l) < n) ++l;
     return (1 << l) == n ? l : -1;
@@ -130,11 +166,6 @@ void to_f32(const cd *src, float2 *dst, size_t n, cd scale = cd(1, 0)) {
     }
 }
 
-// Branch tables of the N = 1024 fast path (sfd_warp1024.cuh) for one axis: the 2N-point DFT split
-// by the parity of the frequency index, w = exp(-2 pi i / 2N):
-//   out[4][N] = pre | pre w^n | post | post w^-n   (each times its scale), formed in float64.
-// Fast-path tables of one pass and one view, layout [2][3][N]: for branch b the vectors
-// pre_b, H_b, conj(post_b) (sfd_warp1024.cuh); H = the float32 M-point kernel spectrum.
 // The butterflies of the warp FFT leave stage-A output k1 multiplied by (-1)^popcount(k1) (sign
 // tracking, sfd_dft32.cuh); k1 is the lane that multiplies table entry lane + 32 r after stage B, so
 // the sign goes into every table that follows an FFT (H_b and the post tables).
@@ -143,6 +174,10 @@ double lane_sign(int n) {
     return ((l ^ (l >> 1) ^ (l >> 2) ^ (l >> 3) ^ (l >> 4)) & 1) ? -1.0 : 1.0;
 }
 
+// Branch tables of an axis of length 1024 (sfd_warp1024.cuh): the 2N-point DFT split by the parity
+// of the frequency index, w = exp(-2 pi i / 2N); layout [2][3][N]: for branch b the vectors
+//   pre_b = pre w^(b n),  H_b[k] = H[2k + b],  conj(post_b) = conj(post w^(-b n))
+// (each times its scale; H = the float32 M-point kernel spectrum), formed in float64.
 void branch_tables(int N, const cd *pre, const cd *post, cd pre_scale, cd post_scale,
                    const float2 *H, float2 *out) {
     for (int n = 0; n < N; ++n) {
@@ -160,8 +195,8 @@ void branch_tables(int N, const cd *pre, const cd *post, cd pre_scale, cd post_s
     }
 }
 
-// Tables of the N = 2048 kernels (sfd_warp2048.cuh) for one axis: the 4096-point DFT split by the
-// frequency index modulo 4, w = exp(-2 pi i / 4096); layout [4][5][1024]: for branch b the vectors
+// Tables of an axis of length 2048 (sfd_warp2048.cuh): the 4096-point DFT split by the frequency
+// index modulo 4, w = exp(-2 pi i / 4096); layout [4][5][1024]: for branch b the vectors
 //   preA_b = pre[n] w^(b n), preB_b = pre[n+1024] w^(b (n+1024)), H_b[k] = H[4k+b],
 //   postA_b = post[n] w^(-b n), postB_b = post[n+1024] w^(-b (n+1024))            (n, k < 1024)
 void branch_tables4(const cd *pre, const cd *post, cd pre_scale, cd post_scale, const float2 *H,
@@ -183,32 +218,58 @@ void branch_tables4(const cd *pre, const cd *post, cd pre_scale, cd post_scale, 
         }
 }
 
-// float32 tables of one view, host staging layout: pre_y[N] post_y[N] pre_x[N] post_x[N] Hy[M]
-// Hx[M]; `fast` (or NULL) receives tabY[6N] tabX[6N] of the fast path.  The y axis uses
-// (p1y, p2y, O0y, Oy), the x axis (p1, p2, O0x, Ox): S_x and S_y may differ (Eq.(2)-(4), L58-67).
-void build_view_f32(const sfd_plan *p, int v, float2 *pre_y, float2 *post_y, float2 *pre_x,
-                    float2 *post_x, float2 *Hy, float2 *Hx, float2 *fast) {
-    const int N = p->d.N, M = p->d.M;
-    std::vector<cd> a(N), b(N), h(M);
-    const double in_scale = p->d.in_dtype == SFD_U8 ? 1.0 / 255.0 : 1.0;
+size_t fast_elems(int n) { return n == 1024 ? 6 * (size_t)1024 : n == 2048 ? 20 * (size_t)1024 : 0; }
+
+// All float32 tables of view v in the device layout of sfd_dev (one contiguous block of
+// d.vstride complex values).  The y axis uses (p1y, p2y, O0y, Oy), the x axis (p1, p2, O0x, Ox):
+// S_x and S_y may differ (Eq.(2)-(4), L58-67).
+void build_view_f32(const sfd_plan *p, int v, float2 *out) {
+    const sfd_dev &d = p->d;
+    const int nmax = d.Nx > d.Ny ? d.Nx : d.Ny;
+    std::vector<cd> a(nmax), b(nmax), h(2 * (size_t)nmax);
+    const double in_scale = d.in_dtype == SFD_U8 ? 1.0 / 255.0 : 1.0;
     const cd c0 = c0_factor(p->lambda, p->p1[v], p->p1y[v], p->z[v]);
-    kernel_spectrum(N, p->lambda, p->p1y[v], p->p2y[v], p->z[v], h.data());
-    to_f32(h.data(), Hy, M);
-    axis_tables(N, p->lambda, p->p1y[v], p->p2y[v], p->z[v], p->Oy[v], a.data(), b.data(), p->O0y[v]);
-    to_f32(a.data(), pre_y, N, cd(in_scale, 0));
-    to_f32(b.data(), post_y, N, c0);
-    if (fast && N == 1024) branch_tables(N, a.data(), b.data(), cd(in_scale, 0), c0, Hy, fast);
-    if (fast && N == 2048) branch_tables4(a.data(), b.data(), cd(in_scale, 0), c0, Hy, fast);
-    kernel_spectrum(N, p->lambda, p->p1[v], p->p2[v], p->z[v], h.data());
-    to_f32(h.data(), Hx, M);
-    axis_tables(N, p->lambda, p->p1[v], p->p2[v], p->z[v], p->Ox[v], a.data(), b.data(), p->O0x[v]);
-    to_f32(a.data(), pre_x, N);
-    to_f32(b.data(), post_x, N);
-    if (fast && N == 1024) branch_tables(N, a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, fast + 6 * (size_t)N);
-    if (fast && N == 2048) branch_tables4(a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, fast + 20 * 1024);
+    float2 *Hy = out + d.off_Hy, *Hx = out + d.off_Hx;
+    // y axis
+    kernel_spectrum(d.Ny, p->lambda, p->p1y[v], p->p2y[v], p->z[v], h.data(), p->wy);
+    to_f32(h.data(), Hy, d.My);
+    axis_tables(d.Ny, p->lambda, p->p1y[v], p->p2y[v], p->z[v], p->Oy[v], a.data(), b.data(),
+                p->O0y[v]);
+    to_f32(a.data(), out + d.off_pre_y, d.Ny, cd(in_scale, 0));
+    to_f32(b.data(), out + d.off_post_y, d.Ny, c0);
+    if (d.off_tabY >= 0 && d.Ny == 1024)
+        branch_tables(d.Ny, a.data(), b.data(), cd(in_scale, 0), c0, Hy, out + d.off_tabY);
+    if (d.off_tabY >= 0 && d.Ny == 2048)
+        branch_tables4(a.data(), b.data(), cd(in_scale, 0), c0, Hy, out + d.off_tabY);
+    // x axis
+    kernel_spectrum(d.Nx, p->lambda, p->p1[v], p->p2[v], p->z[v], h.data(), p->wx);
+    to_f32(h.data(), Hx, d.Mx);
+    axis_tables(d.Nx, p->lambda, p->p1[v], p->p2[v], p->z[v], p->Ox[v], a.data(), b.data(),
+                p->O0x[v]);
+    to_f32(a.data(), out + d.off_pre_x, d.Nx);
+    to_f32(b.data(), out + d.off_post_x, d.Nx);
+    if (d.off_tabX >= 0 && d.Nx == 1024)
+        branch_tables(d.Nx, a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, out + d.off_tabX);
+    if (d.off_tabX >= 0 && d.Nx == 2048)
+        branch_tables4(a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, out + d.off_tabX);
 }
 
-std::atomic<bool> g_init{false};
+// Per-device one-time set-up: cudaFuncSetAttribute applies to the device that is current, so a
+// process that makes plans on several GPUs needs it once on each.
+std::mutex g_init_mutex;
+int g_sms[64] = {};
+
+int device_init(int device, int *sms) {
+    std::lock_guard<std::mutex> lock(g_init_mutex);
+    if (device < 0 || device >= 64) return SFD_EUNSUPPORTED;
+    if (g_sms[device] == 0) {
+        int n = 0;
+        SFD_CUDA(sfd_kernels_init(device, &n));
+        g_sms[device] = n;
+    }
+    *sms = g_sms[device];
+    return SFD_OK;
+}
 
 }  // namespace
 
@@ -219,6 +280,18 @@ struct sfd_stream_state {
     unsigned char *d_out[2] = {nullptr, nullptr};
     cudaEvent_t e_in[2] = {nullptr, nullptr}, e_comp[2] = {nullptr, nullptr},
                 e_out[2] = {nullptr, nullptr}, e_t0 = nullptr, e_t1 = nullptr;
+};
+
+// ---- staging of live view updates ---------------------------------------------------------------
+// sfd_plan_update_view*_async builds a view's tables into one of SLOTS page-locked staging blocks
+// and enqueues ONE host-to-device copy on the caller's stream; the event recorded behind the copy
+// says when the block may be rewritten.
+struct sfd_update_ring {
+    static constexpr int SLOTS = 4;
+    float2 *slot[SLOTS] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t done[SLOTS] = {nullptr, nullptr, nullptr, nullptr};
+    bool used[SLOTS] = {false, false, false, false};
+    int next = 0;
 };
 
 namespace {
@@ -240,12 +313,15 @@ void stream_state_free(sfd_stream_state *s) {
     delete s;
 }
 
+size_t window_elems(const sfd_plan *p) { return (size_t)p->d.Nx * p->d.Ny; }
+
+// the plan's device is current (SFD_ON_DEVICE in the caller)
 int stream_state_make(sfd_plan *p) {
     if (p->ss) return SFD_OK;
     sfd_stream_state *s = new (std::nothrow) sfd_stream_state;
     if (!s) return SFD_ENOMEM;
     p->ss = s;  // freed by sfd_plan_destroy even when half built
-    const size_t nn = (size_t)p->d.N * p->d.N;
+    const size_t nn = window_elems(p);
     const size_t in_bytes = nn * (p->d.in_dtype == SFD_U8 ? 1 : 4);
     SFD_CUDA(cudaStreamCreateWithFlags(&s->s_in, cudaStreamNonBlocking));
     SFD_CUDA(cudaStreamCreateWithFlags(&s->s_comp, cudaStreamNonBlocking));
@@ -263,190 +339,52 @@ int stream_state_make(sfd_plan *p) {
     return SFD_OK;
 }
 
-int upload_view(sfd_plan *p, int v) {
-    const int N = p->d.N, M = p->d.M;
-    const bool fast = p->d.w_twl != nullptr;
-    // fast-path tables of one view and one pass: N = 1024: [2][3][1024], N = 2048: [4][5][1024]
-    const size_t fpass = !fast ? 0 : N == 1024 ? 6 * (size_t)1024 : 20 * (size_t)1024;
-    std::vector<float2> st((size_t)4 * N + 2 * M + 2 * fpass);
-    float2 *fs = fast ? st.data() + 4 * N + 2 * M : nullptr;
-    build_view_f32(p, v, st.data(), st.data() + N, st.data() + 2 * N, st.data() + 3 * N,
-                   st.data() + 4 * N, st.data() + 4 * N + M, fs);
-    if (fast) {
-        SFD_CUDA(cudaMemcpy(p->d.w_tabY + (size_t)v * fpass, fs, fpass * sizeof(float2),
-                            cudaMemcpyHostToDevice));
-        SFD_CUDA(cudaMemcpy(p->d.w_tabX + (size_t)v * fpass, fs + fpass, fpass * sizeof(float2),
-                            cudaMemcpyHostToDevice));
+void update_ring_free(sfd_update_ring *r) {
+    if (!r) return;
+    for (int i = 0; i < sfd_update_ring::SLOTS; ++i) {
+        if (r->slot[i]) cudaFreeHost(r->slot[i]);
+        if (r->done[i]) cudaEventDestroy(r->done[i]);
     }
-    const size_t nb = sizeof(float2) * N;
-    SFD_CUDA(cudaMemcpy(p->d.pre_y + (size_t)v * N, st.data(), nb, cudaMemcpyHostToDevice));
-    SFD_CUDA(cudaMemcpy(p->d.post_y + (size_t)v * N, st.data() + N, nb, cudaMemcpyHostToDevice));
-    SFD_CUDA(cudaMemcpy(p->d.pre_x + (size_t)v * N, st.data() + 2 * N, nb, cudaMemcpyHostToDevice));
-    SFD_CUDA(cudaMemcpy(p->d.post_x + (size_t)v * N, st.data() + 3 * N, nb, cudaMemcpyHostToDevice));
-    SFD_CUDA(cudaMemcpy(p->d.H + (size_t)v * M, st.data() + 4 * N, sizeof(float2) * M,
-                        cudaMemcpyHostToDevice));
-    SFD_CUDA(cudaMemcpy(p->d.Hx + (size_t)v * M, st.data() + 4 * N + M, sizeof(float2) * M,
-                        cudaMemcpyHostToDevice));
+    delete r;
+}
+
+int update_ring_make(sfd_plan *p) {
+    if (p->ur) return SFD_OK;
+    sfd_update_ring *r = new (std::nothrow) sfd_update_ring;
+    if (!r) return SFD_ENOMEM;
+    p->ur = r;
+    for (int i = 0; i < sfd_update_ring::SLOTS; ++i) {
+        SFD_CUDA(cudaMallocHost((void **)&r->slot[i], (size_t)p->d.vstride * sizeof(float2)));
+        SFD_CUDA(cudaEventCreateWithFlags(&r->done[i], cudaEventDisableTiming));
+    }
     return SFD_OK;
 }
 
-}  // namespace
-
-// ---- C ABI -------------------------------------------------------------------------------------
-extern "C" {
-
-int sfd_host_tables(int N, double lambda, double p1, double p2, double z, double off, double *pre,
-                    double *post, double *H) {
-    return sfd_host_tables_general(N, lambda, p1, p2, z, 0.0, off, pre, post, H);
-}
-
-int sfd_host_tables_general(int N, double lambda, double p1, double p2, double z, double off0,
-                            double off, double *pre, double *post, double *H) {
-    if (!pre || !post || !H || log2_exact(N) < 0 || N < 2) return SFD_EINVAL;
-    if (check_view(lambda, p1, p2, z, off, off0) != SFD_OK) return SFD_EINVAL;
-    std::vector<cd> a(N), b(N), h(2 * (size_t)N);
-    axis_tables(N, lambda, p1, p2, z, off, a.data(), b.data(), off0);
-    kernel_spectrum(N, lambda, p1, p2, z, h.data());
-    std::memcpy(pre, a.data(), sizeof(cd) * N);
-    std::memcpy(post, b.data(), sizeof(cd) * N);
-    std::memcpy(H, h.data(), sizeof(cd) * 2 * N);
+// Rebuild the tables of view v from the plan's current parameters and copy them to the device:
+// one cudaMemcpyAsync from a pinned staging slot on `st`, ordered like any other work of that stream
+// (after the executes enqueued before it, before those enqueued after it).  wait = true blocks
+// until the copy has landed.
+int upload_view(sfd_plan *p, int v, cudaStream_t st, bool wait) {
+    int rc = update_ring_make(p);
+    if (rc != SFD_OK) return rc;
+    sfd_update_ring *r = p->ur;
+    const int i = r->next;
+    r->next = (i + 1) % sfd_update_ring::SLOTS;
+    if (r->used[i]) SFD_CUDA(cudaEventSynchronize(r->done[i]));  // the slot's last copy has read it
+    const auto t0 = std::chrono::steady_clock::now();
+    build_view_f32(p, v, r->slot[i]);
+    p->last_update_host_ms =
+        std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    SFD_CUDA(cudaMemcpyAsync(p->d.tabs + (size_t)v * p->d.vstride, r->slot[i],
+                             (size_t)p->d.vstride * sizeof(float2), cudaMemcpyHostToDevice, st));
+    SFD_CUDA(cudaEventRecord(r->done[i], st));
+    r->used[i] = true;
+    if (wait) SFD_CUDA(cudaEventSynchronize(r->done[i]));
     return SFD_OK;
 }
 
-int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const double *p1,
-                    const double *p2, const double *z, const double *Ox, const double *Oy,
-                    int in_dtype) {
-    if (!out) return SFD_EINVAL;
-    *out = nullptr;
-    if (!p1 || !p2 || !z || !Ox || !Oy || n_views < 1) return SFD_EINVAL;
-    const std::vector<double> zero(n_views, 0.0);
-    return sfd_plan_create_general(out, N, n_views, lambda, p1, p1, p2, p2, z, zero.data(),
-                                   zero.data(), Ox, Oy, in_dtype);
-}
-
-int sfd_plan_create_general(sfd_plan **out, int N, int n_views, double lambda, const double *p1x,
-                            const double *p1y, const double *p2x, const double *p2y,
-                            const double *z, const double *O0x, const double *O0y,
-                            const double *O1x, const double *O1y, int in_dtype) {
-    if (!out) return SFD_EINVAL;
-    *out = nullptr;
-    if (!p1x || !p1y || !p2x || !p2y || !z || !O0x || !O0y || !O1x || !O1y) return SFD_EINVAL;
-    const int l2 = log2_exact(N);
-    if (l2 < 6 || l2 > 11 || n_views < 1) return SFD_EINVAL;
-    if (in_dtype != SFD_U8 && in_dtype != SFD_F32) return SFD_EINVAL;
-    for (int v = 0; v < n_views; ++v) {
-        if (check_view(lambda, p1x[v], p2x[v], z[v], O1x[v], O0x[v]) != SFD_OK) return SFD_EINVAL;
-        if (check_view(lambda, p1y[v], p2y[v], z[v], O1y[v], O0y[v]) != SFD_OK) return SFD_EINVAL;
-    }
-    const double *p1 = p1x, *p2 = p2x, *Ox = O1x, *Oy = O1y;
-
-    if (!g_init.load()) {
-        SFD_CUDA(sfd_kernels_init());
-        g_init.store(true);
-    }
-    sfd_plan *p = new (std::nothrow) sfd_plan;
-    if (!p) return SFD_ENOMEM;
-    p->d.N = N;
-    p->d.M = 2 * N;
-    p->d.log2M = l2 + 1;
-    p->d.V = n_views;
-    p->d.in_dtype = in_dtype;
-    p->lambda = lambda;
-    p->p1.assign(p1, p1 + n_views);
-    p->p2.assign(p2, p2 + n_views);
-    p->z.assign(z, z + n_views);
-    p->Ox.assign(Ox, Ox + n_views);
-    p->Oy.assign(Oy, Oy + n_views);
-    p->p1y.assign(p1y, p1y + n_views);
-    p->p2y.assign(p2y, p2y + n_views);
-    p->O0x.assign(O0x, O0x + n_views);
-    p->O0y.assign(O0y, O0y + n_views);
-
-    int rc = SFD_OK;
-    auto fail = [&](int code) {
-        sfd_plan_destroy(p);
-        return code;
-    };
-    if (cudaGetDevice(&p->device) != cudaSuccess) return fail(cuda_fail(cudaGetLastError(), "cudaGetDevice"));
-    const size_t V = n_views, M = 2 * (size_t)N, nn = (size_t)N * N;
-    const size_t n_tab = V * (4 * (size_t)N + 2 * M) + M;  // complex64 elements
-    cudaError_t e;
-    if ((e = cudaMalloc(&p->table_alloc, n_tab * sizeof(float2))) != cudaSuccess)
-        return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc tables"));
-    float2 *t = (float2 *)p->table_alloc;
-    p->d.pre_y = t;
-    p->d.post_y = t + V * N;
-    p->d.pre_x = t + 2 * V * N;
-    p->d.post_x = t + 3 * V * N;
-    p->d.H = t + 4 * V * N;
-    p->d.Hx = p->d.H + V * M;
-    p->d.tw = p->d.Hx + V * M;
-    if ((e = cudaMalloc((void **)&p->d.B, V * nn * sizeof(float2))) != cudaSuccess)
-        return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc B"));
-    if ((e = cudaMalloc((void **)&p->d.inten_ws, V * nn * sizeof(float))) != cudaSuccess)
-        return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc I"));
-    if ((e = cudaMalloc((void **)&p->d.vmax, V * sizeof(unsigned int))) != cudaSuccess)
-        return fail(cuda_fail(e, "cudaMalloc vmax"));
-    p->device_bytes = (long long)(n_tab * sizeof(float2) + V * nn * 12 + V * 4);
-
-    {   // FFT twiddles exp(-2 pi i x / M)
-        std::vector<float2> tw(M);
-        for (size_t x = 0; x < M; ++x) {
-            const cd w = cis_cycles(-(ld)x / (ld)M);
-            tw[x] = make_float2((float)w.real(), (float)w.imag());
-        }
-        if ((e = cudaMemcpy(p->d.tw, tw.data(), M * sizeof(float2), cudaMemcpyHostToDevice)) !=
-            cudaSuccess)
-            return fail(cuda_fail(e, "cudaMemcpy tw"));
-    }
-    if (N == 1024 || N == 2048) {   // fast-path tables (sfd_warp1024.cuh, sfd_warp2048.cuh)
-        const size_t fpass = N == 1024 ? 6 * (size_t)1024 : 20 * (size_t)1024;
-        const size_t n_fast = V * 2 * fpass + 32 * 32;
-        if ((e = cudaMalloc(&p->fast_alloc, n_fast * sizeof(float2))) != cudaSuccess)
-            return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc fast tables"));
-        float2 *f = (float2 *)p->fast_alloc;
-        p->d.w_tabY = f;
-        p->d.w_tabX = f + V * fpass;
-        p->d.w_twl = f + V * 2 * fpass;
-        p->device_bytes += (long long)(n_fast * sizeof(float2));
-        // stage-B twiddles of the warp FFT (sfd_dft32.cuh): [j][lane], j = n/2 - 1 + k,
-        // T_n[k] = exp(-2 pi i (lane + 32 k) / (32 n)), n = 2, 4, .., 32, k < n/2
-        std::vector<float2> twl(32 * 32, make_float2(0.f, 0.f));
-        for (int n = 2; n <= 32; n *= 2)
-            for (int k = 0; k < n / 2; ++k)
-                for (int lane = 0; lane < 32; ++lane) {
-                    const cd w = cis_cycles(-(ld)(lane + 32 * k) / (ld)(32 * n));
-                    twl[(n / 2 - 1 + k) * 32 + lane] = make_float2((float)w.real(), (float)w.imag());
-                }
-        if ((e = cudaMemcpy(p->d.w_twl, twl.data(), twl.size() * sizeof(float2),
-                            cudaMemcpyHostToDevice)) != cudaSuccess)
-            return fail(cuda_fail(e, "cudaMemcpy twl"));
-    }
-    for (int v = 0; v < n_views; ++v)
-        if ((rc = upload_view(p, v)) != SFD_OK) return fail(rc);
-    if ((e = sfd_make_tensormaps(p)) != cudaSuccess) return fail(cuda_fail(e, "cuTensorMapEncodeTiled"));
-    for (int i = 0; i < 4; ++i)
-        if ((e = cudaEventCreate(&p->ev[i])) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
-    *out = p;
-    return SFD_OK;
-}
-
-int sfd_plan_update_view(sfd_plan *p, int view, double p1, double p2, double z, double Ox,
-                         double Oy) {
-    if (!p || view < 0 || view >= p->d.V) return SFD_EINVAL;
-    if (check_view(p->lambda, p1, p2, z, Ox, Oy) != SFD_OK) return SFD_EINVAL;
-    p->p1[view] = p->p1y[view] = p1;
-    p->p2[view] = p->p2y[view] = p2;
-    p->z[view] = z;
-    p->Ox[view] = Ox;
-    p->Oy[view] = Oy;
-    p->O0x[view] = p->O0y[view] = 0.0;
-    return upload_view(p, view);
-}
-
-int sfd_plan_update_view_general(sfd_plan *p, int view, double p1x, double p1y, double p2x,
-                                 double p2y, double z, double O0x, double O0y, double O1x,
-                                 double O1y) {
+int set_view(sfd_plan *p, int view, double p1x, double p1y, double p2x, double p2y, double z,
+             double O0x, double O0y, double O1x, double O1y) {
     if (!p || view < 0 || view >= p->d.V) return SFD_EINVAL;
     if (check_view(p->lambda, p1x, p2x, z, O1x, O0x) != SFD_OK) return SFD_EINVAL;
     if (check_view(p->lambda, p1y, p2y, z, O1y, O0y) != SFD_OK) return SFD_EINVAL;
@@ -459,45 +397,33 @@ int sfd_plan_update_view_general(sfd_plan *p, int view, double p1x, double p1y, 
     p->Oy[view] = O1y;
     p->O0x[view] = O0x;
     p->O0y[view] = O0y;
-    return upload_view(p, view);
-}
-
-int sfd_execute(sfd_plan *p, const void *hologram_dev, void *field_dev, float *intensity_dev,
-                void *stream) {
-    if (!p || !hologram_dev || (!field_dev && !intensity_dev)) return SFD_EINVAL;
-    SFD_CUDA(sfd_launch(p, hologram_dev, (float2 *)field_dev, intensity_dev, nullptr,
-                        (cudaStream_t)stream));
     return SFD_OK;
 }
 
-int sfd_execute_focus(sfd_plan *p, const void *hologram_dev, double *moments_dev,
-                      float *intensity_dev, void *stream) {
-    if (!p || !hologram_dev || !moments_dev) return SFD_EINVAL;
-    SFD_CUDA(sfd_launch(p, hologram_dev, nullptr, intensity_dev, nullptr, (cudaStream_t)stream,
-                        moments_dev));
-    return SFD_OK;
+const void *window_ptr(const sfd_plan *p, const void *frame) {
+    return (const char *)frame + p->d.in_offset * (p->d.in_dtype == SFD_U8 ? 1 : 4);
 }
 
-int sfd_execute_u8(sfd_plan *p, const void *hologram_dev, unsigned char *intensity_u8_dev,
-                   void *stream) {
-    if (!p || !hologram_dev || !intensity_u8_dev) return SFD_EINVAL;
-    SFD_CUDA(sfd_launch(p, hologram_dev, nullptr, nullptr, intensity_u8_dev, (cudaStream_t)stream));
-    return SFD_OK;
-}
-
-int sfd_stream_run(sfd_plan *p, const void *holograms_pinned, int n_frames,
-                   unsigned char *out_pinned, double *seconds) {
-    if (!p || !holograms_pinned || !out_pinned || n_frames < 0) return SFD_EINVAL;
-    if (seconds) *seconds = 0.0;
-    if (n_frames == 0) return SFD_OK;
-    int rc = stream_state_make(p);
-    if (rc != SFD_OK) return rc;
-    sfd_stream_state *s = p->ss;
-    const size_t nn = (size_t)p->d.N * p->d.N;
+// the frame loop of sfd_stream_run; any failure is reported through the single exit of the caller
+int stream_frames(sfd_plan *p, sfd_stream_state *s, const void *holograms_pinned, int n_frames,
+                  unsigned char *out_pinned) {
+    const size_t nn = window_elems(p);
     const size_t in_bytes = nn * (p->d.in_dtype == SFD_U8 ? 1 : 4);
     const size_t out_bytes = nn * p->d.V;
-    const bool timing = p->timing;
-    p->timing = false;  // the per-kernel events belong to sfd_execute*
+    // the device copy of a frame is the dense window: the window set on the plan applies to
+    // sfd_execute*, the stream reads dense [Ny][Nx] frames from the host
+    struct Dense {
+        sfd_plan *p;
+        long long stride, offset;
+        explicit Dense(sfd_plan *q) : p(q), stride(q->d.in_stride), offset(q->d.in_offset) {
+            p->d.in_stride = p->d.Nx;
+            p->d.in_offset = 0;
+        }
+        ~Dense() {
+            p->d.in_stride = stride;
+            p->d.in_offset = offset;
+        }
+    } dense(p);
     SFD_CUDA(cudaEventRecord(s->e_t0, s->s_in));
     for (int f = 0; f < n_frames; ++f) {
         const int b = f & 1;
@@ -518,10 +444,267 @@ int sfd_stream_run(sfd_plan *p, const void *holograms_pinned, int n_frames,
         SFD_CUDA(cudaEventRecord(s->e_out[b], s->s_out));
     }
     SFD_CUDA(cudaEventRecord(s->e_t1, s->s_out));
+    return SFD_OK;
+}
+
+}  // namespace
+
+// ---- C ABI -------------------------------------------------------------------------------------
+extern "C" {
+
+int sfd_host_tables(int N, double lambda, double p1, double p2, double z, double off, double *pre,
+                    double *post, double *H) {
+    return sfd_host_tables_general(N, lambda, p1, p2, z, 0.0, off, pre, post, H);
+}
+
+int sfd_host_tables_general(int N, double lambda, double p1, double p2, double z, double off0,
+                            double off, double *pre, double *post, double *H) {
+    if (!pre || !post || !H || log2_exact(N) < 0 || N < 2) return SFD_EINVAL;
+    if (check_view(lambda, p1, p2, z, off, off0) != SFD_OK) return SFD_EINVAL;
+    std::vector<cd> a(N), b(N), h(2 * (size_t)N);
+    axis_tables(N, lambda, p1, p2, z, off, a.data(), b.data(), off0);
+    kernel_spectrum(N, lambda, p1, p2, z, h.data(), fft_twiddles(2 * (size_t)N));
+    std::memcpy(pre, a.data(), sizeof(cd) * N);
+    std::memcpy(post, b.data(), sizeof(cd) * N);
+    std::memcpy(H, h.data(), sizeof(cd) * 2 * N);
+    return SFD_OK;
+}
+
+int sfd_host_dft32(const float *in, float *out, int lane, int twiddled) {
+    if (!in || !out || lane < 0 || lane > 31) return SFD_EINVAL;
+    sfd_host_dft32_impl(in, out, lane, twiddled);
+    return SFD_OK;
+}
+
+int sfd_plan_create(sfd_plan **out, int N, int n_views, double lambda, const double *p1,
+                    const double *p2, const double *z, const double *Ox, const double *Oy,
+                    int in_dtype) {
+    if (!out) return SFD_EINVAL;
+    *out = nullptr;
+    if (!p1 || !p2 || !z || !Ox || !Oy || n_views < 1) return SFD_EINVAL;
+    const std::vector<double> zero(n_views, 0.0);
+    return sfd_plan_create_rect(out, N, N, n_views, lambda, p1, p1, p2, p2, z, zero.data(),
+                                zero.data(), Ox, Oy, in_dtype);
+}
+
+int sfd_plan_create_general(sfd_plan **out, int N, int n_views, double lambda, const double *p1x,
+                            const double *p1y, const double *p2x, const double *p2y,
+                            const double *z, const double *O0x, const double *O0y,
+                            const double *O1x, const double *O1y, int in_dtype) {
+    return sfd_plan_create_rect(out, N, N, n_views, lambda, p1x, p1y, p2x, p2y, z, O0x, O0y, O1x,
+                                O1y, in_dtype);
+}
+
+int sfd_plan_create_rect(sfd_plan **out, int Nx, int Ny, int n_views, double lambda,
+                         const double *p1x, const double *p1y, const double *p2x,
+                         const double *p2y, const double *z, const double *O0x,
+                         const double *O0y, const double *O1x, const double *O1y, int in_dtype) {
+    if (!out) return SFD_EINVAL;
+    *out = nullptr;
+    if (!p1x || !p1y || !p2x || !p2y || !z || !O0x || !O0y || !O1x || !O1y) return SFD_EINVAL;
+    if (Nx < 1 || Ny < 1 || n_views < 1) return SFD_EINVAL;
+    if (in_dtype != SFD_U8 && in_dtype != SFD_F32) return SFD_EINVAL;
+    for (int v = 0; v < n_views; ++v) {
+        if (check_view(lambda, p1x[v], p2x[v], z[v], O1x[v], O0x[v]) != SFD_OK) return SFD_EINVAL;
+        if (check_view(lambda, p1y[v], p2y[v], z[v], O1y[v], O0y[v]) != SFD_OK) return SFD_EINVAL;
+    }
+    // a size this build has no kernels for is a valid request that is not implemented
+    const int lx = log2_exact(Nx), ly = log2_exact(Ny);
+    if (lx < 6 || lx > 11 || ly < 6 || ly > 11) return SFD_EUNSUPPORTED;
+    int device = 0;
+    SFD_CUDA(cudaGetDevice(&device));
+    int sms = 0;
+    int rc = device_init(device, &sms);
+    if (rc != SFD_OK) return rc;
+
+    sfd_plan *p = new (std::nothrow) sfd_plan;
+    if (!p) return SFD_ENOMEM;
+    sfd_dev &d = p->d;
+    p->device = device;
+    d.sms = sms;
+    d.Nx = Nx;
+    d.Ny = Ny;
+    d.Mx = 2 * Nx;
+    d.My = 2 * Ny;
+    d.log2Mx = lx + 1;
+    d.log2My = ly + 1;
+    d.V = n_views;
+    d.in_dtype = in_dtype;
+    d.in_stride = Nx;
+    d.in_offset = 0;
+    p->lambda = lambda;
+    p->p1.assign(p1x, p1x + n_views);
+    p->p2.assign(p2x, p2x + n_views);
+    p->z.assign(z, z + n_views);
+    p->Ox.assign(O1x, O1x + n_views);
+    p->Oy.assign(O1y, O1y + n_views);
+    p->p1y.assign(p1y, p1y + n_views);
+    p->p2y.assign(p2y, p2y + n_views);
+    p->O0x.assign(O0x, O0x + n_views);
+    p->O0y.assign(O0y, O0y + n_views);
+    p->wy = fft_twiddles((size_t)d.My);
+    p->wx = fft_twiddles((size_t)d.Mx);
+
+    auto fail = [&](int code) {
+        sfd_plan_destroy(p);
+        return code;
+    };
+    // table layout of one view (complex64 elements), the stride rounded up to 128 bytes
+    int o = 0;
+    d.off_pre_y = o;   o += Ny;
+    d.off_post_y = o;  o += Ny;
+    d.off_pre_x = o;   o += Nx;
+    d.off_post_x = o;  o += Nx;
+    d.off_Hy = o;      o += d.My;
+    d.off_Hx = o;      o += d.Mx;
+    if (fast_elems(Ny)) { d.off_tabY = o; o += (int)fast_elems(Ny); }
+    if (fast_elems(Nx)) { d.off_tabX = o; o += (int)fast_elems(Nx); }
+    d.vstride = (o + 15) & ~15;
+    const size_t V = n_views, nn = (size_t)Nx * Ny;
+    const size_t n_tab = V * (size_t)d.vstride + d.My + d.Mx + 32 * 32;  // + FFT twiddles + w_twl
+    cudaError_t e;
+    if ((e = cudaMalloc(&p->table_alloc, n_tab * sizeof(float2))) != cudaSuccess)
+        return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc tables"));
+    d.tabs = (float2 *)p->table_alloc;
+    d.tw_y = d.tabs + V * (size_t)d.vstride;
+    d.tw_x = d.tw_y + d.My;
+    d.w_twl = d.tw_x + d.Mx;
+    if ((e = cudaMalloc((void **)&d.B, V * nn * sizeof(float2))) != cudaSuccess)
+        return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc B"));
+    if ((e = cudaMalloc((void **)&d.inten_ws, V * nn * sizeof(float))) != cudaSuccess)
+        return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : cuda_fail(e, "cudaMalloc I"));
+    if ((e = cudaMalloc((void **)&d.vmax, V * sizeof(unsigned int))) != cudaSuccess)
+        return fail(cuda_fail(e, "cudaMalloc vmax"));
+    p->device_bytes = (long long)(n_tab * sizeof(float2) + V * nn * 12 + V * 4);
+
+    {   // plan constants: FFT twiddles exp(-2 pi i x / M) of both axes (generic kernels) and the
+        // stage-B twiddles of the warp FFT (sfd_dft32.cuh): [j][lane], j = n/2 - 1 + k,
+        // T_n[k] = exp(-2 pi i (lane + 32 k) / (32 n)), n = 2, 4, .., 32, k < n/2
+        std::vector<float2> c((size_t)d.My + d.Mx + 32 * 32, make_float2(0.f, 0.f));
+        for (int x = 0; x < d.My; ++x) {
+            const cd w = cis_cycles(-(ld)x / (ld)d.My);
+            c[x] = make_float2((float)w.real(), (float)w.imag());
+        }
+        for (int x = 0; x < d.Mx; ++x) {
+            const cd w = cis_cycles(-(ld)x / (ld)d.Mx);
+            c[(size_t)d.My + x] = make_float2((float)w.real(), (float)w.imag());
+        }
+        float2 *twl = c.data() + d.My + d.Mx;
+        for (int n = 2; n <= 32; n *= 2)
+            for (int k = 0; k < n / 2; ++k)
+                for (int lane = 0; lane < 32; ++lane) {
+                    const cd w = cis_cycles(-(ld)(lane + 32 * k) / (ld)(32 * n));
+                    twl[(n / 2 - 1 + k) * 32 + lane] = make_float2((float)w.real(), (float)w.imag());
+                }
+        if ((e = cudaMemcpy(d.tw_y, c.data(), c.size() * sizeof(float2), cudaMemcpyHostToDevice)) !=
+            cudaSuccess)
+            return fail(cuda_fail(e, "cudaMemcpy twiddles"));
+    }
+    for (int v = 0; v < n_views; ++v)
+        if ((rc = upload_view(p, v, cudaStreamLegacy, false)) != SFD_OK) return fail(rc);
+    // every table has landed before the plan is handed out: the kernels read them in their prologue,
+    // on whatever stream (possibly a non-blocking one) the caller launches
+    if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail(cuda_fail(e, "cudaDeviceSynchronize"));
+    if ((e = sfd_make_tensormaps(p)) != cudaSuccess) return fail(cuda_fail(e, "cuTensorMapEncodeTiled"));
+    for (int i = 0; i < 4; ++i)
+        if ((e = cudaEventCreate(&p->ev[i])) != cudaSuccess) return fail(cuda_fail(e, "cudaEventCreate"));
+    *out = p;
+    return SFD_OK;
+}
+
+int sfd_plan_set_input_window(sfd_plan *p, long long row_stride, int row0, int col0) {
+    if (!p || row0 < 0 || col0 < 0 || row_stride < 0) return SFD_EINVAL;
+    if (row_stride == 0) row_stride = p->d.Nx;
+    if (row_stride < (long long)col0 + p->d.Nx) return SFD_EINVAL;
+    p->d.in_stride = row_stride;
+    p->d.in_offset = (long long)row0 * row_stride + col0;
+    return SFD_OK;
+}
+
+int sfd_plan_update_view(sfd_plan *p, int view, double p1, double p2, double z, double Ox,
+                         double Oy) {
+    const int rc = set_view(p, view, p1, p1, p2, p2, z, 0.0, 0.0, Ox, Oy);
+    if (rc != SFD_OK) return rc;
+    SFD_ON_DEVICE(p);
+    return upload_view(p, view, cudaStreamLegacy, true);
+}
+
+int sfd_plan_update_view_general(sfd_plan *p, int view, double p1x, double p1y, double p2x,
+                                 double p2y, double z, double O0x, double O0y, double O1x,
+                                 double O1y) {
+    const int rc = set_view(p, view, p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y);
+    if (rc != SFD_OK) return rc;
+    SFD_ON_DEVICE(p);
+    return upload_view(p, view, cudaStreamLegacy, true);
+}
+
+int sfd_plan_update_view_async(sfd_plan *p, int view, double p1, double p2, double z, double Ox,
+                               double Oy, void *stream) {
+    const int rc = set_view(p, view, p1, p1, p2, p2, z, 0.0, 0.0, Ox, Oy);
+    if (rc != SFD_OK) return rc;
+    SFD_ON_DEVICE(p);
+    return upload_view(p, view, (cudaStream_t)stream, false);
+}
+
+int sfd_plan_update_view_general_async(sfd_plan *p, int view, double p1x, double p1y, double p2x,
+                                       double p2y, double z, double O0x, double O0y, double O1x,
+                                       double O1y, void *stream) {
+    const int rc = set_view(p, view, p1x, p1y, p2x, p2y, z, O0x, O0y, O1x, O1y);
+    if (rc != SFD_OK) return rc;
+    SFD_ON_DEVICE(p);
+    return upload_view(p, view, (cudaStream_t)stream, false);
+}
+
+double sfd_plan_last_update_host_ms(const sfd_plan *p) { return p ? p->last_update_host_ms : -1.0; }
+
+int sfd_execute(sfd_plan *p, const void *hologram_dev, void *field_dev, float *intensity_dev,
+                void *stream) {
+    if (!p || !hologram_dev || (!field_dev && !intensity_dev)) return SFD_EINVAL;
+    SFD_ON_DEVICE(p);
+    SFD_CUDA(sfd_launch(p, window_ptr(p, hologram_dev), (float2 *)field_dev, intensity_dev, nullptr,
+                        (cudaStream_t)stream));
+    return SFD_OK;
+}
+
+int sfd_execute_focus(sfd_plan *p, const void *hologram_dev, double *moments_dev,
+                      float *intensity_dev, void *stream) {
+    if (!p || !hologram_dev || !moments_dev) return SFD_EINVAL;
+    SFD_ON_DEVICE(p);
+    SFD_CUDA(sfd_launch(p, window_ptr(p, hologram_dev), nullptr, intensity_dev, nullptr,
+                        (cudaStream_t)stream, moments_dev));
+    return SFD_OK;
+}
+
+int sfd_execute_u8(sfd_plan *p, const void *hologram_dev, unsigned char *intensity_u8_dev,
+                   void *stream) {
+    if (!p || !hologram_dev || !intensity_u8_dev) return SFD_EINVAL;
+    SFD_ON_DEVICE(p);
+    SFD_CUDA(sfd_launch(p, window_ptr(p, hologram_dev), nullptr, nullptr, intensity_u8_dev,
+                        (cudaStream_t)stream));
+    return SFD_OK;
+}
+
+int sfd_stream_run(sfd_plan *p, const void *holograms_pinned, int n_frames,
+                   unsigned char *out_pinned, double *seconds) {
+    if (!p || !holograms_pinned || !out_pinned || n_frames < 0) return SFD_EINVAL;
+    if (seconds) *seconds = 0.0;
+    if (n_frames == 0) return SFD_OK;
+    SFD_ON_DEVICE(p);
+    int rc = stream_state_make(p);
+    if (rc != SFD_OK) return rc;
+    sfd_stream_state *s = p->ss;
+    const bool timing = p->timing;
+    p->timing = false;  // the per-kernel events belong to sfd_execute*
+    rc = stream_frames(p, s, holograms_pinned, n_frames, out_pinned);
     p->timing = timing;
-    SFD_CUDA(cudaEventSynchronize(s->e_t1));
-    SFD_CUDA(cudaStreamSynchronize(s->s_in));
-    SFD_CUDA(cudaStreamSynchronize(s->s_comp));
+    // single exit: whatever was enqueued has drained before the caller may touch (or free) its
+    // pinned buffers, also after a failure half way through the loop
+    const cudaError_t e0 = cudaStreamSynchronize(s->s_in), e1 = cudaStreamSynchronize(s->s_comp),
+                      e2 = cudaStreamSynchronize(s->s_out);
+    if (rc != SFD_OK) return rc;
+    SFD_CUDA(e0);
+    SFD_CUDA(e1);
+    SFD_CUDA(e2);
     float ms = 0.f;
     SFD_CUDA(cudaEventElapsedTime(&ms, s->e_t0, s->e_t1));
     if (seconds) *seconds = (double)ms * 1e-3;
@@ -530,9 +713,10 @@ int sfd_stream_run(sfd_plan *p, const void *holograms_pinned, int n_frames,
 
 int sfd_plan_destroy(sfd_plan *p) {
     if (!p) return SFD_OK;
+    DeviceGuard guard(p->device);
     stream_state_free(p->ss);
+    update_ring_free(p->ur);
     if (p->table_alloc) cudaFree(p->table_alloc);
-    if (p->fast_alloc) cudaFree(p->fast_alloc);
     if (p->d.B) cudaFree(p->d.B);
     if (p->d.inten_ws) cudaFree(p->d.inten_ws);
     if (p->d.vmax) cudaFree(p->d.vmax);
@@ -542,9 +726,12 @@ int sfd_plan_destroy(sfd_plan *p) {
     return SFD_OK;
 }
 
-int sfd_plan_get_n(const sfd_plan *p) { return p ? p->d.N : SFD_EINVAL; }
+int sfd_plan_get_n(const sfd_plan *p) { return p ? p->d.Nx : SFD_EINVAL; }
+int sfd_plan_get_nx(const sfd_plan *p) { return p ? p->d.Nx : SFD_EINVAL; }
+int sfd_plan_get_ny(const sfd_plan *p) { return p ? p->d.Ny : SFD_EINVAL; }
 int sfd_plan_get_views(const sfd_plan *p) { return p ? p->d.V : SFD_EINVAL; }
-int sfd_plan_get_m(const sfd_plan *p) { return p ? p->d.M : SFD_EINVAL; }
+int sfd_plan_get_m(const sfd_plan *p) { return p ? p->d.Mx : SFD_EINVAL; }
+int sfd_plan_get_device(const sfd_plan *p) { return p ? p->device : SFD_EINVAL; }
 long long sfd_plan_device_bytes(const sfd_plan *p) { return p ? p->device_bytes : SFD_EINVAL; }
 
 int sfd_plan_select_kernels(sfd_plan *p, int which) {
@@ -555,10 +742,7 @@ int sfd_plan_select_kernels(sfd_plan *p, int which) {
 
 int sfd_plan_uses_warp_kernels(const sfd_plan *p) {
     if (!p) return SFD_EINVAL;
-    return (p->d.N == 1024 || p->d.N == 2048) && p->kernels != SFD_KERNELS_GENERIC &&
-                   p->d.w_twl != nullptr
-               ? 1
-               : 0;
+    return (sfd_uses_warp_y(p, nullptr) ? 1 : 0) | (sfd_uses_warp_x(p) ? 2 : 0);
 }
 
 int sfd_plan_set_timing(sfd_plan *p, int enable) {
@@ -572,10 +756,17 @@ int sfd_plan_last_kernel_ms(sfd_plan *p, float ms[3]) {
     if (!p || !ms) return SFD_EINVAL;
     ms[0] = ms[1] = ms[2] = 0.f;
     if (!p->ev_valid) return SFD_EINVAL;
+    SFD_ON_DEVICE(p);
     SFD_CUDA(cudaEventSynchronize(p->ev[p->ev_quant ? 3 : 2]));
     SFD_CUDA(cudaEventElapsedTime(&ms[0], p->ev[0], p->ev[1]));
     SFD_CUDA(cudaEventElapsedTime(&ms[1], p->ev[1], p->ev[2]));
     if (p->ev_quant) SFD_CUDA(cudaEventElapsedTime(&ms[2], p->ev[2], p->ev[3]));
+    return SFD_OK;
+}
+
+int sfd_measure_pipes(double out[4]) {
+    if (!out) return SFD_EINVAL;
+    SFD_CUDA(sfd_measure_pipes_impl(out));
     return SFD_OK;
 }
 
@@ -594,6 +785,6 @@ const char *sfd_error_string(int code) {
 
 const char *sfd_last_cuda_error(void) { return g_cuda_err; }
 
-const char *sfd_version(void) { return "sfd 0.1 sm_100a"; }
+const char *sfd_version(void) { return "sfd 0.2 sm_100a"; }
 
 }  // extern "C"

@@ -204,11 +204,11 @@ __device__ __forceinline__ unsigned tm_quarter(unsigned base, int warp) {
 // their quarter: warp w the chunks 0..5 (pre_b and half of H_b), warp w + 4 the chunks 6..11.  All
 // 48 loads of a thread are issued before the first store (and before the allocation): one trip
 // to L2 per set.
-// tab: [V][2][3][N] in global memory
+// tab: the [2][3][N] block of view 0 in global memory, vstride complex values between views
 struct TFill { TChunk c[6]; };
-__device__ __forceinline__ void tm_fill_load(TFill &f, const float2 *__restrict__ tab, int view,
-                                             int warp, int lane) {
-    const float2 *src = tab + (size_t)view * TABS + (size_t)(warp & 1) * 3 * N + lane;
+__device__ __forceinline__ void tm_fill_load(TFill &f, const float2 *__restrict__ tab,
+                                             long long vstride, int view, int warp, int lane) {
+    const float2 *src = tab + (size_t)view * vstride + (size_t)(warp & 1) * 3 * N + lane;
     const int ch0 = 6 * (warp >> 2);  // first chunk of this warp; chunk = 8 values, 4 chunks per table
 #pragma unroll
     for (int j = 0; j < 6; ++j)
@@ -228,13 +228,13 @@ __device__ __forceinline__ void tm_fill_store(const TFill &f, unsigned quarter, 
 // range [total b / g, total (b + 1) / g) of work units touches (per_view units per view), make
 // them visible.  Returns the base address; tm_finish releases it at the end of the kernel.
 __device__ __forceinline__ unsigned tm_setup(unsigned *slot, const float2 *__restrict__ tab,
-                                             int total, int per_view) {
+                                             long long vstride, int total, int per_view) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int a0 = (int)((long long)total * blockIdx.x / gridDim.x);
     const int a1 = (int)((long long)total * (blockIdx.x + 1) / gridDim.x);
     const int view0 = a0 < a1 ? a0 / per_view : 0;
     TFill f;
-    if (a0 < a1) tm_fill_load(f, tab, view0, warp, lane);  // on their way during the allocation
+    if (a0 < a1) tm_fill_load(f, tab, vstride, view0, warp, lane);  // on their way during the allocation
     if (warp == 0) tm_alloc(slot);
     tm_sync_cta();
     const unsigned base = *reinterpret_cast<volatile unsigned *>(slot);
@@ -242,7 +242,7 @@ __device__ __forceinline__ unsigned tm_setup(unsigned *slot, const float2 *__res
         const unsigned q = tm_quarter(base, warp);
         tm_fill_store(f, q, 0, warp);
         if ((a1 - 1) / per_view != view0) {
-            tm_fill_load(f, tab, view0 + 1, warp, lane);
+            tm_fill_load(f, tab, vstride, view0 + 1, warp, lane);
             tm_fill_store(f, q, 1, warp);
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
@@ -407,13 +407,14 @@ template <typename TIn> struct SmemY {
 template <typename TIn> struct TileRegs { typename TileElem<TIn>::slab e[8]; };
 
 // the 128 threads of a half fetch rows ht, ht + 128, .. of the slab that starts at column col
+// (plain loads: the hologram was written by whatever ran before this kernel in the stream)
 template <typename TIn>
-__device__ __forceinline__ void tile_load(TileRegs<TIn> &t, const TIn *__restrict__ holo, int col,
-                                          int ht) {
+__device__ __forceinline__ void tile_load(TileRegs<TIn> &t, const TIn *holo, long long hstride,
+                                          int col, int ht) {
 #pragma unroll
     for (int i = 0; i < 8; ++i)
-        t.e[i] = __ldg(reinterpret_cast<const typename TileElem<TIn>::slab *>(
-            holo + (size_t)(ht + 128 * i) * N + col));
+        t.e[i] = *reinterpret_cast<const typename TileElem<TIn>::slab *>(
+            holo + (size_t)(ht + 128 * i) * hstride + col);
 }
 __device__ __forceinline__ void tile_store(const TileRegs<unsigned char> &t,
                                            unsigned short (*tile)[N], int ht) {
@@ -454,9 +455,11 @@ __device__ __forceinline__ void bulk_wait_read() {
 }
 
 // Persistent CTA of 256 threads: work item = (view, group of 4 columns); a CTA takes a contiguous
-// range of items (at most two views: the launcher sizes the grid accordingly).
-// tabY: [V][2][3][N] (post carries c0, pre the 1/255 of uint8 input); tmB: tensor map of B seen as
-// float [V * N][2 N] with box 4 x YBOX.
+// range of items (at most two views: the launcher sizes the grid accordingly).  The line length is
+// N = 1024 = the number of hologram rows Ny; the number of columns nx (a multiple of 16) and the
+// hologram's row stride are run-time values (rectangular grids, windows inside a wider frame).
+// tabY: [2][3][N] per view (post carries c0, pre the 1/255 of uint8 input); tmB: tensor map of B seen
+// as float [V * N][2 nx] with box 4 x YBOX.
 // Per item a warp (column c of its half, branch B) transforms its column, hands the half of the
 // outputs it does not finish to its partner through its own transpose tile (idle by then), adds
 // what the partner left for it and writes 16 final values per thread into the staging tile.
@@ -481,12 +484,12 @@ __device__ __forceinline__ void y_finish(const float2 (&v)[32], const float2 *xb
 }
 
 template <typename TIn>
-__device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restrict__ holo,
-                                            unsigned tq, const float2 (&tw)[TWN],
+__device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *holo, long long hstride,
+                                            int nx, unsigned tq, const float2 (&tw)[TWN],
                                             const void *tmB, int V) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int half = warp >> 2, c = (warp >> 1) & 1, ht = threadIdx.x & 127, b = warp & 1;
-    constexpr int groups = N / YC;
+    const int groups = nx / YC;
     const int items = V * groups;
     const int i0 = (int)((long long)items * blockIdx.x / gridDim.x);
     const int i1 = (int)((long long)items * (blockIdx.x + 1) / gridDim.x);
@@ -497,10 +500,10 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
     const bool leader = ht == 0;  // issues and retires the half's bulk stores
     const int view0 = i0 / groups;
     constexpr int IPS = TileElem<TIn>::IPS;
-    static_assert(groups % IPS == 0, "a slab never straddles two views");
+    // groups % IPS == 0 (nx is a multiple of 16): a slab never straddles two views
     {
         TileRegs<TIn> t;
-        tile_load<TIn>(t, holo, (i0 % groups) / IPS * (YC * IPS) + 2 * IPS * half, ht);
+        tile_load<TIn>(t, holo, hstride, (i0 % groups) / IPS * (YC * IPS) + 2 * IPS * half, ht);
         tile_store(t, sm.tile[half], ht);
     }
     half_sync(half);
@@ -532,7 +535,7 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *__restric
         // the next slab is fetched behind the tile reads: its loads touch one row per lane (32
         // wavefronts each) and would hold up everything queued after them
         if (has_next)
-            tile_load<TIn>(t, holo, ((item + 1) % groups) / IPS * (YC * IPS) + 2 * IPS * half, ht);
+            tile_load<TIn>(t, holo, hstride, ((item + 1) % groups) / IPS * (YC * IPS) + 2 * IPS * half, ht);
         branch(v, lane, xb, tw, tpre + TM_TAB, turns);
         // the previous item's bulk stores must have left the staging tile before it is rewritten
         if (leader) bulk_wait_read();
@@ -570,7 +573,8 @@ struct SmemX {
 };
 
 // Work unit = (view, group of XP adjacent rows); a CTA takes a contiguous range of units, so all
-// its pairs are always in the same view.  tabX: [V][2][3][N].
+// its pairs are always in the same view.  The line length is N = 1024 = the number of columns Nx;
+// the number of rows per view ny (a multiple of XP) is a run-time value.  tabX: [2][3][N] per view.
 // exchange of the halves, stores, reductions of one line for branch B (see y_hand_over)
 template <int B>
 __device__ __forceinline__ void x_finish(float2 (&v)[32], float2 *xb, const float2 *xbp, int lane,
@@ -614,13 +618,12 @@ __device__ __forceinline__ void x_finish(float2 (&v)[32], float2 *xb, const floa
     }
 }
 
-__device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict__ Bin,
-                                            unsigned tq,
+__device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *Bin, int ny, unsigned tq,
                                             const float2 (&tw)[TWN], float2 *__restrict__ field,
                                             float *__restrict__ inten, unsigned int *vmax,
                                             double *mom, int V) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, pair = warp >> 1;
-    constexpr int gpv = (N + XP - 1) / XP;  // units per view
+    const int gpv = ny / XP;  // units per view
     const int units = V * gpv;
     const int u0 = (int)((long long)units * blockIdx.x / gridDim.x);
     const int u1 = (int)((long long)units * (blockIdx.x + 1) / gridDim.x);
@@ -634,19 +637,18 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
     unsigned iphase = 0;
     bool pending = false;  // the pair's input row is already on its way
     // turn-taking of warps w and w + 4 (needs every warp of the CTA to run the same number of
-    // lines: XP divides N)
-    static_assert(WX == 8 && N % XP == 0, "turn-taking needs equal line counts per warp");
+    // lines: XP divides ny)
+    static_assert(WX == 8, "turn-taking pairs warps w and w + 4");
     const Turns turns = turns_make(warp, true);
     turns_open(turns, warp);
     for (int u = u0; u < u1; ++u) {
         const int view = u / gpv, line = (u % gpv) * XP + pair;
-        if (line >= N) continue;  // pair-uniform (ragged last group of a view when XP does not divide N)
         const unsigned tpre = tq + (view - view0) * TM_SET;  // pre_b | H_b | conj(post_b)
-        const size_t row = (size_t)view * N + line;
+        const size_t row = (size_t)view * ny + line;
         if (!pending && issuer)
             bulk_load(sm.inb[pair], Bin + row * N, N * sizeof(float2), &sm.ibar[pair]);
         const int nu = u + 1, nline = (nu % gpv) * XP + pair;
-        const bool has_next = nu < u1 && nline < N;
+        const bool has_next = nu < u1;
         mbar_wait(&sm.ibar[pair], iphase);
         iphase ^= 1;
         float2 v[32];
@@ -667,7 +669,7 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *__restrict_
         pair_sync(pair);
         if (has_next && issuer) {
             fence_async_smem();
-            bulk_load(sm.inb[pair], Bin + ((size_t)(nu / gpv) * N + nline) * N, N * sizeof(float2),
+            bulk_load(sm.inb[pair], Bin + ((size_t)(nu / gpv) * ny + nline) * N, N * sizeof(float2),
                       &sm.ibar[pair]);
         }
         pending = has_next;

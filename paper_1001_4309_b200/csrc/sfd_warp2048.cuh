@@ -32,8 +32,7 @@ constexpr int NBR = 4;              // branches per line
 constexpr int QTABS = NBR * 5 * N;  // complex elements of one view's tables of one pass: [4][5][N]
 // tensor-memory columns of the five tables of a branch
 constexpr int TQ_PREA = 0, TQ_PREB = 64, TQ_H = 128, TQ_POSTA = 192, TQ_POSTB = 256;
-constexpr int QUX = NL / 2;         // work units per view, pass x: 2 rows
-constexpr int QUY = NL / 4;         // work units per view, pass y: 4 columns (2 per quad)
+// work units per view: pass x 2 rows (ny / 2 units), pass y 4 columns, 2 per quad (nx / 4 units)
 
 __device__ __forceinline__ void quad_sync(int quad) {  // named barrier of the four warps of a quad
     asm volatile("bar.sync %0, 128;" ::"r"(quad + 1) : "memory");
@@ -42,10 +41,11 @@ __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "mem
 
 // The two warps of a sub-partition copy the 20 chunks (5 tables x 4 chunks of 8 values) of
 // `view`, branch warp & 3, into their quarter: warp w chunks 0..9, warp w + 4 chunks 10..19, five
-// chunks (40 loads per thread) in flight at a time.  tab: [V][4][5][N] in global memory.
-__device__ __forceinline__ void tmq_fill(unsigned quarter, const float2 *__restrict__ tab, int view,
-                                         int warp, int lane) {
-    const float2 *src = tab + (size_t)view * QTABS + (size_t)(warp & 3) * 5 * N + lane;
+// chunks (40 loads per thread) in flight at a time.  tab: the [4][5][N] block of view 0 in global
+// memory, vstride complex values between views.
+__device__ __forceinline__ void tmq_fill(unsigned quarter, const float2 *__restrict__ tab,
+                                         long long vstride, int view, int warp, int lane) {
+    const float2 *src = tab + (size_t)view * vstride + (size_t)(warp & 3) * 5 * N + lane;
 #pragma unroll 1
     for (int h = 0; h < 2; ++h) {
         const int ch0 = 10 * (warp >> 2) + 5 * h;
@@ -64,12 +64,12 @@ __device__ __forceinline__ void tmq_fill(unsigned quarter, const float2 *__restr
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 __device__ __forceinline__ unsigned tmq_setup(unsigned *slot, const float2 *__restrict__ tab,
-                                              int view) {
+                                              long long vstride, int view) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (warp == 0) tm_alloc(slot);
     tm_sync_cta();
     const unsigned base = *reinterpret_cast<volatile unsigned *>(slot);
-    tmq_fill(tm_quarter(base, warp), tab, view, warp, lane);
+    tmq_fill(tm_quarter(base, warp), tab, vstride, view, warp, lane);
     tm_sync_cta();
     return base;
 }
@@ -141,7 +141,7 @@ struct SmemXQ {
     unsigned tmem;
 };
 
-__device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *__restrict__ Bin, unsigned tq,
+__device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *Bin, int ny, unsigned tq,
                                             const float2 (&tw)[TWN], float2 *__restrict__ field,
                                             float *__restrict__ inten, unsigned int *vmax,
                                             double *mom, Range rg) {
@@ -154,7 +154,7 @@ __device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *__restrict
     const Turns turns = turns_make(warp, true);
     turns_open(turns, warp);
     for (int u = rg.u0; u < rg.u1; ++u) {
-        const size_t row = (size_t)rg.view * NL + 2 * u + quad;
+        const size_t row = (size_t)rg.view * ny + 2 * u + quad;
         if (!pending && issuer)
             bulk_load(sm.inb[quad], Bin + row * NL, NL * sizeof(float2), &sm.ibar[quad]);
         const bool has_next = u + 1 < rg.u1;
@@ -255,12 +255,12 @@ template <typename TIn> struct SubRegs { typename SubSlab<TIn>::elem e[16]; };
 
 // the 128 threads of a quad fetch rows qt, qt + 128, .. of the slab that starts at column col
 template <typename TIn>
-__device__ __forceinline__ void sub_load(SubRegs<TIn> &t, const TIn *__restrict__ holo, int col,
-                                         int qt) {
+__device__ __forceinline__ void sub_load(SubRegs<TIn> &t, const TIn *holo, long long hstride,
+                                         int col, int qt) {
 #pragma unroll
     for (int i = 0; i < 16; ++i)
-        t.e[i] = __ldg(reinterpret_cast<const typename SubSlab<TIn>::elem *>(
-            holo + (size_t)(qt + 128 * i) * NL + col));
+        t.e[i] = *reinterpret_cast<const typename SubSlab<TIn>::elem *>(
+            holo + (size_t)(qt + 128 * i) * hstride + col);
 }
 __device__ __forceinline__ void sub_store(const SubRegs<unsigned char> &t,
                                           unsigned short (*tile)[N][2], int qt, int quad) {
@@ -291,9 +291,10 @@ __device__ __forceinline__ float2 fold_values(const float2 (&e)[2], int c) {
     return c ? make_float2(w.y, w.w) : make_float2(w.x, w.z);
 }
 
-// tmB: tensor map of B seen as float [V * NL][2 NL] with box YBOXW x YBOX.
+// tmB: tensor map of B seen as float [V * NL][2 nx] with box YBOXW x YBOX; hstride = elements
+// between hologram rows.
 template <typename TIn>
-__device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *__restrict__ holo,
+__device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, long long hstride,
                                             unsigned tq, const float2 (&tw)[TWN], const void *tmB,
                                             Range rg) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, quad = warp >> 2, b = warp & 3;
@@ -305,7 +306,7 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *__restri
     const bool leader = threadIdx.x == 0;  // issues and retires the bulk stores
     {
         SubRegs<TIn> t;
-        sub_load<TIn>(t, holo, SubSlab<TIn>::col(rg.u0, quad), qt);
+        sub_load<TIn>(t, holo, hstride, SubSlab<TIn>::col(rg.u0, quad), qt);
         sub_store(t, sm.tile[quad], qt, quad);
     }
     quad_sync(quad);
@@ -337,7 +338,7 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *__restri
             }
             // the next sub-slab is fetched behind the tile reads of the unit's last column: its
             // loads touch one row per lane (32 wavefronts each)
-            if (cc == 1 && next_slab) sub_load<TIn>(t, holo, SubSlab<TIn>::col(u + 1, quad), qt);
+            if (cc == 1 && next_slab) sub_load<TIn>(t, holo, hstride, SubSlab<TIn>::col(u + 1, quad), qt);
             quad_sync(quad);  // the previous column's exchange area has been read by all four warps
             branch<false>(v, lane, xb, tw, tq + TQ_H, turns);
             // the previous unit's bulk stores must have left the staging tile before it is rewritten

@@ -33,8 +33,21 @@ def test_version_and_error_strings():
     assert B.sfd_launch_count() == 0 or torch.cuda.is_available()
 
 
+@pytest.mark.parametrize("N", [100, 32, 4096, 1000])
+def test_sizes_without_kernels_are_unsupported_not_invalid(N):
+    """A grid side this build has no kernels for is a valid request that is not implemented."""
+    with pytest.raises(B.SfdError) as e:
+        B.sfd_plan_create(N, 1, W.LAMBDA, [W.PITCH], [W.PITCH], [0.05], [0.0], [0.0], B.SFD_F32)
+    assert e.value.code == B.SFD_EUNSUPPORTED
+    one = [W.PITCH]
+    with pytest.raises(B.SfdError) as e:
+        B.sfd_plan_create_rect(64, N, 1, W.LAMBDA, one, one, one, one, [0.05], [0.0], [0.0], [0.0], [0.0],
+                               B.SFD_F32)
+    assert e.value.code == B.SFD_EUNSUPPORTED
+
+
 @pytest.mark.parametrize("bad", [
-    dict(N=100), dict(N=32), dict(N=4096), dict(n_views=0), dict(lam=0.0), dict(lam=-1e-6),
+    dict(N=0), dict(N=-64), dict(n_views=0), dict(lam=0.0), dict(lam=-1e-6),
     dict(p1=[0.0]), dict(p2=[-1e-6]), dict(z=[0.0]), dict(z=[float("nan")]), dict(z=[float("inf")]),
     dict(Ox=[float("nan")]), dict(in_dtype=7),
 ])
@@ -114,7 +127,7 @@ def test_host_tables_general_match_oracle_tables(N, p1, p2, z, off0, off):
 
 
 @pytest.mark.parametrize("bad", [
-    dict(N=96), dict(n_views=0), dict(p1y=[0.0]), dict(p2x=[float("nan")]), dict(z=[0.0]),
+    dict(N=0), dict(n_views=0), dict(p1y=[0.0]), dict(p2x=[float("nan")]), dict(z=[0.0]),
     dict(O0x=[float("inf")]), dict(O1y=[float("nan")]), dict(in_dtype=-1),
 ])
 def test_general_plan_create_rejects_bad_arguments(bad):
@@ -135,3 +148,47 @@ def test_new_entry_points_reject_null():
     assert B._lib.sfd_plan_create_general(None, 64, 1, 1e-6, *([None] * 9), 0) == B.SFD_EINVAL
     with pytest.raises(B.SfdError):
         B.sfd_host_tables_general(100, W.LAMBDA, W.PITCH, W.PITCH, 0.05, 0.0, 0.0)
+
+
+def test_round2_entry_points_reject_null_and_bad_arguments():
+    assert B._lib.sfd_plan_create_rect(None, 64, 128, 1, 1e-6, *([None] * 9), 0) == B.SFD_EINVAL
+    assert B._lib.sfd_plan_set_input_window(None, 0, 0, 0) == B.SFD_EINVAL
+    assert B._lib.sfd_plan_update_view_async(None, 0, 1e-6, 1e-6, 0.1, 0.0, 0.0, None) == B.SFD_EINVAL
+    assert B._lib.sfd_plan_update_view_general_async(None, 0, *([1e-6] * 4), 0.1, 0.0, 0.0, 0.0, 0.0,
+                                                     None) == B.SFD_EINVAL
+    assert B._lib.sfd_plan_last_update_host_ms(None) == -1.0
+    assert B._lib.sfd_plan_get_nx(None) == B.SFD_EINVAL and B._lib.sfd_plan_get_ny(None) == B.SFD_EINVAL
+    assert B._lib.sfd_plan_get_device(None) == B.SFD_EINVAL
+    assert B._lib.sfd_measure_pipes(None) == B.SFD_EINVAL
+    assert B._lib.sfd_host_dft32(None, None, 0, 0) == B.SFD_EINVAL
+    with pytest.raises(B.SfdError):
+        B.sfd_host_dft32(np.zeros(32, np.complex64), lane=32)
+
+
+def test_binding_loads_only_the_in_tree_library(monkeypatch):
+    """No environment override: the product imports paper_1001_4309_b200/libsfd.so and nothing else."""
+    assert B.LIB_PATH.name == "libsfd.so" and B.LIB_PATH.parent.name == "paper_1001_4309_b200"
+    import inspect
+    assert "environ" not in inspect.getsource(B)
+
+
+@pytest.mark.parametrize("lane", [0, 1, 13, 31])
+def test_host_butterflies_equal_the_dft(lane):
+    """Host logic pin of the register butterflies the warp kernels run (sfd_dft32.cuh: FMA-formulated
+    radix-2 stages, sign tracking, inter-stage twiddles folded into stage B): stepped on the CPU they
+    must equal the plain 32-point DFT (numpy) resp. the DFT of the twiddled input, to fp32 rounding."""
+    rng = np.random.default_rng(100 + lane)
+    x = (rng.standard_normal(32) + 1j * rng.standard_normal(32)).astype(np.complex64)
+    r = np.arange(32)
+    a = B.sfd_host_dft32(x, lane, twiddled=False)
+    want = np.fft.fft(x.astype(np.complex128))
+    assert np.linalg.norm(a - want) / np.linalg.norm(want) < 3e-7
+    b = B.sfd_host_dft32(x, lane, twiddled=True)
+    want = np.fft.fft(x.astype(np.complex128) * np.exp(-2j * np.pi * r * lane / 1024))
+    assert np.linalg.norm(b - want) / np.linalg.norm(want) < 3e-7
+    # a delta at input r gives the r-th row of the DFT matrix: every twiddle index is exercised
+    for r0 in (1, 5, 16, 31):
+        e = np.zeros(32, np.complex64)
+        e[r0] = 1
+        got = B.sfd_host_dft32(e, lane, twiddled=True)
+        assert np.max(np.abs(got - np.exp(-2j * np.pi * (r0 * lane / 1024 + r0 * r / 32)))) < 3e-7

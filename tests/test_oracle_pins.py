@@ -328,3 +328,30 @@ def test_focus_moments_closed_forms():
     m = O.focus_moments(img)
     assert m[0, 0] == 40.0 and m[0, 1] == 8 * 9 + 8 * 4
     assert np.isclose(O.normalised_variance(m, 16)[0], 16 * 104 / 1600 - 1)
+
+
+def test_crop_window_reading_13():
+    """PAPER.md L42 / reading 13: the 1 360 x 1 024 frame is cropped to its central 1 024 columns; a
+    window moved off centre by (dr, dc) samples equals the centred transform of the same samples with
+    the hologram-window offset O_0 = (dc p, dr p) (the physical positions of the samples are what count)."""
+    rng = np.random.default_rng(3)
+    frame = rng.integers(0, 256, (1024, 1360), dtype=np.uint8)
+    w = O.crop_window(frame, 1024, 1024)
+    assert w.shape == (1024, 1024) and np.array_equal(w, frame[:, 168:1192])
+    assert np.array_equal(O.crop_window(frame, 64, 32, 5, 7), frame[5:69, 7:39])
+    with pytest.raises(ValueError):
+        O.crop_window(frame, 1024, 1024, 1, 0)
+    # physics: a 24 x 40 frame, window 16 x 16 moved by (dr, dc) = (3, -5) off centre
+    small = rng.random((24, 40))
+    lam, z, p = 632.8e-9, 0.004, 4.65e-6
+    dr, dc = 3, -5
+    win = O.crop_window(small, 16, 16, (24 - 16) // 2 + dr, (40 - 16) // 2 + dc)
+    got = O.separable_matrices(win, lam, z, p, 2e-6, O1=(1e-5, -2e-5), O0=(dc * p, dr * p))
+    # the same samples placed at their physical positions inside a zero frame, centred transform,
+    # evaluated on the same output window
+    big = np.zeros((24, 40))
+    big[4 + dr:20 + dr, 12 + dc:28 + dc] = win
+    Kx = O.fresnel_matrix(40, lam, z, p, 2e-6, 0.0, 1e-5 + (40 - 16) / 2 * 2e-6)[:16]
+    Ky = O.fresnel_matrix(24, lam, z, p, 2e-6, 0.0, -2e-5 + (24 - 16) / 2 * 2e-6)[:16]
+    want = O.c0_factor(lam, z, p, p) * (Ky @ big @ Kx.T)
+    assert np.linalg.norm(got - want) / np.linalg.norm(want) < 1e-12
