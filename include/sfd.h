@@ -52,6 +52,7 @@ typedef struct sfd_plan sfd_plan; /* opaque */
 /* hologram sample types (argument in_dtype) */
 #define SFD_U8 0  /* unsigned 8-bit CCD samples; the method sees value/255 (reading 12) */
 #define SFD_F32 1 /* float32 samples used as they are */
+#define SFD_C64 2 /* complex64 samples (re, im interleaved); angular-spectrum plans only */
 
 /* Create a plan for one hologram size and a fixed set of views (S = p1 p2/(lambda z);
  * Eq.(2)-(4)).  Builds, in float64 on the host, the 1-D chirp tables of Eq.(2)-(3) and the spectrum
@@ -235,6 +236,35 @@ SFD_API int sfd_measure_pipes(double out[4]);
 /* The same for a hologram window shifted by off0 along that axis (general geometry). */
 SFD_API int sfd_host_tables_general(int N, double lambda, double p1, double p2, double z, double off0,
                                     double off, double *pre, double *post, double *H);
+
+/* ---- angular-spectrum propagation -------------------------------------------
+ * Digital holographic microscopy observes "both the amplitude and phase of a specimen".
+ * Next to the paper's Shifted-Fresnel transform the library carries the exact (non-paraxial)
+ * propagator that SURVEY.md 8(d) uses to define the synthetic holograms:
+ *
+ *     u(z) = IFFT2[ FFT2[u0] * H ],   H(fx, fy) = exp(i 2 pi z sqrt(1/lambda^2 - fx^2 - fy^2)),
+ *
+ * on the periodic Ny x Nx grid of pitch (px, py) - a circular convolution, no padding; the caller pads
+ * if wrap-around matters.  fx = kx/(Nx px) with bins kx >= Nx/2 negative; components with
+ * fx^2 + fy^2 >= 1/lambda^2 (evanescent) are set to zero; band_limit != 0 also zeroes, per axis,
+ * |f| > 1/(lambda sqrt((2 z/(N p))^2 + 1)).  One plan holds n_planes depths z[] of one input: the row
+ * transform of the input is shared, H is cached per plane (built on the device in float64 at plan
+ * creation, 8 bytes per sample and plane).  The same fp32 line-FFT kernels as the generic Fresnel
+ * path, three launches per call.
+ *   Nx, Ny     powers of two in 128..4096 (else SFD_EUNSUPPORTED); z[] finite, any sign, 0 allowed.
+ *   in_dtype   SFD_F32 (real input) or SFD_C64.
+ * sfd_asm_execute: u0_dev [Ny][Nx] of in_dtype; outputs [n_planes][Ny][Nx]: field_dev complex64,
+ * intensity_dev float32 = |u|^2, phase_dev float32 = atan2(im, re) in (-pi, pi]; each may be NULL, not
+ * all three.  Asynchronous on `stream`; one execute in flight per plan.
+ * Errors: SFD_EINVAL, SFD_EUNSUPPORTED, SFD_ENOMEM, SFD_ECUDA (text: sfd_asm_last_cuda_error). */
+typedef struct sfd_asm_plan sfd_asm_plan; /* opaque */
+SFD_API int sfd_asm_plan_create(sfd_asm_plan **out, int Nx, int Ny, int n_planes, double lambda,
+                                double px, double py, const double *z, int in_dtype, int band_limit);
+SFD_API int sfd_asm_execute(sfd_asm_plan *plan, const void *u0_dev, void *field_dev,
+                            float *intensity_dev, float *phase_dev, void *stream);
+SFD_API int sfd_asm_plan_destroy(sfd_asm_plan *plan);
+SFD_API long long sfd_asm_plan_device_bytes(const sfd_asm_plan *plan);
+SFD_API const char *sfd_asm_last_cuda_error(void);
 
 /* Static description of an error code / of the last CUDA error seen by this thread. */
 SFD_API const char *sfd_error_string(int code);

@@ -19,7 +19,7 @@ LIB_PATH = _PKG / "libsfd.so"        # the in-tree build, nothing else
 HEADER_PATH = _PKG.parent / "include" / "sfd.h"
 
 SFD_OK, SFD_EINVAL, SFD_ENOMEM, SFD_ECUDA, SFD_EUNSUPPORTED = 0, -1, -2, -3, -4
-SFD_U8, SFD_F32 = 0, 1
+SFD_U8, SFD_F32, SFD_C64 = 0, 1, 2
 SFD_KERNELS_AUTO, SFD_KERNELS_GENERIC = 0, 1
 
 if not LIB_PATH.exists():
@@ -48,6 +48,12 @@ _sig = {
     "sfd_plan_get_device": (C.c_int, [_vp]),
     "sfd_host_dft32": (C.c_int, [C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_int, C.c_int]),
     "sfd_measure_pipes": (C.c_int, [_dp]),
+    "sfd_asm_plan_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
+                                      C.c_double, _dp, C.c_int, C.c_int]),
+    "sfd_asm_execute": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
+    "sfd_asm_plan_destroy": (C.c_int, [_vp]),
+    "sfd_asm_plan_device_bytes": (C.c_longlong, [_vp]),
+    "sfd_asm_last_cuda_error": (C.c_char_p, []),
     "sfd_host_tables_general": (C.c_int, [C.c_int] + [C.c_double] * 6 + [_dp, _dp, _dp]),
     "sfd_execute": (C.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "sfd_execute_u8": (C.c_int, [_vp, _vp, _vp, _vp]),
@@ -313,6 +319,79 @@ def sfd_host_tables_general(N, lam, p1, p2, z, off0, off):
                                       post.ctypes.data_as(_dp), H.ctypes.data_as(_dp)),
          "sfd_host_tables_general")
     return pre, post, H
+
+
+def sfd_asm_plan_create(Nx, Ny, n_planes, lam, px, py, z, in_dtype=SFD_C64, band_limit=False):
+    """Angular-spectrum plan (include/sfd.h); returns the opaque handle."""
+    zz = _darr(z, n_planes)
+    h = _vp()
+    code = _lib.sfd_asm_plan_create(C.byref(h), int(Nx), int(Ny), int(n_planes), float(lam), float(px),
+                                    float(py), zz.ctypes.data_as(_dp), int(in_dtype), int(bool(band_limit)))
+    if code == SFD_ECUDA:
+        raise SfdError(code, "sfd_asm_plan_create: " + _lib.sfd_asm_last_cuda_error().decode())
+    _chk(code, "sfd_asm_plan_create")
+    return h.value
+
+
+def sfd_asm_execute(plan, u0_dev, field_dev, intensity_dev, phase_dev, stream=None):
+    code = _lib.sfd_asm_execute(plan, _ptr(u0_dev), _ptr(field_dev), _ptr(intensity_dev),
+                                _ptr(phase_dev), _stream(stream))
+    if code == SFD_ECUDA:
+        raise SfdError(code, "sfd_asm_execute: " + _lib.sfd_asm_last_cuda_error().decode())
+    _chk(code, "sfd_asm_execute")
+
+
+def sfd_asm_plan_destroy(plan):
+    _chk(_lib.sfd_asm_plan_destroy(plan), "sfd_asm_plan_destroy")
+
+
+def sfd_asm_plan_device_bytes(plan):
+    return int(_lib.sfd_asm_plan_device_bytes(plan))
+
+
+def sfd_asm_last_cuda_error():
+    return _lib.sfd_asm_last_cuda_error().decode()
+
+
+class AsmPlan:
+    """Angular-spectrum plan: ``AsmPlan(Nx, Ny, lam, pitch, z=[...], in_dtype=SFD_C64, band_limit=False)``;
+    ``pitch`` a scalar or ``(px, py)``.  Allocation of outputs is the only thing it adds."""
+
+    def __init__(self, Nx, Ny, lam, pitch, z, in_dtype=SFD_C64, band_limit=False):
+        px, py = (pitch, pitch) if np.ndim(pitch) == 0 else pitch
+        self.Nx, self.Ny, self.P, self.in_dtype = int(Nx), int(Ny), len(np.atleast_1d(z)), int(in_dtype)
+        self.handle = sfd_asm_plan_create(Nx, Ny, self.P, lam, px, py, z, in_dtype, band_limit)
+
+    def close(self):
+        if self.handle:
+            sfd_asm_plan_destroy(self.handle)
+            self.handle = None
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def execute(self, u0, field=True, intensity=True, phase=True, stream=None):
+        """Returns ``(field complex64, intensity float32, phase float32)``, each ``[P, Ny, Nx]`` or None."""
+        import torch
+        want = torch.float32 if self.in_dtype == SFD_F32 else torch.complex64
+        if (u0.dtype != want or tuple(u0.shape) != (self.Ny, self.Nx) or not u0.is_cuda
+                or not u0.is_contiguous()):
+            raise ValueError(f"input must be a contiguous CUDA tensor [{self.Ny},{self.Nx}] {want}")
+        shape = (self.P, self.Ny, self.Nx)
+        f = torch.empty(shape, dtype=torch.complex64, device=u0.device) if field else None
+        I = torch.empty(shape, dtype=torch.float32, device=u0.device) if intensity else None
+        ph = torch.empty(shape, dtype=torch.float32, device=u0.device) if phase else None
+        sfd_asm_execute(self.handle, u0, f, I, ph, stream)
+        return f, I, ph
+
+    @property
+    def device_bytes(self):
+        return sfd_asm_plan_device_bytes(self.handle)
 
 
 # ---- convenience wrapper: owns the handle, allocates outputs with torch --------------------------

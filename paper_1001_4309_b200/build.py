@@ -16,7 +16,7 @@ PKG = pathlib.Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libsfd.so"
-SOURCES = [CSRC / "sfd_kernels.cu", CSRC / "sfd_plan.cpp"]
+SOURCES = [CSRC / "sfd_kernels.cu", CSRC / "sfd_asm.cu", CSRC / "sfd_plan.cpp"]
 HEADERS = [CSRC / "sfd_fft_core.cuh", CSRC / "sfd_dft32.cuh", CSRC / "sfd_warp1024.cuh", CSRC / "sfd_warp2048.cuh", CSRC / "sfd_internal.h", ROOT / "include" / "sfd.h"]
 
 NVCC_FLAGS = [

@@ -154,6 +154,18 @@ template <int LOG2M> struct Sched {
     static constexpr int PADDED = M + M / 16;  // shared-memory elements per line (1 pad per 16)
 };
 
+// CTA shapes of the generic kernels: columns per CTA in a column pass / rows per CTA in a row pass,
+// by transform length M = 2^LOG2M
+template <int LOG2M> struct Tile {
+    static constexpr int T = Sched<LOG2M>::T;
+    static constexpr int C = LOG2M <= 7 ? 16 : LOG2M <= 9 ? 8 : LOG2M <= 11 ? 4 : 2;
+    static constexpr int RPC = T >= 128 ? 1 : 128 / T;
+    static constexpr int THREADS_Y = C * T;
+    static constexpr int THREADS_X = RPC * T;
+    static constexpr size_t SMEM_Y = sizeof(float2) * Sched<LOG2M>::PADDED * C;
+    static constexpr size_t SMEM_X = sizeof(float2) * Sched<LOG2M>::PADDED * RPC;
+};
+
 // Shared-memory view of one line: element pos of the line lives at base[(pos + pos/16) * ISTR].
 template <int ISTR> struct LineSmem {
     float2 *base;

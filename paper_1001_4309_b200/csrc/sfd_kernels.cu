@@ -24,17 +24,6 @@ namespace {
 
 using namespace sfd;
 
-// columns per CTA in pass y / rows per CTA in pass x, by padded length
-template <int LOG2M> struct Tile {
-    static constexpr int T = Sched<LOG2M>::T;
-    static constexpr int C = LOG2M <= 7 ? 16 : LOG2M <= 9 ? 8 : LOG2M <= 11 ? 4 : 2;
-    static constexpr int RPC = T >= 128 ? 1 : 128 / T;
-    static constexpr int THREADS_Y = C * T;
-    static constexpr int THREADS_X = RPC * T;
-    static constexpr size_t SMEM_Y = sizeof(float2) * Sched<LOG2M>::PADDED * C;
-    static constexpr size_t SMEM_X = sizeof(float2) * Sched<LOG2M>::PADDED * RPC;
-};
-
 // tables of one axis as the generic kernels see them: view v at base + v * vstride
 struct AxisTabs {
     const float2 *base;

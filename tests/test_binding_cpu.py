@@ -192,3 +192,23 @@ def test_host_butterflies_equal_the_dft(lane):
         e[r0] = 1
         got = B.sfd_host_dft32(e, lane, twiddled=True)
         assert np.max(np.abs(got - np.exp(-2j * np.pi * (r0 * lane / 1024 + r0 * r / 32)))) < 3e-7
+
+
+@pytest.mark.parametrize("bad,code", [
+    (dict(Nx=100), B.SFD_EUNSUPPORTED), (dict(Ny=64), B.SFD_EUNSUPPORTED), (dict(Nx=8192), B.SFD_EUNSUPPORTED),
+    (dict(Nx=0), B.SFD_EINVAL), (dict(lam=0.0), B.SFD_EINVAL), (dict(px=-1e-6), B.SFD_EINVAL),
+    (dict(z=[float("nan")]), B.SFD_EINVAL), (dict(in_dtype=B.SFD_U8), B.SFD_EINVAL),
+])
+def test_asm_plan_create_rejects_bad_arguments(bad, code):
+    kw = dict(Nx=128, Ny=128, lam=W.LAMBDA, px=W.PITCH, py=W.PITCH, z=[0.05], in_dtype=B.SFD_C64)
+    kw.update(bad)
+    with pytest.raises(B.SfdError) as e:
+        B.sfd_asm_plan_create(kw["Nx"], kw["Ny"], 1, kw["lam"], kw["px"], kw["py"], kw["z"], kw["in_dtype"])
+    assert e.value.code == code
+
+
+def test_asm_entry_points_reject_null():
+    assert B._lib.sfd_asm_plan_create(None, 128, 128, 1, 1e-6, 1e-6, 1e-6, None, 2, 0) == B.SFD_EINVAL
+    assert B._lib.sfd_asm_execute(None, None, None, None, None, None) == B.SFD_EINVAL
+    assert B._lib.sfd_asm_plan_destroy(None) == B.SFD_OK
+    assert B._lib.sfd_asm_plan_device_bytes(None) == B.SFD_EINVAL

@@ -1,0 +1,114 @@
+"""GPU parity of angular-spectrum propagation: sfd_asm_* through the C ABI against
+the float64 oracle (oracle/angular_spectrum.py), element by element, at the north_star tolerance
+(rel-L2 <= 2e-5, max |du| <= 1e-4 max|u| per plane; phase to 2e-4 rad where |u| is not small)."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import angular_spectrum as A
+from paper_1001_4309_b200 import build as sfd_build
+from paper_1001_4309_b200 import workloads as W
+
+sfd_build.build()
+from paper_1001_4309_b200 import binding as B  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+REL_L2, REL_MAX = 2e-5, 1e-4
+
+
+def _dev():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (no CPU fallback exists)"
+    return torch.device("cuda:0")
+
+
+def _check(f, I, ph, want, what):
+    for p in range(want.shape[0]):
+        d = f[p].astype(np.complex128) - want[p]
+        l2 = np.linalg.norm(d) / np.linalg.norm(want[p])
+        mx = np.abs(d).max() / np.abs(want[p]).max()
+        assert l2 <= REL_L2 and mx <= REL_MAX, f"{what} plane {p}: rel-L2 {l2:.2e}, max {mx:.2e}"
+        Iw = A.intensity(want[p])
+        assert np.abs(I[p] - Iw).max() <= REL_MAX * Iw.max()
+        big = np.abs(want[p]) > 0.05 * np.abs(want[p]).max()
+        dphi = np.angle(np.exp(1j * (ph[p] - A.phase(want[p]))))        # wrapped difference
+        assert np.abs(dphi[big]).max() < 2e-4, f"{what} plane {p}: phase off by {np.abs(dphi[big]).max():.2e}"
+        assert ph[p].min() >= -math.pi - 1e-6 and ph[p].max() <= math.pi + 1e-6
+
+
+@pytest.mark.parametrize("Nx,Ny,dtype,pitch,zs,bl", [
+    (128, 128, B.SFD_C64, W.PITCH, [0.01, -0.02], False),
+    (256, 128, B.SFD_F32, (3.0e-6, 5.0e-6), [0.004, 0.05, 0.0], False),      # rectangular, anisotropic, z = 0
+    (512, 1024, B.SFD_C64, W.PITCH, [0.08], True),                           # band limit active
+    (1024, 1024, B.SFD_C64, W.PITCH, [0.08, -0.06], False),
+    (2048, 2048, B.SFD_F32, W.PITCH, [0.08], True),                          # the hologram generator's grid
+    (4096, 2048, B.SFD_C64, 0.4e-6, [20e-6], False),                         # evanescent bins (pitch < lambda/2 .. )
+])
+def test_asm_against_oracle(Nx, Ny, dtype, pitch, zs, bl):
+    rng = np.random.default_rng(Nx + Ny)
+    if dtype == B.SFD_F32:
+        u0 = rng.random((Ny, Nx), dtype=np.float32)
+        u0[Ny - 1, Nx - 1] = 9.0
+    else:
+        u0 = (rng.standard_normal((Ny, Nx)) + 1j * rng.standard_normal((Ny, Nx))).astype(np.complex64)
+        u0[Ny - 1, Nx - 1] = 9.0 - 4.0j
+        u0[0, Nx - 2] = -7.0j
+    with B.AsmPlan(Nx, Ny, W.LAMBDA, pitch, zs, dtype, bl) as plan:
+        n0 = B.sfd_launch_count()
+        f, I, ph = plan.execute(torch.from_numpy(u0).to(_dev()))
+        torch.cuda.synchronize()
+        assert B.sfd_launch_count() - n0 == 3
+        assert plan.device_bytes > 0
+    want, _, _ = A.propagate_planes(u0, W.LAMBDA, zs, pitch, bl)
+    _check(f.cpu().numpy(), I.cpu().numpy(), ph.cpu().numpy(), want, f"{Nx}x{Ny}")
+
+
+def test_plane_wave_eigenvalue_on_gpu_output():
+    """The oracle's pin applied to the CUDA path: a plane wave comes back multiplied by the analytic H."""
+    N, kx, ky, z = 256, 200, 17, 0.031
+    n, m = np.mgrid[0:N, 0:N]
+    u0 = np.exp(2j * np.pi * (kx * m / N + ky * n / N)).astype(np.complex64)
+    with B.AsmPlan(N, N, W.LAMBDA, W.PITCH, [z]) as plan:
+        f, _, _ = plan.execute(torch.from_numpy(u0).to(_dev()), intensity=False, phase=False)
+        torch.cuda.synchronize()
+    fx, fy = (kx - N) / (N * W.PITCH), ky / (N * W.PITCH)
+    cyc = z * math.sqrt(1 / W.LAMBDA ** 2 - fx * fx - fy * fy)
+    eig = np.exp(2j * np.pi * (cyc - round(cyc)))
+    assert np.abs(f[0].cpu().numpy() - eig * u0.astype(np.complex128)).max() < 2e-5
+
+
+def test_gabor_hologram_generator_on_the_gpu():
+    """What row f4 is for: the synthetic-hologram recipe of SURVEY.md 8(d) (object transmittance t on a 2N
+    grid, u = ASM(t - 1), I = |1 + u|^2) with the propagation done by the library, against the oracle."""
+    N, z = 512, 0.05
+    rng = np.random.default_rng(12)
+    t = np.ones((2 * N, 2 * N), np.float32)
+    for _ in range(12):
+        cy, cx, r = rng.integers(N // 2, 3 * N // 2, 2).tolist() + [int(rng.integers(2, 9))]
+        yy, xx = np.ogrid[-r:r + 1, -r:r + 1]
+        t[cy - r:cy + r + 1, cx - r:cx + r + 1][yy * yy + xx * xx <= r * r] = 0.0
+    with B.AsmPlan(2 * N, 2 * N, W.LAMBDA, W.PITCH, [z], B.SFD_F32, band_limit=True) as plan:
+        f, _, _ = plan.execute(torch.from_numpy(t - 1.0).to(_dev()), intensity=False, phase=False)
+        I = (1.0 + f[0]).abs().square()[N // 2:N // 2 + N, N // 2:N // 2 + N]
+        torch.cuda.synchronize()
+    u = A.propagate((t - 1.0).astype(np.float64), W.LAMBDA, z, W.PITCH, band_limit=True)
+    Iw = np.abs(1.0 + u[N // 2:N // 2 + N, N // 2:N // 2 + N]) ** 2
+    assert np.abs(I.cpu().numpy() - Iw).max() < 1e-4 * Iw.max()
+    g8, w8 = np.rint(255 * I.cpu().numpy() / I.max().item()), np.rint(255 * Iw / Iw.max())
+    assert np.abs(g8 - w8).max() <= 1 and (g8 != w8).mean() < 1e-3
+
+
+def test_asm_outputs_optional_and_reusable():
+    N = 128
+    u0 = torch.randn(N, N, dtype=torch.complex64, device=_dev())
+    with B.AsmPlan(N, N, W.LAMBDA, W.PITCH, [0.02]) as plan:
+        f, I, ph = plan.execute(u0)
+        f2, none_i, none_p = plan.execute(u0, intensity=False, phase=False)
+        none_f, I2, ph2 = plan.execute(u0, field=False)
+        torch.cuda.synchronize()
+        assert none_i is None and none_p is None and none_f is None
+        assert torch.equal(f, f2) and torch.equal(I, I2) and torch.equal(ph, ph2)
+        with pytest.raises(B.SfdError) as e:
+            plan.execute(u0, field=False, intensity=False, phase=False)
+        assert e.value.code == B.SFD_EINVAL
