@@ -2,6 +2,10 @@
 """bench.py — throughput of the Shifted-Fresnel hot path on B200 (BASELINE.json `metric`).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl sfd|reference] [--config 1|2|4]
+    python bench.py --peaks          # measured pipe rates of this GPU (sfd_measure_pipes), one JSON line
+
+Started bare with --gpus N > 1 (no WORLD_SIZE in the environment) it launches its N ranks itself, one
+process per GPU, rendezvous on 127.0.0.1; under torchrun it is one of the ranks.
 
 A *step* is one pass of the whole hot path (convert, pre-chirp,
 zero-pad, forward FFT, kernel-spectrum multiply, inverse FFT, crop, post-chirp, |u|^2) over one
@@ -13,8 +17,12 @@ Own arm (`--impl sfd`, default)
   value      reconstructions/s (views/s) with inputs resident in HBM; K back-to-back steps timed
              with one CUDA-event pair on the launching stream, max over ranks.  The R input/output
              buffer sets the steps rotate through are larger than L2 together.
-  roofline   the dominant kernel's algorithmic bytes / its mean CUDA-event duration, against the
-             measured HBM copy bandwidth of MEASURED_PEAKS.json, plus an ALU-side figure.
+  roofline   the dominant kernel's nominal flops / its mean CUDA-event duration against the fp32 FMA
+             rate MEASURED on this GPU in the same run (sfd_measure_pipes), with the HBM figures
+             (algorithmic bytes against MEASURED_PEAKS.json) beside it; traffic from profiles/.
+  clocks     SM clock, throttle reasons and power sampled through NVML during a block of >= 0.5 s of
+             the same steps run right before the timed region (and during the timed region itself
+             when that is long enough to be seen by a 5 ms sampler).
   e2e        the same metric through `sfd_stream_run`: pinned HOST holograms in, 8-bit intensity
              images in pinned HOST memory out, H2D + kernels + D2H all inside the timed region.
   cpu_baseline  the float64 oracle (form B) on the host cores, bounded sample (N=1, rank 0 only).
@@ -27,6 +35,8 @@ import argparse
 import json
 import os
 import pathlib
+import socket
+import subprocess
 import sys
 import threading
 import time
@@ -50,7 +60,12 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="sfd", choices=["sfd", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=[1, 2, 4])
-    ap.add_argument("--e2e-frames", type=int, default=128)
+    ap.add_argument("--e2e-frames", type=int, default=256,
+                    help="frames of the real-time stream (BASELINE.json configs[3]: 256)")
+    ap.add_argument("--peaks", action="store_true",
+                    help="print the measured pipe rates of this GPU (sfd_measure_pipes) and exit")
+    ap.add_argument("--no-extras", action="store_true",
+                    help="skip the secondary measurements (live steering, angular spectrum)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--kernels", default="auto", choices=["auto", "generic"],
@@ -60,9 +75,21 @@ def parse_args():
     return ap.parse_args()
 
 
-def fp32_floor_us(N, V, sms=148, ghz=1.965):
-    """Time one pass of the warp-per-branch kernels needs if the fp32 pipes never idle (us)."""
-    return V * N * (N // 512) * 2730.0 / (4 * sms) / (ghz * 1e3)
+def fp32_floor_us(N, V, cycles_per_branch, sms=148, ghz=1.965):
+    """Time one pass of the warp-per-branch kernels needs if the fp32 pipes never idle (us):
+    V N lines x N/512 branches, each `cycles_per_branch` pipe cycles of one of 4 x sms sub-partitions."""
+    return V * N * (N // 512) * cycles_per_branch / (4 * sms) / (ghz * 1e3)
+
+
+def ncu_traffic(workload, kernel):
+    """DRAM read + write bytes per launch of `kernel` from the committed ncu --set full capture
+    (profiles/r02_traffic.json, written from the capture named inside it); None if not recorded."""
+    f = ROOT / "profiles" / "r02_traffic.json"
+    try:
+        rec = json.loads(f.read_text())[workload][kernel]
+        return int(rec["dram_read_bytes"]) + int(rec["dram_write_bytes"]), rec.get("source")
+    except Exception:
+        return None, None
 
 
 def measured_peaks():
@@ -82,7 +109,7 @@ class ClockSampler(threading.Thread):
     REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
                0x4: "sw_power_cap", 0x80: "hw_power_brake_slowdown"}
 
-    def __init__(self, index, period=0.01):
+    def __init__(self, index, period=0.005):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples = []            # (t, sm_mhz, reasons bitmask, watts)
@@ -124,14 +151,17 @@ class ClockSampler(threading.Thread):
         if self.is_alive():
             self.join(timeout=2)
 
-    def summary(self, t0, t1):
+    def summary(self, t0, t1, fallback=None):
+        """Samples inside [t0, t1]; if the region is too short to hold two samples, those of the
+        `fallback` window (the sustained block of the same steps right before it) are reported."""
         if not self.ok:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "note": "NVML unavailable"}
         inside = [s for s in self.samples if t0 <= s[0] <= t1]
         note = "sampled inside the timed region"
-        if not inside:               # region shorter than one sampling period
-            inside = [s for s in self.samples if t0 - 0.5 <= s[0] <= t1 + 0.5] or self.samples
-            note = "timed region shorter than the sampling period; nearest samples under load"
+        if len(inside) < 2 and fallback is not None:
+            inside = [s for s in self.samples if fallback[0] <= s[0] <= fallback[1]]
+            note = ("timed region shorter than two sampling periods: samples of the sustained block of "
+                    "the same steps that ends where the timed region starts")
         mhz = sorted(s[1] for s in inside)
         bits = 0
         for s in inside:
@@ -169,6 +199,12 @@ def oracle_view_seconds(holo, wl, v):
     return time.perf_counter() - t0
 
 
+ORACLE_CAVEAT = ("the oracle does more work per reconstruction than the GPU path: float64, the paper's "
+                 "un-pruned 2-D 2N x 2N FFTs, chirp tables and kernel spectrum rebuilt for every view "
+                 "(steps (v)-(vi) every frame, as the paper's step list has it); the GPU path is fp32, "
+                 "pruned, and caches the tables per plan - a baseline, not a like-for-like comparison")
+
+
 def cpu_baseline(wl, holo, budget_s=12.0, max_views=400):
     from oracle import shifted_fresnel as O
     oracle_view_seconds(holo, wl, 0)                 # untimed warm-up (FFT plan cache, page faults)
@@ -179,12 +215,19 @@ def cpu_baseline(wl, holo, budget_s=12.0, max_views=400):
     return {"value": done / spent, "unit": UNIT, "cores": int(O.FFT_WORKERS), "kind": "oracle",
             "sample": f"{done} single-view reconstructions of {wl.name} (oracle form B, float64, "
                       f"scipy.fft workers={O.FFT_WORKERS}) in {spent:.2f} s after 1 warm-up",
+            "caveat": ORACLE_CAVEAT,
             "frames_per_s": done / spent / wl.n_views}
 
 
 def run_reference(args, info):
-    """Reference arm: the oracle, untuned, on the host cores; rank 0 only."""
+    """Reference arm: the oracle, untuned, on the host cores; rank 0 only (the other ranks join the
+    process group, meet rank 0 at a barrier and exit 0 without work)."""
+    from paper_1001_4309_b200 import dist as D
+    D.init(info, "gloo")
+    D.barrier(info)
     if not info.is_root:
+        D.barrier(info)
+        D.finalize(info)
         return 0
     from oracle import shifted_fresnel as O
     from paper_1001_4309_b200 import workloads as W
@@ -207,17 +250,20 @@ def run_reference(args, info):
               f"({t_total:.1f} s; capped at {budget:.0f} s)")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "ranks_joined": info.world,
         "steps": done, "steps_requested": args.steps, "warmup": min(args.warmup, 3),
         "ms_per_step": 1e3 * t_total / done, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": wl.name, "N": wl.N, "views": wl.n_views, "unit_per_step": 1},
         "frames_per_s": value / wl.n_views,
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": int(O.FFT_WORKERS),
-                         "kind": "oracle", "sample": sample},
+                         "kind": "oracle", "sample": sample, "caveat": ORACLE_CAVEAT},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+    D.barrier(info)
+    D.finalize(info)
     return 0
 
 
@@ -231,6 +277,9 @@ def run_sfd(args, info):
 
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py --impl sfd needs a CUDA device: the hot path has no CPU fallback")
+    if info.local_rank >= torch.cuda.device_count():
+        raise RuntimeError(f"rank {info.rank}: local rank {info.local_rank} but only "
+                           f"{torch.cuda.device_count()} CUDA device(s) visible")
     torch.cuda.set_device(info.local_rank)
     dev = torch.device("cuda", info.local_rank)
     D.init(info, "nccl")
@@ -255,6 +304,8 @@ def run_sfd(args, info):
     if args.kernels == "generic":
         plan.select_kernels(B.SFD_KERNELS_GENERIC)
     stream = torch.cuda.current_stream()
+    # measured pipe rates of this GPU (a few ms of FMA kernels), the roofline's denominator
+    pipe_tflops, cyc_a, cyc_b, pipe_ghz = B.sfd_measure_pipes()
     sampler = ClockSampler(torch.cuda._get_nvml_device_index(dev) if hasattr(
         torch.cuda, "_get_nvml_device_index") else info.local_rank)
     sampler.start()
@@ -263,30 +314,39 @@ def run_sfd(args, info):
         r = i % R
         B.sfd_execute(plan.handle, holos[r], fields[r], intens[r], stream)
 
+    def timed(n, first=0):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for i in range(n):
+            step(first + i)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3, t0, time.perf_counter()
+
     for i in range(max(args.warmup, 3)):
         step(i)
     torch.cuda.synchronize()
+    # sustained block: the same steps for >= 0.5 s with the clock sampler running, so that the clock
+    # record does not depend on the length of the timed region (a --steps 20 region lasts 1 ms)
+    probe, _, _ = timed(50)
+    n_sus = max(200, int(0.6 / (probe / 50)))
+    sec_sus, ts0, ts1 = timed(n_sus)
     D.barrier(info)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     n0 = B.sfd_launch_count()
-    t0 = time.perf_counter()
-    e0.record(stream)
-    for i in range(args.steps):
-        step(i)
-    e1.record(stream)
-    torch.cuda.synchronize()
-    t1 = time.perf_counter()
+    sec_rank, t0, t1 = timed(args.steps)
     launches = B.sfd_launch_count() - n0
     D.barrier(info)
-    sec_rank = e0.elapsed_time(e1) * 1e-3
-    clocks = sampler.summary(t0, t1)
+    clocks = sampler.summary(t0, t1, fallback=(ts0, ts1))
+    clocks["sustained_block"] = dict(sampler.summary(ts0, ts1), steps=n_sus, seconds=round(sec_sus, 4))
     units, sec, value = D.aggregate_throughput(info, args.steps * V, sec_rank, dev)
+    _, sec_s, value_sus = D.aggregate_throughput(info, n_sus * V, sec_sus, dev)
     launches_all = int(D.sum_over_ranks(info, launches, dev))
 
     # per-kernel CUDA-event durations (events recorded by the library around each kernel, on the
     # launching stream), same rotation, right after the timed region
     plan.set_timing(True)
-    ksteps = min(args.steps, 200)
+    ksteps = min(max(args.steps, 20), 200)
     kms = np.zeros(3)
     for i in range(ksteps):
         step(i)
@@ -297,7 +357,7 @@ def run_sfd(args, info):
     alg = algorithmic(N, V, in_bytes, want_field, True)
     peak, peak_src = measured_peaks()
     keys = ["k_pass_y", "k_pass_x"]                    # rows of algorithmic()
-    # the kernels that actually ran: N = 1024 has its own pair (sfd_plan_uses_warp_kernels)
+    # the kernels that actually ran: N = 1024 / 2048 have their own pair (sfd_plan_uses_warp_kernels)
     names = [f"k_cols_{wl.N}", f"k_rows_{wl.N}"] if plan.uses_warp_kernels else keys
     dom = int(np.argmax(kms[:2]))
     per_kernel = {}
@@ -310,23 +370,28 @@ def run_sfd(args, info):
             "gbs": round(alg[name]["bytes"] / dur / 1e9, 1) if dur > 0 else None,
             "hbm_frac": round(alg[name]["bytes"] / dur / 1e9 / peak, 4) if dur > 0 else None,
             "nominal_tflops": round(alg[name]["flops"] / dur / 1e12, 2) if dur > 0 else None,
-            "alu_frac": round(alg[name]["flops"] / dur / 1e12 / ALU_PEAK_TFLOPS, 4) if dur > 0 else None,
+            "alu_frac": round(alg[name]["flops"] / dur / 1e12 / pipe_tflops, 4) if dur > 0 else None,
         }
     dname = names[dom]
     step_bytes = alg["k_pass_y"]["bytes"] + alg["k_pass_x"]["bytes"]
+    traffic, traffic_src = ncu_traffic(wl.name, dname)
+    # pipe model of the warp-per-branch kernels with the butterfly cycles measured in this run: a
+    # 1024-point branch of a line = 2 stage-A + 2 stage-B butterflies + 3 table multiplies (4 operations
+    # per complex value; the pre-chirp of pass y multiplies a real sample: 2)
+    cyc_branch = [2 * cyc_a + 2 * cyc_b + 2 * 128 + 64, 2 * cyc_a + 2 * cyc_b + 3 * 128]
     # Binding roof: with the traffic cut to 28 MiB per view the path runs at
-    # ~16 flop/B, above the fp32 ridge (11.4 flop/B), so the plain fp32 pipe bounds it.  The HBM
+    # ~16 flop/B, above the fp32 ridge (11 flop/B), so the plain fp32 pipe bounds it.  The HBM
     # figures BASELINE.json's metric asks for are reported beside it under "hbm".
     roofline = {
         "bound": "alu", "kernel": dname, "achieved": per_kernel[dname]["nominal_tflops"],
-        "peak": round(ALU_PEAK_TFLOPS, 1), "unit": "TFLOP/s",
+        "peak": round(pipe_tflops, 2), "unit": "TFLOP/s",
         "frac": per_kernel[dname]["alu_frac"],
-        "peak_source": "derived: 148 SMs x 128 fp32 lanes x 2 flop x 1.965 GHz (DESIGN.md section 7)",
+        "peak_source": f"measured in this run: sfd_measure_pipes, {pipe_tflops:.2f} TFLOP/s of plain fp32 FMA "
+                       f"(2 flop each) over all SMs at {pipe_ghz:.3f} GHz; derived figure for comparison: "
+                       f"148 SMs x 128 lanes x 2 x 1.965 GHz = {ALU_PEAK_TFLOPS:.1f}",
+        "peak_derived": round(ALU_PEAK_TFLOPS, 1),
         "flops_model": "nominal 5 M log2 M per M-point FFT, M = 2N, two FFTs per line, + pointwise",
-        "traffic": NCU_TRAFFIC.get((wl.name, dname)),
-        "traffic_source": "profiles/ (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum, "
-                          "per launch, caches flushed by ncu before the launch)"
-        if NCU_TRAFFIC.get((wl.name, dname)) else None,
+        "traffic": traffic, "traffic_source": traffic_src,
         "hbm": {"kernel": dname, "achieved": per_kernel[dname]["gbs"], "peak": peak, "unit": "GB/s",
                 "frac": per_kernel[dname]["hbm_frac"], "peak_source": peak_src,
                 "algorithmic_bytes": alg[dname]["bytes"],
@@ -334,13 +399,14 @@ def run_sfd(args, info):
                          "gbs": round(step_bytes / (sec_rank / args.steps) / 1e9, 1),
                          "frac": round(step_bytes / (sec_rank / args.steps) / 1e9 / peak, 4)}},
         "kernels": per_kernel,
-        # measured pipe model of the warp-per-branch kernels: a 1024-point
-        # branch of a line costs 2730 fp32-pipe cycles of one of the 4 x 148 sub-partitions
-        "fp32_pipe": ({"floor_us_per_kernel": round(fp32_floor_us(N, V), 2),
-                       "frac": round(fp32_floor_us(N, V) / (1e3 * float(kms[dom])), 4),
-                       "model": "2730 pipe cycles per 1024-point branch and line (4 radix-32 butterflies of "
-                                "464 cycles, 2 twiddle and 3 table multiplies), N/512 branches per line, "
-                                "V N lines per kernel, 592 sub-partitions at 1.965 GHz"}
+        "fp32_pipe": ({"floor_us_per_kernel": [round(fp32_floor_us(N, V, c, plan_sms(torch, dev), pipe_ghz), 2)
+                                               for c in cyc_branch],
+                       "frac": round(fp32_floor_us(N, V, cyc_branch[dom], plan_sms(torch, dev), pipe_ghz)
+                                     / (1e3 * float(kms[dom])), 4),
+                       "cycles_stage_a": round(cyc_a, 1), "cycles_stage_b": round(cyc_b, 1),
+                       "model": "measured cycles of the two radix-32 butterfly stages (a warp alone on its "
+                                "sub-partition) x 2 each + table multiplies per 1024-point branch, N/512 "
+                                "branches per line, V N lines per kernel, 4 sub-partitions per SM"}
                       if plan.uses_warp_kernels else None),
         "timing": f"library CUDA events around each kernel on the launching stream, mean of "
                   f"{ksteps} steps after the timed region (kernel sum "
@@ -364,10 +430,20 @@ def run_sfd(args, info):
         u_all, s_max, e_val = D.aggregate_throughput(info, F * V, s, dev)
         e2e = {"value": e_val, "unit": UNIT, "h2d_bytes_per_step": N * N * in_bytes,
                "d2h_bytes_per_step": V * N * N, "frames": F, "frames_per_s": e_val / V,
+               "frames_are": f"{F} distinct pinned host frames = the seeded hologram of {wl.name} rolled by "
+                             "(11 f, 5 f) pixels (the path is data-oblivious; the 256 independently seeded "
+                             "frames of configs[3] take 8 min to generate and are covered by the parity test "
+                             "on 6 of them)",
                "api": f"sfd_stream_run: pinned host holograms -> double-buffered H2D -> {names[0]}, "
                       f"{names[1]}, k_quantise -> D2H of 8-bit intensity images to pinned host memory",
                "pcie_gbs_d2h": round(V * N * N * F / s / 1e9, 2),
                "warmup": "one untimed pass over the same ring of F pinned host frames"}
+        del hp, op
+
+    extras = None
+    if info.is_root and not args.no_extras:
+        extras = {"steering": steering(plan, wl, holos[0], stream, torch, B),
+                  "angular_spectrum": asm_line(wl, dev, torch, B, np)}
     sampler.stop()
 
     cpu = None
@@ -390,8 +466,10 @@ def run_sfd(args, info):
                          f"{R * set_bytes / 2**20:.0f} MiB > L2 ({L2_BYTES / 1e6:.0f} MB)",
                    "sharding": "whole frames per rank, no collective on the data path"},
         "frames_per_s": value / V,
+        "value_sustained": value_sus,
+        "sustained": f"{n_sus} steps in {sec_s:.3f} s right before the timed region, same loop",
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
-        "gpu_launches": launches_all,
+        "gpu_launches": launches_all, "extras": extras,
         "paper_context": "paper: 4 views in ~60 ms on four GTX 295 chips (66.7 reconstructions/s), "
                          "9542 ms on a Core2Quad; other hardware, context only",
     }
@@ -399,23 +477,121 @@ def run_sfd(args, info):
     return 0
 
 
-# ncu `--set full` DRAM traffic per launch (bytes), copied from profiles/ by hand after each capture;
-# key = (workload name, kernel).  Absent = null in the JSON line.
-NCU_TRAFFIC = {
-    # profiles/r01_final_launches.md (final round-1 kernels, config 2)
-    ("paper_4view_1024", "k_cols_1024"): 16894720 + 15644928,
-    ("paper_4view_1024", "k_rows_1024"): 33795584 + 3111168,
-    # profiles/r01_v9_config4.md (N = 2048 warp kernels, config 4)
-    ("scale_stress_2048", "k_cols_2048"): 10770688 + 533581050,
-    ("scale_stress_2048", "k_rows_2048"): 539547390 + 753424640,
-}
+def plan_sms(torch, dev):
+    return torch.cuda.get_device_properties(dev).multi_processor_count
+
+
+def steering(plan, wl, holo, stream, torch, B, frames=400, every=10):
+    """Row f1: what live steering costs.  A device-resident loop of sfd_execute_u8 (the real-time
+    mode's kernels) with and without an asynchronous update of one view every `every` frames."""
+    V = wl.n_views
+
+    def run(update):
+        out = None
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        host_ms = []
+        e0.record(stream)
+        for f in range(frames):
+            if update and f % every == 0:
+                v = (f // every) % V
+                plan.update_view_async(v, wl.p1[v], wl.p2[v], wl.z[v] * (1.0 + 1e-3 * (f % 7)), wl.Ox[v],
+                                       wl.Oy[v], stream)
+                host_ms.append(plan.last_update_host_ms)
+            out = plan.execute_u8(holo, out, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return frames / (e0.elapsed_time(e1) * 1e-3), host_ms
+
+    run(False)
+    plain, _ = run(False)
+    steered, host_ms = run(True)
+    for v in range(V):                                   # leave the plan as it was
+        plan.update_view(v, wl.p1[v], wl.p2[v], wl.z[v], wl.Ox[v], wl.Oy[v])
+    return {"frames_per_s_plain": round(plain, 1), "frames_per_s_steered": round(steered, 1),
+            "update_every_frames": every,
+            "host_build_ms": round(sum(host_ms) / len(host_ms), 3),
+            "api": "sfd_plan_update_view_async on the execute stream (float64 tables on the host into pinned "
+                   "staging, one H2D copy, no synchronisation) between sfd_execute_u8 calls"}
+
+
+def asm_line(wl, dev, torch, B, np, reps=200):
+    """Row f4: angular-spectrum propagations per second at the workload's size, complex64 in,
+    field + intensity + phase out, inputs resident, distinct buffers rotated through L2."""
+    N = wl.N
+    R = 6
+    u0 = [torch.randn(N, N, dtype=torch.complex64, device=dev) for _ in range(R)]
+    outs = [(torch.empty((1, N, N), dtype=torch.complex64, device=dev),
+             torch.empty((1, N, N), dtype=torch.float32, device=dev),
+             torch.empty((1, N, N), dtype=torch.float32, device=dev)) for _ in range(R)]
+    stream = torch.cuda.current_stream()
+    with B.AsmPlan(N, N, wl.lam, 4.65e-6, [0.08]) as plan:
+        for i in range(10):
+            B.sfd_asm_execute(plan.handle, u0[i % R], *outs[i % R], stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for i in range(reps):
+            B.sfd_asm_execute(plan.handle, u0[i % R], *outs[i % R], stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3 / reps
+    by = N * N * (8 + 8 + 8 + 8 + 8 + 8 + 8 + 4 + 4)     # in, A w/r, H, W w/r, field, intensity, phase
+    return {"propagations_per_s": round(1.0 / sec, 1), "us": round(sec * 1e6, 2), "N": N,
+            "algorithmic_bytes": by, "gbs": round(by / sec / 1e9, 1),
+            "api": "sfd_asm_execute: 3 launches (rows FFT, columns FFT x H x IFFT, rows IFFT + |u|^2 + arg u)"}
+
+
+def run_peaks():
+    import torch
+    from paper_1001_4309_b200 import binding as B
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --peaks needs a CUDA device")
+    B.sfd_measure_pipes()                                  # warm-up (clocks, instruction cache)
+    tf, ca, cb, ghz = B.sfd_measure_pipes()
+    hbm, src = measured_peaks()
+    print(json.dumps({"peaks": {"fp32_fma_tflops": round(tf, 2), "dft32_stage_a_cycles": round(ca, 1),
+                                "dft32_stage_b_cycles": round(cb, 1), "sm_ghz": round(ghz, 3),
+                                "fp32_derived_tflops": round(ALU_PEAK_TFLOPS, 1), "hbm_gbs": hbm,
+                                "hbm_source": src, "gpu": torch.cuda.get_device_name(0),
+                                "how": "sfd_measure_pipes (include/sfd.h): FFMA chains on all SMs; "
+                                       "sfdb::dft32 / dft32_tw in a register-only loop, one warp per "
+                                       "sub-partition, clock64"}}), flush=True)
+    return 0
+
+
+# ---- launcher: `python bench.py --gpus N` started bare spawns its own N ranks -------------------------
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def spawn_ranks(args):
+    """One process per GPU with RANK / LOCAL_RANK / WORLD_SIZE / MASTER_* set, as torchrun would; the
+    output of every rank passes through (rank 0 prints the JSON line).  Returns the worst exit code."""
+    port = _free_port()
+    procs = []
+    for r in range(args.gpus):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(args.gpus),
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        if args.impl == "sfd":
+            env.setdefault("NCCL_DEBUG", "INFO")          # the communicator log (stderr) stays on
+            env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__)] + sys.argv[1:], env=env))
+    rc = 0
+    for p in procs:
+        rc = max(rc, abs(p.wait()))
+    return rc
 
 
 def main():
     args = parse_args()
+    if args.peaks:
+        return run_peaks()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_ranks(args)
     from paper_1001_4309_b200 import dist as D
     info = D.rank_info()
-    if info.world != args.gpus and info.world > 1:
+    if info.world != args.gpus:
         raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={info.world}")
     if args.impl == "reference":
         return run_reference(args, info)

@@ -69,9 +69,15 @@ private:
 const ld TWO_PI = 6.283185307179586476925286766559005768L;
 
 inline ld frac1(ld c) { return c - rintl(c); }  // cycles -> (-1/2, 1/2]
+// exp(2 pi i c): the phase is summed and reduced modulo 1 in extended precision (it reaches 1e5
+// cycles); the reduced phase |c| <= 1/2 then goes through the double-precision sincos (error 1e-16,
+// nine orders below the float32 rounding that follows, and five times faster than cosl/sinl: the
+// table builder is what a live view update costs on the host)
 inline cd cis_cycles(ld c) {
-    c = frac1(c);
-    return cd((double)cosl(TWO_PI * c), (double)sinl(TWO_PI * c));
+    const double r = (double)(TWO_PI * frac1(c));
+    double sn, cs;
+    sincos(r, &sn, &cs);
+    return cd(cs, sn);
 }
 
 // exp(-2 pi i k / n), k < n/2, evaluated directly (no recurrence)
@@ -178,10 +184,11 @@ double lane_sign(int n) {
 // of the frequency index, w = exp(-2 pi i / 2N); layout [2][3][N]: for branch b the vectors
 //   pre_b = pre w^(b n),  H_b[k] = H[2k + b],  conj(post_b) = conj(post w^(-b n))
 // (each times its scale; H = the float32 M-point kernel spectrum), formed in float64.
+// tw = fft_twiddles(2N): tw[n] = exp(-2 pi i n / 2N) = w^n.
 void branch_tables(int N, const cd *pre, const cd *post, cd pre_scale, cd post_scale,
-                   const float2 *H, float2 *out) {
+                   const float2 *H, float2 *out, const std::vector<cd> &tw) {
     for (int n = 0; n < N; ++n) {
-        const cd w = cis_cycles(-(ld)n / (ld)(2 * N));
+        const cd w = tw[n];
         const float sg = (float)lane_sign(n);
         const cd t[4] = {pre[n] * pre_scale, pre[n] * pre_scale * w,
                          (double)sg * std::conj(post[n] * post_scale),
@@ -199,15 +206,17 @@ void branch_tables(int N, const cd *pre, const cd *post, cd pre_scale, cd post_s
 // index modulo 4, w = exp(-2 pi i / 4096); layout [4][5][1024]: for branch b the vectors
 //   preA_b = pre[n] w^(b n), preB_b = pre[n+1024] w^(b (n+1024)), H_b[k] = H[4k+b],
 //   postA_b = post[n] w^(-b n), postB_b = post[n+1024] w^(-b (n+1024))            (n, k < 1024)
+// tw = fft_twiddles(4096): w^e = tw[e] for e < 2048, -tw[e - 2048] above.
 void branch_tables4(const cd *pre, const cd *post, cd pre_scale, cd post_scale, const float2 *H,
-                    float2 *out) {
+                    float2 *out, const std::vector<cd> &tw) {
     const int Nb = 1024;
     for (int b = 0; b < 4; ++b)
         for (int n = 0; n < Nb; ++n) {
             float2 *o = out + (size_t)b * 5 * Nb + n;
             for (int half = 0; half < 2; ++half) {
                 const int m = n + half * Nb;
-                const cd w = cis_cycles(-(ld)((long long)b * m) / (ld)4096);
+                const int e = (b * m) & 4095;
+                const cd w = e < 2048 ? tw[e] : -tw[e - 2048];
                 const cd a = pre[m] * pre_scale * w,
                          c = lane_sign(n) * post[m] * post_scale * std::conj(w);
                 o[(size_t)half * Nb] = make_float2((float)a.real(), (float)a.imag());
@@ -238,9 +247,9 @@ void build_view_f32(const sfd_plan *p, int v, float2 *out) {
     to_f32(a.data(), out + d.off_pre_y, d.Ny, cd(in_scale, 0));
     to_f32(b.data(), out + d.off_post_y, d.Ny, c0);
     if (d.off_tabY >= 0 && d.Ny == 1024)
-        branch_tables(d.Ny, a.data(), b.data(), cd(in_scale, 0), c0, Hy, out + d.off_tabY);
+        branch_tables(d.Ny, a.data(), b.data(), cd(in_scale, 0), c0, Hy, out + d.off_tabY, p->wy);
     if (d.off_tabY >= 0 && d.Ny == 2048)
-        branch_tables4(a.data(), b.data(), cd(in_scale, 0), c0, Hy, out + d.off_tabY);
+        branch_tables4(a.data(), b.data(), cd(in_scale, 0), c0, Hy, out + d.off_tabY, p->wy);
     // x axis
     kernel_spectrum(d.Nx, p->lambda, p->p1[v], p->p2[v], p->z[v], h.data(), p->wx);
     to_f32(h.data(), Hx, d.Mx);
@@ -249,9 +258,9 @@ void build_view_f32(const sfd_plan *p, int v, float2 *out) {
     to_f32(a.data(), out + d.off_pre_x, d.Nx);
     to_f32(b.data(), out + d.off_post_x, d.Nx);
     if (d.off_tabX >= 0 && d.Nx == 1024)
-        branch_tables(d.Nx, a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, out + d.off_tabX);
+        branch_tables(d.Nx, a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, out + d.off_tabX, p->wx);
     if (d.off_tabX >= 0 && d.Nx == 2048)
-        branch_tables4(a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, out + d.off_tabX);
+        branch_tables4(a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, out + d.off_tabX, p->wx);
 }
 
 // Per-device one-time set-up: cudaFuncSetAttribute applies to the device that is current, so a

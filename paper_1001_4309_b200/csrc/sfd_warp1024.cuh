@@ -489,7 +489,7 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *holo, lon
                                             const void *tmB, int V) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int half = warp >> 2, c = (warp >> 1) & 1, ht = threadIdx.x & 127, b = warp & 1;
-    const int groups = nx / YC;
+    const int groups = nx / YC, lgg = 31 - __clz(groups);  // nx is a power of two: shifts, not divisions
     const int items = V * groups;
     const int i0 = (int)((long long)items * blockIdx.x / gridDim.x);
     const int i1 = (int)((long long)items * (blockIdx.x + 1) / gridDim.x);
@@ -498,19 +498,19 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *holo, lon
     const float2 *xbp = sm.xb[warp ^ 1];
     float2 *stg = &sm.stage[half][0][0];
     const bool leader = ht == 0;  // issues and retires the half's bulk stores
-    const int view0 = i0 / groups;
+    const int view0 = i0 >> lgg;
     constexpr int IPS = TileElem<TIn>::IPS;
     // groups % IPS == 0 (nx is a multiple of 16): a slab never straddles two views
     {
         TileRegs<TIn> t;
-        tile_load<TIn>(t, holo, hstride, (i0 % groups) / IPS * (YC * IPS) + 2 * IPS * half, ht);
+        tile_load<TIn>(t, holo, hstride, (i0 & (groups - 1)) / IPS * (YC * IPS) + 2 * IPS * half, ht);
         tile_store(t, sm.tile[half], ht);
     }
     half_sync(half);
     const Turns turns = turns_make(warp, true);
     turns_open(turns, warp);
     for (int item = i0; item < i1; ++item) {
-        const int view = item / groups, g = item % groups, k = g % IPS;
+        const int view = item >> lgg, g = item & (groups - 1), k = g % IPS;
         const int colh = g / IPS * (YC * IPS) + 2 * IPS * half + 2 * k;
         const unsigned tpre = tq + (view - view0) * TM_SET;  // pre_b | H_b | conj(post_b)
         const bool has_next = item + 1 < i1 && k == IPS - 1;  // the next item opens a new slab
@@ -535,7 +535,7 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *holo, lon
         // the next slab is fetched behind the tile reads: its loads touch one row per lane (32
         // wavefronts each) and would hold up everything queued after them
         if (has_next)
-            tile_load<TIn>(t, holo, hstride, ((item + 1) % groups) / IPS * (YC * IPS) + 2 * IPS * half, ht);
+            tile_load<TIn>(t, holo, hstride, ((item + 1) & (groups - 1)) / IPS * (YC * IPS) + 2 * IPS * half, ht);
         branch(v, lane, xb, tw, tpre + TM_TAB, turns);
         // the previous item's bulk stores must have left the staging tile before it is rewritten
         if (leader) bulk_wait_read();
@@ -623,7 +623,7 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *Bin, int ny
                                             float *__restrict__ inten, unsigned int *vmax,
                                             double *mom, int V) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, pair = warp >> 1;
-    const int gpv = ny / XP;  // units per view
+    const int gpv = ny / XP, lgv = 31 - __clz(gpv);  // units per view; ny is a power of two
     const int units = V * gpv;
     const int u0 = (int)((long long)units * blockIdx.x / gridDim.x);
     const int u1 = (int)((long long)units * (blockIdx.x + 1) / gridDim.x);
@@ -633,7 +633,7 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *Bin, int ny
     const float2 *in = sm.inb[pair] + lane;
     const int b = warp & 1;
     const bool issuer = b == 0 && lane == 0;
-    const int view0 = u0 / gpv;
+    const int view0 = u0 >> lgv;
     unsigned iphase = 0;
     bool pending = false;  // the pair's input row is already on its way
     // turn-taking of warps w and w + 4 (needs every warp of the CTA to run the same number of
@@ -642,12 +642,12 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *Bin, int ny
     const Turns turns = turns_make(warp, true);
     turns_open(turns, warp);
     for (int u = u0; u < u1; ++u) {
-        const int view = u / gpv, line = (u % gpv) * XP + pair;
+        const int view = u >> lgv, line = (u & (gpv - 1)) * XP + pair;
         const unsigned tpre = tq + (view - view0) * TM_SET;  // pre_b | H_b | conj(post_b)
         const size_t row = (size_t)view * ny + line;
         if (!pending && issuer)
             bulk_load(sm.inb[pair], Bin + row * N, N * sizeof(float2), &sm.ibar[pair]);
-        const int nu = u + 1, nline = (nu % gpv) * XP + pair;
+        const int nu = u + 1, nline = (nu & (gpv - 1)) * XP + pair;
         const bool has_next = nu < u1;
         mbar_wait(&sm.ibar[pair], iphase);
         iphase ^= 1;
@@ -669,7 +669,7 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *Bin, int ny
         pair_sync(pair);
         if (has_next && issuer) {
             fence_async_smem();
-            bulk_load(sm.inb[pair], Bin + ((size_t)(nu / gpv) * ny + nline) * N, N * sizeof(float2),
+            bulk_load(sm.inb[pair], Bin + ((size_t)(nu >> lgv) * ny + nline) * N, N * sizeof(float2),
                       &sm.ibar[pair]);
         }
         pending = has_next;

@@ -86,21 +86,50 @@ def test_shard_range_partitions_every_unit_once(n, world):
         W.shard_range(n, world, world)
 
 
-def test_reference_arm_prints_on_rank0_only():
-    """`bench.py --impl reference` under a 2-rank environment: rank 1 exits 0 without output and
-    without touching a process group; rank 0 (here run alone, world 1) prints the JSON line."""
-    env = dict(os.environ, RANK="1", LOCAL_RANK="1", WORLD_SIZE="2", MASTER_ADDR="127.0.0.1",
-               MASTER_PORT=str(_free_port()))
-    r1 = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference",
-                         "--gpus", "2", "--steps", "1", "--warmup", "0", "--config", "1"],
-                        env=env, capture_output=True, text=True, timeout=300)
-    assert r1.returncode == 0 and r1.stdout.strip() == ""
-    env0 = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE")}
-    r0 = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference",
-                         "--steps", "2", "--warmup", "1", "--config", "1"],
-                        env=env0, capture_output=True, text=True, timeout=600)
-    assert r0.returncode == 0, r0.stderr
-    line = json.loads(r0.stdout.strip().splitlines()[-1])
-    assert line["impl"] == "reference" and line["unit"] == "reconstructions/s"
-    assert line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
+def _json_lines(text):
+    return [json.loads(l) for l in text.splitlines() if l.startswith("{")]
+
+
+def test_bare_bench_starts_its_own_ranks():
+    """`python bench.py --impl reference --gpus 2` with no WORLD_SIZE in the environment launches two
+    ranks itself (one process each, rendezvous on 127.0.0.1); both join the process group, rank 0 alone
+    works and prints ONE JSON line, rank 1 exits 0 without output."""
+    env = {k: v for k, v in os.environ.items()
+           if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                        "--steps", "2", "--warmup", "1", "--config", "1"],
+                       env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr
+    lines = _json_lines(r.stdout)
+    assert len(lines) == 1
+    line = lines[0]
+    assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["ranks_joined"] == 2
+    assert line["unit"] == "reconstructions/s" and line["value"] > 0
+    assert line["cpu_baseline"]["kind"] == "oracle" and "caveat" in line["cpu_baseline"]
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["gpu_launches"] == 0
+
+
+def test_reference_arm_under_a_torchrun_style_launch():
+    """The driver's launch: every rank started with RANK / WORLD_SIZE / MASTER_* in its environment.
+    Rank 1 joins, waits for rank 0 and exits 0 with empty stdout; rank 0 prints the line."""
+    port = _free_port()
+    procs = []
+    for rank in (0, 1):
+        env = dict(os.environ, RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE="2",
+                   MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference",
+                                       "--gpus", "2", "--steps", "1", "--warmup", "0", "--config", "1"],
+                                      env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    outs = [p.communicate(timeout=600) for p in procs]
+    assert [p.returncode for p in procs] == [0, 0], outs
+    assert outs[1][0].strip() == ""
+    line = _json_lines(outs[0][0])[-1]
+    assert line["impl"] == "reference" and line["ranks_joined"] == 2
+
+
+def test_world_size_must_match_gpus():
+    env = dict(os.environ, RANK="0", LOCAL_RANK="0", WORLD_SIZE="3", MASTER_ADDR="127.0.0.1",
+               MASTER_PORT=str(_free_port()))
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
+                       env=env, capture_output=True, text=True, timeout=120)
+    assert r.returncode != 0 and "WORLD_SIZE" in (r.stderr + r.stdout)
