@@ -262,6 +262,12 @@ __device__ __forceinline__ void sub_load(SubRegs<TIn> &t, const TIn *holo, long 
         t.e[i] = *reinterpret_cast<const typename SubSlab<TIn>::elem *>(
             holo + (size_t)(qt + 128 * i) * hstride + col);
 }
+template <typename TIn>
+__device__ __forceinline__ void sub_prefetch(const TIn *holo, long long hstride, int col, int qt) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(holo + (size_t)(qt + 128 * i) * hstride + col));
+}
 __device__ __forceinline__ void sub_store(const SubRegs<unsigned char> &t,
                                           unsigned short (*tile)[N][2], int qt, int quad) {
 #pragma unroll
@@ -315,7 +321,6 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, lo
     for (int u = rg.u0; u < rg.u1; ++u) {
         const int k = u % IPS;
         const bool next_slab = u + 1 < rg.u1 && k == IPS - 1;
-        SubRegs<TIn> t;
 #pragma unroll 1
         for (int cc = 0; cc < 2; ++cc) {  // the quad's two columns, one after the other
             float2 v[32];
@@ -336,9 +341,10 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, lo
                     }
                 }
             }
-            // the next sub-slab is fetched behind the tile reads of the unit's last column: its
-            // loads touch one row per lane (32 wavefronts each)
-            if (cc == 1 && next_slab) sub_load<TIn>(t, holo, hstride, SubSlab<TIn>::col(u + 1, quad), qt);
+            // the next sub-slab is pulled towards L2 now and loaded after the branch: 32 registers of
+            // slab held across the butterflies spilled (measured: 0.91 ms per launch of config 4 with
+            // the loads here, 0.72 ms with the prefetch)
+            if (cc == 1 && next_slab) sub_prefetch<TIn>(holo, hstride, SubSlab<TIn>::col(u + 1, quad), qt);
             quad_sync(quad);  // the previous column's exchange area has been read by all four warps
             branch<false>(v, lane, xb, tw, tq + TQ_H, turns);
             // the previous unit's bulk stores must have left the staging tile before it is rewritten
@@ -353,7 +359,11 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, lo
 #pragma unroll
             for (int i = 0; i < 16; ++i) stg[(lane + 32 * (16 * b + i)) * 4 + 2 * quad + cc] = mine[i];
             if (cc == 1) {
-                if (next_slab) sub_store(t, sm.tile[quad], qt, quad);  // the tile was last read before this column's first barrier
+                if (next_slab) {  // the tile was last read before this column's first barrier
+                    SubRegs<TIn> t;
+                    sub_load<TIn>(t, holo, hstride, SubSlab<TIn>::col(u + 1, quad), qt);
+                    sub_store(t, sm.tile[quad], qt, quad);
+                }
                 fence_async_smem();  // staging writes -> async proxy
                 cta_sync();          // staging tile complete (both quads), next slab visible
                 if (leader) {
