@@ -111,27 +111,25 @@ k_quantise(const float4 *inten, const unsigned int *vmax, uchar4 *__restrict__ o
 // One CTA per SM.  Even warps run branch 0 (even bins), odd warps branch 1.
 // k_cols_1024: Ny = 1024 rows, nx columns (lines).  k_rows_1024: Nx = 1024 columns, ny rows (lines).
 template <typename TIn>
-__global__ void __launch_bounds__(sfdw::WY * 32, 1)
+__global__ void __launch_bounds__(sfdw::NW1024 * 32, 1)
 k_cols_1024(const TIn *holo, long long hstride, int nx, const float2 *__restrict__ tabY,
             long long vstride, const float2 *__restrict__ twl,
             const __grid_constant__ CUtensorMap tmB, unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
-    sfdw::SmemY<TIn> &sm = *reinterpret_cast<sfdw::SmemY<TIn> *>(smem4);
+    using SM = sfdw::SmemY<TIn, sfdw::NW1024>;
+    SM &sm = *reinterpret_cast<SM *>(smem4);
     sfdw::pdl_launch_dependents();
-    float2 tw[sfdw::TWN];
-    sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
-    const int groups = nx / sfdw::YC;
+    const int ipv = sfdw::YItems<TIn, sfdw::NW1024>::per_view(nx);  // items per view, as in pass_y_loop
     {   // pull the first slab of this CTA towards L2 while the prologue runs (a prefetch reads nothing:
         // it may precede griddepcontrol.wait)
-        constexpr int IPS = sfdw::TileElem<TIn>::IPS;
-        const int i0 = (int)((long long)V * groups * blockIdx.x / gridDim.x);
-        const TIn *p0 = holo + (i0 % groups) / IPS * (sfdw::YC * IPS);
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(p0 + (size_t)(threadIdx.x + 256 * i) * hstride));
+        using YI = sfdw::YItems<TIn, sfdw::NW1024>;
+        const int i0 = (int)((long long)V * ipv * blockIdx.x / gridDim.x);
+        const TIn *p0 = holo + (i0 % ipv) / YI::IPS * YI::COLS;
+        for (int r = threadIdx.x; r < sfdw::N; r += blockDim.x)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(p0 + (size_t)r * hstride));
     }
     // tables of this CTA's view(s) -> tensor memory
-    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabY, vstride, V * groups, groups);
+    const unsigned tbase = sfdw::tm_setup<sfdw::NW1024>(&sm.tmem, tabY, vstride, V * ipv, ipv, twl);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     // everything above touches plan constants only; the hologram, B, vmax and mom belong to the
     // kernels before this one in the stream
@@ -140,28 +138,26 @@ k_cols_1024(const TIn *holo, long long hstride, int nx, const float2 *__restrict
         for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
     if (mom != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
-    sfdw::pass_y_loop<TIn>(sm, holo, hstride, nx, tq, tw, &tmB, V);
+    sfdw::pass_y_loop<TIn, sfdw::NW1024, sfdw::TURNSY>(sm, holo, hstride, nx, tq, tq + sfdw::TM_TW, &tmB, V);
     sfdw::tm_finish(tbase);
 }
 
-__global__ void __launch_bounds__(sfdw::WX * 32, 1)
+__global__ void __launch_bounds__(sfdw::NW1024 * 32, 1)
 k_rows_1024(const float2 *B, int ny, const float2 *__restrict__ tabX, long long vstride,
             const float2 *__restrict__ twl, float2 *__restrict__ field, float *__restrict__ inten,
             unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
-    sfdw::SmemX &sm = *reinterpret_cast<sfdw::SmemX *>(smem4);
+    using SM = sfdw::SmemX<sfdw::NW1024>;
+    SM &sm = *reinterpret_cast<SM *>(smem4);
     sfdw::pdl_launch_dependents();
     if (threadIdx.x == 0) {
-        for (int i = 0; i < sfdw::XP; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
+        for (int i = 0; i < sfdw::NW1024 / 2; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
         sfdw::mbar_fence_init();
     }
-    float2 tw[sfdw::TWN];
-    sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
-    const int gpv = ny / sfdw::XP;  // units per view, as in pass_x_loop
-    const unsigned tbase = sfdw::tm_setup(&sm.tmem, tabX, vstride, V * gpv, gpv);
+    const unsigned tbase = sfdw::tm_setup<sfdw::NW1024>(&sm.tmem, tabX, vstride, V * ny, ny, twl);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
-    sfdw::pass_x_loop(sm, B, ny, tq, tw, field, inten, vmax, mom, V);
+    sfdw::pass_x_loop<sfdw::NW1024, sfdw::TURNSX>(sm, B, ny, tq, tq + sfdw::TM_TW, field, inten, vmax, mom, V);
     sfdw::tm_finish(tbase);
 }
 
@@ -176,17 +172,15 @@ k_cols_2048(const TIn *holo, long long hstride, int nx, const float2 *__restrict
     extern __shared__ float4 smem4[];
     sfdq::SmemYQ<TIn> &sm = *reinterpret_cast<sfdq::SmemYQ<TIn> *>(smem4);
     sfdw::pdl_launch_dependents();
-    float2 tw[sfdw::TWN];
-    sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
     const sfdq::Range rg = sfdq::cta_range(cpv, nx / 4);
-    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabY, vstride, rg.view);
+    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabY, vstride, rg.view, twl);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     sfdw::pdl_wait();
     if (vmax != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
     if (mom != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
-    sfdq::pass_y_quad<TIn>(sm, holo, hstride, tq, tw, &tmB, rg);
+    sfdq::pass_y_quad<TIn>(sm, holo, hstride, tq, tq + sfdq::TQ_TW, &tmB, rg);
     sfdw::tm_finish(tbase);
 }
 
@@ -202,13 +196,11 @@ k_rows_2048(const float2 *B, int ny, const float2 *__restrict__ tabX, long long 
         sfdw::mbar_init(&sm.ibar[1], 1);
         sfdw::mbar_fence_init();
     }
-    float2 tw[sfdw::TWN];
-    sfdw::load_twiddles(tw, threadIdx.x & 31, twl);
     const sfdq::Range rg = sfdq::cta_range(cpv, ny / 2);
-    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabX, vstride, rg.view);
+    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabX, vstride, rg.view, twl);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
-    sfdq::pass_x_quad(sm, B, ny, tq, tw, field, inten, vmax, mom, rg);
+    sfdq::pass_x_quad(sm, B, ny, tq, tq + sfdq::TQ_TW, field, inten, vmax, mom, rg);
     sfdw::tm_finish(tbase);
 }
 
@@ -312,12 +304,12 @@ cudaError_t launch_y(sfd_plan *p, const void *holo, unsigned int *vmax, double *
         // two views (the kernel holds two table sets)
         const int grid = d.V > d.sms ? d.V : d.sms;
         if (d.in_dtype == 0) {
-            Launch l(dim3(grid), dim3(sfdw::WY * 32), sizeof(sfdw::SmemY<unsigned char>), st);
+            Launch l(dim3(grid), dim3(sfdw::NW1024 * 32), sizeof(sfdw::SmemY<unsigned char, sfdw::NW1024>), st);
             return cudaLaunchKernelEx(&l.cfg, k_cols_1024<unsigned char>, (const unsigned char *)holo,
                                       d.in_stride, d.Nx, tabY, d.vstride, (const float2 *)d.w_twl, tmB,
                                       vmax, mom, d.V);
         }
-        Launch l(dim3(grid), dim3(sfdw::WY * 32), sizeof(sfdw::SmemY<float>), st);
+        Launch l(dim3(grid), dim3(sfdw::NW1024 * 32), sizeof(sfdw::SmemY<float, sfdw::NW1024>), st);
         return cudaLaunchKernelEx(&l.cfg, k_cols_1024<float>, (const float *)holo, d.in_stride, d.Nx,
                                   tabY, d.vstride, (const float2 *)d.w_twl, tmB, vmax, mom, d.V);
     }
@@ -362,7 +354,7 @@ cudaError_t launch_x(sfd_plan *p, float2 *field, float *inten, unsigned int *vma
     const sfd_dev &d = p->d;
     const float2 *tabX = d.tabs + d.off_tabX;
     if (sfd_uses_warp_x(p) && d.Nx == sfdw::N) {
-        Launch l(dim3(d.V > d.sms ? d.V : d.sms), dim3(sfdw::WX * 32), sizeof(sfdw::SmemX), st);
+        Launch l(dim3(d.V > d.sms ? d.V : d.sms), dim3(sfdw::NW1024 * 32), sizeof(sfdw::SmemX<sfdw::NW1024>), st);
         return cudaLaunchKernelEx(&l.cfg, k_rows_1024, (const float2 *)d.B, d.Ny, tabX, d.vstride,
                                   (const float2 *)d.w_twl, field, inten, vmax, mom, d.V);
     }
@@ -447,9 +439,9 @@ cudaError_t sfd_kernels_init(int device, int *sms) {
     if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,        \
                                   (int)(bytes))) != cudaSuccess)                              \
         return e;
-    SFD_SMEM(k_cols_1024<unsigned char>, sizeof(sfdw::SmemY<unsigned char>))
-    SFD_SMEM(k_cols_1024<float>, sizeof(sfdw::SmemY<float>))
-    SFD_SMEM(k_rows_1024, sizeof(sfdw::SmemX))
+    SFD_SMEM(k_cols_1024<unsigned char>, sizeof(sfdw::SmemY<unsigned char, sfdw::NW1024>))
+    SFD_SMEM(k_cols_1024<float>, sizeof(sfdw::SmemY<float, sfdw::NW1024>))
+    SFD_SMEM(k_rows_1024, sizeof(sfdw::SmemX<sfdw::NW1024>))
     SFD_SMEM(k_cols_2048<unsigned char>, sizeof(sfdq::SmemYQ<unsigned char>))
     SFD_SMEM(k_cols_2048<float>, sizeof(sfdq::SmemYQ<float>))
     SFD_SMEM(k_rows_2048, sizeof(sfdq::SmemXQ))

@@ -140,6 +140,7 @@ constexpr int TABS = 2 * 3 * N;  // complex elements
 constexpr int TM_COLS = 512;      // allocated columns (all of it: one CTA per SM)
 constexpr int TM_SET = 192;       // columns of one view set
 constexpr int TM_TAB = 64;        // columns of one table
+constexpr int TM_TW = 2 * TM_SET;  // 64 columns of stage-B twiddles (31 per-lane values + pad)
 struct TChunk { unsigned w[16]; };
 #define SFDW_O16(c) "=r"(c.w[0]), "=r"(c.w[1]), "=r"(c.w[2]), "=r"(c.w[3]), "=r"(c.w[4]), "=r"(c.w[5]), \
     "=r"(c.w[6]), "=r"(c.w[7]), "=r"(c.w[8]), "=r"(c.w[9]), "=r"(c.w[10]), "=r"(c.w[11]), "=r"(c.w[12]), \
@@ -200,18 +201,20 @@ __device__ __forceinline__ void tm_sync_cta() {  // makes tcgen05.st of other wa
 __device__ __forceinline__ unsigned tm_quarter(unsigned base, int warp) {
     return base + ((unsigned)(32 * (warp & 3)) << 16);
 }
-// The two warps of a sub-partition copy the tables of `view`, branch warp & 1, into set `set` of
-// their quarter: warp w the chunks 0..5 (pre_b and half of H_b), warp w + 4 the chunks 6..11.  All
-// 48 loads of a thread are issued before the first store (and before the allocation): one trip
-// to L2 per set.
+// The R = NW / 4 warps of a sub-partition copy the tables of `view`, branch warp & 1, into set `set`
+// of their quarter: warp w + 4 r the chunks 12 r / R .. (12 of them: pre_b, H_b, conj(post_b), four
+// chunks of 8 values each).  All loads of a thread are issued before the first store (and before
+// the allocation): one trip to L2 per set.
 // tab: the [2][3][N] block of view 0 in global memory, vstride complex values between views
-struct TFill { TChunk c[6]; };
-__device__ __forceinline__ void tm_fill_load(TFill &f, const float2 *__restrict__ tab,
+template <int NW> struct TFill { TChunk c[12 / (NW / 4)]; };
+template <int NW>
+__device__ __forceinline__ void tm_fill_load(TFill<NW> &f, const float2 *__restrict__ tab,
                                              long long vstride, int view, int warp, int lane) {
+    constexpr int CH = 12 / (NW / 4);
     const float2 *src = tab + (size_t)view * vstride + (size_t)(warp & 1) * 3 * N + lane;
-    const int ch0 = 6 * (warp >> 2);  // first chunk of this warp; chunk = 8 values, 4 chunks per table
+    const int ch0 = CH * (warp >> 2);  // first chunk of this warp; chunk = 8 values, 4 chunks per table
 #pragma unroll
-    for (int j = 0; j < 6; ++j)
+    for (int j = 0; j < CH; ++j)
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
             const float2 x = __ldg(src + 32 * (8 * (ch0 + j) + i));  // table t = chunk / 4 starts at t * N
@@ -219,34 +222,55 @@ __device__ __forceinline__ void tm_fill_load(TFill &f, const float2 *__restrict_
             f.c[j].w[2 * i + 1] = __float_as_uint(x.y);
         }
 }
-__device__ __forceinline__ void tm_fill_store(const TFill &f, unsigned quarter, int set, int warp) {
-    const int ch0 = 6 * (warp >> 2);
+template <int NW>
+__device__ __forceinline__ void tm_fill_store(const TFill<NW> &f, unsigned quarter, int set, int warp) {
+    constexpr int CH = 12 / (NW / 4);
+    const int ch0 = CH * (warp >> 2);
 #pragma unroll
-    for (int j = 0; j < 6; ++j) tm_st(f.c[j], quarter + set * TM_SET + 16 * (ch0 + j));
+    for (int j = 0; j < CH; ++j) tm_st(f.c[j], quarter + set * TM_SET + 16 * (ch0 + j));
 }
-// Kernel prologue (all threads): allocate, fill the one or two view sets this CTA's contiguous
-// range [total b / g, total (b + 1) / g) of work units touches (per_view units per view), make
-// them visible.  Returns the base address; tm_finish releases it at the end of the kernel.
+// twl: [31][32] at [j][lane] (plan constant) -> 4 chunks of 8 values in this lane quarter
+__device__ __forceinline__ void tm_fill_twiddles(unsigned taddr, const float2 *__restrict__ twl, int lane) {
+#pragma unroll 1
+    for (int j = 0; j < 4; ++j) {
+        TChunk c;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const float2 x = (8 * j + i < 31) ? __ldg(twl + (8 * j + i) * 32 + lane) : make_float2(0.f, 0.f);
+            c.w[2 * i] = __float_as_uint(x.x);
+            c.w[2 * i + 1] = __float_as_uint(x.y);
+        }
+        tm_st(c, taddr + 16 * j);
+    }
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+// Kernel prologue (all NW warps): allocate, fill the one or two view sets this CTA's contiguous
+// range [total b / g, total (b + 1) / g) of work units touches (per_view units per view) and the
+// twiddle columns, make them visible.  Returns the base address; tm_finish releases it at the end of
+// the kernel.
+template <int NW>
 __device__ __forceinline__ unsigned tm_setup(unsigned *slot, const float2 *__restrict__ tab,
-                                             long long vstride, int total, int per_view) {
+                                             long long vstride, int total, int per_view,
+                                             const float2 *__restrict__ twl) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int a0 = (int)((long long)total * blockIdx.x / gridDim.x);
     const int a1 = (int)((long long)total * (blockIdx.x + 1) / gridDim.x);
     const int view0 = a0 < a1 ? a0 / per_view : 0;
-    TFill f;
-    if (a0 < a1) tm_fill_load(f, tab, vstride, view0, warp, lane);  // on their way during the allocation
+    TFill<NW> f;
+    if (a0 < a1) tm_fill_load<NW>(f, tab, vstride, view0, warp, lane);  // on their way during the allocation
     if (warp == 0) tm_alloc(slot);
     tm_sync_cta();
     const unsigned base = *reinterpret_cast<volatile unsigned *>(slot);
     if (a0 < a1) {
         const unsigned q = tm_quarter(base, warp);
-        tm_fill_store(f, q, 0, warp);
+        tm_fill_store<NW>(f, q, 0, warp);
         if ((a1 - 1) / per_view != view0) {
-            tm_fill_load(f, tab, vstride, view0 + 1, warp, lane);
-            tm_fill_store(f, q, 1, warp);
+            tm_fill_load<NW>(f, tab, vstride, view0 + 1, warp, lane);
+            tm_fill_store<NW>(f, q, 1, warp);
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
+    if (warp < 4) tm_fill_twiddles(tm_quarter(base, warp) + TM_TW, twl, lane);
     tm_sync_cta();
     return base;
 }
@@ -254,55 +278,89 @@ __device__ __forceinline__ void tm_finish(unsigned base) {
     tm_sync_cta();
     if ((threadIdx.x >> 5) == 0) tm_free(base);
 }
-// Coupling of the two warps that share an SM sub-partition (warps w and w + 4 of an 8-warp CTA).
+// Coupling of the warps that share an SM sub-partition (warps w, w + 4, w + 8, .. of a CTA).
 // The butterfly phases of a line load the sub-partition's fp32 pipe, the phases between them
 // (transposes, table and input reads, exchange, stores) the SM-wide shared-memory pipe; left alone
-// the warps of an SM drift into the same phase and the shared-memory pipe sees bursts.  The two
-// warps hand a turn to each other around the two transposes of a branch: bar.sync on one's own
-// named barrier before the stores into the tile, bar.arrive on the partner's after the loads from it
-// (thread count 64).  This does not exclude anything; it bounds how far the two warps drift apart.
-// Measured against the alternatives in round 1 (no coupling, strict mbarrier tokens,
-// rendezvous, the same hand-off around the butterfly phases): the fastest by 1 to 11 %.
+// the warps of an SM drift into the same phase and the shared-memory pipe sees bursts.  The warps of
+// a sub-partition pass a turn round a ring (w -> w + 4 -> .. -> w) around the two transposes of a
+// branch: bar.sync on one's own named barrier before the stores into the tile, bar.arrive on the
+// successor's after the loads from it (thread count 64).  This does not exclude anything; it bounds
+// how far the warps drift apart.  Measured with two warps per sub-partition in round 1 (DESIGN.md
+// 5.4: no coupling, strict mbarrier tokens, rendezvous, the same hand-off around the butterfly
+// phases): the fastest by 1 to 11 %.
 struct Turns {
-    unsigned mine, theirs;  // named barriers 5..12
+    unsigned mine, next;  // named barriers first .. first + NW - 1
     bool on;
 };
 __device__ __forceinline__ void turn_begin(const Turns &t) {
     if (t.on) asm volatile("bar.sync %0, 64;" ::"r"(t.mine) : "memory");
 }
 __device__ __forceinline__ void turn_end(const Turns &t) {
-    if (t.on) asm volatile("bar.arrive %0, 64;" ::"r"(t.theirs) : "memory");
+    if (t.on) asm volatile("bar.arrive %0, 64;" ::"r"(t.next) : "memory");
 }
-// Warps 0..3 own the first turn; warps 4..7 pass on their first one and warps 0..3 add one after
-// their last line, so that both warps of a sub-partition take the same number of turns.
-__device__ __forceinline__ Turns turns_make(int warp, bool on) {
-    const unsigned sp = warp & 3, up = warp >> 2;
-    return Turns{5u + 2 * sp + up, 5u + 2 * sp + 1 - up, on};
+// Warps 0..3 own the first turn: the last warps of the ring pass on a turn at the start and warps
+// 0..3 take one more after their last line, so that every barrier sees as many arrivals as waits.
+// Every warp of a sub-partition must take the same number of turns (a warp without work in a round
+// takes empty ones: turns_skip).
+__device__ __forceinline__ Turns turns_make(int warp, int nwarps, unsigned first, bool on) {
+    const int succ = warp + 4 < nwarps ? warp + 4 : (warp & 3);
+    return Turns{first + warp, first + succ, on};
 }
-__device__ __forceinline__ void turns_open(const Turns &t, int warp) {
-    if ((warp >> 2) == 1) turn_end(t);
+__device__ __forceinline__ void turns_open(const Turns &t, int warp, int nwarps) {
+    if (warp + 4 >= nwarps) turn_end(t);
 }
 __device__ __forceinline__ void turns_close(const Turns &t, int warp) {
-    if ((warp >> 2) == 0) turn_begin(t);
+    if (warp < 4) turn_begin(t);
+}
+__device__ __forceinline__ void turns_skip(const Turns &t) {  // the two turns of a line, empty
+    turn_begin(t);
+    turn_end(t);
+    turn_begin(t);
+    turn_end(t);
 }
 
-// One branch of a line, in place (the caller has applied pre): forward FFT, x H_b, inverse FFT,
-// x post_b.  The inverse is run as conj(FFT(conj(.))) so that both transforms execute the same code:
-//     v <- conj(FFT(v) H_b);  v <- conj(FFT(v) conj(post_b)) = post_b IFFT(H_b FFT(v)) N
-// (the 1/N sits in H).  t = tensor-memory address of H_b in this warp's quarter; conj(post_b) follows it.
-// Both tables carry the lane sign of sfd_dft32.cuh: entry lane + 32 r is multiplied by out_sign(lane).
-// A 1024-point FFT of a warp (four-step, in v[r] = x[lane + 32 r], out v[r] = X[lane + 32 r]):
-//     stage A   32-point DFT over n1 (element lane + 32 n1) in registers            sfdb::dft32
-//     transpose 32 x 32 through the warp's tile xb: lane becomes k1, register n2
-//     stage B   32-point DFT over n2 with the inter-stage twiddles exp(-2 pi i k1 n2 / 1024)
-//               folded into its butterflies (tw: 31 per-lane constants)             sfdb::dft32_tw
-// The two FFTs of the branch share one copy of the code (rolled loop): the line transform then fits
-// the instruction cache.  On return v = this warp's partial sums for all 1024 outputs.
-// POST = false (N = 2048 kernels, sfd_warp2048.cuh): the last multiply is left to the caller, on
-// return v = IFFT(H_b FFT(v)) N.
+// stage B with its 31 twiddles streamed from tensor memory (tt: first twiddle column of this
+// quarter) through the two chunk buffers: chunk j = t[8j .. 8j+7] of sfdb::dft32_tw
+__device__ __forceinline__ void tw_bf(float2 &a, float2 &b, const TChunk &c, int i) {
+    const float2 w = tm_val(c, i);
+    sfdb::bf(a, b, w.x, w.y);
+}
+__device__ __forceinline__ void dft32_tw_tm(float2 (&a)[32], unsigned tt, TChunk &c0, TChunk &c1) {
+    tm_ld(c0, tt);
+    tm_ld(c1, tt + 16);
+    sfdb::bit_reverse(a);
+    tm_wait(c0);
+    tm_wait(c1);
+#pragma unroll
+    for (int q = 0; q < 32; q += 2) tw_bf(a[q], a[q + 1], c0, 0);                     // level 2: t[0]
+#pragma unroll
+    for (int q = 0; q < 32; q += 4)
+#pragma unroll
+        for (int k = 0; k < 2; ++k) tw_bf(a[q + k], a[q + k + 2], c0, 1 + k);        // level 4: t[1..2]
+#pragma unroll
+    for (int q = 0; q < 32; q += 8)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) tw_bf(a[q + k], a[q + k + 4], c0, 3 + k);        // level 8: t[3..6]
+    tw_bf(a[0], a[8], c0, 7);                                                        // level 16, k = 0: t[7]
+    tw_bf(a[16], a[24], c0, 7);
+    tm_ld_before(c0, tt + 32, a[0].x);                                               // t[16..23] on their way
+#pragma unroll
+    for (int q = 0; q < 32; q += 16)
+#pragma unroll
+        for (int k = 1; k < 8; ++k) tw_bf(a[q + k], a[q + k + 8], c1, k - 1);        // k = 1..7: t[8..14]
+    tw_bf(a[0], a[16], c1, 7);                                                       // level 32, k = 0: t[15]
+    tm_wait(c0);
+    tm_ld_before(c1, tt + 48, a[0].x);                                               // t[24..30]
+#pragma unroll
+    for (int k = 1; k < 9; ++k) tw_bf(a[k], a[k + 16], c0, k - 1);                   // k = 1..8: t[16..23]
+    tm_wait(c1);
+#pragma unroll
+    for (int k = 9; k < 16; ++k) tw_bf(a[k], a[k + 16], c1, k - 9);                  // k = 9..15: t[24..30]
+}
+
 template <bool POST = true>
 __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
-                                       const float2 (&tw)[TWN], unsigned t, const Turns &turns) {
+                                       unsigned tt, unsigned t, const Turns &turns) {
 #pragma unroll 1
     for (int f = 0; f < 2; ++f) {
         sfdb::dft32(v);
@@ -322,8 +380,8 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
         TChunk c0, c1;
         const unsigned ta = t + f * TM_TAB;
         const bool mul = POST || f == 0;
-        if (mul) tm_ld_before(c0, ta, v[0].x);  // in flight during the butterflies
-        sfdb::dft32_tw(v, tw);
+        dft32_tw_tm(v, tt, c0, c1);
+        if (mul) tm_ld(c0, ta);
         // v[k] now holds out_sign(k) x the FFT value (sign tracking of sfd_dft32.cuh; the sign stage A
         // left behind depends on the lane and sits in the tables): the compile-time sign is applied
         // together with the conjugation / the table multiply
@@ -368,25 +426,34 @@ __device__ __forceinline__ void add_halves(float2 (&v)[32], float2 *mine, const 
     for (int q = 0; q < 16; ++q) v[16 * B + q] = padd(v[16 * B + q], theirs[q * 32 + lane]);
 }
 
-// ---- pass y: 4 adjacent hologram columns per CTA ---------------------------------------------------
-// The CTA is two independent halves of four warps (half h = warps 4h .. 4h+3 = two warp pairs);
-// half h transforms columns col0 + 2h and col0 + 2h + 1 of the CTA's current item.  Nothing
-// synchronises the two halves with each other except the turn-taking of the warps that share a
-// sub-partition (warps w and w + 4).
+// ---- pass y: 2 adjacent hologram columns per group of four warps ------------------------------------
+// The CTA is G = NW / 4 independent groups of four warps (group g = warps 4g .. 4g+3 = two warp
+// pairs); a group transforms two adjacent columns of the CTA's current item.  Nothing synchronises
+// the groups with each other except the turn-taking of the warps that share a sub-partition.
 //
 // Write-out.  B is [n1][m0] and a column's outputs are one element per row: written by the LSU
-// that is one 128-byte wavefront per row and store instruction (the v5 profile: 28 % of the
-// data-pipe time of this kernel).  Instead the warps of a half put their final sums into a dense
-// staging tile [n1][2 columns] (16 bytes per row) and one thread hands the tile to the TMA unit
-// (cp.async.bulk.tensor, shared -> global, four boxes of 256 rows x 16 bytes): the scatter costs the
-// LSU pipe nothing and runs beside the next item's butterflies.
-constexpr int WY = 8;  // warps per CTA
-constexpr int YC = 4;  // columns per item
-constexpr int YBOX = 256;  // rows of one TMA store box (the tensor map is built with this box)
-// Input slab of a half: SLAB_BYTES = 8 bytes of every hologram row = 2 columns x IPS items.  Half h
-// of item (slab s, k) transforms columns YC IPS s + 2 IPS h + 2 k + {0, 1}: the half reads its slab
-// once per IPS items with one 8-byte load per row (a 2-byte load per row and item costs the LSU one
-// wavefront per row just the same) and keeps it in shared memory as [k][n0] column pairs.
+// that is one 128-byte wavefront per row and store instruction.  Instead the warps of a group put
+// their final sums into a dense staging tile [n1][2 columns] (16 bytes per row) and one thread hands
+// the tile to the TMA unit (cp.async.bulk.tensor, shared -> global, four boxes of 256 rows x 16
+// bytes): the scatter costs the LSU pipe nothing and runs beside the next item's butterflies.
+// Warps per CTA of the N = 1024 kernels.  The loops below are written for any multiple of four and
+// were measured with 12 (three warps per sub-partition, 148 registers per thread with the twiddles in
+// tensor memory): per line 5 to 9 % faster, but V N / 148 = 27.7 lines per CTA are 7 rounds of 4 lines
+// (99 % full) against 5 rounds of 6 (92 %), which eats the gain: config 2 65.4k against 67k
+// reconstructions/s.  Turn-taking (Turns) needs one named barrier per warp: with 12 warps pass x has
+// none left for it (6 pair barriers + 12 > 15).
+#ifndef SFD_NW1024
+#define SFD_NW1024 8
+#endif
+constexpr int NW1024 = SFD_NW1024;
+constexpr bool TURNSY = true, TURNSX = NW1024 + NW1024 / 2 <= 15;  // turn-taking of the warps of a sub-partition
+constexpr int YBOX = 256;   // rows of one TMA store box (the tensor map is built with this box)
+// Input slab of a group: SLAB_BYTES = 8 bytes of every hologram row = 2 columns x IPS items.  An
+// item-group of IPS items covers 2 G IPS adjacent columns, group g owning the 2 IPS columns from
+// 2 IPS g on: the group reads its slab once per IPS items with one 8-byte load per row (a 2-byte load
+// per row and item costs the LSU one wavefront per row just the same) and keeps it in shared memory
+// as [k][n0] column pairs.  nx need not be a multiple of 2 G IPS: in the last item-group of a view
+// the groups whose columns lie beyond nx idle.
 template <typename TIn> struct TileElem {            // uint8: 4 items per slab
     using type = unsigned short;                     // 2 uint8 columns of a row
     using slab = uint2;
@@ -397,16 +464,16 @@ template <> struct TileElem<float> {                 // float: 1 item per slab
     using slab = float2;
     static constexpr int IPS = 1;
 };
-template <typename TIn> struct SmemY {
-    float2 xb[WY][XB];
-    alignas(128) float2 stage[2][N][2];  // [half][n1][column of the half]: final sums, TMA store source
-    typename TileElem<TIn>::type tile[2][TileElem<TIn>::IPS][N];  // [half][k][n0]: the half's slab
+template <typename TIn, int NW> struct SmemY {
+    float2 xb[NW][XB];
+    alignas(128) float2 stage[NW / 4][N][2];  // [group][n1][column of the group]: final sums, TMA store source
+    typename TileElem<TIn>::type tile[NW / 4][TileElem<TIn>::IPS][N];  // [group][k][n0]: the group's slab
     unsigned tmem;  // base address of the tensor-memory allocation
 };
 
 template <typename TIn> struct TileRegs { typename TileElem<TIn>::slab e[8]; };
 
-// the 128 threads of a half fetch rows ht, ht + 128, .. of the slab that starts at column col
+// the 128 threads of a group fetch rows ht, ht + 128, .. of the slab that starts at column col
 // (plain loads: the hologram was written by whatever ran before this kernel in the stream)
 template <typename TIn>
 __device__ __forceinline__ void tile_load(TileRegs<TIn> &t, const TIn *holo, long long hstride,
@@ -437,8 +504,8 @@ __device__ __forceinline__ float tile_value(unsigned short e, int c) {
 }
 __device__ __forceinline__ float tile_value(float2 e, int c) { return c ? e.y : e.x; }
 
-__device__ __forceinline__ void half_sync(int half) {  // named barrier of the four warps of a half
-    asm volatile("bar.sync %0, 128;" ::"r"(half + 1) : "memory");
+__device__ __forceinline__ void group_sync(int group) {  // named barrier of the four warps of a group
+    asm volatile("bar.sync %0, 128;" ::"r"(group + 1) : "memory");
 }
 // 2-D tiled bulk store shared -> global through tensor map `tm` (box fixed by the map); c0 = float
 // index within the row of B, c1 = row of B (view * N + n1)
@@ -454,18 +521,28 @@ __device__ __forceinline__ void bulk_wait_read() {
     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
-// Persistent CTA of 256 threads: work item = (view, group of 4 columns); a CTA takes a contiguous
-// range of items (at most two views: the launcher sizes the grid accordingly).  The line length is
-// N = 1024 = the number of hologram rows Ny; the number of columns nx (a multiple of 16) and the
-// hologram's row stride are run-time values (rectangular grids, windows inside a wider frame).
+// Columns of one view are cut into item-groups of 2 G IPS columns, IPS items each.
+template <typename TIn, int NW> struct YItems {
+    static constexpr int IPS = TileElem<TIn>::IPS, G = NW / 4, COLS = 2 * G * IPS;
+    static constexpr bool POW2 = (COLS & (COLS - 1)) == 0;  // then items per view is a power of two too
+    __device__ static int per_view(int nx) { return (nx + COLS - 1) / COLS * IPS; }
+    // item -> (view, item of the view): shifts when per_view is a power of two (nx is one)
+    __device__ static int view_of(int item, int ipv) { return POW2 ? item >> (31 - __clz(ipv)) : item / ipv; }
+    __device__ static int wrap(int g, int ipv) { return POW2 ? g & (ipv - 1) : g % ipv; }
+};
+
+// Persistent CTA of NW warps: work item = (view, 2 G columns); a CTA takes a contiguous range of
+// items (at most two views: the launcher sizes the grid accordingly).  The line length is N = 1024
+// = the number of hologram rows Ny; the number of columns nx (a multiple of 16) and the hologram's
+// row stride are run-time values (rectangular grids, windows inside a wider frame).
 // tabY: [2][3][N] per view (post carries c0, pre the 1/255 of uint8 input); tmB: tensor map of B seen
 // as float [V * N][2 nx] with box 4 x YBOX.
-// Per item a warp (column c of its half, branch B) transforms its column, hands the half of the
+// Per item a warp (column c of its group, branch B) transforms its column, hands the half of the
 // outputs it does not finish to its partner through its own transpose tile (idle by then), adds
 // what the partner left for it and writes 16 final values per thread into the staging tile.
 // The two places of a line that depend on the branch index at compile time (which half of the
 // register vector stays) are small functions instantiated for B = 0, 1 and entered through a
-// warp-uniform branch; everything else is ONE copy of code for all eight warps (half the
+// warp-uniform branch; everything else is ONE copy of code for all warps (half the
 // instruction-cache footprint of two template copies of the whole loop: measured, the
 // no_instruction stalls of the N = 2048 kernels, written this way, are a third of those of two copies).
 template <int B>
@@ -483,37 +560,55 @@ __device__ __forceinline__ void y_finish(const float2 (&v)[32], const float2 *xb
     }
 }
 
-template <typename TIn>
-__device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *holo, long long hstride,
-                                            int nx, unsigned tq, const float2 (&tw)[TWN],
-                                            const void *tmB, int V) {
+template <typename TIn, int NW, bool TURNS>
+__device__ __forceinline__ void pass_y_loop(SmemY<TIn, NW> &sm, const TIn *holo, long long hstride,
+                                            int nx, unsigned tq, unsigned tt, const void *tmB,
+                                            int V) {
+    using YI = YItems<TIn, NW>;
+    constexpr int IPS = YI::IPS, G = YI::G;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int half = warp >> 2, c = (warp >> 1) & 1, ht = threadIdx.x & 127, b = warp & 1;
-    const int groups = nx / YC, lgg = 31 - __clz(groups);  // nx is a power of two: shifts, not divisions
-    const int items = V * groups;
+    const int group = warp >> 2, c = (warp >> 1) & 1, ht = threadIdx.x & 127, b = warp & 1;
+    const int ipv = YI::per_view(nx);
+    const int items = V * ipv;
     const int i0 = (int)((long long)items * blockIdx.x / gridDim.x);
     const int i1 = (int)((long long)items * (blockIdx.x + 1) / gridDim.x);
     if (i0 >= i1) return;  // CTA-uniform
     float2 *xb = sm.xb[warp];
     const float2 *xbp = sm.xb[warp ^ 1];
-    float2 *stg = &sm.stage[half][0][0];
-    const bool leader = ht == 0;  // issues and retires the half's bulk stores
-    const int view0 = i0 >> lgg;
-    constexpr int IPS = TileElem<TIn>::IPS;
-    // groups % IPS == 0 (nx is a multiple of 16): a slab never straddles two views
+    float2 *stg = &sm.stage[group][0][0];
+    const bool leader = ht == 0;  // issues and retires the group's bulk stores
+    const int view0 = YI::view_of(i0, ipv);
+    // first column of this group's slab in the item-group of item g (of a view)
+    auto slab_col = [&](int g) { return g / IPS * YI::COLS + 2 * IPS * group; };
     {
-        TileRegs<TIn> t;
-        tile_load<TIn>(t, holo, hstride, (i0 & (groups - 1)) / IPS * (YC * IPS) + 2 * IPS * half, ht);
-        tile_store(t, sm.tile[half], ht);
+        const int col = slab_col(YI::wrap(i0, ipv));
+        if (YI::POW2 || col < nx) {
+            TileRegs<TIn> t;
+            tile_load<TIn>(t, holo, hstride, col, ht);
+            tile_store(t, sm.tile[group], ht);
+        }
     }
-    half_sync(half);
-    const Turns turns = turns_make(warp, true);
-    turns_open(turns, warp);
+    group_sync(group);
+    const Turns turns = turns_make(warp, NW, G + 1, TURNS);
+    turns_open(turns, warp, NW);
     for (int item = i0; item < i1; ++item) {
-        const int view = item >> lgg, g = item & (groups - 1), k = g % IPS;
-        const int colh = g / IPS * (YC * IPS) + 2 * IPS * half + 2 * k;
+        const int view = YI::view_of(item, ipv), g = item - view * ipv, k = g % IPS;
+        const int scol = slab_col(g), colh = scol + 2 * k;
         const unsigned tpre = tq + (view - view0) * TM_SET;  // pre_b | H_b | conj(post_b)
-        const bool has_next = item + 1 < i1 && k == IPS - 1;  // the next item opens a new slab
+        // the next item opens a new slab (that lies inside the hologram)
+        const int ncol = slab_col(YI::wrap(g + 1, ipv));
+        // (with COLS a power of two every item-group is complete: nx is a multiple of 16)
+        const bool has_next = item + 1 < i1 && k == IPS - 1 && (YI::POW2 || ncol < nx);
+        if (!YI::POW2 && scol >= nx) {  // group-uniform: this group's columns of the view's last item-group do not exist
+            turns_skip(turns);
+            if (has_next) {
+                TileRegs<TIn> t;
+                tile_load<TIn>(t, holo, hstride, ncol, ht);
+                tile_store(t, sm.tile[group], ht);
+                group_sync(group);
+            }
+            continue;
+        }
         TileRegs<TIn> t;
         float2 v[32];
         {
@@ -526,7 +621,7 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *holo, lon
                 if (j < 3) tm_ld((j & 1) ? c0 : c1, tpre + 16 * (j + 1));
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
-                    const float a = tile_value(sm.tile[half][k][lane + 32 * (8 * j + i)], c);
+                    const float a = tile_value(sm.tile[group][k][lane + 32 * (8 * j + i)], c);
                     const float2 p = tm_val(ch, i);
                     v[8 * j + i] = make_float2(a * p.x, a * p.y);
                 }
@@ -534,23 +629,22 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *holo, lon
         }
         // the next slab is fetched behind the tile reads: its loads touch one row per lane (32
         // wavefronts each) and would hold up everything queued after them
-        if (has_next)
-            tile_load<TIn>(t, holo, hstride, ((item + 1) & (groups - 1)) / IPS * (YC * IPS) + 2 * IPS * half, ht);
-        branch(v, lane, xb, tw, tpre + TM_TAB, turns);
+        if (has_next) tile_load<TIn>(t, holo, hstride, ncol, ht);
+        branch(v, lane, xb, tt, tpre + TM_TAB, turns);
         // the previous item's bulk stores must have left the staging tile before it is rewritten
         if (leader) bulk_wait_read();
         if (b == 0)
             y_hand_over<0>(v, xb, lane);
         else
             y_hand_over<1>(v, xb, lane);
-        half_sync(half);  // partner's hand-over visible; staging tile and input tile free
+        group_sync(group);  // partner's hand-over visible; staging tile and input tile free
         if (b == 0)
             y_finish<0>(v, xbp, stg, lane, c);
         else
             y_finish<1>(v, xbp, stg, lane, c);
-        if (has_next) tile_store(t, sm.tile[half], ht);
+        if (has_next) tile_store(t, sm.tile[group], ht);
         fence_async_smem();  // staging writes -> async proxy
-        half_sync(half);     // staging tile complete, next input tile visible, hand-over tiles free
+        group_sync(group);   // staging tile complete, next input tile visible, hand-over tiles free
         if (leader) {
 #pragma unroll
             for (int j = 0; j < N / YBOX; ++j)
@@ -563,18 +657,13 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *holo, lon
 }
 
 // ---- pass x: one row of B per warp pair -----------------------------------------------------------
-constexpr int WX = 8;        // warps per CTA
-constexpr int XP = WX / 2;   // pairs per CTA = rows in flight per CTA
-struct SmemX {
-    float2 xb[WX][XB];
-    float2 inb[XP][N];  // input row of each pair (bulk async copy destination)
-    unsigned long long ibar[XP];
+template <int NW> struct SmemX {
+    float2 xb[NW][XB];
+    float2 inb[NW / 2][N];  // input row of each pair (bulk async copy destination)
+    unsigned long long ibar[NW / 2];
     unsigned tmem;  // base address of the tensor-memory allocation
 };
 
-// Work unit = (view, group of XP adjacent rows); a CTA takes a contiguous range of units, so all
-// its pairs are always in the same view.  The line length is N = 1024 = the number of columns Nx;
-// the number of rows per view ny (a multiple of XP) is a run-time value.  tabX: [2][3][N] per view.
 // exchange of the halves, stores, reductions of one line for branch B (see y_hand_over)
 template <int B>
 __device__ __forceinline__ void x_finish(float2 (&v)[32], float2 *xb, const float2 *xbp, int lane,
@@ -618,37 +707,43 @@ __device__ __forceinline__ void x_finish(float2 (&v)[32], float2 *xb, const floa
     }
 }
 
-__device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *Bin, int ny, unsigned tq,
-                                            const float2 (&tw)[TWN], float2 *__restrict__ field,
+// A CTA takes a contiguous range of the V ny rows (at most two views: the launcher sizes the grid
+// accordingly) and walks it in rounds of XP = NW / 2 rows, pair p taking row l0 + XP r + p of round
+// r; in the last round the pairs beyond the end of the range idle.  The line length is N = 1024 =
+// the number of columns Nx; the number of rows per view ny (a power of two) is a run-time value.
+// tabX: [2][3][N] per view.
+template <int NW, bool TURNS>
+__device__ __forceinline__ void pass_x_loop(SmemX<NW> &sm, const float2 *Bin, int ny, unsigned tq,
+                                            unsigned tt, float2 *__restrict__ field,
                                             float *__restrict__ inten, unsigned int *vmax,
                                             double *mom, int V) {
+    constexpr int XP = NW / 2;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, pair = warp >> 1;
-    const int gpv = ny / XP, lgv = 31 - __clz(gpv);  // units per view; ny is a power of two
-    const int units = V * gpv;
-    const int u0 = (int)((long long)units * blockIdx.x / gridDim.x);
-    const int u1 = (int)((long long)units * (blockIdx.x + 1) / gridDim.x);
-    if (u0 >= u1) return;  // CTA-uniform
+    const int lgn = 31 - __clz(ny);
+    const int lines = V * ny;
+    const int l0 = (int)((long long)lines * blockIdx.x / gridDim.x);
+    const int l1 = (int)((long long)lines * (blockIdx.x + 1) / gridDim.x);
+    if (l0 >= l1) return;  // CTA-uniform
     float2 *xb = sm.xb[warp];
     const float2 *xbp = sm.xb[warp ^ 1];
     const float2 *in = sm.inb[pair] + lane;
     const int b = warp & 1;
     const bool issuer = b == 0 && lane == 0;
-    const int view0 = u0 >> lgv;
+    const int view0 = l0 >> lgn;
     unsigned iphase = 0;
-    bool pending = false;  // the pair's input row is already on its way
-    // turn-taking of warps w and w + 4 (needs every warp of the CTA to run the same number of
-    // lines: XP divides ny)
-    static_assert(WX == 8, "turn-taking pairs warps w and w + 4");
-    const Turns turns = turns_make(warp, true);
-    turns_open(turns, warp);
-    for (int u = u0; u < u1; ++u) {
-        const int view = u >> lgv, line = (u & (gpv - 1)) * XP + pair;
+    // turn-taking of the warps w, w + 4, .. of a sub-partition: named barriers behind the pairs' ones
+    const Turns turns = turns_make(warp, NW, XP + 1, TURNS);
+    turns_open(turns, warp, NW);
+    if (issuer && l0 + pair < l1)
+        bulk_load(sm.inb[pair], Bin + (size_t)(l0 + pair) * N, N * sizeof(float2), &sm.ibar[pair]);
+    for (int L = l0 + pair; L - pair < l1; L += XP) {
+        if (L >= l1) {  // pair-uniform: no row left for this pair in the last round
+            turns_skip(turns);
+            continue;
+        }
+        const int view = L >> lgn;
         const unsigned tpre = tq + (view - view0) * TM_SET;  // pre_b | H_b | conj(post_b)
-        const size_t row = (size_t)view * ny + line;
-        if (!pending && issuer)
-            bulk_load(sm.inb[pair], Bin + row * N, N * sizeof(float2), &sm.ibar[pair]);
-        const int nu = u + 1, nline = (nu & (gpv - 1)) * XP + pair;
-        const bool has_next = nu < u1;
+        const bool has_next = L + XP < l1;
         mbar_wait(&sm.ibar[pair], iphase);
         iphase ^= 1;
         float2 v[32];
@@ -669,15 +764,13 @@ __device__ __forceinline__ void pass_x_loop(SmemX &sm, const float2 *Bin, int ny
         pair_sync(pair);
         if (has_next && issuer) {
             fence_async_smem();
-            bulk_load(sm.inb[pair], Bin + ((size_t)(nu >> lgv) * ny + nline) * N, N * sizeof(float2),
-                      &sm.ibar[pair]);
+            bulk_load(sm.inb[pair], Bin + (size_t)(L + XP) * N, N * sizeof(float2), &sm.ibar[pair]);
         }
-        pending = has_next;
-        branch(v, lane, xb, tw, tpre + TM_TAB, turns);
+        branch(v, lane, xb, tt, tpre + TM_TAB, turns);
         if (b == 0)
-            x_finish<0>(v, xb, xbp, lane, pair, field, inten, row * N, mom, vmax, view);
+            x_finish<0>(v, xb, xbp, lane, pair, field, inten, (size_t)L * N, mom, vmax, view);
         else
-            x_finish<1>(v, xb, xbp, lane, pair, field, inten, row * N, mom, vmax, view);
+            x_finish<1>(v, xb, xbp, lane, pair, field, inten, (size_t)L * N, mom, vmax, view);
     }
     turns_close(turns, warp);
 }

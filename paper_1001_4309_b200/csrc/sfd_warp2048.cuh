@@ -31,7 +31,7 @@ constexpr int NL = 2048;            // line length
 constexpr int NBR = 4;              // branches per line
 constexpr int QTABS = NBR * 5 * N;  // complex elements of one view's tables of one pass: [4][5][N]
 // tensor-memory columns of the five tables of a branch
-constexpr int TQ_PREA = 0, TQ_PREB = 64, TQ_H = 128, TQ_POSTA = 192, TQ_POSTB = 256;
+constexpr int TQ_PREA = 0, TQ_PREB = 64, TQ_H = 128, TQ_POSTA = 192, TQ_POSTB = 256, TQ_TW = 320;
 // work units per view: pass x 2 rows (ny / 2 units), pass y 4 columns, 2 per quad (nx / 4 units)
 
 __device__ __forceinline__ void quad_sync(int quad) {  // named barrier of the four warps of a quad
@@ -64,12 +64,13 @@ __device__ __forceinline__ void tmq_fill(unsigned quarter, const float2 *__restr
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 __device__ __forceinline__ unsigned tmq_setup(unsigned *slot, const float2 *__restrict__ tab,
-                                              long long vstride, int view) {
+                                              long long vstride, int view, const float2 *__restrict__ twl) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (warp == 0) tm_alloc(slot);
     tm_sync_cta();
     const unsigned base = *reinterpret_cast<volatile unsigned *>(slot);
     tmq_fill(tm_quarter(base, warp), tab, vstride, view, warp, lane);
+    if (warp < 4) tm_fill_twiddles(tm_quarter(base, warp) + TQ_TW, twl, lane);
     tm_sync_cta();
     return base;
 }
@@ -142,7 +143,7 @@ struct SmemXQ {
 };
 
 __device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *Bin, int ny, unsigned tq,
-                                            const float2 (&tw)[TWN], float2 *__restrict__ field,
+                                            unsigned tt, float2 *__restrict__ field,
                                             float *__restrict__ inten, unsigned int *vmax,
                                             double *mom, Range rg) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, quad = warp >> 2, b = warp & 3;
@@ -151,8 +152,8 @@ __device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *Bin, int n
     const bool issuer = b == 0 && lane == 0;
     unsigned iphase = 0;
     bool pending = false;
-    const Turns turns = turns_make(warp, true);
-    turns_open(turns, warp);
+    const Turns turns = turns_make(warp, 8, 5, true);  // named barriers 5..12
+    turns_open(turns, warp, 8);
     for (int u = rg.u0; u < rg.u1; ++u) {
         const size_t row = (size_t)rg.view * ny + 2 * u + quad;
         if (!pending && issuer)
@@ -183,7 +184,7 @@ __device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *Bin, int n
             bulk_load(sm.inb[quad], Bin + (row + 2) * NL, NL * sizeof(float2), &sm.ibar[quad]);
         }
         pending = has_next;
-        branch<false>(v, lane, xb, tw, tq + TQ_H, turns);
+        branch<false>(v, lane, xb, tt, tq + TQ_H, turns);
         float2 mine[16];
         quad_scatter(v, mine, tq, b, lane, sm.xb, sm.ex, warp);
         quad_sync(quad);
@@ -301,7 +302,7 @@ __device__ __forceinline__ float2 fold_values(const float2 (&e)[2], int c) {
 // between hologram rows.
 template <typename TIn>
 __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, long long hstride,
-                                            unsigned tq, const float2 (&tw)[TWN], const void *tmB,
+                                            unsigned tq, unsigned tt, const void *tmB,
                                             Range rg) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, quad = warp >> 2, b = warp & 3;
     const int qt = threadIdx.x & 127;
@@ -316,8 +317,8 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, lo
         sub_store(t, sm.tile[quad], qt, quad);
     }
     quad_sync(quad);
-    const Turns turns = turns_make(warp, true);
-    turns_open(turns, warp);
+    const Turns turns = turns_make(warp, 8, 5, true);  // named barriers 5..12
+    turns_open(turns, warp, 8);
     for (int u = rg.u0; u < rg.u1; ++u) {
         const int k = u % IPS;
         const bool next_slab = u + 1 < rg.u1 && k == IPS - 1;
@@ -346,7 +347,7 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, lo
             // the loads here, 0.72 ms with the prefetch)
             if (cc == 1 && next_slab) sub_prefetch<TIn>(holo, hstride, SubSlab<TIn>::col(u + 1, quad), qt);
             quad_sync(quad);  // the previous column's exchange area has been read by all four warps
-            branch<false>(v, lane, xb, tw, tq + TQ_H, turns);
+            branch<false>(v, lane, xb, tt, tq + TQ_H, turns);
             // the previous unit's bulk stores must have left the staging tile before it is rewritten
             if (cc == 0 && leader) bulk_wait_read();
             float2 mine[16];
