@@ -19,6 +19,7 @@
 #include "sfd_internal.h"
 #include "sfd_warp1024.cuh"
 #include "sfd_warp2048.cuh"
+#include "sfd_warp512.cuh"
 
 namespace {
 
@@ -161,6 +162,45 @@ k_rows_1024(const float2 *B, int ny, const float2 *__restrict__ tabX, long long 
     sfdw::tm_finish(tbase);
 }
 
+// ---- axis length 512 (sfd_warp512.cuh): one warp per line, no branch split ---------------------------
+template <typename TIn>
+__global__ void __launch_bounds__(256, 1)
+k_cols_512(const TIn *holo, long long hstride, int nx, const float2 *__restrict__ tabY,
+           long long vstride, const float2 *__restrict__ twl, const __grid_constant__ CUtensorMap tmB,
+           unsigned int *vmax, double *mom, int V) {
+    extern __shared__ float4 smem4[];
+    sfdh::SmemYH<TIn> &sm = *reinterpret_cast<sfdh::SmemYH<TIn> *>(smem4);
+    sfdw::pdl_launch_dependents();
+    const int ipv = nx >> 3;  // items (8 columns) per view, as in pass_y_half
+    const unsigned tbase = sfdh::tmh_setup(&sm.tmem, tabY, vstride, V * ipv, ipv, twl);
+    const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
+    sfdw::pdl_wait();
+    if (vmax != nullptr && blockIdx.x == 0)
+        for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
+    if (mom != nullptr && blockIdx.x == 0)
+        for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
+    sfdh::pass_y_half<TIn>(sm, holo, hstride, nx, tq, &tmB, V);
+    sfdw::tm_finish(tbase);
+}
+
+__global__ void __launch_bounds__(256, 1)
+k_rows_512(const float2 *B, int ny, const float2 *__restrict__ tabX, long long vstride,
+           const float2 *__restrict__ twl, float2 *__restrict__ field, float *__restrict__ inten,
+           unsigned int *vmax, double *mom, int V) {
+    extern __shared__ float4 smem4[];
+    sfdh::SmemXH &sm = *reinterpret_cast<sfdh::SmemXH *>(smem4);
+    sfdw::pdl_launch_dependents();
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < 8; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
+        sfdw::mbar_fence_init();
+    }
+    const unsigned tbase = sfdh::tmh_setup(&sm.tmem, tabX, vstride, V * ny, ny, twl);
+    const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
+    sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
+    sfdh::pass_x_half(sm, B, ny, tq, field, inten, vmax, mom, V);
+    sfdw::tm_finish(tbase);
+}
+
 // ---- axis length 2048 (sfd_warp2048.cuh): four branches per line, a quad of warps per line ----------
 // grid = V * cpv CTAs: CTA c works on view c / cpv.  tab: [4][5][1024] per view.
 template <typename TIn>
@@ -272,10 +312,12 @@ struct Launch {
     }
 };
 
-// the slab loads of the warp kernels read 8 bytes of a hologram row at once
+// the slab loads of the warp kernels read 8 bytes of a hologram row at once (Ny = 512 with float
+// input: 16 bytes)
 bool slab_aligned(const sfd_plan *p, const void *holo) {
     const size_t es = p->d.in_dtype == 0 ? 1 : 4;
-    return (reinterpret_cast<size_t>(holo) & 7) == 0 && ((size_t)p->d.in_stride * es & 7) == 0;
+    const size_t mask = p->d.Ny == sfdh::NH && p->d.in_dtype != 0 ? 15 : 7;
+    return (reinterpret_cast<size_t>(holo) & mask) == 0 && ((size_t)p->d.in_stride * es & mask) == 0;
 }
 
 AxisTabs axis_y(const sfd_dev &d) { return AxisTabs{d.tabs, d.vstride, d.off_pre_y, d.off_Hy, d.off_post_y}; }
@@ -312,6 +354,18 @@ cudaError_t launch_y(sfd_plan *p, const void *holo, unsigned int *vmax, double *
         Launch l(dim3(grid), dim3(sfdw::NW1024 * 32), sizeof(sfdw::SmemY<float, sfdw::NW1024>), st);
         return cudaLaunchKernelEx(&l.cfg, k_cols_1024<float>, (const float *)holo, d.in_stride, d.Nx,
                                   tabY, d.vstride, (const float2 *)d.w_twl, tmB, vmax, mom, d.V);
+    }
+    if (sfd_uses_warp_y(p, holo) && d.Ny == sfdh::NH) {
+        const int grid = d.V > d.sms ? d.V : d.sms;
+        if (d.in_dtype == 0) {
+            Launch l(dim3(grid), dim3(256), sizeof(sfdh::SmemYH<unsigned char>), st);
+            return cudaLaunchKernelEx(&l.cfg, k_cols_512<unsigned char>, (const unsigned char *)holo,
+                                      d.in_stride, d.Nx, tabY, d.vstride, (const float2 *)d.w_twl, tmB,
+                                      vmax, mom, d.V);
+        }
+        Launch l(dim3(grid), dim3(256), sizeof(sfdh::SmemYH<float>), st);
+        return cudaLaunchKernelEx(&l.cfg, k_cols_512<float>, (const float *)holo, d.in_stride, d.Nx, tabY,
+                                  d.vstride, (const float2 *)d.w_twl, tmB, vmax, mom, d.V);
     }
     if (sfd_uses_warp_y(p, holo) && d.Ny == sfdq::NL) {
         const int cpv = d.sms / d.V > 0 ? d.sms / d.V : 1;  // CTAs per view: a CTA works inside one view
@@ -356,6 +410,11 @@ cudaError_t launch_x(sfd_plan *p, float2 *field, float *inten, unsigned int *vma
     if (sfd_uses_warp_x(p) && d.Nx == sfdw::N) {
         Launch l(dim3(d.V > d.sms ? d.V : d.sms), dim3(sfdw::NW1024 * 32), sizeof(sfdw::SmemX<sfdw::NW1024>), st);
         return cudaLaunchKernelEx(&l.cfg, k_rows_1024, (const float2 *)d.B, d.Ny, tabX, d.vstride,
+                                  (const float2 *)d.w_twl, field, inten, vmax, mom, d.V);
+    }
+    if (sfd_uses_warp_x(p) && d.Nx == sfdh::NH) {
+        Launch l(dim3(d.V > d.sms ? d.V : d.sms), dim3(256), sizeof(sfdh::SmemXH), st);
+        return cudaLaunchKernelEx(&l.cfg, k_rows_512, (const float2 *)d.B, d.Ny, tabX, d.vstride,
                                   (const float2 *)d.w_twl, field, inten, vmax, mom, d.V);
     }
     if (sfd_uses_warp_x(p) && d.Nx == sfdq::NL) {
@@ -442,6 +501,9 @@ cudaError_t sfd_kernels_init(int device, int *sms) {
     SFD_SMEM(k_cols_1024<unsigned char>, sizeof(sfdw::SmemY<unsigned char, sfdw::NW1024>))
     SFD_SMEM(k_cols_1024<float>, sizeof(sfdw::SmemY<float, sfdw::NW1024>))
     SFD_SMEM(k_rows_1024, sizeof(sfdw::SmemX<sfdw::NW1024>))
+    SFD_SMEM(k_cols_512<unsigned char>, sizeof(sfdh::SmemYH<unsigned char>))
+    SFD_SMEM(k_cols_512<float>, sizeof(sfdh::SmemYH<float>))
+    SFD_SMEM(k_rows_512, sizeof(sfdh::SmemXH))
     SFD_SMEM(k_cols_2048<unsigned char>, sizeof(sfdq::SmemYQ<unsigned char>))
     SFD_SMEM(k_cols_2048<float>, sizeof(sfdq::SmemYQ<float>))
     SFD_SMEM(k_rows_2048, sizeof(sfdq::SmemXQ))

@@ -227,7 +227,25 @@ void branch_tables4(const cd *pre, const cd *post, cd pre_scale, cd post_scale, 
         }
 }
 
-size_t fast_elems(int n) { return n == 1024 ? 6 * (size_t)1024 : n == 2048 ? 20 * (size_t)1024 : 0; }
+// Tables of an axis of length 512 (sfd_warp512.cuh): the padded transform is the 1024-point warp FFT
+// itself, no branch split; layout pre[512] | H[1024] | conj(post)[512], the two tables that follow an
+// FFT with the lane sign.
+void tables512(const cd *pre, const cd *post, cd pre_scale, cd post_scale, const float2 *H,
+               float2 *out) {
+    for (int n = 0; n < 512; ++n) {
+        const cd a = pre[n] * pre_scale, c = lane_sign(n) * std::conj(post[n] * post_scale);
+        out[n] = make_float2((float)a.real(), (float)a.imag());
+        out[512 + 1024 + n] = make_float2((float)c.real(), (float)c.imag());
+    }
+    for (int k = 0; k < 1024; ++k) {
+        const float sg = (float)lane_sign(k);
+        out[512 + k] = make_float2(sg * H[k].x, sg * H[k].y);
+    }
+}
+
+size_t fast_elems(int n) {
+    return n == 512 ? (size_t)2048 : n == 1024 ? 6 * (size_t)1024 : n == 2048 ? 20 * (size_t)1024 : 0;
+}
 
 // All float32 tables of view v in the device layout of sfd_dev (one contiguous block of
 // d.vstride complex values).  The y axis uses (p1y, p2y, O0y, Oy), the x axis (p1, p2, O0x, Ox):
@@ -246,6 +264,8 @@ void build_view_f32(const sfd_plan *p, int v, float2 *out) {
                 p->O0y[v]);
     to_f32(a.data(), out + d.off_pre_y, d.Ny, cd(in_scale, 0));
     to_f32(b.data(), out + d.off_post_y, d.Ny, c0);
+    if (d.off_tabY >= 0 && d.Ny == 512)
+        tables512(a.data(), b.data(), cd(in_scale, 0), c0, Hy, out + d.off_tabY);
     if (d.off_tabY >= 0 && d.Ny == 1024)
         branch_tables(d.Ny, a.data(), b.data(), cd(in_scale, 0), c0, Hy, out + d.off_tabY, p->wy);
     if (d.off_tabY >= 0 && d.Ny == 2048)
@@ -257,6 +277,8 @@ void build_view_f32(const sfd_plan *p, int v, float2 *out) {
                 p->O0x[v]);
     to_f32(a.data(), out + d.off_pre_x, d.Nx);
     to_f32(b.data(), out + d.off_post_x, d.Nx);
+    if (d.off_tabX >= 0 && d.Nx == 512)
+        tables512(a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, out + d.off_tabX);
     if (d.off_tabX >= 0 && d.Nx == 1024)
         branch_tables(d.Nx, a.data(), b.data(), cd(1, 0), cd(1, 0), Hx, out + d.off_tabX, p->wx);
     if (d.off_tabX >= 0 && d.Nx == 2048)

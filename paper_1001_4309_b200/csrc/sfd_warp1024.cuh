@@ -229,20 +229,28 @@ __device__ __forceinline__ void tm_fill_store(const TFill<NW> &f, unsigned quart
 #pragma unroll
     for (int j = 0; j < CH; ++j) tm_st(f.c[j], quarter + set * TM_SET + 16 * (ch0 + j));
 }
-// twl: [31][32] at [j][lane] (plan constant) -> 4 chunks of 8 values in this lane quarter
-__device__ __forceinline__ void tm_fill_twiddles(unsigned taddr, const float2 *__restrict__ twl, int lane) {
-#pragma unroll 1
-    for (int j = 0; j < 4; ++j) {
-        TChunk c;
+// twl: [31][32] at [j][lane] (plan constant) -> 4 chunks of 8 values in this lane quarter; all 31
+// loads of a thread in flight together (tw_load before the allocation, tw_store after it)
+struct TwFill { TChunk c[4]; };
+__device__ __forceinline__ void tw_load(TwFill &f, const float2 *__restrict__ twl, int lane) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
             const float2 x = (8 * j + i < 31) ? __ldg(twl + (8 * j + i) * 32 + lane) : make_float2(0.f, 0.f);
-            c.w[2 * i] = __float_as_uint(x.x);
-            c.w[2 * i + 1] = __float_as_uint(x.y);
+            f.c[j].w[2 * i] = __float_as_uint(x.x);
+            f.c[j].w[2 * i + 1] = __float_as_uint(x.y);
         }
-        tm_st(c, taddr + 16 * j);
-    }
+}
+__device__ __forceinline__ void tw_store(const TwFill &f, unsigned taddr) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) tm_st(f.c[j], taddr + 16 * j);
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tm_fill_twiddles(unsigned taddr, const float2 *__restrict__ twl, int lane) {
+    TwFill f;
+    tw_load(f, twl, lane);
+    tw_store(f, taddr);
 }
 // Kernel prologue (all NW warps): allocate, fill the one or two view sets this CTA's contiguous
 // range [total b / g, total (b + 1) / g) of work units touches (per_view units per view) and the
@@ -257,7 +265,9 @@ __device__ __forceinline__ unsigned tm_setup(unsigned *slot, const float2 *__res
     const int a1 = (int)((long long)total * (blockIdx.x + 1) / gridDim.x);
     const int view0 = a0 < a1 ? a0 / per_view : 0;
     TFill<NW> f;
+    TwFill ft;
     if (a0 < a1) tm_fill_load<NW>(f, tab, vstride, view0, warp, lane);  // on their way during the allocation
+    if (warp < 4) tw_load(ft, twl, lane);
     if (warp == 0) tm_alloc(slot);
     tm_sync_cta();
     const unsigned base = *reinterpret_cast<volatile unsigned *>(slot);
@@ -270,7 +280,7 @@ __device__ __forceinline__ unsigned tm_setup(unsigned *slot, const float2 *__res
         }
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     }
-    if (warp < 4) tm_fill_twiddles(tm_quarter(base, warp) + TM_TW, twl, lane);
+    if (warp < 4) tw_store(ft, tm_quarter(base, warp) + TM_TW);
     tm_sync_cta();
     return base;
 }
@@ -358,7 +368,9 @@ __device__ __forceinline__ void dft32_tw_tm(float2 (&a)[32], unsigned tt, TChunk
     for (int k = 9; k < 16; ++k) tw_bf(a[k], a[k + 16], c1, k - 9);                  // k = 9..15: t[24..30]
 }
 
-template <bool POST = true>
+// NOUT: chunks of 8 registers of the result that the caller keeps (the N = 512 kernels need the first
+// two: the post multiply skips the rest).
+template <bool POST = true, int NOUT = 4>
 __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
                                        unsigned tt, unsigned t, const Turns &turns) {
 #pragma unroll 1
@@ -396,9 +408,10 @@ __device__ __forceinline__ void branch(float2 (&v)[32], int lane, float2 *xb,
         } else {
 #pragma unroll
             for (int j = 0; j < 4; ++j) {  // v = conj(sign v * table)
+                if (NOUT < 4 && f == 1 && j >= NOUT) break;
                 TChunk &c = (j & 1) ? c1 : c0;
                 tm_wait(c);
-                if (j < 3) tm_ld((j & 1) ? c0 : c1, ta + 16 * (j + 1));
+                if (j < 3 && !(NOUT < 4 && f == 1 && j + 1 >= NOUT)) tm_ld((j & 1) ? c0 : c1, ta + 16 * (j + 1));
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
                     const float sg = (float)sfdb::out_sign(8 * j + i);

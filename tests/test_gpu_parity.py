@@ -504,6 +504,50 @@ def test_warp_kernels_bit_identical_under_concurrent_load(N, V, in_dtype, iters)
             assert torch.equal(f, f0) and torch.equal(I, I0), f"run {it} differs from the first"
 
 
+@pytest.mark.parametrize("in_dtype,V", [(B.SFD_U8, 4), (B.SFD_F32, 150)])
+def test_512_warp_and_generic_kernels_agree_with_oracle(in_dtype, V):
+    """N = 512 has two kernel sets: one warp per line (sfd_warp512.cuh: the padded line is exactly the
+    1024-point warp FFT) and the generic Stockham kernels.  Both against the oracle, with marked samples
+    in the last row/column; V = 150 > SMs makes CTA ranges straddle views; then the 8-bit mode and the
+    focus moments through the warp kernels."""
+    N = 512
+    rng = np.random.default_rng(512 + V)
+    base = W.config(2)
+    pick = rng.integers(0, 4, V)
+    if in_dtype == B.SFD_F32:
+        holo = rng.random((N, N), dtype=np.float32)
+        holo[N - 1, N - 1] = 40.0
+        holo[0, N - 3] = 25.0
+    else:
+        holo = rng.integers(0, 256, (N, N), dtype=np.uint8)
+        holo[N - 1, N - 1] = 255
+        holo[0, N - 3] = 0
+    kw = dict(N=N, lam=base.lam, p1=base.p1[pick], p2=base.p2[pick], z=base.z[pick] / 2, Ox=base.Ox[pick] / 2,
+              Oy=base.Oy[pick] / 2, in_dtype=in_dtype)
+    h = torch.from_numpy(holo).to(_dev())
+    with B.Plan(**kw) as plan:
+        assert plan.uses_warp_kernels
+        f, I = plan.execute(h)
+        mom, _ = plan.execute_focus(h)
+        u8 = plan.execute_u8(h) if V <= 8 else None
+        plan.select_kernels(B.SFD_KERNELS_GENERIC)
+        assert not plan.uses_warp_kernels
+        fg, _ = plan.execute(h)
+        torch.cuda.synchronize()
+    want, Iw = O.reconstruct_views(holo, base.lam, base.p1, base.p2, base.z / 2, base.Ox / 2, base.Oy / 2)
+    first = {int(k): int(np.flatnonzero(pick == k)[0]) for k in np.unique(pick)}
+    for k, v0 in first.items():
+        _assert_close(f[v0:v0 + 1].cpu().numpy(), want[k:k + 1], f"N=512 warp kernels, view {v0}")
+        _assert_close(I[v0:v0 + 1].cpu().numpy(), Iw[k:k + 1], f"N=512 warp kernels intensity, view {v0}")
+        _assert_close(fg[v0:v0 + 1].cpu().numpy(), want[k:k + 1], f"N=512 generic kernels, view {v0}")
+    for v in range(V):
+        assert torch.equal(f[v], f[first[int(pick[v])]]), f"view {v} differs from its twin"
+    m = mom.cpu().numpy()
+    assert np.max(np.abs(m / O.focus_moments(Iw)[pick] - 1.0)) < 1e-5
+    if u8 is not None:
+        _u8_check(u8.cpu().numpy(), Iw[pick], "N=512 u8")
+
+
 @pytest.mark.parametrize("N", [128, 1024])
 def test_execute_is_capturable_in_a_cuda_graph(N):
     """sfd_execute only enqueues kernels on the caller's stream (no allocation, no synchronisation), so a
@@ -587,9 +631,11 @@ def _rect_oracle(holo, g, form="B"):
 
 @pytest.mark.parametrize("Nx,Ny,in_dtype,mask", [
     (128, 64, B.SFD_F32, 0),        # generic kernels on both axes, two radix schedules
-    (64, 512, B.SFD_U8, 0),
+    (64, 512, B.SFD_U8, 1),         # pass y = k_cols_512 over 64 columns, pass x generic
+    (512, 128, B.SFD_F32, 2),       # pass y generic, pass x = k_rows_512 over 128 rows
     (256, 1024, B.SFD_U8, 1),       # pass y = k_cols_1024 over 256 columns, pass x generic
-    (1024, 512, B.SFD_U8, 2),       # pass y generic over 1024 columns, pass x = k_rows_1024 over 512 rows
+    (1024, 512, B.SFD_U8, 3),       # pass y = k_cols_512 over 1024 columns, pass x = k_rows_1024 over 512 rows
+    (512, 2048, B.SFD_F32, 3),      # k_cols_2048 + k_rows_512
     (2048, 1024, B.SFD_F32, 3),     # k_cols_1024 + k_rows_2048
     (1024, 2048, B.SFD_U8, 3),      # k_cols_2048 + k_rows_1024
 ])
