@@ -202,32 +202,37 @@ k_rows_512(const float2 *B, int ny, const float2 *__restrict__ tabX, long long v
 }
 
 // ---- axis length 2048 (sfd_warp2048.cuh): four branches per line, a quad of warps per line ----------
-// grid = V * cpv CTAs: CTA c works on view c / cpv.  tab: [4][5][1024] per view.
+// One CTA per SM (at least V); a CTA's range of work units may cross into the next view once
+// (sfdq::Span).  tab: [4][5][1024] per view.
 template <typename TIn>
 __global__ void __launch_bounds__(256, 1)
 k_cols_2048(const TIn *holo, long long hstride, int nx, const float2 *__restrict__ tabY,
             long long vstride, const float2 *__restrict__ twl,
-            const __grid_constant__ CUtensorMap tmB, unsigned int *vmax, double *mom, int V,
-            int cpv) {
+            const __grid_constant__ CUtensorMap tmB, unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
     sfdq::SmemYQ<TIn> &sm = *reinterpret_cast<sfdq::SmemYQ<TIn> *>(smem4);
     sfdw::pdl_launch_dependents();
-    const sfdq::Range rg = sfdq::cta_range(cpv, nx / 4);
-    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabY, vstride, rg.view, twl);
+    const sfdq::Span span = sfdq::cta_span(V, nx / 4);
+    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabY, vstride, span.first_view(), twl);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     sfdw::pdl_wait();
     if (vmax != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
     if (mom != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
-    sfdq::pass_y_quad<TIn>(sm, holo, hstride, tq, tq + sfdq::TQ_TW, &tmB, rg);
+    for (int s = 0; s < 2; ++s) {
+        const sfdq::Range rg = span.segment(s);
+        if (rg.u0 >= rg.u1) break;
+        if (s == 1) sfdq::tmq_refill(tbase, tabY, vstride, rg.view);
+        sfdq::pass_y_quad<TIn>(sm, holo, hstride, tq, tq + sfdq::TQ_TW, &tmB, rg);
+    }
     sfdw::tm_finish(tbase);
 }
 
 __global__ void __launch_bounds__(256, 1)
 k_rows_2048(const float2 *B, int ny, const float2 *__restrict__ tabX, long long vstride,
             const float2 *__restrict__ twl, float2 *__restrict__ field, float *__restrict__ inten,
-            unsigned int *vmax, double *mom, int cpv) {
+            unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
     sfdq::SmemXQ &sm = *reinterpret_cast<sfdq::SmemXQ *>(smem4);
     sfdw::pdl_launch_dependents();
@@ -236,11 +241,17 @@ k_rows_2048(const float2 *B, int ny, const float2 *__restrict__ tabX, long long 
         sfdw::mbar_init(&sm.ibar[1], 1);
         sfdw::mbar_fence_init();
     }
-    const sfdq::Range rg = sfdq::cta_range(cpv, ny / 2);
-    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabX, vstride, rg.view, twl);
+    const sfdq::Span span = sfdq::cta_span(V, ny / 2);
+    const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabX, vstride, span.first_view(), twl);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
-    sfdq::pass_x_quad(sm, B, ny, tq, tq + sfdq::TQ_TW, field, inten, vmax, mom, rg);
+    unsigned iphase = 0;
+    for (int s = 0; s < 2; ++s) {
+        const sfdq::Range rg = span.segment(s);
+        if (rg.u0 >= rg.u1) break;
+        if (s == 1) sfdq::tmq_refill(tbase, tabX, vstride, rg.view);
+        sfdq::pass_x_quad(sm, B, ny, tq, tq + sfdq::TQ_TW, field, inten, vmax, mom, rg, iphase);
+    }
     sfdw::tm_finish(tbase);
 }
 
@@ -368,16 +379,16 @@ cudaError_t launch_y(sfd_plan *p, const void *holo, unsigned int *vmax, double *
                                   d.vstride, (const float2 *)d.w_twl, tmB, vmax, mom, d.V);
     }
     if (sfd_uses_warp_y(p, holo) && d.Ny == sfdq::NL) {
-        const int cpv = d.sms / d.V > 0 ? d.sms / d.V : 1;  // CTAs per view: a CTA works inside one view
+        const int grid = d.V > d.sms ? d.V : d.sms;
         if (d.in_dtype == 0) {
-            Launch l(dim3(d.V * cpv), dim3(256), sizeof(sfdq::SmemYQ<unsigned char>), st);
+            Launch l(dim3(grid), dim3(256), sizeof(sfdq::SmemYQ<unsigned char>), st);
             return cudaLaunchKernelEx(&l.cfg, k_cols_2048<unsigned char>, (const unsigned char *)holo,
                                       d.in_stride, d.Nx, tabY, d.vstride, (const float2 *)d.w_twl, tmB,
-                                      vmax, mom, d.V, cpv);
+                                      vmax, mom, d.V);
         }
-        Launch l(dim3(d.V * cpv), dim3(256), sizeof(sfdq::SmemYQ<float>), st);
+        Launch l(dim3(grid), dim3(256), sizeof(sfdq::SmemYQ<float>), st);
         return cudaLaunchKernelEx(&l.cfg, k_cols_2048<float>, (const float *)holo, d.in_stride, d.Nx,
-                                  tabY, d.vstride, (const float2 *)d.w_twl, tmB, vmax, mom, d.V, cpv);
+                                  tabY, d.vstride, (const float2 *)d.w_twl, tmB, vmax, mom, d.V);
     }
     switch (d.log2My) {
         case 7: return launch_y_generic<7>(d, holo, vmax, mom, st);
@@ -418,10 +429,9 @@ cudaError_t launch_x(sfd_plan *p, float2 *field, float *inten, unsigned int *vma
                                   (const float2 *)d.w_twl, field, inten, vmax, mom, d.V);
     }
     if (sfd_uses_warp_x(p) && d.Nx == sfdq::NL) {
-        const int cpv = d.sms / d.V > 0 ? d.sms / d.V : 1;
-        Launch l(dim3(d.V * cpv), dim3(256), sizeof(sfdq::SmemXQ), st);
+        Launch l(dim3(d.V > d.sms ? d.V : d.sms), dim3(256), sizeof(sfdq::SmemXQ), st);
         return cudaLaunchKernelEx(&l.cfg, k_rows_2048, (const float2 *)d.B, d.Ny, tabX, d.vstride,
-                                  (const float2 *)d.w_twl, field, inten, vmax, mom, cpv);
+                                  (const float2 *)d.w_twl, field, inten, vmax, mom, d.V);
     }
     switch (d.log2Mx) {
         case 7: return launch_x_generic<7>(d, field, inten, vmax, mom, st);

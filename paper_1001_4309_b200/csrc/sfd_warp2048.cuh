@@ -75,11 +75,29 @@ __device__ __forceinline__ unsigned tmq_setup(unsigned *slot, const float2 *__re
     return base;
 }
 
-// This CTA's view and its contiguous range of the view's `units` work units (cpv CTAs per view).
+// A CTA takes a contiguous range [a0, a1) of the V * units work units of a launch.  The five tables
+// of a branch fill 320 of the 512 tensor-memory columns, so only one view's tables are resident: a
+// range that crosses into the next view (at most once: the grid has at least V CTAs) is walked as
+// two segments with the tables reloaded in between (segment() is CTA-uniform).
 struct Range { int view, u0, u1; };
-__device__ __forceinline__ Range cta_range(int cpv, int units) {
-    const int view = blockIdx.x / cpv, idx = blockIdx.x % cpv;
-    return Range{view, (int)((long long)units * idx / cpv), (int)((long long)units * (idx + 1) / cpv)};
+struct Span {
+    int a0, a1, units;
+    __device__ int first_view() const { return a0 < a1 ? a0 / units : 0; }
+    __device__ Range segment(int s) const {  // s = 0, 1; empty if u0 >= u1
+        const int view = first_view() + s, lo = view * units, hi = lo + units;
+        return Range{view, (a0 > lo ? a0 : lo) - lo, (a1 < hi ? a1 : hi) - lo};
+    }
+};
+__device__ __forceinline__ Span cta_span(int V, int units) {
+    const long long total = (long long)V * units;
+    return Span{(int)(total * blockIdx.x / gridDim.x), (int)(total * (blockIdx.x + 1) / gridDim.x), units};
+}
+// all warps have finished with the resident tables: load those of `view`
+__device__ __forceinline__ void tmq_refill(unsigned base, const float2 *__restrict__ tab,
+                                           long long vstride, int view) {
+    tm_sync_cta();
+    tmq_fill(tm_quarter(base, threadIdx.x >> 5), tab, vstride, view, threadIdx.x >> 5, threadIdx.x & 31);
+    tm_sync_cta();
 }
 
 // Exchange area of a warp: three quarters of 16 x 32 values for the other three warps of the quad
@@ -145,13 +163,12 @@ struct SmemXQ {
 __device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *Bin, int ny, unsigned tq,
                                             unsigned tt, float2 *__restrict__ field,
                                             float *__restrict__ inten, unsigned int *vmax,
-                                            double *mom, Range rg) {
+                                            double *mom, Range rg, unsigned &iphase) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, quad = warp >> 2, b = warp & 3;
     float2 *xb = sm.xb[warp];
     const float2 *in = sm.inb[quad] + lane;
     const bool issuer = b == 0 && lane == 0;
-    unsigned iphase = 0;
-    bool pending = false;
+    bool pending = false;  // (iphase: parity of the quad's input barrier, carried across segments)
     const Turns turns = turns_make(warp, 8, 5, true);  // named barriers 5..12
     turns_open(turns, warp, 8);
     for (int u = rg.u0; u < rg.u1; ++u) {
