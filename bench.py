@@ -443,7 +443,8 @@ def run_sfd(args, info):
     extras = None
     if info.is_root and not args.no_extras:
         extras = {"steering": steering(plan, wl, holos[0], stream, torch, B),
-                  "angular_spectrum": asm_line(wl, dev, torch, B, np)}
+                  "angular_spectrum": asm_line(wl, dev, torch, B, np),
+                  "other_sizes": sizes_line(wl, dev, torch, B)}
     sampler.stop()
 
     cpu = None
@@ -538,6 +539,32 @@ def asm_line(wl, dev, torch, B, np, reps=200):
     return {"propagations_per_s": round(1.0 / sec, 1), "us": round(sec * 1e6, 2), "N": N,
             "algorithmic_bytes": by, "gbs": round(by / sec / 1e9, 1),
             "api": "sfd_asm_execute: 3 launches (rows FFT, columns FFT x H x IFFT, rows IFFT + |u|^2 + arg u)"}
+
+
+def sizes_line(wl, dev, torch, B, steps=600):
+    """The same views on smaller square holograms (uint8, field + intensity out): us per frame.
+    N = 512 runs the one-warp-per-line kernels, the smaller sizes the generic Stockham kernels."""
+    out = {}
+    stream = torch.cuda.current_stream()
+    for N in (512, 256, 128):
+        R = 8
+        holos = [torch.randint(0, 256, (N, N), dtype=torch.uint8, device=dev) for _ in range(R)]
+        f = [torch.empty((wl.n_views, N, N), dtype=torch.complex64, device=dev) for _ in range(R)]
+        I = [torch.empty((wl.n_views, N, N), dtype=torch.float32, device=dev) for _ in range(R)]
+        with B.Plan(N=N, lam=wl.lam, p1=wl.p1, p2=wl.p2, z=wl.z, Ox=wl.Ox, Oy=wl.Oy, in_dtype=B.SFD_U8) as plan:
+            for i in range(20):
+                B.sfd_execute(plan.handle, holos[i % R], f[i % R], I[i % R], stream)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for i in range(steps):
+                B.sfd_execute(plan.handle, holos[i % R], f[i % R], I[i % R], stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            out[f"N{N}"] = {"us_per_frame": round(e0.elapsed_time(e1) * 1e3 / steps, 2),
+                            "warp_kernels": plan.uses_warp_kernels}
+    out["note"] = (f"{wl.n_views} views of {wl.name}, uint8 in, complex64 field + float32 intensity out; the small "
+                   "sizes are bound by the launch rate of the host (a CUDA graph of sfd_execute calls removes that)")
+    return out
 
 
 def run_peaks():
