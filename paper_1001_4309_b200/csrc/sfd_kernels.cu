@@ -132,13 +132,16 @@ k_cols_1024(const TIn *holo, long long hstride, int nx, const float2 *__restrict
     // tables of this CTA's view(s) -> tensor memory
     const unsigned tbase = sfdw::tm_setup<sfdw::NW1024>(&sm.tmem, tabY, vstride, V * ipv, ipv, twl);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
-    // everything above touches plan constants only; the hologram, B, vmax and mom belong to the
-    // kernels before this one in the stream
-    sfdw::pdl_wait();
-    if (vmax != nullptr && blockIdx.x == 0)
-        for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
-    if (mom != nullptr && blockIdx.x == 0)
-        for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
+    // everything above touches plan constants only.  B, vmax and mom belong to the kernels before
+    // this one in the stream: the threads that write them wait for those kernels first - block 0 here
+    // (8-bit and focus modes only), the store leaders in front of their first store of B
+    if ((vmax != nullptr || mom != nullptr) && blockIdx.x == 0) {
+        sfdw::pdl_wait();
+        if (vmax != nullptr)
+            for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
+        if (mom != nullptr)
+            for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
+    }
     sfdw::pass_y_loop<TIn, sfdw::NW1024, sfdw::TURNSY>(sm, holo, hstride, nx, tq, tq + sfdw::TM_TW, &tmB, V);
     sfdw::tm_finish(tbase);
 }

@@ -659,6 +659,15 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn, NW> &sm, const TIn *holo,
         fence_async_smem();  // staging writes -> async proxy
         group_sync(group);   // staging tile complete, next input tile visible, hand-over tiles free
         if (leader) {
+            // Programmatic dependent launch: the only thing pass y does to memory that the kernel
+            // before it may still be using is to overwrite B (pass x of the frame before reads it),
+            // and the only thread that does so is this one.  It waits here, in front of its first
+            // store, instead of at the top of the kernel: a CTA that got its SM early (the CTAs of the
+            // kernel before do not all finish together) works on its first columns meanwhile.  The
+            // hologram is never written by a kernel of this library; whatever else produced it was
+            // complete before this kernel could start (only our own kernels release their dependents
+            // early).
+            if (item == i0) pdl_wait();
 #pragma unroll
             for (int j = 0; j < N / YBOX; ++j)
                 tma_store_2d(tmB, stg + j * YBOX * 2, 2 * colh, view * N + j * YBOX);
