@@ -108,29 +108,38 @@ k_quantise(const float4 *inten, const unsigned int *vmax, uchar4 *__restrict__ o
     }
 }
 
-// ---- axis length 1024 (sfd_warp1024.cuh): persistent kernels, one warp pair per line ---------------
-// One CTA per SM.  Even warps run branch 0 (even bins), odd warps branch 1.
-// k_cols_1024: Ny = 1024 rows, nx columns (lines).  k_rows_1024: Nx = 1024 columns, ny rows (lines).
+// ---- axis length 1024 (sfd_warp1024.cuh): persistent kernels ------------------------------------------
+// One CTA per SM.  k_cols_1024: Ny = 1024 rows, nx columns (lines); grid = V * cpv, CTA c works on
+// view c / cpv (solo and split rounds, see pass_y_loop).  k_rows_1024: Nx = 1024 columns, ny rows
+// (lines), a warp pair per line, even warps branch 0 (even bins), odd warps branch 1.
 template <typename TIn>
-__global__ void __launch_bounds__(sfdw::NW1024 * 32, 1)
+__global__ void __launch_bounds__(256, 1)
 k_cols_1024(const TIn *holo, long long hstride, int nx, const float2 *__restrict__ tabY,
             long long vstride, const float2 *__restrict__ twl,
-            const __grid_constant__ CUtensorMap tmB, unsigned int *vmax, double *mom, int V) {
+            const __grid_constant__ CUtensorMap tmB, unsigned int *vmax, double *mom, int V,
+            int cpv) {
     extern __shared__ float4 smem4[];
-    using SM = sfdw::SmemY<TIn, sfdw::NW1024>;
+    using SM = sfdw::SmemY<TIn>;
     SM &sm = *reinterpret_cast<SM *>(smem4);
     sfdw::pdl_launch_dependents();
-    const int ipv = sfdw::YItems<TIn, sfdw::NW1024>::per_view(nx);  // items per view, as in pass_y_loop
-    {   // pull the first slab of this CTA towards L2 while the prologue runs (a prefetch reads nothing:
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < 2; ++i) {
+            sfdw::mbar_init(&sm.full[i], 8);
+            sfdw::mbar_init(&sm.empty[i], 8);
+        }
+        sfdw::mbar_fence_init();
+    }
+    const int view = blockIdx.x / cpv;
+    const sfdw::YPlan yp = sfdw::YPlan::make(nx, blockIdx.x % cpv, cpv);
+    if (yp.rounds() > 0) {
+        // pull the first slab of this CTA towards L2 while the prologue runs (a prefetch reads nothing:
         // it may precede griddepcontrol.wait)
-        using YI = sfdw::YItems<TIn, sfdw::NW1024>;
-        const int i0 = (int)((long long)V * ipv * blockIdx.x / gridDim.x);
-        const TIn *p0 = holo + (i0 % ipv) / YI::IPS * YI::COLS;
+        const TIn *p0 = holo + (yp.col(0) & ~7);
         for (int r = threadIdx.x; r < sfdw::N; r += blockDim.x)
             asm volatile("prefetch.global.L2 [%0];" ::"l"(p0 + (size_t)r * hstride));
     }
-    // tables of this CTA's view(s) -> tensor memory
-    const unsigned tbase = sfdw::tm_setup<sfdw::NW1024>(&sm.tmem, tabY, vstride, V * ipv, ipv, twl);
+    // tables of both branches of this CTA's view -> tensor memory
+    const unsigned tbase = sfdw::tm_setup_both(&sm.tmem, tabY, vstride, view, twl);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     // everything above touches plan constants only.  B, vmax and mom belong to the kernels before
     // this one in the stream: the threads that write them wait for those kernels first - block 0 here
@@ -142,26 +151,26 @@ k_cols_1024(const TIn *holo, long long hstride, int nx, const float2 *__restrict
         if (mom != nullptr)
             for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
     }
-    sfdw::pass_y_loop<TIn, sfdw::NW1024, sfdw::TURNSY>(sm, holo, hstride, nx, tq, tq + sfdw::TM_TW, &tmB, V);
+    sfdw::pass_y_loop<TIn>(sm, holo, hstride, nx, tq, tq + sfdw::TM_TW, &tmB, view, yp);
     sfdw::tm_finish(tbase);
 }
 
-__global__ void __launch_bounds__(sfdw::NW1024 * 32, 1)
+__global__ void __launch_bounds__(sfdw::NWX * 32, 1)
 k_rows_1024(const float2 *B, int ny, const float2 *__restrict__ tabX, long long vstride,
             const float2 *__restrict__ twl, float2 *__restrict__ field, float *__restrict__ inten,
             unsigned int *vmax, double *mom, int V) {
     extern __shared__ float4 smem4[];
-    using SM = sfdw::SmemX<sfdw::NW1024>;
+    using SM = sfdw::SmemX<sfdw::NWX>;
     SM &sm = *reinterpret_cast<SM *>(smem4);
     sfdw::pdl_launch_dependents();
     if (threadIdx.x == 0) {
-        for (int i = 0; i < sfdw::NW1024 / 2; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
+        for (int i = 0; i < sfdw::NWX / 2; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
         sfdw::mbar_fence_init();
     }
-    const unsigned tbase = sfdw::tm_setup<sfdw::NW1024>(&sm.tmem, tabX, vstride, V * ny, ny, twl);
+    const unsigned tbase = sfdw::tm_setup<sfdw::NWX>(&sm.tmem, tabX, vstride, V * ny, ny, twl);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
     sfdw::pdl_wait();  // B (and vmax, mom) come from pass y
-    sfdw::pass_x_loop<sfdw::NW1024, sfdw::TURNSX>(sm, B, ny, tq, tq + sfdw::TM_TW, field, inten, vmax, mom, V);
+    sfdw::pass_x_loop<sfdw::NWX, true>(sm, B, ny, tq, tq + sfdw::TM_TW, field, inten, vmax, mom, V);
     sfdw::tm_finish(tbase);
 }
 
@@ -327,10 +336,10 @@ struct Launch {
 };
 
 // the slab loads of the warp kernels read 8 bytes of a hologram row at once (Ny = 512 with float
-// input: 16 bytes)
+// or 1024 with float input: 16 bytes)
 bool slab_aligned(const sfd_plan *p, const void *holo) {
     const size_t es = p->d.in_dtype == 0 ? 1 : 4;
-    const size_t mask = p->d.Ny == sfdh::NH && p->d.in_dtype != 0 ? 15 : 7;
+    const size_t mask = (p->d.Ny == sfdh::NH || p->d.Ny == sfdw::N) && p->d.in_dtype != 0 ? 15 : 7;
     return (reinterpret_cast<size_t>(holo) & mask) == 0 && ((size_t)p->d.in_stride * es & mask) == 0;
 }
 
@@ -356,18 +365,18 @@ cudaError_t launch_y(sfd_plan *p, const void *holo, unsigned int *vmax, double *
     const CUtensorMap &tmB = *reinterpret_cast<const CUtensorMap *>(p->tmapB);
     const float2 *tabY = d.tabs + d.off_tabY;
     if (sfd_uses_warp_y(p, holo) && d.Ny == sfdw::N) {
-        // one CTA per SM, but at least V CTAs: a CTA's contiguous range of items then touches at most
-        // two views (the kernel holds two table sets)
-        const int grid = d.V > d.sms ? d.V : d.sms;
+        // a CTA works inside one view (its tensor memory holds both branches' tables of that view):
+        // SMs / V CTAs per view
+        const int cpv = d.sms / d.V > 0 ? d.sms / d.V : 1;
         if (d.in_dtype == 0) {
-            Launch l(dim3(grid), dim3(sfdw::NW1024 * 32), sizeof(sfdw::SmemY<unsigned char, sfdw::NW1024>), st);
+            Launch l(dim3(d.V * cpv), dim3(256), sizeof(sfdw::SmemY<unsigned char>), st);
             return cudaLaunchKernelEx(&l.cfg, k_cols_1024<unsigned char>, (const unsigned char *)holo,
                                       d.in_stride, d.Nx, tabY, d.vstride, (const float2 *)d.w_twl, tmB,
-                                      vmax, mom, d.V);
+                                      vmax, mom, d.V, cpv);
         }
-        Launch l(dim3(grid), dim3(sfdw::NW1024 * 32), sizeof(sfdw::SmemY<float, sfdw::NW1024>), st);
+        Launch l(dim3(d.V * cpv), dim3(256), sizeof(sfdw::SmemY<float>), st);
         return cudaLaunchKernelEx(&l.cfg, k_cols_1024<float>, (const float *)holo, d.in_stride, d.Nx,
-                                  tabY, d.vstride, (const float2 *)d.w_twl, tmB, vmax, mom, d.V);
+                                  tabY, d.vstride, (const float2 *)d.w_twl, tmB, vmax, mom, d.V, cpv);
     }
     if (sfd_uses_warp_y(p, holo) && d.Ny == sfdh::NH) {
         const int grid = d.V > d.sms ? d.V : d.sms;
@@ -422,7 +431,7 @@ cudaError_t launch_x(sfd_plan *p, float2 *field, float *inten, unsigned int *vma
     const sfd_dev &d = p->d;
     const float2 *tabX = d.tabs + d.off_tabX;
     if (sfd_uses_warp_x(p) && d.Nx == sfdw::N) {
-        Launch l(dim3(d.V > d.sms ? d.V : d.sms), dim3(sfdw::NW1024 * 32), sizeof(sfdw::SmemX<sfdw::NW1024>), st);
+        Launch l(dim3(d.V > d.sms ? d.V : d.sms), dim3(sfdw::NWX * 32), sizeof(sfdw::SmemX<sfdw::NWX>), st);
         return cudaLaunchKernelEx(&l.cfg, k_rows_1024, (const float2 *)d.B, d.Ny, tabX, d.vstride,
                                   (const float2 *)d.w_twl, field, inten, vmax, mom, d.V);
     }
@@ -511,9 +520,9 @@ cudaError_t sfd_kernels_init(int device, int *sms) {
     if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,        \
                                   (int)(bytes))) != cudaSuccess)                              \
         return e;
-    SFD_SMEM(k_cols_1024<unsigned char>, sizeof(sfdw::SmemY<unsigned char, sfdw::NW1024>))
-    SFD_SMEM(k_cols_1024<float>, sizeof(sfdw::SmemY<float, sfdw::NW1024>))
-    SFD_SMEM(k_rows_1024, sizeof(sfdw::SmemX<sfdw::NW1024>))
+    SFD_SMEM(k_cols_1024<unsigned char>, sizeof(sfdw::SmemY<unsigned char>))
+    SFD_SMEM(k_cols_1024<float>, sizeof(sfdw::SmemY<float>))
+    SFD_SMEM(k_rows_1024, sizeof(sfdw::SmemX<sfdw::NWX>))
     SFD_SMEM(k_cols_512<unsigned char>, sizeof(sfdh::SmemYH<unsigned char>))
     SFD_SMEM(k_cols_512<float>, sizeof(sfdh::SmemYH<float>))
     SFD_SMEM(k_rows_512, sizeof(sfdh::SmemXH))

@@ -439,76 +439,96 @@ __device__ __forceinline__ void add_halves(float2 (&v)[32], float2 *mine, const 
     for (int q = 0; q < 16; ++q) v[16 * B + q] = padd(v[16 * B + q], theirs[q * 32 + lane]);
 }
 
-// ---- pass y: 2 adjacent hologram columns per group of four warps ------------------------------------
-// The CTA is G = NW / 4 independent groups of four warps (group g = warps 4g .. 4g+3 = two warp
-// pairs); a group transforms two adjacent columns of the CTA's current item.  Nothing synchronises
-// the groups with each other except the turn-taking of the warps that share a sub-partition.
+// ---- pass y: hologram columns, 8 warps per CTA ------------------------------------------------------
+// A CTA works inside one view (the launcher gives every view cpv = SMs / V CTAs) and its tensor-memory
+// quarters hold the tables of BOTH branches of that view (2 x 192 columns + the twiddles).  Its
+// columns come in two kinds of rounds:
 //
-// Write-out.  B is [n1][m0] and a column's outputs are one element per row: written by the LSU
-// that is one 128-byte wavefront per row and store instruction.  Instead the warps of a group put
-// their final sums into a dense staging tile [n1][2 columns] (16 bytes per row) and one thread hands
-// the tile to the TMA unit (cp.async.bulk.tensor, shared -> global, four boxes of 256 rows x 16
-// bytes): the scatter costs the LSU pipe nothing and runs beside the next item's butterflies.
-// Warps per CTA of the N = 1024 kernels.  The loops below are written for any multiple of four and
-// were measured with 12 (three warps per sub-partition, 148 registers per thread with the twiddles in
-// tensor memory): per line 5 to 9 % faster, but V N / 148 = 27.7 lines per CTA are 7 rounds of 4 lines
-// (99 % full) against 5 rounds of 6 (92 %), which eats the gain: config 2 65.4k against 67k
-// reconstructions/s.  Turn-taking (Turns) needs one named barrier per warp: with 12 warps pass x has
-// none left for it (6 pair barriers + 12 > 15).
-#ifndef SFD_NW1024
-#define SFD_NW1024 8
-#endif
-constexpr int NW1024 = SFD_NW1024;
-constexpr bool TURNSY = true, TURNSX = NW1024 + NW1024 / 2 <= 15;  // turn-taking of the warps of a sub-partition
+//   solo rounds   8 adjacent columns, one per warp.  A warp runs branch 0 of its column, parks the
+//                 partial sums in registers, runs branch 1 and adds: no partner, no exchange through
+//                 shared memory, no barrier between warps on the transform path.  The two warps of a
+//                 pair (columns 2p, 2p + 1) meet only at their staging tile [n1][2 columns], from
+//                 which one thread hands 16-byte rows of B to the TMA unit.
+//   split rounds  4 adjacent columns, a group of four warps per 2 columns, one warp per (column,
+//                 branch): the two warps of a column exchange halves of their partial sums through
+//                 their transpose tiles (idle by then) and each finishes half of the outputs; the
+//                 group's four warps meet at a staging tile.  This is how every column ran in round 1.
+//
+// Why both: a warp runs a line in two branch-runs when it runs it alone, so solo work comes in units
+// of two runs, and V N / (8 x 148) = 3.46 columns per warp would round up to 4 columns = 8 runs.  The
+// CTA's whole blocks of 8 columns run solo (3 rounds = 6 runs at config 2), the columns left over in a
+// view (136 of 1024) are dealt out in half blocks and run split (1 run): 7 runs, as before, six of
+// them without exchange.  Measured on the way: a round of the split kernels 4.31 us, a round of the
+// exchange-free N = 512 kernels 3.59 us.
+//
+// Write-out.  B is [n1][m0] and a column's outputs are one element per row: written by the LSU that
+// is one 128-byte wavefront per row and store instruction.  Instead the warps put their final sums
+// into a dense staging tile [n1][2 columns] (16 bytes per row) and one thread hands the tile to the
+// TMA unit (cp.async.bulk.tensor, shared -> global, four boxes of 256 rows x 16 bytes): the scatter
+// costs the LSU pipe nothing and runs beside the next butterflies.
+// Read-in.  The CTA reads the 8 hologram columns of a round as one slab (uint8: 8 bytes of every row,
+// float: 32) and keeps it in shared memory as four planes [pair of columns][n0] (a 2-byte load per
+// row and column costs the LSU one wavefront per row just the same as the 8-byte one); the slab of
+// the next round is fetched into registers behind the tile reads of this round and stored into the
+// second buffer after the first branch.  The two buffers are handed over with mbarriers (full: all 8
+// warps have stored their rows; empty: all 8 warps have read theirs), NOT with a CTA-wide barrier: a
+// __syncthreads per round lines up the two warps of every sub-partition, which then run their
+// butterflies at the same time and their shared-memory phases at the same time - measured 4.9 us per
+// run against 4.3 us for the split rounds it was meant to beat.  With the mbarriers a warp may be up
+// to a run ahead of the slowest, and the stagger the turn-taking builds up survives.
 constexpr int YBOX = 256;   // rows of one TMA store box (the tensor map is built with this box)
-// Input slab of a group: SLAB_BYTES = 8 bytes of every hologram row = 2 columns x IPS items.  An
-// item-group of IPS items covers 2 G IPS adjacent columns, group g owning the 2 IPS columns from
-// 2 IPS g on: the group reads its slab once per IPS items with one 8-byte load per row (a 2-byte load
-// per row and item costs the LSU one wavefront per row just the same) and keeps it in shared memory
-// as [k][n0] column pairs.  nx need not be a multiple of 2 G IPS: in the last item-group of a view
-// the groups whose columns lie beyond nx idle.
-template <typename TIn> struct TileElem {            // uint8: 4 items per slab
+template <typename TIn> struct TileElem {            // uint8
     using type = unsigned short;                     // 2 uint8 columns of a row
-    using slab = uint2;
-    static constexpr int IPS = 4;
 };
-template <> struct TileElem<float> {                 // float: 1 item per slab
+template <> struct TileElem<float> {
     using type = float2;                             // 2 float columns of a row
-    using slab = float2;
-    static constexpr int IPS = 1;
 };
-template <typename TIn, int NW> struct SmemY {
-    float2 xb[NW][XB];
-    alignas(128) float2 stage[NW / 4][N][2];  // [group][n1][column of the group]: final sums, TMA store source
-    typename TileElem<TIn>::type tile[NW / 4][TileElem<TIn>::IPS][N];  // [group][k][n0]: the group's slab
+template <typename TIn> struct SmemY {
+    float2 xb[8][XB];
+    alignas(128) float2 stage[4][N][2];  // [pair][n1][column of the pair]: final sums, TMA store source
+    typename TileElem<TIn>::type tile[2][4][N];  // [buffer][pair of columns][n0]: the slab of a round
+    unsigned long long full[2], empty[2];  // slab buffers: stored by all 8 warps / read by all 8 warps
     unsigned tmem;  // base address of the tensor-memory allocation
 };
 
-template <typename TIn> struct TileRegs { typename TileElem<TIn>::slab e[8]; };
-
-// the 128 threads of a group fetch rows ht, ht + 128, .. of the slab that starts at column col
+// the 256 threads of the CTA fetch rows tid, tid + 256, .. of the 8 columns that start at column col
 // (plain loads: the hologram was written by whatever ran before this kernel in the stream)
-template <typename TIn>
-__device__ __forceinline__ void tile_load(TileRegs<TIn> &t, const TIn *holo, long long hstride,
-                                          int col, int ht) {
+template <typename TIn> struct SlabRegs;
+template <> struct SlabRegs<unsigned char> { uint2 e[4]; };
+template <> struct SlabRegs<float> { float4 e[4][2]; };
+__device__ __forceinline__ void slab_load(SlabRegs<unsigned char> &t, const unsigned char *holo,
+                                          long long hstride, int col, int tid) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
-        t.e[i] = *reinterpret_cast<const typename TileElem<TIn>::slab *>(
-            holo + (size_t)(ht + 128 * i) * hstride + col);
+    for (int i = 0; i < 4; ++i)
+        t.e[i] = *reinterpret_cast<const uint2 *>(holo + (size_t)(tid + 256 * i) * hstride + col);
 }
-__device__ __forceinline__ void tile_store(const TileRegs<unsigned char> &t,
-                                           unsigned short (*tile)[N], int ht) {
+__device__ __forceinline__ void slab_load(SlabRegs<float> &t, const float *holo, long long hstride,
+                                          int col, int tid) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        tile[0][ht + 128 * i] = (unsigned short)(t.e[i].x & 0xffffu);
-        tile[1][ht + 128 * i] = (unsigned short)(t.e[i].x >> 16);
-        tile[2][ht + 128 * i] = (unsigned short)(t.e[i].y & 0xffffu);
-        tile[3][ht + 128 * i] = (unsigned short)(t.e[i].y >> 16);
+    for (int i = 0; i < 4; ++i) {
+        const float4 *p = reinterpret_cast<const float4 *>(holo + (size_t)(tid + 256 * i) * hstride + col);
+        t.e[i][0] = p[0];
+        t.e[i][1] = p[1];
     }
 }
-__device__ __forceinline__ void tile_store(const TileRegs<float> &t, float2 (*tile)[N], int ht) {
+__device__ __forceinline__ void slab_store(const SlabRegs<unsigned char> &t, unsigned short (*tile)[N],
+                                           int tid) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) tile[0][ht + 128 * i] = t.e[i];
+    for (int i = 0; i < 4; ++i) {
+        tile[0][tid + 256 * i] = (unsigned short)(t.e[i].x & 0xffffu);
+        tile[1][tid + 256 * i] = (unsigned short)(t.e[i].x >> 16);
+        tile[2][tid + 256 * i] = (unsigned short)(t.e[i].y & 0xffffu);
+        tile[3][tid + 256 * i] = (unsigned short)(t.e[i].y >> 16);
+    }
+}
+__device__ __forceinline__ void slab_store(const SlabRegs<float> &t, float2 (*tile)[N], int tid) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        tile[0][tid + 256 * i] = make_float2(t.e[i][0].x, t.e[i][0].y);
+        tile[1][tid + 256 * i] = make_float2(t.e[i][0].z, t.e[i][0].w);
+        tile[2][tid + 256 * i] = make_float2(t.e[i][1].x, t.e[i][1].y);
+        tile[3][tid + 256 * i] = make_float2(t.e[i][1].z, t.e[i][1].w);
+    }
 }
 // uint8 -> float without the conversion unit (I2F shares the MIO queue with shared memory and is
 // quarter rate): one byte permute drops the sample into the mantissa of 2^23, one add removes 2^23
@@ -519,6 +539,9 @@ __device__ __forceinline__ float tile_value(float2 e, int c) { return c ? e.y : 
 
 __device__ __forceinline__ void group_sync(int group) {  // named barrier of the four warps of a group
     asm volatile("bar.sync %0, 128;" ::"r"(group + 1) : "memory");
+}
+__device__ __forceinline__ void ypair_sync(int pair) {  // pass y: the two warps of a pair (solo rounds)
+    asm volatile("bar.sync %0, 64;" ::"r"(pair + 11) : "memory");
 }
 // 2-D tiled bulk store shared -> global through tensor map `tm` (box fixed by the map); c0 = float
 // index within the row of B, c1 = row of B (view * N + n1)
@@ -534,30 +557,56 @@ __device__ __forceinline__ void bulk_wait_read() {
     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
-// Columns of one view are cut into item-groups of 2 G IPS columns, IPS items each.
-template <typename TIn, int NW> struct YItems {
-    static constexpr int IPS = TileElem<TIn>::IPS, G = NW / 4, COLS = 2 * G * IPS;
-    static constexpr bool POW2 = (COLS & (COLS - 1)) == 0;  // then items per view is a power of two too
-    __device__ static int per_view(int nx) { return (nx + COLS - 1) / COLS * IPS; }
-    // item -> (view, item of the view): shifts when per_view is a power of two (nx is one)
-    __device__ static int view_of(int item, int ipv) { return POW2 ? item >> (31 - __clz(ipv)) : item / ipv; }
-    __device__ static int wrap(int g, int ipv) { return POW2 ? g & (ipv - 1) : g % ipv; }
+// Columns of a view for CTA j of cpv: whole blocks of 8 columns (solo rounds), then half blocks of 4
+// out of what cpv does not divide (split rounds).
+struct YPlan {
+    int solo, split, blk0, half0, cpv;  // rounds of each kind, first block, first leftover column
+    __device__ static YPlan make(int nx, int j, int cpv) {
+        const int nblk = nx >> 3, solo = nblk / cpv, left = nblk - solo * cpv, halves = 2 * left;
+        return YPlan{solo, halves > j ? (halves - j + cpv - 1) / cpv : 0, j * solo, 8 * solo * cpv + 4 * j, cpv};
+    }
+    __device__ int rounds() const { return solo + split; }
+    // first of the 4 (split) or 8 (solo) columns of round r
+    __device__ int col(int r) const { return r < solo ? 8 * (blk0 + r) : half0 + 4 * cpv * (r - solo); }
 };
 
-// Persistent CTA of NW warps: work item = (view, 2 G columns); a CTA takes a contiguous range of
-// items (at most two views: the launcher sizes the grid accordingly).  The line length is N = 1024
-// = the number of hologram rows Ny; the number of columns nx (a multiple of 16) and the hologram's
-// row stride are run-time values (rectangular grids, windows inside a wider frame).
-// tabY: [2][3][N] per view (post carries c0, pre the 1/255 of uint8 input); tmB: tensor map of B seen
-// as float [V * N][2 nx] with box 4 x YBOX.
-// Per item a warp (column c of its group, branch B) transforms its column, hands the half of the
-// outputs it does not finish to its partner through its own transpose tile (idle by then), adds
-// what the partner left for it and writes 16 final values per thread into the staging tile.
-// The two places of a line that depend on the branch index at compile time (which half of the
-// register vector stays) are small functions instantiated for B = 0, 1 and entered through a
-// warp-uniform branch; everything else is ONE copy of code for all warps (half the
-// instruction-cache footprint of two template copies of the whole loop: measured, the
-// no_instruction stalls of the N = 2048 kernels, written this way, are a third of those of two copies).
+// Both branches' tables of `view` into every lane quarter: branch b at column b * TM_SET.  The two
+// warps of a sub-partition copy 12 chunks each, six at a time.  tab: the [2][3][N] block of view 0.
+__device__ __forceinline__ unsigned tm_setup_both(unsigned *slot, const float2 *__restrict__ tab,
+                                                  long long vstride, int view,
+                                                  const float2 *__restrict__ twl) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const float2 *src = tab + (size_t)view * vstride + lane;
+    const int ch0 = 12 * (warp >> 2);
+    TFill<8> f;
+    TwFill ft;
+    auto load = [&](int first) {
+#pragma unroll
+        for (int j = 0; j < 6; ++j)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const float2 x = __ldg(src + 32 * (8 * (first + j) + i));
+                f.c[j].w[2 * i] = __float_as_uint(x.x);
+                f.c[j].w[2 * i + 1] = __float_as_uint(x.y);
+            }
+    };
+    load(ch0);
+    if (warp < 4) tw_load(ft, twl, lane);
+    if (warp == 0) tm_alloc(slot);
+    tm_sync_cta();
+    const unsigned base = *reinterpret_cast<volatile unsigned *>(slot);
+    const unsigned q = tm_quarter(base, warp);
+#pragma unroll
+    for (int j = 0; j < 6; ++j) tm_st(f.c[j], q + 16 * (ch0 + j));
+    load(ch0 + 6);
+#pragma unroll
+    for (int j = 0; j < 6; ++j) tm_st(f.c[j], q + 16 * (ch0 + 6 + j));
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    if (warp < 4) tw_store(ft, q + TM_TW);
+    tm_sync_cta();
+    return base;
+}
+
 template <int B>
 __device__ __forceinline__ void y_hand_over(const float2 (&v)[32], float2 *xb, int lane) {
 #pragma unroll
@@ -573,56 +622,55 @@ __device__ __forceinline__ void y_finish(const float2 (&v)[32], const float2 *xb
     }
 }
 
-template <typename TIn, int NW, bool TURNS>
-__device__ __forceinline__ void pass_y_loop(SmemY<TIn, NW> &sm, const TIn *holo, long long hstride,
+// tabY: [2][3][N] per view (post carries c0, pre the 1/255 of uint8 input) in tensor memory, branch b
+// at tq + b * TM_SET; tmB: tensor map of B seen as float [V * N][2 nx] with box 4 x YBOX.  The line
+// length is N = 1024 = the number of hologram rows Ny; the number of columns nx (a multiple of 16) and
+// the hologram's row stride are run-time values.  The loop runs over branch-runs so that the line
+// transform (branch()) exists once in the code: a solo round is two runs, a split round one.
+template <typename TIn>
+__device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *holo, long long hstride,
                                             int nx, unsigned tq, unsigned tt, const void *tmB,
-                                            int V) {
-    using YI = YItems<TIn, NW>;
-    constexpr int IPS = YI::IPS, G = YI::G;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int group = warp >> 2, c = (warp >> 1) & 1, ht = threadIdx.x & 127, b = warp & 1;
-    const int ipv = YI::per_view(nx);
-    const int items = V * ipv;
-    const int i0 = (int)((long long)items * blockIdx.x / gridDim.x);
-    const int i1 = (int)((long long)items * (blockIdx.x + 1) / gridDim.x);
-    if (i0 >= i1) return;  // CTA-uniform
+                                            int view, const YPlan yp) {
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, tid = threadIdx.x;
+    const int pair = warp >> 1, b = warp & 1, group = warp >> 2, c = pair & 1;
+    const int runs = 2 * yp.solo + yp.split;
+    if (runs == 0) return;  // CTA-uniform
     float2 *xb = sm.xb[warp];
     const float2 *xbp = sm.xb[warp ^ 1];
-    float2 *stg = &sm.stage[group][0][0];
-    const bool leader = ht == 0;  // issues and retires the group's bulk stores
-    const int view0 = YI::view_of(i0, ipv);
-    // first column of this group's slab in the item-group of item g (of a view)
-    auto slab_col = [&](int g) { return g / IPS * YI::COLS + 2 * IPS * group; };
+    const bool pair_leader = b == 0 && lane == 0;       // solo rounds: the pair's bulk stores
+    const bool group_leader = (tid & 127) == 0;         // split rounds: the group's (the leader of pair 2 group)
+    bool waited = false;  // this thread has waited for the kernel before this one (see the first store)
+    auto warp_arrive = [&](unsigned long long *bar) {  // this warp's rows are stored / read
+        __syncwarp();
+        if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+    };
     {
-        const int col = slab_col(YI::wrap(i0, ipv));
-        if (YI::POW2 || col < nx) {
-            TileRegs<TIn> t;
-            tile_load<TIn>(t, holo, hstride, col, ht);
-            tile_store(t, sm.tile[group], ht);
-        }
+        SlabRegs<TIn> t;
+        slab_load(t, holo, hstride, yp.col(0) & ~7, tid);
+        slab_store(t, sm.tile[0], tid);
+        warp_arrive(&sm.full[0]);
     }
-    group_sync(group);
-    const Turns turns = turns_make(warp, NW, G + 1, TURNS);
-    turns_open(turns, warp, NW);
-    for (int item = i0; item < i1; ++item) {
-        const int view = YI::view_of(item, ipv), g = item - view * ipv, k = g % IPS;
-        const int scol = slab_col(g), colh = scol + 2 * k;
-        const unsigned tpre = tq + (view - view0) * TM_SET;  // pre_b | H_b | conj(post_b)
-        // the next item opens a new slab (that lies inside the hologram)
-        const int ncol = slab_col(YI::wrap(g + 1, ipv));
-        // (with COLS a power of two every item-group is complete: nx is a multiple of 16)
-        const bool has_next = item + 1 < i1 && k == IPS - 1 && (YI::POW2 || ncol < nx);
-        if (!YI::POW2 && scol >= nx) {  // group-uniform: this group's columns of the view's last item-group do not exist
-            turns_skip(turns);
-            if (has_next) {
-                TileRegs<TIn> t;
-                tile_load<TIn>(t, holo, hstride, ncol, ht);
-                tile_store(t, sm.tile[group], ht);
-                group_sync(group);
-            }
-            continue;
+    unsigned ph_full = 0, ph_empty = 0;  // bit b: parity of the next completion of full[b] / empty[b] to wait for
+    const Turns turns = turns_make(warp, 8, 3, true);  // named barriers 3..10
+    turns_open(turns, warp, 8);
+    SlabRegs<TIn> t;
+    float2 acc[32];
+    int round = -1;
+    for (int run = 0; run < runs; ++run) {
+        const bool solo = run < 2 * yp.solo, first = !solo || (run & 1) == 0;
+        if (first) {
+            ++round;
+            // the slab of this round is complete (all 8 warps stored their rows during the round before)
+            mbar_wait(&sm.full[round & 1], (ph_full >> (round & 1)) & 1u);
+            ph_full ^= 1u << (round & 1);
         }
-        TileRegs<TIn> t;
+        const int col0 = yp.col(round), buf = round & 1;
+        const bool has_next = first && round + 1 < yp.rounds();
+        // this warp's column of the round, its place in the slab, its branch
+        const int br = solo ? (run & 1) : b;
+        const int plane = solo ? pair : ((col0 & 7) >> 1) + group;
+        const int byte = solo ? b : c;
+        const unsigned tpre = tq + br * TM_SET;  // pre_b | H_b | conj(post_b)
         float2 v[32];
         {
             TChunk c0, c1;
@@ -634,7 +682,7 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn, NW> &sm, const TIn *holo,
                 if (j < 3) tm_ld((j & 1) ? c0 : c1, tpre + 16 * (j + 1));
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
-                    const float a = tile_value(sm.tile[group][k][lane + 32 * (8 * j + i)], c);
+                    const float a = tile_value(sm.tile[buf][plane][lane + 32 * (8 * j + i)], byte);
                     const float2 p = tm_val(ch, i);
                     v[8 * j + i] = make_float2(a * p.x, a * p.y);
                 }
@@ -642,43 +690,81 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn, NW> &sm, const TIn *holo,
         }
         // the next slab is fetched behind the tile reads: its loads touch one row per lane (32
         // wavefronts each) and would hold up everything queued after them
-        if (has_next) tile_load<TIn>(t, holo, hstride, ncol, ht);
+        if (has_next) slab_load(t, holo, hstride, yp.col(round + 1) & ~7, tid);
+        if (!solo || br == 1) warp_arrive(&sm.empty[buf]);  // this warp's last read of the round's slab
         branch(v, lane, xb, tt, tpre + TM_TAB, turns);
-        // the previous item's bulk stores must have left the staging tile before it is rewritten
-        if (leader) bulk_wait_read();
-        if (b == 0)
-            y_hand_over<0>(v, xb, lane);
-        else
-            y_hand_over<1>(v, xb, lane);
-        group_sync(group);  // partner's hand-over visible; staging tile and input tile free
-        if (b == 0)
-            y_finish<0>(v, xbp, stg, lane, c);
-        else
-            y_finish<1>(v, xbp, stg, lane, c);
-        if (has_next) tile_store(t, sm.tile[group], ht);
-        fence_async_smem();  // staging writes -> async proxy
-        group_sync(group);   // staging tile complete, next input tile visible, hand-over tiles free
-        if (leader) {
-            // Programmatic dependent launch: the only thing pass y does to memory that the kernel
-            // before it may still be using is to overwrite B (pass x of the frame before reads it),
-            // and the only thread that does so is this one.  It waits here, in front of its first
-            // store, instead of at the top of the kernel: a CTA that got its SM early (the CTAs of the
-            // kernel before do not all finish together) works on its first columns meanwhile.  The
-            // hologram is never written by a kernel of this library; whatever else produced it was
-            // complete before this kernel could start (only our own kernels release their dependents
-            // early).
-            if (item == i0) pdl_wait();
+        if (has_next) {
+            if (round >= 1) {  // all 8 warps have read the slab of the round before out of that buffer
+                mbar_wait(&sm.empty[buf ^ 1], (ph_empty >> (buf ^ 1)) & 1u);
+                ph_empty ^= 1u << (buf ^ 1);
+            }
+            slab_store(t, sm.tile[buf ^ 1], tid);
+            warp_arrive(&sm.full[buf ^ 1]);
+        }
+        if (solo && br == 0) {  // park branch 0
 #pragma unroll
-            for (int j = 0; j < N / YBOX; ++j)
-                tma_store_2d(tmB, stg + j * YBOX * 2, 2 * colh, view * N + j * YBOX);
-            bulk_commit();
+            for (int r = 0; r < 32; ++r) acc[r] = v[r];
+            continue;
+        }
+        // Programmatic dependent launch: the only thing pass y does to memory that the kernel before
+        // it may still be using is to overwrite B (pass x of the frame before reads it), and the only
+        // threads that do so are the store leaders.  They wait in front of their first store instead
+        // of at the top of the kernel: a CTA that got its SM early (the CTAs of the kernel before do
+        // not all finish together) works on its first columns meanwhile.  The hologram is never written
+        // by a kernel of this library; whatever else produced it was complete before this kernel could
+        // start (only our own kernels release their dependents early).
+        if (solo) {
+            float2 *stg = &sm.stage[pair][0][0];
+            // the pair's previous bulk store has left the staging tile before it is rewritten
+            if (pair_leader) bulk_wait_read();
+            ypair_sync(pair);
+#pragma unroll
+            for (int r = 0; r < 32; ++r) stg[(lane + 32 * r) * 2 + b] = padd(v[r], acc[r]);
+            fence_async_smem();  // staging writes -> async proxy
+            ypair_sync(pair);    // both columns of the pair are in the staging tile
+            if (pair_leader) {
+                if (!waited) pdl_wait();
+                waited = true;
+#pragma unroll
+                for (int j = 0; j < N / YBOX; ++j)
+                    tma_store_2d(tmB, stg + j * YBOX * 2, 2 * (col0 + 2 * pair), view * N + j * YBOX);
+                bulk_commit();
+            }
+        } else {
+            float2 *stg = &sm.stage[2 * group][0][0];
+            if (group_leader) bulk_wait_read();
+            if (b == 0)
+                y_hand_over<0>(v, xb, lane);
+            else
+                y_hand_over<1>(v, xb, lane);
+            group_sync(group);  // partner's hand-over visible; staging tile free
+            if (b == 0)
+                y_finish<0>(v, xbp, stg, lane, c);
+            else
+                y_finish<1>(v, xbp, stg, lane, c);
+            fence_async_smem();  // staging writes -> async proxy
+            group_sync(group);   // staging tile complete, hand-over tiles free
+            if (group_leader) {
+                if (!waited) pdl_wait();
+                waited = true;
+#pragma unroll
+                for (int j = 0; j < N / YBOX; ++j)
+                    tma_store_2d(tmB, stg + j * YBOX * 2, 2 * (col0 + 2 * group), view * N + j * YBOX);
+                bulk_commit();
+            }
         }
     }
-    if (leader) bulk_wait_read();  // shared memory must outlive the last store's reads
+    if (lane == 0) bulk_wait_read();  // shared memory must outlive the last stores' reads
     turns_close(turns, warp);
 }
 
 // ---- pass x: one row of B per warp pair -----------------------------------------------------------
+// Warps per CTA of pass x.  The loop below is written for any multiple of four and was measured with
+// 12 (three warps per sub-partition, 132 registers per thread with the twiddles in tensor memory):
+// per line 5 to 9 % faster, but V N / 148 = 27.7 lines per CTA are 7 rounds of 4 lines (99 % full)
+// against 5 rounds of 6 (92 %), which eats the gain, and 6 pair barriers + 12 turn barriers exceed the
+// 15 named barriers a CTA has.
+constexpr int NWX = 8;
 template <int NW> struct SmemX {
     float2 xb[NW][XB];
     float2 inb[NW / 2][N];  // input row of each pair (bulk async copy destination)
