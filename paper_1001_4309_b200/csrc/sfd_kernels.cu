@@ -183,14 +183,25 @@ k_cols_512(const TIn *holo, long long hstride, int nx, const float2 *__restrict_
     extern __shared__ float4 smem4[];
     sfdh::SmemYH<TIn> &sm = *reinterpret_cast<sfdh::SmemYH<TIn> *>(smem4);
     sfdw::pdl_launch_dependents();
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < 2; ++i) {
+            sfdw::mbar_init(&sm.full[i], 8);
+            sfdw::mbar_init(&sm.empty[i], 8);
+        }
+        sfdw::mbar_fence_init();
+    }
     const int ipv = nx >> 3;  // items (8 columns) per view, as in pass_y_half
     const unsigned tbase = sfdh::tmh_setup(&sm.tmem, tabY, vstride, V * ipv, ipv, twl);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
-    sfdw::pdl_wait();
-    if (vmax != nullptr && blockIdx.x == 0)
-        for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
-    if (mom != nullptr && blockIdx.x == 0)
-        for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
+    // B, vmax and mom belong to the kernels before this one: block 0 waits before it clears the latter
+    // two, the store leaders wait in front of their first store of B (as in k_cols_1024)
+    if ((vmax != nullptr || mom != nullptr) && blockIdx.x == 0) {
+        sfdw::pdl_wait();
+        if (vmax != nullptr)
+            for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
+        if (mom != nullptr)
+            for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
+    }
     sfdh::pass_y_half<TIn>(sm, holo, hstride, nx, tq, &tmB, V);
     sfdw::tm_finish(tbase);
 }

@@ -9,8 +9,9 @@
 // the output registers dropped.  No split by the parity of the frequency index, hence no partner
 // warp, no exchange of partial sums and no barrier on the transform path: a warp loads a line,
 // transforms it and stores it.  What is left of the inter-warp traffic of the N = 1024 kernels:
-//   pass y  the 8 warps of a CTA share the 8-byte input slab of a round (8 adjacent columns: one
-//           __syncthreads per round, slab double-buffered), and the two warps of a pair share a
+//   pass y  the 8 warps of a CTA share the 8-byte input slab of a round (8 adjacent columns; the two
+//           slab buffers are handed over with mbarriers, not with a CTA-wide barrier, which would line
+//           up the two warps of every sub-partition: see pass_y_loop), and the two warps of a pair share a
 //           staging tile [n1][2 columns] so that the TMA store writes 16-byte rows of B (one pair
 //           barrier per line, staging double-buffered);
 //   pass x  nothing (rows arrive by per-warp bulk copies, outputs leave as coalesced stores);
@@ -203,12 +204,9 @@ template <typename TIn> struct SmemYH {
     float2 xb[8][XB];
     alignas(128) float2 stage[4][2][NH][2];  // [pair][buffer][n1][column of the pair]: TMA store source
     typename TileElem<TIn>::type tile[2][4][NH];  // [buffer][pair][n0]: the CTA's slab
+    unsigned long long full[2], empty[2];  // slab buffers: stored by all 8 warps / read by all 8 warps
     unsigned tmem;
 };
-
-__device__ __forceinline__ void bulk_wait_read1() {  // all but the most recent bulk group have read
-    asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
-}
 
 // Work item = (view, 8 adjacent columns); a CTA takes a contiguous range of items.  nx (a multiple
 // of 16) and the hologram's row stride are run-time values.  tmB: tensor map of B seen as float
@@ -225,18 +223,24 @@ __device__ __forceinline__ void pass_y_half(SmemYH<TIn> &sm, const TIn *holo, lo
     float2 *xb = sm.xb[warp];
     const bool leader = c == 0 && lane == 0;  // issues and retires the pair's bulk stores
     const int view0 = i0 >> lgi;
+    auto warp_arrive = [&](unsigned long long *bar) {  // this warp's rows are stored / read
+        __syncwarp();
+        if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+    };
     typename SlabH<TIn>::Regs t;
     SlabH<TIn>::load(t, holo, hstride, 8 * (i0 & (ipv - 1)), threadIdx.x);
     SlabH<TIn>::store(t, sm.tile[0], threadIdx.x);
+    warp_arrive(&sm.full[0]);
+    unsigned ph_full = 0, ph_empty = 0;  // bit b: parity of the next completion of full[b] / empty[b]
     const Turns turns = turns_make(warp, 8, 5, true);
     turns_open(turns, warp, 8);
     for (int item = i0; item < i1; ++item) {
         const int view = item >> lgi, g = item & (ipv - 1), buf = (item - i0) & 1;
         const unsigned tpre = tq + (view - view0) * TH_SET;
         const bool has_next = item + 1 < i1;
-        // the slab of this round is complete (stored during the round before); every warp has read
-        // the slab of the round before, whose buffer the next slab goes into
-        __syncthreads();
+        // the slab of this round is complete (all 8 warps stored their rows during the round before)
+        mbar_wait(&sm.full[buf], (ph_full >> buf) & 1u);
+        ph_full ^= 1u << buf;
         float2 v[32];
         {
             TChunk c0, c1;
@@ -256,21 +260,30 @@ __device__ __forceinline__ void pass_y_half(SmemYH<TIn> &sm, const TIn *holo, lo
             for (int r = 16; r < 32; ++r) v[r] = make_float2(0.f, 0.f);
         }
         if (has_next) SlabH<TIn>::load(t, holo, hstride, 8 * ((g + 1) & (ipv - 1)), threadIdx.x);
+        warp_arrive(&sm.empty[buf]);  // this warp has read its column of the slab
         branch<true, 2>(v, lane, xb, tq + TH_TW, tpre + TH_H, turns);
-        if (has_next) SlabH<TIn>::store(t, sm.tile[buf ^ 1], threadIdx.x);
-        // staging buffer `buf` of the pair: its last bulk store (two lines ago) has read it (the leader
-        // waited for that before the pair barrier of the line before)
+        if (has_next) {
+            if (item > i0) {  // all 8 warps have read the slab of the round before out of that buffer
+                mbar_wait(&sm.empty[buf ^ 1], (ph_empty >> (buf ^ 1)) & 1u);
+                ph_empty ^= 1u << (buf ^ 1);
+            }
+            SlabH<TIn>::store(t, sm.tile[buf ^ 1], threadIdx.x);
+            warp_arrive(&sm.full[buf ^ 1]);
+        }
+        // staging buffer `buf` of the pair: its last bulk store (two lines ago) has read it - the leader
+        // made sure of that before the pair barrier of the line before, which orders it before these writes
         float2 *stg = &sm.stage[pair][buf][0][0];
 #pragma unroll
         for (int q = 0; q < 16; ++q) stg[(lane + 32 * q) * 2 + c] = v[q];
         fence_async_smem();  // staging writes -> async proxy
-        pair_sync(pair);     // both columns of the pair are in the staging tile
+        if (leader) bulk_wait_read();  // the store of the line before (other buffer) has read its tile
+        pair_sync(pair);               // both columns of the pair are in the staging tile
         if (leader) {
+            if (item == i0) pdl_wait();  // B belongs to the kernel before this one until it has completed
 #pragma unroll
             for (int j = 0; j < NH / YBOX; ++j)
                 tma_store_2d(tmB, stg + j * YBOX * 2, 2 * (8 * g + 2 * pair), view * NH + j * YBOX);
             bulk_commit();
-            bulk_wait_read1();
         }
     }
     if (leader) bulk_wait_read();  // shared memory must outlive the last store's reads
