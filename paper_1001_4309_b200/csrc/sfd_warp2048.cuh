@@ -365,14 +365,23 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, lo
             if (cc == 1 && next_slab) sub_prefetch<TIn>(holo, hstride, SubSlab<TIn>::col(u + 1, quad), qt);
             quad_sync(quad);  // the previous column's exchange area has been read by all four warps
             branch<false>(v, lane, xb, tt, tq + TQ_H, turns);
-            // the previous unit's bulk stores must have left the staging tile before it is rewritten
-            if (cc == 0 && leader) bulk_wait_read();
+            // The two quads share the staging tile (32-byte rows of B need all four columns of the
+            // unit) but must not share a CTA-wide barrier: that lines up the two warps of every
+            // sub-partition (w and w + 4 sit in different quads), which then run their butterflies at
+            // the same time and their shared-memory phases at the same time.  Instead warp 0, which
+            // issues the bulk stores, tells quad 1 when the tile is free (named barrier 13: it arrives,
+            // quad 1 waits - it has arrived long before) and is told when the tile is complete (named
+            // barrier 14: everybody else arrives, warp 0 waits).
+            if (cc == 0 && warp == 0) {
+                // the previous unit's bulk stores must have left the staging tile before it is rewritten
+                if (leader) bulk_wait_read();
+                __syncwarp();
+                asm volatile("bar.arrive 13, 160;" ::: "memory");
+            }
             float2 mine[16];
             quad_scatter(v, mine, tq, b, lane, sm.xb, sm.ex, warp);
-            if (cc == 0)
-                cta_sync();  // also: the staging tile is free (the leader sits in quad 0)
-            else
-                quad_sync(quad);
+            quad_sync(quad);
+            if (cc == 0 && quad == 1) asm volatile("bar.sync 13, 160;" ::: "memory");
             quad_collect(mine, b, lane, sm.xb, sm.ex, warp);
 #pragma unroll
             for (int i = 0; i < 16; ++i) stg[(lane + 32 * (16 * b + i)) * 4 + 2 * quad + cc] = mine[i];
@@ -383,7 +392,11 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, lo
                     sub_store(t, sm.tile[quad], qt, quad);
                 }
                 fence_async_smem();  // staging writes -> async proxy
-                cta_sync();          // staging tile complete (both quads), next slab visible
+                quad_sync(quad);     // this quad's columns are in the staging tile, its next slab visible
+                if (warp == 0)
+                    asm volatile("bar.sync 14, 256;" ::: "memory");  // staging tile complete (both quads)
+                else
+                    asm volatile("bar.arrive 14, 256;" ::: "memory");
                 if (leader) {
 #pragma unroll
                     for (int j = 0; j < NL / YBOX; ++j)
