@@ -16,15 +16,20 @@
 // chirp-kernel spectra of the Fresnel path, built once on the device in float64 (the phase
 // z sqrt(.) is about 1e5 cycles: float32 cannot hold it) with the 1/(Nx Ny) of the inverse folded in.
 // Line FFTs: the Stockham register/shared-memory code of sfd_fft_core.cuh (fft_line), 128..4096
-// points.  All three kernels are chained by programmatic dependent launch.
+// points.  All three kernels are chained by programmatic dependent launch.  A 1024 x 1024 grid runs
+// the same three steps as warp-FFT kernels (k_asm1024_*, sfd_asm1024.cuh) on a transposed,
+// sign-folded copy of H.
+#include <cuda.h>  // CUtensorMap (types only: the encoder is fetched through the runtime)
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <cstdint>
 #include <cstdio>
 #include <new>
 #include <vector>
 
 #include "sfd.h"
+#include "sfd_asm1024.cuh"
 #include "sfd_fft_core.cuh"
 #include "sfd_internal.h"
 
@@ -41,9 +46,10 @@ __device__ __forceinline__ float2 load_sample(const float *p, size_t i) { return
 __device__ __forceinline__ float2 load_sample(const float2 *p, size_t i) { return p[i]; }
 
 // H[p][ky][kx] in float64, stored as complex64 with the 1/(Nx Ny) of the inverse transforms
+// (warp_layout: transposed and sign-folded for the 1024 x 1024 kernels)
 __global__ void __launch_bounds__(256)
 k_asm_transfer(float2 *H, int Nx, int Ny, double lambda, double px, double py, const double *z,
-               int band_limit) {
+               int band_limit, int warp_layout) {
     const int kx = blockIdx.x * blockDim.x + threadIdx.x, ky = blockIdx.y, p = blockIdx.z;
     if (kx >= Nx) return;
     const double fx = (double)(2 * kx < Nx ? kx : kx - Nx) / ((double)Nx * px);
@@ -65,7 +71,56 @@ k_asm_transfer(float2 *H, int Nx, int Ny, double lambda, double px, double py, c
         const double sc = 1.0 / ((double)Nx * (double)Ny);
         h = make_float2((float)(cs * sc), (float)(sn * sc));
     }
-    H[((size_t)p * Ny + ky) * Nx + kx] = h;
+    if (!warp_layout) {
+        H[((size_t)p * Ny + ky) * Nx + kx] = h;
+    } else {  // T_p[kx][ky] = sigma(ky) sigma(kx) H_p[ky][kx] / (Nx Ny), sfd_asm1024.cuh
+        if ((__popc(kx) + __popc(ky)) & 1) h = make_float2(-h.x, -h.y);
+        H[((size_t)p * Nx + kx) * Ny + ky] = h;
+    }
+}
+
+// ---- 1024 x 1024: warp-FFT kernels (sfd_asm1024.cuh), 8 warps per CTA, one CTA per SM ---------------
+template <typename TIn>
+__global__ void __launch_bounds__(256, 1)
+k_asm1024_rows_fwd(const TIn *u0, const float2 *__restrict__ twl, float2 *A, int rows) {
+    extern __shared__ float4 smem4[];
+    pdl_launch_dependents();
+    sfda::rows_fwd<TIn>(*reinterpret_cast<sfda::SmemR *>(smem4), u0, twl, A, rows);
+}
+
+__global__ void __launch_bounds__(sfda::NTC, 1)
+k_asm1024_cols(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmW,
+               const float2 *__restrict__ Tt, const float2 *__restrict__ twl, int P) {
+    extern __shared__ float4 smem4[];
+    // the swizzle pattern of the tile is a function of the shared-memory address: 1024-byte alignment
+    sfda::SmemC &sm = *reinterpret_cast<sfda::SmemC *>(
+        (reinterpret_cast<uintptr_t>(smem4) + 1023) & ~(uintptr_t)1023);
+    pdl_launch_dependents();
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < sfda::NWA; ++i) sfdw::mbar_init(&sm.tbar[i], 1);
+        sfdw::mbar_init(&sm.in_full, 1);
+        sfdw::mbar_init(&sm.in_read, sfda::NWA);
+        sfdw::mbar_init(&sm.staged, sfda::NWA);
+        sfdw::mbar_init(&sm.empty, 1);
+        sfdw::mbar_fence_init();
+    }
+    __syncthreads();
+    sfda::cols(sm, &tmA, &tmW, Tt, twl, P);
+}
+
+template <bool PHASE>
+__global__ void __launch_bounds__(256, 1)
+k_asm1024_rows_inv(const float2 *W, const float2 *__restrict__ twl, float2 *__restrict__ field,
+                   float *__restrict__ inten, float *__restrict__ phase, int rows) {
+    extern __shared__ float4 smem4[];
+    sfda::SmemI &sm = *reinterpret_cast<sfda::SmemI *>(smem4);
+    pdl_launch_dependents();
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < sfda::NWA; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
+        sfdw::mbar_fence_init();
+    }
+    __syncthreads();
+    sfda::rows_inv<PHASE>(sm, W, twl, field, inten, phase, rows);
 }
 
 template <int LOG2N, typename TIn>
@@ -164,6 +219,12 @@ struct sfd_asm_plan {
     float2 *W = nullptr;     // [P][Ny][Nx]   after the column pass
     float2 *tw_x = nullptr;  // [Nx] exp(-2 pi i k / Nx)
     float2 *tw_y = nullptr;  // [Ny]
+    // 1024 x 1024: warp-FFT kernels; H holds T[p][kx][ky] then (sfd_asm1024.cuh)
+    bool warp = false;
+    int sms = 0;
+    float2 *twl = nullptr;  // [31][32] stage-B twiddles of the warp FFT (sfd_dft32.cuh)
+    alignas(64) unsigned char tmapA[128] = {};
+    alignas(64) unsigned char tmapW[128] = {};
     long long device_bytes = 0;
 };
 
@@ -243,6 +304,52 @@ fwd_fn pick_fwd(int l) { ASM_DISPATCH(l, rows_fwd) }
 cols_fn pick_cols(int l) { ASM_DISPATCH(l, cols) }
 inv_fn pick_inv(int l) { ASM_DISPATCH(l, rows_inv) }
 
+cudaError_t asm_attrs_1024() {
+    cudaError_t e;
+#define ASM_SMEM(kernel, bytes)                                                            \
+    if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,     \
+                                  (int)(bytes))) != cudaSuccess)                           \
+        return e;
+    ASM_SMEM(k_asm1024_rows_fwd<float>, sizeof(sfda::SmemR))
+    ASM_SMEM(k_asm1024_rows_fwd<float2>, sizeof(sfda::SmemR))
+    ASM_SMEM(k_asm1024_cols, sizeof(sfda::SmemC) + 1024)
+    ASM_SMEM(k_asm1024_rows_inv<false>, sizeof(sfda::SmemI))
+    ASM_SMEM(k_asm1024_rows_inv<true>, sizeof(sfda::SmemI))
+#undef ASM_SMEM
+    return cudaSuccess;
+}
+
+// the three kernels of the 1024 x 1024 path
+cudaError_t launch_1024(const sfd_asm_plan *p, const void *in, float2 *field, float *inten,
+                        float *phase, cudaStream_t st) {
+    constexpr int NW = sfda::NWA, N = sfdw::N;
+    cudaError_t e;
+    {
+        Launch l(dim3(N / NW), dim3(32 * NW), sizeof(sfda::SmemR), st);
+        if (p->in_dtype == SFD_F32)
+            e = cudaLaunchKernelEx(&l.cfg, k_asm1024_rows_fwd<float>, (const float *)in,
+                                   (const float2 *)p->twl, p->A, N);
+        else
+            e = cudaLaunchKernelEx(&l.cfg, k_asm1024_rows_fwd<float2>, (const float2 *)in,
+                                   (const float2 *)p->twl, p->A, N);
+        if (e != cudaSuccess) return e;
+    }
+    {
+        Launch l(dim3(N / NW), dim3(sfda::NTC), sizeof(sfda::SmemC) + 1024, st);
+        e = cudaLaunchKernelEx(&l.cfg, k_asm1024_cols, *reinterpret_cast<const CUtensorMap *>(p->tmapA),
+                               *reinterpret_cast<const CUtensorMap *>(p->tmapW), (const float2 *)p->H,
+                               (const float2 *)p->twl, p->P);
+        if (e != cudaSuccess) return e;
+    }
+    const int rows = p->P * N, ctas = rows / NW < p->sms ? rows / NW : p->sms;
+    Launch l(dim3(ctas), dim3(32 * NW), sizeof(sfda::SmemI), st);
+    if (phase)
+        return cudaLaunchKernelEx(&l.cfg, k_asm1024_rows_inv<true>, (const float2 *)p->W,
+                                  (const float2 *)p->twl, field, inten, phase, rows);
+    return cudaLaunchKernelEx(&l.cfg, k_asm1024_rows_inv<false>, (const float2 *)p->W,
+                              (const float2 *)p->twl, field, inten, phase, rows);
+}
+
 bool g_attr_done[64] = {};
 
 }  // namespace
@@ -272,6 +379,7 @@ int sfd_asm_plan_create(sfd_asm_plan **out, int Nx, int Ny, int n_planes, double
         ASM_CUDA(asm_attrs<10>());
         ASM_CUDA(asm_attrs<11>());
         ASM_CUDA(asm_attrs<12>());
+        ASM_CUDA(asm_attrs_1024());
         g_attr_done[device] = true;
     }
     sfd_asm_plan *p = new (std::nothrow) sfd_asm_plan;
@@ -279,6 +387,8 @@ int sfd_asm_plan_create(sfd_asm_plan **out, int Nx, int Ny, int n_planes, double
     p->Nx = Nx; p->Ny = Ny; p->lx = lx; p->ly = ly; p->P = n_planes;
     p->in_dtype = in_dtype; p->band_limit = band_limit != 0; p->device = device;
     p->lambda = lambda; p->px = px; p->py = py;
+    p->warp = Nx == sfdw::N && Ny == sfdw::N;
+    ASM_CUDA(cudaDeviceGetAttribute(&p->sms, cudaDevAttrMultiProcessorCount, device));
     const size_t nn = (size_t)Nx * Ny, P = n_planes;
     auto fail = [&](int code) {
         sfd_asm_plan_destroy(p);
@@ -288,13 +398,23 @@ int sfd_asm_plan_create(sfd_asm_plan **out, int Nx, int Ny, int n_planes, double
     if ((e = cudaMalloc((void **)&p->H, P * nn * sizeof(float2))) != cudaSuccess ||
         (e = cudaMalloc((void **)&p->W, P * nn * sizeof(float2))) != cudaSuccess ||
         (e = cudaMalloc((void **)&p->A, nn * sizeof(float2))) != cudaSuccess ||
-        (e = cudaMalloc((void **)&p->tw_x, (size_t)(Nx + Ny) * sizeof(float2))) != cudaSuccess)
+        (e = cudaMalloc((void **)&p->tw_x, (size_t)(Nx + Ny + 32 * 32) * sizeof(float2))) != cudaSuccess)
         return fail(e == cudaErrorMemoryAllocation ? SFD_ENOMEM : asm_fail(e, "cudaMalloc"));
     p->tw_y = p->tw_x + Nx;
-    p->device_bytes = (long long)((2 * P + 1) * nn * sizeof(float2) + (size_t)(Nx + Ny) * sizeof(float2));
+    p->twl = p->tw_y + Ny;
+    p->device_bytes =
+        (long long)((2 * P + 1) * nn * sizeof(float2) + (size_t)(Nx + Ny + 32 * 32) * sizeof(float2));
     {
-        std::vector<float2> tw((size_t)Nx + Ny);
+        std::vector<float2> tw((size_t)Nx + Ny + 32 * 32, make_float2(0.f, 0.f));
         const long double two_pi = 6.283185307179586476925286766559005768L;
+        // stage-B twiddles of the warp FFT: [j][lane], j = n/2 - 1 + k, exp(-2 pi i (lane + 32 k)/(32 n))
+        for (int n = 2; n <= 32; n *= 2)
+            for (int k = 0; k < n / 2; ++k)
+                for (int lane = 0; lane < 32; ++lane) {
+                    const long double a = two_pi * (lane + 32 * k) / (32 * n);
+                    tw[(size_t)Nx + Ny + (n / 2 - 1 + k) * 32 + lane] =
+                        make_float2((float)cosl(a), (float)-sinl(a));
+                }
         for (int k = 0; k < Nx; ++k)
             tw[k] = make_float2((float)cosl(two_pi * k / Nx), (float)-sinl(two_pi * k / Nx));
         for (int k = 0; k < Ny; ++k)
@@ -309,12 +429,20 @@ int sfd_asm_plan_create(sfd_asm_plan **out, int Nx, int Ny, int n_planes, double
     e = cudaMemcpy(zd, z, P * sizeof(double), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) {
         k_asm_transfer<<<dim3((Nx + 255) / 256, Ny, n_planes), 256>>>(p->H, Nx, Ny, lambda, px, py, zd,
-                                                                     p->band_limit);
+                                                                     p->band_limit, p->warp ? 1 : 0);
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     cudaFree(zd);
     if (e != cudaSuccess) return fail(asm_fail(e, "k_asm_transfer"));
+    if (p->warp) {
+        static_assert(sizeof(CUtensorMap) <= sizeof(p->tmapA), "tensor map storage");
+        if ((e = sfd_encode_rows_tmap(p->tmapA, p->A, (unsigned long long)Ny, Nx, 2 * sfda::NWA,
+                                      sfdw::YBOX, true)) != cudaSuccess ||
+            (e = sfd_encode_rows_tmap(p->tmapW, p->W, P * (unsigned long long)Ny, Nx, 2 * sfda::NWA,
+                                      sfdw::YBOX, true)) != cudaSuccess)
+            return fail(asm_fail(e, "cuTensorMapEncodeTiled"));
+    }
     sfd_count_launch(1);
     *out = p;
     return SFD_OK;
@@ -327,9 +455,14 @@ int sfd_asm_execute(sfd_asm_plan *p, const void *u0_dev, void *field_dev, float 
     ASM_CUDA(cudaGetDevice(&prev));
     if (prev != p->device) ASM_CUDA(cudaSetDevice(p->device));
     cudaStream_t st = (cudaStream_t)stream;
-    cudaError_t e = pick_fwd(p->lx)(p, u0_dev, st);
-    if (e == cudaSuccess) e = pick_cols(p->ly)(p, st);
-    if (e == cudaSuccess) e = pick_inv(p->lx)(p, (float2 *)field_dev, intensity_dev, phase_dev, st);
+    cudaError_t e;
+    if (p->warp) {
+        e = launch_1024(p, u0_dev, (float2 *)field_dev, intensity_dev, phase_dev, st);
+    } else {
+        e = pick_fwd(p->lx)(p, u0_dev, st);
+        if (e == cudaSuccess) e = pick_cols(p->ly)(p, st);
+        if (e == cudaSuccess) e = pick_inv(p->lx)(p, (float2 *)field_dev, intensity_dev, phase_dev, st);
+    }
     if (prev != p->device) cudaSetDevice(prev);
     if (e != cudaSuccess) return asm_fail(e, "sfd_asm_execute");
     sfd_count_launch(3);

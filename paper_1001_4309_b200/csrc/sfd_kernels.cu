@@ -493,9 +493,8 @@ bool sfd_uses_warp_x(const sfd_plan *p) {
 // [V * Ny][2 Nx], box = 4 floats (two complex columns; Ny = 2048: 8 floats, four columns) x YBOX rows,
 // no swizzle.  The encoder is a driver entry point; it is fetched through the runtime so that the
 // library does not link libcuda.
-cudaError_t sfd_make_tensormaps(sfd_plan *p) {
-    static_assert(sizeof(CUtensorMap) <= sizeof(p->tmapB), "tensor map storage");
-    if (p->d.off_tabY < 0) return cudaSuccess;
+cudaError_t sfd_encode_rows_tmap(void *out, float2 *base, unsigned long long rows, int nx,
+                                 unsigned box_floats, unsigned box_rows, bool swizzle64) {
     typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
                                   const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
                                   const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -505,15 +504,23 @@ cudaError_t sfd_make_tensormaps(sfd_plan *p) {
     cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
     if (e != cudaSuccess) return e;
     if (fn == nullptr || qr != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
-    const cuuint64_t dims[2] = {2 * (cuuint64_t)p->d.Nx, (cuuint64_t)p->d.V * p->d.Ny};
-    const cuuint64_t strides[1] = {2 * (cuuint64_t)p->d.Nx * sizeof(float)};
-    const cuuint32_t box[2] = {p->d.Ny == sfdq::NL ? (cuuint32_t)sfdq::YBOXW : 4u, sfdw::YBOX};
+    const cuuint64_t dims[2] = {2 * (cuuint64_t)nx, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {2 * (cuuint64_t)nx * sizeof(float)};
+    const cuuint32_t box[2] = {box_floats, box_rows};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = ((encode_fn)fn)(
-        reinterpret_cast<CUtensorMap *>(p->tmapB), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, p->d.B, dims,
-        strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+        reinterpret_cast<CUtensorMap *>(out), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims,
+        strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+        swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
         CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+cudaError_t sfd_make_tensormaps(sfd_plan *p) {
+    static_assert(sizeof(CUtensorMap) <= sizeof(p->tmapB), "tensor map storage");
+    if (p->d.off_tabY < 0) return cudaSuccess;
+    return sfd_encode_rows_tmap(p->tmapB, p->d.B, (unsigned long long)p->d.V * p->d.Ny, p->d.Nx,
+                                p->d.Ny == sfdq::NL ? (unsigned)sfdq::YBOXW : 4u, sfdw::YBOX);
 }
 
 void sfd_count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }

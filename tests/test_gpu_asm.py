@@ -41,7 +41,8 @@ def _check(f, I, ph, want, what):
     (128, 128, B.SFD_C64, W.PITCH, [0.01, -0.02], False),
     (256, 128, B.SFD_F32, (3.0e-6, 5.0e-6), [0.004, 0.05, 0.0], False),      # rectangular, anisotropic, z = 0
     (512, 1024, B.SFD_C64, W.PITCH, [0.08], True),                           # band limit active
-    (1024, 1024, B.SFD_C64, W.PITCH, [0.08, -0.06], False),
+    (1024, 1024, B.SFD_C64, W.PITCH, [0.08, -0.06], False),                  # the warp-FFT kernels
+    (1024, 1024, B.SFD_F32, (4.0e-6, 5.5e-6), [0.03, 0.0, -0.11, 0.2, 0.051], True),  # 5 planes: tile and table reuse
     (2048, 2048, B.SFD_F32, W.PITCH, [0.08], True),                          # the hologram generator's grid
     (4096, 2048, B.SFD_C64, 0.4e-6, [20e-6], False),                         # evanescent bins (pitch < lambda/2 .. )
 ])
