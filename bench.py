@@ -516,29 +516,43 @@ def steering(plan, wl, holo, stream, torch, B, frames=400, every=10):
 
 
 def asm_line(wl, dev, torch, B, np, reps=200):
-    """Row f4: angular-spectrum propagations per second at the workload's size, complex64 in,
-    field + intensity + phase out, inputs resident, distinct buffers rotated through L2."""
+    """Row f4: angular-spectrum propagations per second at the workload's size, complex64 in, inputs
+    resident, distinct buffers rotated through L2: one plane with field + intensity + phase out, and
+    an 8-plane focus stack (field + intensity) from one input."""
     N = wl.N
-    R = 6
-    u0 = [torch.randn(N, N, dtype=torch.complex64, device=dev) for _ in range(R)]
-    outs = [(torch.empty((1, N, N), dtype=torch.complex64, device=dev),
-             torch.empty((1, N, N), dtype=torch.float32, device=dev),
-             torch.empty((1, N, N), dtype=torch.float32, device=dev)) for _ in range(R)]
     stream = torch.cuda.current_stream()
-    with B.AsmPlan(N, N, wl.lam, 4.65e-6, [0.08]) as plan:
-        for i in range(10):
-            B.sfd_asm_execute(plan.handle, u0[i % R], *outs[i % R], stream)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        for i in range(reps):
-            B.sfd_asm_execute(plan.handle, u0[i % R], *outs[i % R], stream)
-        e1.record(stream)
-        torch.cuda.synchronize()
-    sec = e0.elapsed_time(e1) * 1e-3 / reps
+
+    def run(P, with_phase, R):
+        u0 = [torch.randn(N, N, dtype=torch.complex64, device=dev) for _ in range(R)]
+        outs = [(torch.empty((P, N, N), dtype=torch.complex64, device=dev),
+                 torch.empty((P, N, N), dtype=torch.float32, device=dev),
+                 torch.empty((P, N, N), dtype=torch.float32, device=dev) if with_phase else None)
+                for _ in range(R)]
+        with B.AsmPlan(N, N, wl.lam, 4.65e-6, [0.08 + 0.002 * i for i in range(P)]) as plan:
+            for i in range(10):
+                B.sfd_asm_execute(plan.handle, u0[i % R], *outs[i % R], stream)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for i in range(reps):
+                B.sfd_asm_execute(plan.handle, u0[i % R], *outs[i % R], stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3 / reps
+
+    sec = run(1, True, 6)
+    sec8 = run(8, False, 2)
     by = N * N * (8 + 8 + 8 + 8 + 8 + 8 + 8 + 4 + 4)     # in, A w/r, H, W w/r, field, intensity, phase
+    by8 = N * N * (8 + 8 + 8 + 8 * (8 + 8 + 8 + 8 + 4))  # in, A w/r; per plane H, W w/r, field, intensity
+    io, io8 = N * N * (8 + 8 + 4 + 4), N * N * (8 + 8 * (8 + 4))  # input + outputs only (what must touch HBM)
     return {"propagations_per_s": round(1.0 / sec, 1), "us": round(sec * 1e6, 2), "N": N,
             "algorithmic_bytes": by, "gbs": round(by / sec / 1e9, 1),
-            "api": "sfd_asm_execute: 3 launches (rows FFT, columns FFT x H x IFFT, rows IFFT + |u|^2 + arg u)"}
+            "io_bytes": io, "io_gbs": round(io / sec / 1e9, 1),
+            "stack8": {"us_per_plane": round(sec8 * 1e6 / 8, 2), "planes_per_s": round(8.0 / sec8, 1),
+                       "algorithmic_bytes": by8, "gbs": round(by8 / sec8 / 1e9, 1),
+                       "io_bytes": io8, "io_gbs": round(io8 / sec8 / 1e9, 1)},
+            "note": "algorithmic_bytes counts the intermediates (A, W, H) written and read between the "
+                    "kernels, which stay in L2 at this size; io_bytes is the input and the outputs only",
+            "api": "sfd_asm_execute: 3 launches (rows FFT, columns FFT x H x IFFT per plane, rows IFFT + |u|^2 + arg u)"}
 
 
 def sizes_line(wl, dev, torch, B, steps=600):
