@@ -235,6 +235,11 @@ k_cols_2048(const TIn *holo, long long hstride, int nx, const float2 *__restrict
     extern __shared__ float4 smem4[];
     sfdq::SmemYQ<TIn> &sm = *reinterpret_cast<sfdq::SmemYQ<TIn> *>(smem4);
     sfdw::pdl_launch_dependents();
+    if (threadIdx.x == 0) {
+        sfdw::mbar_init(&sm.full, 8);
+        sfdw::mbar_init(&sm.empty, 8);
+        sfdw::mbar_fence_init();
+    }
     const sfdq::Span span = sfdq::cta_span(V, nx / 4);
     const unsigned tbase = sfdq::tmq_setup(&sm.tmem, tabY, vstride, span.first_view(), twl);
     const unsigned tq = sfdw::tm_quarter(tbase, threadIdx.x >> 5);
@@ -243,11 +248,12 @@ k_cols_2048(const TIn *holo, long long hstride, int nx, const float2 *__restrict
         for (int i = threadIdx.x; i < V; i += blockDim.x) vmax[i] = 0u;
     if (mom != nullptr && blockIdx.x == 0)
         for (int i = threadIdx.x; i < 2 * V; i += blockDim.x) mom[i] = 0.0;
+    unsigned ph_full = 0, ph_empty = 0;  // parities of the slab barriers, carried across segments
     for (int s = 0; s < 2; ++s) {
         const sfdq::Range rg = span.segment(s);
         if (rg.u0 >= rg.u1) break;
         if (s == 1) sfdq::tmq_refill(tbase, tabY, vstride, rg.view);
-        sfdq::pass_y_quad<TIn>(sm, holo, hstride, tq, tq + sfdq::TQ_TW, &tmB, rg);
+        sfdq::pass_y_quad<TIn>(sm, holo, hstride, tq, tq + sfdq::TQ_TW, &tmB, rg, ph_full, ph_empty);
     }
     sfdw::tm_finish(tbase);
 }
@@ -346,11 +352,13 @@ struct Launch {
     }
 };
 
-// the slab loads of the warp kernels read 8 bytes of a hologram row at once (Ny = 512 with float
-// or 1024 with float input: 16 bytes)
+// the slab loads of the warp kernels read 8 bytes of a hologram row at once (Ny = 512 or 1024 with
+// float input, Ny = 2048 with uint8 input: 16 bytes)
 bool slab_aligned(const sfd_plan *p, const void *holo) {
     const size_t es = p->d.in_dtype == 0 ? 1 : 4;
-    const size_t mask = (p->d.Ny == sfdh::NH || p->d.Ny == sfdw::N) && p->d.in_dtype != 0 ? 15 : 7;
+    const bool wide = p->d.Ny == sfdq::NL ? p->d.in_dtype == 0
+                                          : (p->d.Ny == sfdh::NH || p->d.Ny == sfdw::N) && p->d.in_dtype != 0;
+    const size_t mask = wide ? 15 : 7;
     return (reinterpret_cast<size_t>(holo) & mask) == 0 && ((size_t)p->d.in_stride * es & mask) == 0;
 }
 

@@ -247,18 +247,25 @@ __device__ __forceinline__ void pass_x_quad(SmemXQ &sm, const float2 *Bin, int n
 // [n1][4] that one thread hands to the TMA unit: 32 bytes = one full sector per row of B.  (With
 // 16-byte rows B, which at this size does not fit L2, cost 1.2 GB of DRAM traffic per launch for
 // 0.5 GB of payload: half-written sectors are read back and merged.)
-// A quad reads its hologram samples as a slab of 8 bytes per row: uint8 = the 8 columns of two
-// units (its own are bytes 4 k + 2 q + c, k = u % 2), float = its 2 columns of one unit, and keeps
-// them in shared memory as [k][n'][h] column pairs with rows n' and n' + 1024 side by side (one
-// read gives both samples a thread folds together).
+// Hologram samples reach shared memory as slabs, kept as [quad][k][n'][h] column pairs with rows n' and
+// n' + 1024 side by side (one read gives both samples a thread folds together):
+//   float  each quad fetches its own 2 columns of one unit, 8 bytes per row (sub_load / sub_store);
+//   uint8  the CTA fetches the 16 columns of FOUR units, 16 bytes per row, once (slab16_*): a row of
+//          the hologram is one shared-memory wavefront per load instruction however few of its bytes
+//          are wanted, and the two quads want the same rows - per-quad slabs of 8 columns cost four
+//          times the wavefronts per unit (measured: the slab tail was 15 % of a line's period).
+//          The tile is handed over with two mbarriers (empty: all 8 warps have read their last
+//          column of the slab; full: all 8 warps have stored their rows of the next one).
 template <typename TIn> struct SubSlab {  // uint8
     using elem = uint2;
-    static constexpr int IPS = 2;
-    __device__ static int col(int u, int q) { return 8 * (u / 2); }
+    static constexpr int IPS = 4;
+    static constexpr bool CTA_WIDE = true;
+    __device__ static int col(int u, int q) { return 16 * (u / 4); }
 };
 template <> struct SubSlab<float> {
     using elem = float2;
     static constexpr int IPS = 1;
+    static constexpr bool CTA_WIDE = false;
     __device__ static int col(int u, int q) { return 4 * u + 2 * q; }
 };
 constexpr int YBOXW = 8;  // floats per row of a TMA store box of pass y (4 complex columns)
@@ -267,6 +274,7 @@ template <typename TIn> struct SmemYQ {
     Exch ex;
     alignas(128) float2 stage[NL][4];  // [n1][column of the unit]: final sums, TMA store source
     typename TileElem<TIn>::type tile[2][SubSlab<TIn>::IPS][N][2];  // [quad][k][n'][h]
+    unsigned long long full, empty;  // hand-over of the CTA-wide slab (uint8), 8 arrivals each
     unsigned tmem;
 };
 template <typename TIn> struct SubRegs { typename SubSlab<TIn>::elem e[16]; };
@@ -303,6 +311,29 @@ __device__ __forceinline__ void sub_store(const SubRegs<float> &t, float2 (*tile
         tile[0][n0 & (N - 1)][n0 >> 10] = t.e[i];
     }
 }
+// uint8, CTA-wide: the 256 threads fetch rows tid, tid + 256, .. (16 bytes each) of the slab that starts
+// at column col and split them into the two quads' tiles: byte 4 k + 2 q + c = unit k, quad q, column c
+struct Slab16 { uint4 e[8]; };
+__device__ __forceinline__ void slab16_load(Slab16 &t, const unsigned char *holo, long long hstride,
+                                            int col, int tid) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+        t.e[i] = *reinterpret_cast<const uint4 *>(holo + (size_t)(tid + 256 * i) * hstride + col);
+}
+__device__ __forceinline__ void slab16_store(const Slab16 &t, unsigned short (*tile)[4][N][2], int tid) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int n0 = tid + 256 * i, n = n0 & (N - 1), h = n0 >> 10;
+        const unsigned w[4] = {t.e[i].x, t.e[i].y, t.e[i].z, t.e[i].w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            tile[0][k][n][h] = (unsigned short)(w[k] & 0xffffu);
+            tile[1][k][n][h] = (unsigned short)(w[k] >> 16);
+        }
+    }
+}
+__device__ __forceinline__ void slab16_load(Slab16 &, const float *, long long, int, int) {}
+__device__ __forceinline__ void slab16_store(const Slab16 &, float2 (*)[1][N][2], int) {}
 // both samples (rows n' and n' + 1024) of column c of the pair
 __device__ __forceinline__ float2 fold_values(const unsigned short (&e)[2], int c) {
     const unsigned w = *reinterpret_cast<const unsigned *>(e);  // [n'] low half, [n' + 1024] high half
@@ -320,7 +351,7 @@ __device__ __forceinline__ float2 fold_values(const float2 (&e)[2], int c) {
 template <typename TIn>
 __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, long long hstride,
                                             unsigned tq, unsigned tt, const void *tmB,
-                                            Range rg) {
+                                            Range rg, unsigned &ph_full, unsigned &ph_empty) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, quad = warp >> 2, b = warp & 3;
     const int qt = threadIdx.x & 127;
     constexpr int IPS = SubSlab<TIn>::IPS;
@@ -328,12 +359,23 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, lo
     float2 *xb = sm.xb[warp];
     float2 *stg = &sm.stage[0][0];
     const bool leader = threadIdx.x == 0;  // issues and retires the bulk stores
-    {
+    constexpr bool CTA_WIDE = SubSlab<TIn>::CTA_WIDE;
+    auto warp_arrive = [&](unsigned long long *bar) {
+        __syncwarp();
+        if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+    };
+    if (CTA_WIDE) {
+        Slab16 t;
+        slab16_load(t, holo, hstride, SubSlab<TIn>::col(rg.u0, quad), threadIdx.x);
+        slab16_store(t, sm.tile, threadIdx.x);
+        warp_arrive(&sm.full);
+    } else {
         SubRegs<TIn> t;
         sub_load<TIn>(t, holo, hstride, SubSlab<TIn>::col(rg.u0, quad), qt);
         sub_store(t, sm.tile[quad], qt, quad);
+        quad_sync(quad);
     }
-    quad_sync(quad);
+    bool fresh = CTA_WIDE;  // a slab this warp has not yet waited for is on its way into the tile
     const Turns turns = turns_make(warp, 8, 5, true);  // named barriers 5..12
     turns_open(turns, warp, 8);
     for (int u = rg.u0; u < rg.u1; ++u) {
@@ -342,6 +384,11 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, lo
 #pragma unroll 1
         for (int cc = 0; cc < 2; ++cc) {  // the quad's two columns, one after the other
             float2 v[32];
+            if (CTA_WIDE && fresh) {  // all 8 warps have stored their rows of this slab
+                mbar_wait(&sm.full, ph_full);
+                ph_full ^= 1;
+                fresh = false;
+            }
             {   // v = a[n'] preA_b + a[n' + 1024] preB_b (a real)
                 TChunk ca, cb;
 #pragma unroll
@@ -362,7 +409,12 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, lo
             // the next sub-slab is pulled towards L2 now and loaded after the branch: 32 registers of
             // slab held across the butterflies spilled (measured: 0.91 ms per launch of config 4 with
             // the loads here, 0.72 ms with the prefetch)
-            if (cc == 1 && next_slab) sub_prefetch<TIn>(holo, hstride, SubSlab<TIn>::col(u + 1, quad), qt);
+            if (cc == 1 && next_slab) {
+                if (CTA_WIDE)
+                    warp_arrive(&sm.empty);  // this warp's last read of the slab
+                else
+                    sub_prefetch<TIn>(holo, hstride, SubSlab<TIn>::col(u + 1, quad), qt);
+            }
             quad_sync(quad);  // the previous column's exchange area has been read by all four warps
             branch<false>(v, lane, xb, tt, tq + TQ_H, turns);
             // The two quads share the staging tile (32-byte rows of B need all four columns of the
@@ -386,7 +438,15 @@ __device__ __forceinline__ void pass_y_quad(SmemYQ<TIn> &sm, const TIn *holo, lo
 #pragma unroll
             for (int i = 0; i < 16; ++i) stg[(lane + 32 * (16 * b + i)) * 4 + 2 * quad + cc] = mine[i];
             if (cc == 1) {
-                if (next_slab) {  // the tile was last read before this column's first barrier
+                if (next_slab && CTA_WIDE) {
+                    Slab16 t;
+                    slab16_load(t, holo, hstride, SubSlab<TIn>::col(u + 1, quad), threadIdx.x);
+                    mbar_wait(&sm.empty, ph_empty);  // both quads have read their last column of the slab
+                    ph_empty ^= 1;
+                    slab16_store(t, sm.tile, threadIdx.x);
+                    warp_arrive(&sm.full);
+                    fresh = true;
+                } else if (next_slab) {  // the tile was last read before this column's first barrier
                     SubRegs<TIn> t;
                     sub_load<TIn>(t, holo, hstride, SubSlab<TIn>::col(u + 1, quad), qt);
                     sub_store(t, sm.tile[quad], qt, quad);

@@ -100,8 +100,8 @@ def test_gabor_hologram_generator_on_the_gpu():
     assert np.abs(g8 - w8).max() <= 1 and (g8 != w8).mean() < 1e-3
 
 
-def test_asm_outputs_optional_and_reusable():
-    N = 128
+@pytest.mark.parametrize("N", [128, 1024])      # generic line kernels, warp-FFT kernels
+def test_asm_outputs_optional_and_reusable(N):
     u0 = torch.randn(N, N, dtype=torch.complex64, device=_dev())
     with B.AsmPlan(N, N, W.LAMBDA, W.PITCH, [0.02]) as plan:
         f, I, ph = plan.execute(u0)
@@ -113,3 +113,22 @@ def test_asm_outputs_optional_and_reusable():
         with pytest.raises(B.SfdError) as e:
             plan.execute(u0, field=False, intensity=False, phase=False)
         assert e.value.code == B.SFD_EINVAL
+
+
+def test_asm_1024_back_to_back_calls_do_not_interfere():
+    """The three warp-FFT kernels are chained by programmatic dependent launch and reuse the plan's A and W
+    buffers: calls queued without synchronisation on different inputs must each give their own result."""
+    N, zs = 1024, [0.05, 0.09, -0.02]
+    rng = np.random.default_rng(5)
+    ins = [(rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))).astype(np.complex64) for _ in range(3)]
+    dev_in = [torch.from_numpy(u).to(_dev()) for u in ins]
+    with B.AsmPlan(N, N, W.LAMBDA, W.PITCH, zs) as plan:
+        outs = [plan.execute(d, phase=False) for d in dev_in for _ in range(2)]   # a, a, b, b, c, c
+        torch.cuda.synchronize()
+    for i, u in enumerate(ins):
+        want, _, _ = A.propagate_planes(u, W.LAMBDA, zs, W.PITCH)
+        for f, I, _ in outs[2 * i:2 * i + 2]:
+            d = f.cpu().numpy().astype(np.complex128) - want
+            assert np.linalg.norm(d) / np.linalg.norm(want) <= REL_L2
+            assert np.abs(I.cpu().numpy() - A.intensity(want)).max() <= REL_MAX * A.intensity(want).max()
+        assert torch.equal(outs[2 * i][0], outs[2 * i + 1][0])
