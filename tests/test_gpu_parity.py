@@ -578,6 +578,26 @@ def test_execute_is_capturable_in_a_cuda_graph(N):
             assert torch.equal(f, f0) and torch.equal(I, I0)
 
 
+@pytest.mark.parametrize("col0", [16, 8])
+def test_2048_uint8_window_alignment(col0):
+    """The N = 2048 column kernel reads 16 bytes of a uint8 hologram row at once (the 16 columns of four
+    units).  A window of a 2 080-wide frame that starts on a 16-byte boundary runs the warp kernels with
+    a row stride that is not N; one that starts on an 8-byte boundary only silently takes the generic
+    pass y (a 16-byte load there would fault).  Both against the oracle on the oracle's own crop."""
+    N, stride, row0 = 2048, 2080, 1
+    rng = np.random.default_rng(col0)
+    frame = rng.integers(0, 256, (N + 2, stride), dtype=np.uint8)
+    g = {k: v[:2] for k, v in _GENERAL.items()}
+    win = np.ascontiguousarray(O.crop_window(frame, N, N, row0, col0))
+    fr = torch.from_numpy(frame).to(_dev())
+    assert fr.data_ptr() % 16 == 0
+    with B.Plan(N=N, lam=W.LAMBDA, in_dtype=B.SFD_U8, **g) as plan:
+        plan.set_input_window((N + 2, stride), row0, col0)
+        f, _ = plan.execute(fr)
+        torch.cuda.synchronize()
+    _assert_close(f.cpu().numpy(), _general_oracle(win, g, "B"), f"2048 window at column {col0}")
+
+
 # ---- round 2: tight regression bound, P5 on the GPU, rectangular grids, frame windows, live updates ------
 REG_L2, REG_MAX = 2e-6, 1e-5   # measured 1.5e-7 .. 3.5e-7 / 4e-7 .. 1.1e-6: a 10x loss of precision turns this red
 
