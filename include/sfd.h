@@ -250,11 +250,11 @@ SFD_API int sfd_host_tables_general(int N, double lambda, double p1, double p2, 
  * |f| > 1/(lambda sqrt((2 z/(N p))^2 + 1)).  One plan holds n_planes depths z[] of one input: the row
  * transform of the input is shared, H is cached per plane (built on the device in float64 at plan
  * creation, 8 bytes per sample and plane).  Three launches per call: the fp32 line-FFT kernels of the
- * generic Fresnel path, and for a 1024 x 1024 grid the warp FFT of the Fresnel fast
- * path, whose column kernel transforms a column forward once for all planes.
+ * generic Fresnel path, and for 1024 x 1024 and 2048 x 2048 grids the warp FFT of the
+ * Fresnel fast path, whose column kernel transforms a column forward once for all planes.
  *   Nx, Ny     powers of two in 128..4096 (else SFD_EUNSUPPORTED); z[] finite, any sign, 0 allowed.
  *   in_dtype   SFD_F32 (real input) or SFD_C64.
- * sfd_asm_execute: u0_dev [Ny][Nx] of in_dtype; outputs [n_planes][Ny][Nx]: field_dev complex64,
+ * sfd_asm_execute: u0_dev [Ny][Nx] of in_dtype (16-byte aligned for a 2048 x 2048 plan); outputs [n_planes][Ny][Nx]: field_dev complex64,
  * intensity_dev float32 = |u|^2, phase_dev float32 = atan2(im, re) in (-pi, pi]; each may be NULL, not
  * all three.  Asynchronous on `stream`; calls on one plan must be ordered (one stream, or events): the
  * plan owns the intermediates between its three kernels.

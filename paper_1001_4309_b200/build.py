@@ -17,7 +17,7 @@ ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libsfd.so"
 SOURCES = [CSRC / "sfd_kernels.cu", CSRC / "sfd_asm.cu", CSRC / "sfd_plan.cpp"]
-HEADERS = [CSRC / "sfd_fft_core.cuh", CSRC / "sfd_dft32.cuh", CSRC / "sfd_warp1024.cuh", CSRC / "sfd_warp2048.cuh", CSRC / "sfd_warp512.cuh", CSRC / "sfd_asm1024.cuh", CSRC / "sfd_internal.h", ROOT / "include" / "sfd.h"]
+HEADERS = [CSRC / "sfd_fft_core.cuh", CSRC / "sfd_dft32.cuh", CSRC / "sfd_warp1024.cuh", CSRC / "sfd_warp2048.cuh", CSRC / "sfd_warp512.cuh", CSRC / "sfd_asm1024.cuh", CSRC / "sfd_asm2048.cuh", CSRC / "sfd_internal.h", ROOT / "include" / "sfd.h"]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -30,6 +30,7 @@
 
 #include "sfd.h"
 #include "sfd_asm1024.cuh"
+#include "sfd_asm2048.cuh"
 #include "sfd_fft_core.cuh"
 #include "sfd_internal.h"
 
@@ -73,9 +74,12 @@ k_asm_transfer(float2 *H, int Nx, int Ny, double lambda, double px, double py, c
     }
     if (!warp_layout) {
         H[((size_t)p * Ny + ky) * Nx + kx] = h;
-    } else {  // T_p[kx][ky] = sigma(ky) sigma(kx) H_p[ky][kx] / (Nx Ny), sfd_asm1024.cuh
+    } else if (warp_layout == 1) {  // T_p[kx][ky] = sigma(ky) sigma(kx) H_p[ky][kx] / (Nx Ny), sfd_asm1024.cuh
         if ((__popc(kx) + __popc(ky)) & 1) h = make_float2(-h.x, -h.y);
         H[((size_t)p * Nx + kx) * Ny + ky] = h;
+    } else {  // T_p[kx][ky & 1][ky >> 1] = sigma(ky >> 1) sigma(kx mod 1024) H_p[ky][kx] / (Nx Ny), sfd_asm2048.cuh
+        if ((__popc(kx & 1023) + __popc(ky >> 1)) & 1) h = make_float2(-h.x, -h.y);
+        H[(((size_t)p * Nx + kx) * 2 + (ky & 1)) * 1024 + (ky >> 1)] = h;
     }
 }
 
@@ -106,6 +110,58 @@ k_asm1024_cols(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     }
     __syncthreads();
     sfda::cols(sm, &tmA, &tmW, Tt, twl, P);
+}
+
+// ---- 2048 x 2048: a pair of warps per line (sfd_asm2048.cuh) -----------------------------------------
+template <typename TIn>
+__global__ void __launch_bounds__(256, 1)
+k_asm2048_rows_fwd(const TIn *u0, const float2 *__restrict__ twl, const float2 *__restrict__ w2048,
+                   float2 *A, int rows) {
+    extern __shared__ float4 smem4[];
+    sfda2::SmemI2 &sm = *reinterpret_cast<sfda2::SmemI2 *>(smem4);
+    pdl_launch_dependents();
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < sfda2::NPAIR; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
+        sfdw::mbar_fence_init();
+    }
+    __syncthreads();
+    sfda2::rows_fwd<TIn>(sm, u0, twl, w2048, A, rows);
+}
+
+__global__ void __launch_bounds__(sfda::NTC, 1)
+k_asm2048_cols(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmW,
+               const float2 *__restrict__ Tt, const float2 *__restrict__ twl,
+               const float2 *__restrict__ w2048, int P) {
+    extern __shared__ float4 smem4[];
+    sfda2::SmemC2 &sm = *reinterpret_cast<sfda2::SmemC2 *>(
+        (reinterpret_cast<uintptr_t>(smem4) + 1023) & ~(uintptr_t)1023);
+    pdl_launch_dependents();
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < sfda::NWA; ++i) sfdw::mbar_init(&sm.tbar[i], 1);
+        sfdw::mbar_init(&sm.in_full, 1);
+        sfdw::mbar_init(&sm.in_read, sfda::NWA);
+        sfdw::mbar_init(&sm.staged, sfda::NWA);
+        sfdw::mbar_init(&sm.empty, 1);
+        sfdw::mbar_fence_init();
+    }
+    __syncthreads();
+    sfda2::cols(sm, &tmA, &tmW, Tt, twl, w2048, P);
+}
+
+template <bool PHASE>
+__global__ void __launch_bounds__(256, 1)
+k_asm2048_rows_inv(const float2 *W, const float2 *__restrict__ twl, const float2 *__restrict__ w2048,
+                   float2 *__restrict__ field, float *__restrict__ inten, float *__restrict__ phase,
+                   int rows) {
+    extern __shared__ float4 smem4[];
+    sfda2::SmemI2 &sm = *reinterpret_cast<sfda2::SmemI2 *>(smem4);
+    pdl_launch_dependents();
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < sfda2::NPAIR; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
+        sfdw::mbar_fence_init();
+    }
+    __syncthreads();
+    sfda2::rows_inv<PHASE>(sm, W, twl, w2048, field, inten, phase, rows);
 }
 
 template <bool PHASE>
@@ -219,8 +275,8 @@ struct sfd_asm_plan {
     float2 *W = nullptr;     // [P][Ny][Nx]   after the column pass
     float2 *tw_x = nullptr;  // [Nx] exp(-2 pi i k / Nx)
     float2 *tw_y = nullptr;  // [Ny]
-    // 1024 x 1024: warp-FFT kernels; H holds T[p][kx][ky] then (sfd_asm1024.cuh)
-    bool warp = false;
+    // 1 = 1024 x 1024, 2 = 2048 x 2048: warp-FFT kernels; H holds T then (sfd_asm1024.cuh / sfd_asm2048.cuh)
+    int warp = 0;
     int sms = 0;
     float2 *twl = nullptr;  // [31][32] stage-B twiddles of the warp FFT (sfd_dft32.cuh)
     alignas(64) unsigned char tmapA[128] = {};
@@ -315,6 +371,11 @@ cudaError_t asm_attrs_1024() {
     ASM_SMEM(k_asm1024_cols, sizeof(sfda::SmemC) + 1024)
     ASM_SMEM(k_asm1024_rows_inv<false>, sizeof(sfda::SmemI))
     ASM_SMEM(k_asm1024_rows_inv<true>, sizeof(sfda::SmemI))
+    ASM_SMEM(k_asm2048_rows_fwd<float>, sizeof(sfda2::SmemI2))
+    ASM_SMEM(k_asm2048_rows_fwd<float2>, sizeof(sfda2::SmemI2))
+    ASM_SMEM(k_asm2048_cols, sizeof(sfda2::SmemC2) + 1024)
+    ASM_SMEM(k_asm2048_rows_inv<false>, sizeof(sfda2::SmemI2))
+    ASM_SMEM(k_asm2048_rows_inv<true>, sizeof(sfda2::SmemI2))
 #undef ASM_SMEM
     return cudaSuccess;
 }
@@ -348,6 +409,38 @@ cudaError_t launch_1024(const sfd_asm_plan *p, const void *in, float2 *field, fl
                                   (const float2 *)p->twl, field, inten, phase, rows);
     return cudaLaunchKernelEx(&l.cfg, k_asm1024_rows_inv<false>, (const float2 *)p->W,
                               (const float2 *)p->twl, field, inten, phase, rows);
+}
+
+// the three kernels of the 2048 x 2048 path
+cudaError_t launch_2048(const sfd_asm_plan *p, const void *in, float2 *field, float *inten,
+                        float *phase, cudaStream_t st) {
+    constexpr int NW = sfda::NWA, NP = sfda2::NPAIR, NL = sfda2::NL;
+    const float2 *w = p->tw_x;  // exp(-2 pi i k / 2048): its first 1024 entries are the radix-2 twiddles
+    cudaError_t e;
+    {
+        Launch l(dim3(NL / NP < p->sms ? NL / NP : p->sms), dim3(32 * NW), sizeof(sfda2::SmemI2), st);
+        if (p->in_dtype == SFD_F32)
+            e = cudaLaunchKernelEx(&l.cfg, k_asm2048_rows_fwd<float>, (const float *)in,
+                                   (const float2 *)p->twl, w, p->A, NL);
+        else
+            e = cudaLaunchKernelEx(&l.cfg, k_asm2048_rows_fwd<float2>, (const float2 *)in,
+                                   (const float2 *)p->twl, w, p->A, NL);
+        if (e != cudaSuccess) return e;
+    }
+    {
+        Launch l(dim3(NL / NP < p->sms ? NL / NP : p->sms), dim3(sfda::NTC), sizeof(sfda2::SmemC2) + 1024, st);
+        e = cudaLaunchKernelEx(&l.cfg, k_asm2048_cols, *reinterpret_cast<const CUtensorMap *>(p->tmapA),
+                               *reinterpret_cast<const CUtensorMap *>(p->tmapW), (const float2 *)p->H,
+                               (const float2 *)p->twl, w, p->P);
+        if (e != cudaSuccess) return e;
+    }
+    const int rows = p->P * NL, ctas = rows / NP < p->sms ? rows / NP : p->sms;
+    Launch l(dim3(ctas), dim3(32 * NW), sizeof(sfda2::SmemI2), st);
+    if (phase)
+        return cudaLaunchKernelEx(&l.cfg, k_asm2048_rows_inv<true>, (const float2 *)p->W,
+                                  (const float2 *)p->twl, w, field, inten, phase, rows);
+    return cudaLaunchKernelEx(&l.cfg, k_asm2048_rows_inv<false>, (const float2 *)p->W,
+                              (const float2 *)p->twl, w, field, inten, phase, rows);
 }
 
 bool g_attr_done[64] = {};
@@ -387,7 +480,7 @@ int sfd_asm_plan_create(sfd_asm_plan **out, int Nx, int Ny, int n_planes, double
     p->Nx = Nx; p->Ny = Ny; p->lx = lx; p->ly = ly; p->P = n_planes;
     p->in_dtype = in_dtype; p->band_limit = band_limit != 0; p->device = device;
     p->lambda = lambda; p->px = px; p->py = py;
-    p->warp = Nx == sfdw::N && Ny == sfdw::N;
+    p->warp = Nx == sfdw::N && Ny == sfdw::N ? 1 : Nx == sfda2::NL && Ny == sfda2::NL ? 2 : 0;
     ASM_CUDA(cudaDeviceGetAttribute(&p->sms, cudaDevAttrMultiProcessorCount, device));
     const size_t nn = (size_t)Nx * Ny, P = n_planes;
     auto fail = [&](int code) {
@@ -429,7 +522,7 @@ int sfd_asm_plan_create(sfd_asm_plan **out, int Nx, int Ny, int n_planes, double
     e = cudaMemcpy(zd, z, P * sizeof(double), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) {
         k_asm_transfer<<<dim3((Nx + 255) / 256, Ny, n_planes), 256>>>(p->H, Nx, Ny, lambda, px, py, zd,
-                                                                     p->band_limit, p->warp ? 1 : 0);
+                                                                     p->band_limit, p->warp);
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
@@ -437,10 +530,13 @@ int sfd_asm_plan_create(sfd_asm_plan **out, int Nx, int Ny, int n_planes, double
     if (e != cudaSuccess) return fail(asm_fail(e, "k_asm_transfer"));
     if (p->warp) {
         static_assert(sizeof(CUtensorMap) <= sizeof(p->tmapA), "tensor map storage");
-        if ((e = sfd_encode_rows_tmap(p->tmapA, p->A, (unsigned long long)Ny, Nx, 2 * sfda::NWA,
-                                      sfdw::YBOX, true)) != cudaSuccess ||
-            (e = sfd_encode_rows_tmap(p->tmapW, p->W, P * (unsigned long long)Ny, Nx, 2 * sfda::NWA,
-                                      sfdw::YBOX, true)) != cudaSuccess)
+        // column tiles: 8 columns (64-byte rows) at 1024, 4 columns (32-byte rows) at 2048
+        const unsigned bw = p->warp == 1 ? 2 * sfda::NWA : 2 * sfda2::NPAIR;
+        const int swz = p->warp == 1 ? 64 : 32;
+        if ((e = sfd_encode_rows_tmap(p->tmapA, p->A, (unsigned long long)Ny, Nx, bw, sfdw::YBOX, swz)) !=
+                cudaSuccess ||
+            (e = sfd_encode_rows_tmap(p->tmapW, p->W, P * (unsigned long long)Ny, Nx, bw, sfdw::YBOX, swz)) !=
+                cudaSuccess)
             return fail(asm_fail(e, "cuTensorMapEncodeTiled"));
     }
     sfd_count_launch(1);
@@ -451,13 +547,17 @@ int sfd_asm_plan_create(sfd_asm_plan **out, int Nx, int Ny, int n_planes, double
 int sfd_asm_execute(sfd_asm_plan *p, const void *u0_dev, void *field_dev, float *intensity_dev,
                     float *phase_dev, void *stream) {
     if (!p || !u0_dev || (!field_dev && !intensity_dev && !phase_dev)) return SFD_EINVAL;
+    // the 2048 x 2048 kernels fetch input rows as bulk copies
+    if (p->warp == 2 && (reinterpret_cast<uintptr_t>(u0_dev) & 15) != 0) return SFD_EINVAL;
     int prev = -1;
     ASM_CUDA(cudaGetDevice(&prev));
     if (prev != p->device) ASM_CUDA(cudaSetDevice(p->device));
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e;
-    if (p->warp) {
+    if (p->warp == 1) {
         e = launch_1024(p, u0_dev, (float2 *)field_dev, intensity_dev, phase_dev, st);
+    } else if (p->warp == 2) {
+        e = launch_2048(p, u0_dev, (float2 *)field_dev, intensity_dev, phase_dev, st);
     } else {
         e = pick_fwd(p->lx)(p, u0_dev, st);
         if (e == cudaSuccess) e = pick_cols(p->ly)(p, st);

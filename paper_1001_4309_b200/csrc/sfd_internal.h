@@ -79,9 +79,10 @@ void sfd_count_launch(int n);
 cudaError_t sfd_make_tensormaps(sfd_plan *p);
 // Tensor map (128 bytes at `out`, 64-byte aligned) of a complex64 matrix [rows][nx] seen as float
 // [rows][2 nx], tiled in boxes of box_floats x box_rows (the column tiles of the warp kernels);
-// swizzle64: the 16-byte chunks of a 64-byte box row are permuted in shared memory (SWIZZLE_64B)
+// swizzle = 32 / 64: the 16-byte chunks of a 32- / 64-byte box row are permuted in shared memory
+// (SWIZZLE_32B / SWIZZLE_64B), 0: none
 cudaError_t sfd_encode_rows_tmap(void *out, float2 *base, unsigned long long rows, int nx,
-                                 unsigned box_floats, unsigned box_rows, bool swizzle64 = false);
+                                 unsigned box_floats, unsigned box_rows, int swizzle = 0);
 // fp32 pipe micro-benchmarks (sfd_kernels.cu), see sfd_measure_pipes in sfd.h
 cudaError_t sfd_measure_pipes_impl(double out[4]);
 // host-side step of the register butterflies (sfd_kernels.cu, compiled for the host as well)

@@ -502,7 +502,7 @@ bool sfd_uses_warp_x(const sfd_plan *p) {
 // no swizzle.  The encoder is a driver entry point; it is fetched through the runtime so that the
 // library does not link libcuda.
 cudaError_t sfd_encode_rows_tmap(void *out, float2 *base, unsigned long long rows, int nx,
-                                 unsigned box_floats, unsigned box_rows, bool swizzle64) {
+                                 unsigned box_floats, unsigned box_rows, int swizzle) {
     typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *,
                                   const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
                                   const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -519,7 +519,8 @@ cudaError_t sfd_encode_rows_tmap(void *out, float2 *base, unsigned long long row
     const CUresult r = ((encode_fn)fn)(
         reinterpret_cast<CUtensorMap *>(out), CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base, dims,
         strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-        swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
+        swizzle == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
+                      : swizzle == 32 ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_NONE,
         CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }

@@ -43,7 +43,8 @@ def _check(f, I, ph, want, what):
     (512, 1024, B.SFD_C64, W.PITCH, [0.08], True),                           # band limit active
     (1024, 1024, B.SFD_C64, W.PITCH, [0.08, -0.06], False),                  # the warp-FFT kernels
     (1024, 1024, B.SFD_F32, (4.0e-6, 5.5e-6), [0.03, 0.0, -0.11, 0.2, 0.051], True),  # 5 planes: tile and table reuse
-    (2048, 2048, B.SFD_F32, W.PITCH, [0.08], True),                          # the hologram generator's grid
+    (2048, 2048, B.SFD_F32, W.PITCH, [0.08], True),                          # the hologram generator's grid: pair-of-warps kernels
+    (2048, 2048, B.SFD_C64, (4.0e-6, 5.5e-6), [0.05, -0.12, 0.0], False),    # 3 planes: spectrum kept, tile and table reuse
     (4096, 2048, B.SFD_C64, 0.4e-6, [20e-6], False),                         # evanescent bins (pitch < lambda/2 .. )
 ])
 def test_asm_against_oracle(Nx, Ny, dtype, pitch, zs, bl):
