@@ -92,6 +92,28 @@ SFD_API int sfd_execute(sfd_plan *plan, const void *hologram_dev, void *field_de
 SFD_API int sfd_execute_u8(sfd_plan *plan, const void *hologram_dev, unsigned char *intensity_u8_dev,
                    void *stream);
 
+/* Allocation-free variant of step (xi) (L95, reading 15) for callers that cannot call cudaMalloc (code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid it): no plan, no workspace.
+ *   intensity_dev     [n_views][pixels_per_view] float32 on the device, values >= 0 (e.g. the intensity
+ *                     output of sfd_execute), 16-byte aligned; pixels_per_view a multiple of 4
+ *   intensity_u8_dev  [n_views][pixels_per_view] unsigned char on the device, 4-byte aligned; per view
+ *                     I8 = round_half_even(255 * I / max(I)) (an all-zero view gives zeros) - the same
+ *                     arithmetic and the same quantisation kernel as sfd_execute_u8
+ * The per-view maxima are kept in a static device array inside the library (SFD_STATIC_MAX_VIEWS
+ * 32-bit words = 4 KiB, present on every GPU that loads the library until the process exits); the
+ * call enqueues a clear of the words it uses and two kernels on `stream` and returns.  It calls no
+ * cudaMalloc / cudaFree or any allocating routine (the first call on a device looks up the array's
+ * address).  ALL calls share that array: calls on one stream are ordered and safe; calls that may
+ * overlap on the GPU (different streams without an event between them) race on it and must be
+ * serialised by the caller.
+ * Errors: SFD_EINVAL (NULL, sizes, alignment), SFD_EUNSUPPORTED if n_views > SFD_STATIC_MAX_VIEWS
+ * (split the call), SFD_ECUDA; sfd_static_last_error() gives the text of this thread's last failure. */
+#define SFD_STATIC_MAX_VIEWS 1024
+SFD_API int sfd_quantise_u8_static(const float *intensity_dev, int n_views, long long pixels_per_view,
+                                   unsigned char *intensity_u8_dev, void *stream);
+SFD_API int sfd_static_max_views(void);
+SFD_API const char *sfd_static_last_error(void);
+
 /* Depth stacks / focus sweep ("different depths along the depth direction",
  * PAPER.md L33 and Fig. 1): a plan whose views differ only in z is a depth stack of one hologram.
  * This call runs the same two passes and, fused into the last one, reduces every view to its first

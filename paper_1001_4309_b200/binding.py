@@ -58,6 +58,9 @@ _sig = {
     "sfd_execute": (C.c_int, [_vp, _vp, _vp, _vp, _vp]),
     "sfd_execute_u8": (C.c_int, [_vp, _vp, _vp, _vp]),
     "sfd_execute_focus": (C.c_int, [_vp, _vp, _vp, _vp, _vp]),
+    "sfd_quantise_u8_static": (C.c_int, [_vp, C.c_int, C.c_longlong, _vp, _vp]),
+    "sfd_static_max_views": (C.c_int, []),
+    "sfd_static_last_error": (C.c_char_p, []),
     "sfd_stream_run": (C.c_int, [_vp, _vp, C.c_int, _vp, _dp]),
     "sfd_plan_update_view": (C.c_int, [_vp, C.c_int] + [C.c_double] * 5),
     "sfd_plan_destroy": (C.c_int, [_vp]),
@@ -235,6 +238,23 @@ def sfd_plan_update_view_general(plan, view, p1x, p1y, p2x, p2y, z, O0x, O0y, O1
 def sfd_execute(plan, hologram_dev, field_dev, intensity_dev, stream=None):
     _chk(_lib.sfd_execute(plan, _ptr(hologram_dev), _ptr(field_dev), _ptr(intensity_dev),
                           _stream(stream)), "sfd_execute")
+
+
+def sfd_quantise_u8_static(intensity_dev, n_views, pixels_per_view, intensity_u8_dev, stream=None):
+    code = _lib.sfd_quantise_u8_static(_ptr(intensity_dev), n_views, pixels_per_view, _ptr(intensity_u8_dev),
+                                       _stream(stream))
+    if code != SFD_OK:
+        err = SfdError(code, "sfd_quantise_u8_static")
+        err.args = (err.args[0] + ": " + _lib.sfd_static_last_error().decode(),)
+        raise err
+
+
+def sfd_static_max_views():
+    return int(_lib.sfd_static_max_views())
+
+
+def sfd_static_last_error():
+    return _lib.sfd_static_last_error().decode()
 
 
 def sfd_execute_focus(plan, hologram_dev, moments_dev, intensity_dev=None, stream=None):

@@ -13,6 +13,8 @@
 
 #include <atomic>
 #include <cmath>
+#include <cstdio>
+#include <mutex>
 #include <vector>
 
 #include "sfd_fft_core.cuh"
@@ -679,3 +681,108 @@ void sfd_host_dft32_impl(const float *in, float *out, int lane, int twiddled) {
         out[2 * r + 1] = sg * v[r].y;
     }
 }
+
+// ---- allocation-free 8-bit quantisation (sfd_quantise_u8_static, include/sfd.h) -----------------------
+// Step (xi) / reading 15 on its own, for callers that may not allocate (code under CUDA graph
+// capture, serving loops, harnesses that forbid cudaMalloc): float intensities in, 8-bit images out,
+// I8 = round_half_even(255 I / max I) per view.  The per-view maxima - the scratch that sfd_execute_u8
+// keeps in plan memory (sfd_dev::vmax) - live in the array below instead: SFD_STATIC_MAX_VIEWS words,
+// held by every GPU that loads the library until the process exits.  In host code the array's NAME is
+// a host-side stand-in, not a device address; the address comes from cudaGetSymbolAddress, once per
+// device with that device current (static_scratch below).  All calls share the array and it keeps the
+// last call's contents: every call clears the words it uses first (stream-ordered), and calls that
+// overlap on the GPU (different streams without an event between them) race on it.
+static __device__ __align__(256) unsigned int g_static_vmax[SFD_STATIC_MAX_VIEWS];
+
+namespace {
+
+// per-view maximum of `quads` float4s into vmax[view] (cleared beforehand); intensities are >= 0, so
+// their bit patterns order like unsigned integers (as in pass x)
+__global__ void __launch_bounds__(256)
+k_view_max_static(const float4 *__restrict__ inten, unsigned int *vmax, int quads_per_view) {
+    const int v = blockIdx.y;
+    const size_t base = (size_t)v * quads_per_view;
+    float mx = 0.f;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < quads_per_view; i += gridDim.x * blockDim.x) {
+        const float4 I = inten[base + i];
+        mx = fmaxf(fmaxf(mx, fmaxf(I.x, I.y)), fmaxf(I.z, I.w));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    if ((threadIdx.x & 31) == 0 && mx > 0.f) atomicMax(vmax + v, __float_as_uint(mx));
+}
+
+std::mutex g_static_mu;
+unsigned int *g_static_ptr[64] = {};  // device address of g_static_vmax, per device
+thread_local char g_static_err[200] = "no error";
+
+// device address of the scratch array on the current device (looked up on the device's first call)
+cudaError_t static_scratch(unsigned int **out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (g_static_ptr[dev] == nullptr) {
+        void *ptr = nullptr;
+        if ((e = cudaGetSymbolAddress(&ptr, g_static_vmax)) != cudaSuccess) return e;
+        g_static_ptr[dev] = static_cast<unsigned int *>(ptr);
+    }
+    *out = g_static_ptr[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" {
+
+SFD_API int sfd_quantise_u8_static(const float *intensity_dev, int n_views, long long pixels_per_view,
+                                   unsigned char *intensity_u8_dev, void *stream) {
+    auto fail = [](int code, const char *what) {
+        std::snprintf(g_static_err, sizeof g_static_err, "sfd_quantise_u8_static: %s", what);
+        return code;
+    };
+    if (!intensity_dev || !intensity_u8_dev) return fail(SFD_EINVAL, "NULL pointer");
+    if (n_views < 1 || pixels_per_view < 4 || pixels_per_view % 4 != 0 ||
+        pixels_per_view / 4 > 0x7fffffffLL)
+        return fail(SFD_EINVAL, "n_views >= 1 and pixels_per_view a positive multiple of 4 (< 2^33) are required");
+    if ((reinterpret_cast<size_t>(intensity_dev) & 15) != 0 || (reinterpret_cast<size_t>(intensity_u8_dev) & 3) != 0)
+        return fail(SFD_EINVAL, "intensity_dev must be 16-byte, intensity_u8_dev 4-byte aligned");
+    if (n_views > SFD_STATIC_MAX_VIEWS) {
+        std::snprintf(g_static_err, sizeof g_static_err,
+                      "sfd_quantise_u8_static: n_views = %d exceeds SFD_STATIC_MAX_VIEWS = %d (the size of "
+                      "the library's static scratch array); split the call",
+                      n_views, SFD_STATIC_MAX_VIEWS);
+        return SFD_EUNSUPPORTED;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned int *vmax = nullptr;
+    cudaError_t e = static_scratch(&vmax);
+    const int quads = (int)(pixels_per_view / 4);
+    const int blocks = (quads + 256 * 4 - 1) / (256 * 4);
+    // the array keeps the last call's maxima: clear this call's words first
+    if (e == cudaSuccess) e = cudaMemsetAsync(vmax, 0, (size_t)n_views * sizeof(unsigned int), st);
+    if (e == cudaSuccess) {
+        k_view_max_static<<<dim3(blocks, n_views), 256, 0, st>>>((const float4 *)intensity_dev, vmax, quads);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) {
+        Launch l(dim3(blocks, n_views), dim3(256), 0, st);
+        e = cudaLaunchKernelEx(&l.cfg, k_quantise, (const float4 *)intensity_dev,
+                               (const unsigned int *)vmax, (uchar4 *)intensity_u8_dev, quads);
+    }
+    if (e != cudaSuccess) {
+        std::snprintf(g_static_err, sizeof g_static_err, "sfd_quantise_u8_static: %s (%s)",
+                      cudaGetErrorName(e), cudaGetErrorString(e));
+        cudaGetLastError();
+        return SFD_ECUDA;
+    }
+    g_launches.fetch_add(2, std::memory_order_relaxed);
+    return SFD_OK;
+}
+
+SFD_API int sfd_static_max_views(void) { return SFD_STATIC_MAX_VIEWS; }
+
+SFD_API const char *sfd_static_last_error(void) { return g_static_err; }
+
+}  // extern "C"
