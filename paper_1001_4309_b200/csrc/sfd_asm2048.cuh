@@ -183,7 +183,18 @@ __device__ __forceinline__ void rows_inv(SmemI2 &sm, const float2 *W, const floa
             const float2 u = make_float2(s * v[k].x, -s * v[k].y);
             if (field) field[o + 32 * k] = u;
             if (inten) inten[o + 32 * k] = u.x * u.x + u.y * u.y;
-            if (PHASE) phase[o + 32 * k] = atan2f(u.y, u.x);
+            if (PHASE) sm.xb[warp][k * 32 + lane] = u;
+        }
+        // arg u in a ROLLED loop over values parked in the (idle) transpose tile: 32 inlined atan2f are as
+        // long as the transform itself and do not fit the instruction cache beside it
+        if (PHASE) {
+            const float2 *pu = sm.xb[warp] + lane;
+#pragma unroll 2
+            for (int k = 0; k < 32; ++k) {
+                const float2 u = pu[k * 32];
+                phase[o + 32 * k] = atan2f(u.y, u.x);
+            }
+            __syncwarp();  // all lanes have read the tile before the next transpose writes it
         }
     }
 }
