@@ -133,3 +133,18 @@ def test_asm_1024_back_to_back_calls_do_not_interfere():
             assert np.linalg.norm(d) / np.linalg.norm(want) <= REL_L2
             assert np.abs(I.cpu().numpy() - A.intensity(want)).max() <= REL_MAX * A.intensity(want).max()
         assert torch.equal(outs[2 * i][0], outs[2 * i + 1][0])
+
+
+def test_asm_2048_rejects_an_input_that_is_not_16_byte_aligned():
+    """The 2048 x 2048 kernels fetch input rows as bulk copies (16-byte granules): an input 8 bytes off is an
+    argument error, not a fault; the same view shifted back works."""
+    N = 2048
+    buf = torch.randn(N * N + 2, dtype=torch.complex64, device=_dev())
+    assert buf.data_ptr() % 16 == 0
+    with B.AsmPlan(N, N, W.LAMBDA, W.PITCH, [0.05]) as plan:
+        with pytest.raises(B.SfdError) as e:
+            plan.execute(buf[1:1 + N * N].view(N, N), intensity=False, phase=False)
+        assert e.value.code == B.SFD_EINVAL
+        f, _, _ = plan.execute(buf[2:2 + N * N].view(N, N), intensity=False, phase=False)
+        torch.cuda.synchronize()
+        assert torch.isfinite(f.abs().max())
