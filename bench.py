@@ -445,6 +445,8 @@ def run_sfd(args, info):
         extras = {"steering": steering(plan, wl, holos[0], stream, torch, B),
                   "angular_spectrum": asm_line(wl, dev, torch, B, np),
                   "other_sizes": sizes_line(wl, dev, torch, B)}
+        if 2 * wl.N <= 2048:    # the 2N grid of the hologram generator
+            extras["angular_spectrum_2N"] = asm_line(wl, dev, torch, B, np, reps=100, N=2 * wl.N)
     sampler.stop()
 
     cpu = None
@@ -515,11 +517,11 @@ def steering(plan, wl, holo, stream, torch, B, frames=400, every=10):
                    "staging, one H2D copy, no synchronisation) between sfd_execute_u8 calls"}
 
 
-def asm_line(wl, dev, torch, B, np, reps=200):
-    """Row f4: angular-spectrum propagations per second at the workload's size, complex64 in, inputs
-    resident, distinct buffers rotated through L2: one plane with field + intensity + phase out, and
-    an 8-plane focus stack (field + intensity) from one input."""
-    N = wl.N
+def asm_line(wl, dev, torch, B, np, reps=200, N=None):
+    """Row f4: angular-spectrum propagations per second on an N x N grid (default: the workload's size),
+    complex64 in, inputs resident, distinct buffers rotated through L2: one plane with field + intensity
+    + phase out, and an 8-plane focus stack (field + intensity) from one input."""
+    N = N or wl.N
     stream = torch.cuda.current_stream()
 
     def run(P, with_phase, R):
@@ -550,8 +552,9 @@ def asm_line(wl, dev, torch, B, np, reps=200):
             "stack8": {"us_per_plane": round(sec8 * 1e6 / 8, 2), "planes_per_s": round(8.0 / sec8, 1),
                        "algorithmic_bytes": by8, "gbs": round(by8 / sec8 / 1e9, 1),
                        "io_bytes": io8, "io_gbs": round(io8 / sec8 / 1e9, 1)},
-            "note": "algorithmic_bytes counts the intermediates (A, W, H) written and read between the "
-                    "kernels, which stay in L2 at this size; io_bytes is the input and the outputs only",
+            "note": "algorithmic_bytes counts the intermediates (A, W, H) written and read between the kernels"
+                    + (", which stay in L2 at this size" if N <= 1024 else " (larger than L2 at this size)")
+                    + "; io_bytes is the input and the outputs only",
             "api": "sfd_asm_execute: 3 launches (rows FFT, columns FFT x H x IFFT per plane, rows IFFT + |u|^2 + arg u)"}
 
 
