@@ -167,6 +167,7 @@ k_rows_1024(const float2 *B, int ny, const float2 *__restrict__ tabX, long long 
     sfdw::pdl_launch_dependents();
     if (threadIdx.x == 0) {
         for (int i = 0; i < sfdw::NWX / 2; ++i) sfdw::mbar_init(&sm.ibar[i], 1);
+        for (int i = 0; i < sfdw::NWX; ++i) sfdw::mbar_init(&sm.tbar[i], 1);
         sfdw::mbar_fence_init();
     }
     const unsigned tbase = sfdw::tm_setup<sfdw::NWX>(&sm.tmem, tabX, vstride, V * ny, ny, twl);

@@ -298,15 +298,44 @@ __device__ __forceinline__ void tm_finish(unsigned base) {
 // how far the warps drift apart.  Measured with two warps per sub-partition in round 1 (DESIGN.md
 // 5.4: no coupling, strict mbarrier tokens, rendezvous, the same hand-off around the butterfly
 // phases): the fastest by 1 to 11 %.
+// A CTA has 15 named barriers; a kernel with more warps than that leaves for turns (pass x: 12 warps,
+// 6 pair barriers) keeps the ring on mbarriers instead (count 1: the predecessor's lane 0 arrives after
+// its __syncwarp, the warp polls the parity of its own): `mb` set, mine / next shared-memory addresses.
+// At most one arrival is ever pending on a barrier (a warp's next turn needs the whole ring to go round),
+// so a phase cannot be overrun.
 struct Turns {
-    unsigned mine, next;  // named barriers first .. first + NW - 1
+    unsigned mine, next;  // named barriers first .. first + NW - 1 (or mbarrier addresses)
     bool on;
+    bool mb = false;
+    mutable unsigned ph = 0;  // mbarrier mode: parity of this warp's next turn
 };
 __device__ __forceinline__ void turn_begin(const Turns &t) {
-    if (t.on) asm volatile("bar.sync %0, 64;" ::"r"(t.mine) : "memory");
+    if (!t.on) return;
+    if (t.mb) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "W_%=:\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+            "@p bra D_%=;\n"
+            "bra W_%=;\n"
+            "D_%=:\n"
+            "}\n" ::"r"(t.mine),
+            "r"(t.ph)
+            : "memory");
+        t.ph ^= 1;
+    } else {
+        asm volatile("bar.sync %0, 64;" ::"r"(t.mine) : "memory");
+    }
 }
-__device__ __forceinline__ void turn_end(const Turns &t) {
-    if (t.on) asm volatile("bar.arrive %0, 64;" ::"r"(t.next) : "memory");
+__device__ __forceinline__ void turn_end(const Turns &t) {  // (the callers put a __syncwarp in front)
+    if (!t.on) return;
+    if (t.mb) {
+        if ((threadIdx.x & 31) == 0)
+            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(t.next) : "memory");
+    } else {
+        asm volatile("bar.arrive %0, 64;" ::"r"(t.next) : "memory");
+    }
 }
 // Warps 0..3 own the first turn: the last warps of the ring pass on a turn at the start and warps
 // 0..3 take one more after their last line, so that every barrier sees as many arrivals as waits.
@@ -315,6 +344,13 @@ __device__ __forceinline__ void turn_end(const Turns &t) {
 __device__ __forceinline__ Turns turns_make(int warp, int nwarps, unsigned first, bool on) {
     const int succ = warp + 4 < nwarps ? warp + 4 : (warp & 3);
     return Turns{first + warp, first + succ, on};
+}
+// the same ring on the mbarriers bars[0 .. nwarps) (initialised with count 1)
+__device__ __forceinline__ Turns turns_make_mb(int warp, int nwarps, unsigned long long *bars, bool on) {
+    const int succ = warp + 4 < nwarps ? warp + 4 : (warp & 3);
+    Turns t{smem_u32(bars + warp), smem_u32(bars + succ), on};
+    t.mb = true;
+    return t;
 }
 __device__ __forceinline__ void turns_open(const Turns &t, int warp, int nwarps) {
     if (warp + 4 >= nwarps) turn_end(t);
@@ -759,16 +795,19 @@ __device__ __forceinline__ void pass_y_loop(SmemY<TIn> &sm, const TIn *holo, lon
 }
 
 // ---- pass x: one row of B per warp pair -----------------------------------------------------------
-// Warps per CTA of pass x.  The loop below is written for any multiple of four and was measured with
-// 12 (three warps per sub-partition, 132 registers per thread with the twiddles in tensor memory):
-// per line 5 to 9 % faster, but V N / 148 = 27.7 lines per CTA are 7 rounds of 4 lines (99 % full)
-// against 5 rounds of 6 (92 %), which eats the gain, and 6 pair barriers + 12 turn barriers exceed the
-// 15 named barriers a CTA has.
-constexpr int NWX = 8;
+// Warps per CTA of pass x: 12, three per sub-partition (147 registers per thread with the twiddles in
+// tensor memory).  The loop below is written for any multiple of four; measured at config 2 with the
+// turn-taking ring on mbarriers (6 pair barriers + 12 turn barriers exceed the 15 named barriers of a
+// CTA): 8 warps 34.3 us per launch (33.7 with the ring on named barriers), 12 warps 32.4, 14 warps 34.8
+// (128 registers, spills, uneven sub-partitions), 16 warps 32.6 with a slower step.  V N / 148 = 27.7
+// lines per CTA are 5 rounds of 6 lines (92 % full) against 7 rounds of 4 (99 %): without the ring the
+// third warp only made up for that (33.9 us); with it, it is 4 % ahead.
+constexpr int NWX = 12;
 template <int NW> struct SmemX {
     float2 xb[NW][XB];
     float2 inb[NW / 2][N];  // input row of each pair (bulk async copy destination)
     unsigned long long ibar[NW / 2];
+    unsigned long long tbar[NW];  // turn-taking ring (mbarriers, count 1)
     unsigned tmem;  // base address of the tensor-memory allocation
 };
 
@@ -839,8 +878,8 @@ __device__ __forceinline__ void pass_x_loop(SmemX<NW> &sm, const float2 *Bin, in
     const bool issuer = b == 0 && lane == 0;
     const int view0 = l0 >> lgn;
     unsigned iphase = 0;
-    // turn-taking of the warps w, w + 4, .. of a sub-partition: named barriers behind the pairs' ones
-    const Turns turns = turns_make(warp, NW, XP + 1, TURNS);
+    // turn-taking of the warps w, w + 4, .. of a sub-partition (named barriers 1 .. XP are the pairs')
+    const Turns turns = turns_make_mb(warp, NW, sm.tbar, TURNS);
     turns_open(turns, warp, NW);
     if (issuer && l0 + pair < l1)
         bulk_load(sm.inb[pair], Bin + (size_t)(l0 + pair) * N, N * sizeof(float2), &sm.ibar[pair]);
