@@ -45,14 +45,15 @@ SFD_CE float cos64(int r) {  // cos(2 pi r / 64), r < 32
 }
 SFD_CE float sin64(int r) { return r <= 16 ? cos64(16 - r) : cos64(r - 16); }
 
-// v = this warp's 1024-point transform (E for h = 0, O for h = 1) -> its half of the 2048-point one
-// (wl = w^lane; the factor exp(-2 pi i r / 64) is folded into the add: e +- c_r (wl o))
-// e + exp(-2 pi i r / 64) (wd o); wd = w^lane for warp 0, -w^lane for warp 1 (which subtracts)
+// e + exp(-2 pi i r / 64) (wd o); wd = w^lane for warp 0, -w^lane for warp 1 (which subtracts): the
+// constant factor is folded into the add
 __device__ __forceinline__ float2 dit_one(float2 e, float2 o, float2 wd, int r) {
     const float2 t = make_float2(wd.x * o.x - wd.y * o.y, wd.x * o.y + wd.y * o.x);
     return make_float2(fmaf(cos64(r), t.x, fmaf(sin64(r), t.y, e.x)),
                        fmaf(cos64(r), t.y, fmaf(-sin64(r), t.x, e.y)));
 }
+// v = this warp's 1024-point transform (E for h = 0, O for h = 1), theirs = the partner's, already in
+// its tile -> this warp's half of the 2048-point transform (wl = w^lane)
 __device__ __forceinline__ void dit_finish(float2 (&v)[32], int h, int lane, const float2 *theirs, float2 wl) {
     if (h == 0) {
 #pragma unroll
