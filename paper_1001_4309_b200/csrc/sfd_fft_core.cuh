@@ -37,6 +37,17 @@
 
 namespace sfd {
 
+// Plan constants (FFT twiddles, pre / H / post tables) of the Fresnel line code: for padded lengths up to
+// M = 1024 the generic kernels hand in shared-memory copies (sfd_kernels.cu, Staged), read with plain
+// loads; otherwise they are global pointers read through the non-coherent path.
+SFD_CE bool tables_staged(int log2m) { return log2m <= 10; }
+template <bool SM> SFD_HD float2 tab_ld(const float2 *p) {
+    if constexpr (SM)
+        return *p;
+    else
+        return SFD_LDG(p);
+}
+
 SFD_HD float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 SFD_HD float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 SFD_HD float2 cmul(float2 a, float2 b) {
@@ -173,7 +184,7 @@ template <int ISTR> struct LineSmem {
 };
 
 // Twiddle (pass P >= 1) and butterfly of pass P on the register slots.  tw[x] = exp(-2 pi i x/M).
-template <int LOG2M, int P, int DIR, bool HALF_IN>
+template <int LOG2M, int P, int DIR, bool HALF_IN, bool SMTW = false>
 SFD_HD void pass_compute(float2 (&v)[16], int j, const float2 *__restrict__ tw) {
     using S = Sched<LOG2M>;
     constexpr int R = S::radix(P), Q = 16 / R, NS = S::ns(P), STEP = S::M / (NS * R);
@@ -186,7 +197,7 @@ SFD_HD void pass_compute(float2 (&v)[16], int j, const float2 *__restrict__ tw) 
         if (P > 0) {
 #pragma unroll
             for (int t = 1; t < R; ++t) {
-                float2 w = SFD_LDG(tw + k * t * STEP);
+                float2 w = tab_ld<SMTW>(tw + k * t * STEP);
                 if (DIR > 0) w.y = -w.y;
                 a[t] = cmul(a[t], w);
             }
@@ -220,22 +231,22 @@ template <int LOG2M, int ISTR> SFD_HD void gather(float2 (&v)[16], int j, LineSm
 
 // One whole FFT of direction DIR on the slots (all passes; SYNC() is a barrier over every thread
 // that shares this shared-memory buffer).
-template <int LOG2M, int DIR, bool HALF_IN, int ISTR, class SyncF>
+template <int LOG2M, int DIR, bool HALF_IN, int ISTR, class SyncF, bool SMTW = false>
 SFD_HD void fft_line(float2 (&v)[16], int j, LineSmem<ISTR> sm, const float2 *__restrict__ tw,
                      SyncF sync) {
     using S = Sched<LOG2M>;
-    pass_compute<LOG2M, 0, DIR, HALF_IN>(v, j, tw);
+    pass_compute<LOG2M, 0, DIR, HALF_IN, SMTW>(v, j, tw);
     scatter<LOG2M, 0, ISTR>(v, j, sm);
     sync();
     gather<LOG2M, ISTR>(v, j, sm);
     sync();
-    pass_compute<LOG2M, 1, DIR, false>(v, j, tw);
+    pass_compute<LOG2M, 1, DIR, false, SMTW>(v, j, tw);
     if constexpr (S::NP == 3) {
         scatter<LOG2M, 1, ISTR>(v, j, sm);
         sync();
         gather<LOG2M, ISTR>(v, j, sm);
         sync();
-        pass_compute<LOG2M, 2, DIR, false>(v, j, tw);
+        pass_compute<LOG2M, 2, DIR, false, SMTW>(v, j, tw);
     }
 }
 
@@ -248,10 +259,11 @@ SFD_HD void chirpz_line(float2 (&v)[16], int j, LineSmem<ISTR> sm, const float2 
     using S = Sched<LOG2M>;
 #pragma unroll
     for (int s = 8; s < 16; ++s) v[s] = make_float2(0.f, 0.f);
-    fft_line<LOG2M, -1, true, ISTR>(v, j, sm, tw, sync);
+    constexpr bool SM = tables_staged(LOG2M);
+    fft_line<LOG2M, -1, true, ISTR, SyncF, SM>(v, j, sm, tw, sync);
 #pragma unroll
-    for (int s = 0; s < 16; ++s) v[s] = cmul(v[s], SFD_LDG(H + j + s * S::T));
-    fft_line<LOG2M, +1, false, ISTR>(v, j, sm, tw, sync);
+    for (int s = 0; s < 16; ++s) v[s] = cmul(v[s], tab_ld<SM>(H + j + s * S::T));
+    fft_line<LOG2M, +1, false, ISTR, SyncF, SM>(v, j, sm, tw, sync);
 }
 
 // ---- the two passes of a reconstruction --------------------------------------------------------
@@ -277,7 +289,7 @@ SFD_HD void pass_y_body(int tid, int tile, float2 *smem, const TIn *holo, long l
     for (int s = 0; s < 8; ++s) {
         const int n0 = j + s * T;
         const float a = (float)holo[(size_t)n0 * hstride + col];
-        const float2 p = SFD_LDG(pre_y + n0);
+        const float2 p = tab_ld<tables_staged(LOG2M)>(pre_y + n0);
         v[s] = make_float2(a * p.x, a * p.y);
     }
     LineSmem<C> sm{smem + l};
@@ -285,7 +297,7 @@ SFD_HD void pass_y_body(int tid, int tile, float2 *smem, const TIn *holo, long l
 #pragma unroll
     for (int s = 0; s < 8; ++s) {
         const int n1 = j + s * T;
-        B[(size_t)n1 * nx + col] = cmul(v[s], SFD_LDG(post_y + n1));
+        B[(size_t)n1 * nx + col] = cmul(v[s], tab_ld<tables_staged(LOG2M)>(post_y + n1));
     }
 }
 
@@ -308,7 +320,7 @@ SFD_HD float pass_x_body(int tid, int tile, float2 *smem, const float2 *B,
 #pragma unroll
     for (int s = 0; s < 8; ++s) {
         const int m0 = j + s * T;
-        v[s] = cmul(in[m0], SFD_LDG(pre_x + m0));
+        v[s] = cmul(in[m0], tab_ld<tables_staged(LOG2M)>(pre_x + m0));
     }
     LineSmem<1> sm{smem + l * S::PADDED};
     chirpz_line<LOG2M, 1>(v, j, sm, tw, Hx, sync);
@@ -316,7 +328,7 @@ SFD_HD float pass_x_body(int tid, int tile, float2 *smem, const float2 *B,
 #pragma unroll
     for (int s = 0; s < 8; ++s) {
         const int m1 = j + s * T;
-        const float2 u = cmul(v[s], SFD_LDG(post_x + m1));
+        const float2 u = cmul(v[s], tab_ld<tables_staged(LOG2M)>(post_x + m1));
         if (field) field[row * N + m1] = u;
         const float I = u.x * u.x + u.y * u.y;
         if (inten) inten[row * N + m1] = I;
