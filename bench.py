@@ -615,14 +615,23 @@ def run_peaks():
         raise RuntimeError("bench.py --peaks needs a CUDA device")
     B.sfd_measure_pipes()                                  # warm-up (clocks, instruction cache)
     tf, ca, cb, ghz = B.sfd_measure_pipes()
+    B.sfd_measure_memory_pipes()
+    smem, tm1, tm2, tmlat = B.sfd_measure_memory_pipes()
     hbm, src = measured_peaks()
     print(json.dumps({"peaks": {"fp32_fma_tflops": round(tf, 2), "dft32_stage_a_cycles": round(ca, 1),
                                 "dft32_stage_b_cycles": round(cb, 1), "sm_ghz": round(ghz, 3),
                                 "fp32_derived_tflops": round(ALU_PEAK_TFLOPS, 1), "hbm_gbs": hbm,
                                 "hbm_source": src, "gpu": torch.cuda.get_device_name(0),
+                                "smem_bytes_per_clk_sm": round(smem, 1),
+                                "tmem_ld_bytes_per_clk_subpartition": [round(tm1, 1), round(tm2, 1)],
+                                "tmem_ld_dependent_cycles": round(tmlat, 1),
                                 "how": "sfd_measure_pipes (include/sfd.h): FFMA chains on all SMs; "
                                        "sfdb::dft32 / dft32_tw in a register-only loop, one warp per "
-                                       "sub-partition, clock64"}}), flush=True)
+                                       "sub-partition, clock64.  sfd_measure_memory_pipes: shared memory "
+                                       "in the access pattern of the 32 x 32 transposes (8 warps per SM); "
+                                       "tcgen05.ld.32x32b.x16, four in flight per warp, with one and two "
+                                       "warps per sub-partition; one dependent tcgen05.ld + wait::ld"}}),
+          flush=True)
     return 0
 
 

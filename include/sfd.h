@@ -255,6 +255,15 @@ SFD_API int sfd_host_dft32(const float *in, float *out, int lane, int twiddled);
  * the legacy default stream and synchronises.  Errors: SFD_EINVAL, SFD_ECUDA. */
 SFD_API int sfd_measure_pipes(double out[4]);
 
+/* Measured rates of the two on-chip memories as the warp kernels use them, current device:
+ * out[0] shared memory in bytes per clock and SM for the access pattern of the 32 x 32 transposes
+ * (16-byte row reads + 8-byte column writes, 8 warps per SM); out[1] / out[2] tensor-memory load rate
+ * in bytes per clock and sub-partition with one / two warps per sub-partition (four
+ * tcgen05.ld.32x32b.x16 in flight per warp, as the table reads of a line are issued); out[3] cycles of
+ * one dependent tcgen05.ld + tcgen05.wait::ld.  Runs a few milliseconds of kernels on the legacy
+ * default stream and synchronises.  Errors: SFD_EINVAL, SFD_ECUDA (text: sfd_static_last_error). */
+SFD_API int sfd_measure_memory_pipes(double out[4]);
+
 /* The same for a hologram window shifted by off0 along that axis (general geometry). */
 SFD_API int sfd_host_tables_general(int N, double lambda, double p1, double p2, double z, double off0,
                                     double off, double *pre, double *post, double *H);

@@ -48,6 +48,7 @@ _sig = {
     "sfd_plan_get_device": (C.c_int, [_vp]),
     "sfd_host_dft32": (C.c_int, [C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_int, C.c_int]),
     "sfd_measure_pipes": (C.c_int, [_dp]),
+    "sfd_measure_memory_pipes": (C.c_int, [_dp]),
     "sfd_asm_plan_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
                                       C.c_double, _dp, C.c_int, C.c_int]),
     "sfd_asm_execute": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
@@ -226,6 +227,14 @@ def sfd_measure_pipes():
     """(fp32 FMA TFLOP/s, cycles per stage-A butterfly, cycles per stage-B butterfly, SM GHz)."""
     out = np.zeros(4, np.float64)
     _chk(_lib.sfd_measure_pipes(out.ctypes.data_as(_dp)), "sfd_measure_pipes")
+    return tuple(float(v) for v in out)
+
+
+def sfd_measure_memory_pipes():
+    """(shared memory B/clk/SM in the transposes' access pattern, tensor-memory load B/clk/sub-partition with
+    one warp, with two warps per sub-partition, cycles of a dependent tcgen05.ld)."""
+    out = np.zeros(4, np.float64)
+    _chk(_lib.sfd_measure_memory_pipes(out.ctypes.data_as(_dp)), "sfd_measure_memory_pipes")
     return tuple(float(v) for v in out)
 
 

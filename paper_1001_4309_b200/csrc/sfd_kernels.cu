@@ -819,3 +819,130 @@ SFD_API int sfd_static_max_views(void) { return SFD_STATIC_MAX_VIEWS; }
 SFD_API const char *sfd_static_last_error(void) { return g_static_err; }
 
 }  // extern "C"
+
+// ---- sfd_measure_memory_pipes: shared memory and tensor memory as the warp kernels use them ----------
+namespace {
+
+// shared memory: every warp reads its own 4 KB tile with 16-byte loads (the row reads of the transposes:
+// 4 wavefronts per instruction, conflict-free) and writes it with 8-byte stores (their column writes)
+__global__ void __launch_bounds__(256, 1)
+k_peak_smem(float *out, long long *cycles, int reps) {
+    __shared__ float4 tile[8][256];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int i = lane; i < 256; i += 32) tile[warp][i] = make_float4((float)i, 1.f, 2.f, 3.f);
+    __syncthreads();
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    const long long t0 = clock64();
+    for (int r = 0; r < reps; ++r) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const float4 w = tile[warp][q * 32 + lane];
+            acc.x += w.x; acc.y += w.y; acc.z += w.z; acc.w += w.w;
+        }
+        float2 *t2 = reinterpret_cast<float2 *>(tile[warp]);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) t2[q * 32 + lane] = make_float2(acc.x, acc.y + (float)q);
+        __syncwarp();
+    }
+    __syncthreads();
+    const long long t1 = clock64();
+    out[blockIdx.x * 256 + threadIdx.x] = acc.x + acc.y + acc.z + acc.w;
+    if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
+}
+
+// tensor memory: (a) four 16-column loads in flight per warp and wait, as the table reads of a line are
+// issued; (b) one load, wait, and the next address taken from the loaded value: the dependent latency
+__global__ void __launch_bounds__(256, 1)
+k_peak_tmem(float *out, long long *cycles, int reps, int warps_per_quarter) {
+    __shared__ unsigned slot;
+    const int warp = threadIdx.x >> 5;
+    if (warp == 0) sfdw::tm_alloc(&slot);
+    sfdw::tm_sync_cta();
+    const unsigned base = *reinterpret_cast<volatile unsigned *>(&slot), q = sfdw::tm_quarter(base, warp);
+    sfdw::TChunk c[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int i = 0; i < 16; ++i) c[j].w[i] = 0u;
+    if (warp < 4) {
+        for (int col = 0; col < sfdw::TM_COLS; col += 16) sfdw::tm_st(c[0], q + col);
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    }
+    sfdw::tm_sync_cta();
+    const bool active = (warp >> 2) < warps_per_quarter;
+    unsigned sum = 0;
+    long long t0 = clock64();
+    if (active)
+        for (int r = 0; r < reps; ++r) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) sfdw::tm_ld(c[j], q + 64 * (r & 7) + 16 * j);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                sfdw::tm_wait(c[j]);
+                sum += c[j].w[0] + c[j].w[15];
+            }
+        }
+    long long t1 = clock64();
+    if (threadIdx.x == 0) cycles[2 * blockIdx.x] = t1 - t0;
+    __syncthreads();
+    unsigned off = 0;
+    t0 = clock64();
+    if (warp == 0)
+        for (int r = 0; r < reps; ++r) {
+            sfdw::tm_ld(c[0], q + off);
+            sfdw::tm_wait(c[0]);
+            off = (c[0].w[3] & 0x10u) + 16u * (unsigned)(r & 15);  // (the columns hold zeros)
+            sum += off;
+        }
+    t1 = clock64();
+    if (threadIdx.x == 0) cycles[2 * blockIdx.x + 1] = t1 - t0;
+    out[blockIdx.x * 256 + threadIdx.x] = (float)sum;
+    sfdw::tm_finish(base);
+}
+
+}  // namespace
+
+// out[0] shared memory, bytes per clock and SM, in the access pattern of the transposes (16-byte row
+// reads + 8-byte column writes, 8 warps); out[1] / out[2] tensor-memory load rate in bytes per clock
+// and sub-partition with one / two warps per sub-partition (four tcgen05.ld.32x32b.x16 in flight per
+// warp); out[3] cycles of one dependent tcgen05.ld + wait::ld.
+extern "C" SFD_API int sfd_measure_memory_pipes(double out[4]) {
+    if (!out) return SFD_EINVAL;
+    int dev = 0, sms = 0;
+    float *res = nullptr;
+    long long *cyc = nullptr;
+    cudaError_t e;
+    auto done = [&](cudaError_t err) {
+        cudaFree(res);
+        cudaFree(cyc);
+        if (err == cudaSuccess) return (int)SFD_OK;
+        std::snprintf(g_static_err, sizeof g_static_err, "sfd_measure_memory_pipes: %s (%s)",
+                      cudaGetErrorName(err), cudaGetErrorString(err));
+        cudaGetLastError();
+        return (int)SFD_ECUDA;
+    };
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return done(e);
+    if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return done(e);
+    if ((e = cudaMalloc((void **)&res, (size_t)sms * 256 * sizeof(float))) != cudaSuccess) return done(e);
+    if ((e = cudaMalloc((void **)&cyc, (size_t)sms * 2 * sizeof(long long))) != cudaSuccess) return done(e);
+    std::vector<long long> hc(2 * (size_t)sms);
+    auto mean = [&](int stride, int which) {
+        double m = 0;
+        for (int i = 0; i < sms; ++i) m += (double)hc[(size_t)stride * i + which];
+        return m / sms;
+    };
+    const int reps = 2000;
+    for (int pass = 0; pass < 2; ++pass) k_peak_smem<<<sms, 256>>>(res, cyc, reps);
+    if ((e = cudaMemcpy(hc.data(), cyc, sms * sizeof(long long), cudaMemcpyDeviceToHost)) != cudaSuccess) return done(e);
+    out[0] = 8.0 * 32.0 * (8.0 * 16.0 + 16.0 * 8.0) * reps / mean(1, 0);
+    for (int wq = 1; wq <= 2; ++wq) {
+        for (int pass = 0; pass < 2; ++pass) k_peak_tmem<<<sms, 256>>>(res, cyc, reps, wq);
+        if ((e = cudaMemcpy(hc.data(), cyc, 2 * sms * sizeof(long long), cudaMemcpyDeviceToHost)) != cudaSuccess)
+            return done(e);
+        out[wq] = (double)wq * 4.0 * 16.0 * 32.0 * 4.0 * reps / mean(2, 0);
+        out[3] = mean(2, 1) / reps;
+    }
+    if ((e = cudaDeviceSynchronize()) != cudaSuccess) return done(e);
+    g_launches.fetch_add(6, std::memory_order_relaxed);
+    return done(cudaSuccess);
+}

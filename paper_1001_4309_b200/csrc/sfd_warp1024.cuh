@@ -130,9 +130,9 @@ constexpr int TABS = 2 * 3 * N;  // complex elements
 // shared memory that is a third of all shared-memory wavefronts of a line, on the pipe that also
 // carries the transposes.  Tensor memory (256 KB per SM, 128 lanes x 512 columns of 32 bits, unused
 // here otherwise: there is no MMA on this path) has its own read path into the register file
-// (tcgen05.ld, 64 B/clk per sub-partition measured, no contention between sub-partitions), and its
-// shape fits: a warp may touch only the 32 lanes of its sub-partition, lane l of warp w holds what
-// thread l needs.  Both warps of a sub-partition (w, w + 4) run the same branch b = w & 1, so each
+// (tcgen05.ld, 148 B/clk per sub-partition measured - sfd_measure_memory_pipes -, no contention between
+// sub-partitions), and its shape fits: a warp may touch only the 32 lanes of its sub-partition, lane l
+// of warp w holds what thread l needs.  Both warps of a sub-partition (w, w + 4) run the same branch b = w & 1, so each
 // lane quarter holds, per view set s (a CTA's lines lie in at most two views), 192 columns:
 //     column 192 s + 64 t + 2 r + {0, 1} = re, im of table t (pre_b, H_b, conj(post_b)) at lane + 32 r
 // A chunk is 16 columns = 8 complex values; tcgen05.wait::ld waits for every load in flight, so

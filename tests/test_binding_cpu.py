@@ -160,6 +160,7 @@ def test_round2_entry_points_reject_null_and_bad_arguments():
     assert B._lib.sfd_plan_get_nx(None) == B.SFD_EINVAL and B._lib.sfd_plan_get_ny(None) == B.SFD_EINVAL
     assert B._lib.sfd_plan_get_device(None) == B.SFD_EINVAL
     assert B._lib.sfd_measure_pipes(None) == B.SFD_EINVAL
+    assert B._lib.sfd_measure_memory_pipes(None) == B.SFD_EINVAL
     assert B._lib.sfd_host_dft32(None, None, 0, 0) == B.SFD_EINVAL
     with pytest.raises(B.SfdError):
         B.sfd_host_dft32(np.zeros(32, np.complex64), lane=32)

@@ -815,3 +815,10 @@ def test_measure_pipes_reports_sane_numbers():
     assert 40.0 < tf < 90.0            # 148 SMs x 128 lanes x 2 x ~1.9 GHz = 72 nominal
     assert 300.0 < cyc_a < 700.0 and 380.0 < cyc_b < 900.0
     assert 1.0 < ghz < 2.3
+
+
+def test_measure_memory_pipes_reports_sane_numbers():
+    smem, tm1, tm2, lat = B.sfd_measure_memory_pipes()
+    assert 60.0 < smem <= 130.0          # 128 B/clk and SM is the architectural rate
+    assert 40.0 < tm1 <= 300.0 and tm1 * 0.9 < tm2 <= 400.0   # measured 148 / 215 B/clk and sub-partition
+    assert 10.0 < lat < 200.0
