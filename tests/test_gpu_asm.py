@@ -148,3 +148,28 @@ def test_asm_2048_rejects_an_input_that_is_not_16_byte_aligned():
         f, _, _ = plan.execute(buf[2:2 + N * N].view(N, N), intensity=False, phase=False)
         torch.cuda.synchronize()
         assert torch.isfinite(f.abs().max())
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_random_asm_plans_against_oracle(seed):
+    """Seeded sweep: grid sides drawn from 128 .. 2048 independently (square 1024 and 2048 forced in for two seeds:
+    the warp-FFT paths), 1 - 3 planes of either sign, real or complex input, anisotropic pitch, band limit on or off."""
+    rng = np.random.default_rng(2000 + seed)
+    Nx, Ny = (int(2 ** rng.integers(7, 12)) for _ in range(2))
+    if seed == 0:
+        Nx = Ny = 1024
+    if seed == 1:
+        Nx = Ny = 2048
+    zs = list(rng.uniform(0.005, 0.2, int(rng.integers(1, 4))) * rng.choice([-1.0, 1.0]))
+    dtype = B.SFD_F32 if rng.random() < 0.5 else B.SFD_C64
+    pitch = (float(rng.uniform(2e-6, 6e-6)), float(rng.uniform(2e-6, 6e-6)))
+    bl = bool(rng.random() < 0.5)
+    if dtype == B.SFD_F32:
+        u0 = rng.random((Ny, Nx), dtype=np.float32)
+    else:
+        u0 = (rng.standard_normal((Ny, Nx)) + 1j * rng.standard_normal((Ny, Nx))).astype(np.complex64)
+    with B.AsmPlan(Nx, Ny, W.LAMBDA, pitch, zs, dtype, bl) as plan:
+        f, I, ph = plan.execute(torch.from_numpy(u0).to(_dev()))
+        torch.cuda.synchronize()
+    want, _, _ = A.propagate_planes(u0, W.LAMBDA, zs, pitch, bl)
+    _check(f.cpu().numpy(), I.cpu().numpy(), ph.cpu().numpy(), want, f"seed {seed}: {Nx}x{Ny}, {len(zs)} planes")

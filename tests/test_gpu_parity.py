@@ -691,6 +691,31 @@ def test_rectangular_grids_against_oracle(Nx, Ny, in_dtype, mask):
         _u8_check(u8.cpu().numpy(), O.intensity(want), f"{Nx}x{Ny} u8")
 
 
+@pytest.mark.parametrize("seed", range(10))
+def test_random_plans_against_oracle(seed):
+    """Seeded sweep over what a plan can be: grid sides drawn from 64 .. 1024 independently (every pairing of
+    the generic, N = 512 and N = 1024 kernels comes up), 1 - 5 views, uint8 or float32 input, pitches,
+    distances of either sign and window shifts drawn per view.  Field and intensity against form B."""
+    rng = np.random.default_rng(1000 + seed)
+    Nx, Ny = (int(2 ** rng.integers(6, 11)) for _ in range(2))
+    V = int(rng.integers(1, 6))
+    in_dtype = B.SFD_U8 if rng.random() < 0.5 else B.SFD_F32
+    g = dict(p1x=rng.uniform(3e-6, 7e-6, V), p1y=rng.uniform(3e-6, 7e-6, V),
+             p2x=rng.uniform(0.8e-6, 6e-6, V), p2y=rng.uniform(0.8e-6, 6e-6, V),
+             z=rng.uniform(0.03, 0.15, V) * rng.choice([-1.0, 1.0], V),
+             O0x=rng.uniform(-3e-4, 3e-4, V), O0y=rng.uniform(-3e-4, 3e-4, V),
+             O1x=rng.uniform(-8e-4, 8e-4, V), O1y=rng.uniform(-8e-4, 8e-4, V))
+    holo = (rng.integers(0, 256, (Ny, Nx), dtype=np.uint8) if in_dtype == B.SFD_U8
+            else rng.random((Ny, Nx), dtype=np.float32))
+    with B.Plan(Nx=Nx, Ny=Ny, lam=W.LAMBDA, in_dtype=in_dtype, **g) as plan:
+        f, I = plan.execute(torch.from_numpy(holo).to(_dev()))
+        torch.cuda.synchronize()
+    want = _rect_oracle(holo, g, "B")
+    what = f"seed {seed}: {Nx}x{Ny}, {V} views, dtype {in_dtype}"
+    _assert_close(f.cpu().numpy(), want, what + " field")
+    _assert_close(I.cpu().numpy(), O.intensity(want), what + " intensity")
+
+
 @pytest.mark.parametrize("col0,row0,warp", [(168, 0, True), (165, 0, False), (8, 3, True)])
 def test_ccd_frame_window_read_in_place(col0, row0, warp):
     """Row f3 / PAPER.md L42 (reading 13): the plan reads its 1024 x 1024 window out of a 1 360-wide 8-bit
